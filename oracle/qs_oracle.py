@@ -1,0 +1,587 @@
+"""CPU FP64 oracle for the quench-simulation hot path.  TEST INFRASTRUCTURE ONLY.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this file.  It shares no code with the CUDA path
+(``paper_2403_07666_b200/``) and never imports it; the product never imports this.
+
+Plain numpy/scipy, float64, written to be checked against the text by eye.  Citations are
+``PAPER.md:<line>`` (= /root/reference/PAPER.md) and ``SURVEY.md §8(c) C<k>`` (the readings
+of the points on which the paper's main text is silent; the same list is in DESIGN.md).
+
+Route taken here on purpose differs from the GPU's: K(k), E(k) come from the library
+(``scipy.special.ellipkm1`` / ``ellipe``, Cephes) and enter Maxwell's textbook bracket; dense
+matrices are formed explicitly; the per-step linear system is solved by dense Cholesky + Schur
+complement (its plain definition), with a projected CG only for sizes a dense solve cannot hold.
+
+Pins (tests/test_oracle_*.py, all ``-m "not gpu"``):
+  mutual_pair        Neumann double integral by quadrature; thin-ring self-inductance
+  field_pair         Biot-Savart quadrature; on-axis loop field; curl of A from mutual_pair
+  material_law       closed forms E(Jc)=Ec, E'->n Ec/Jc, Jc(4.2 K,0,0), strain zero, dE/dJ by FD
+  heat_substeps      exact discrete 1-D steady state; energy balance to rounding
+  kkt_dense / pcg    constraint C^T I' = d, KKT residual, dense vs CG, single-ring L-R circuit
+  lattice tables     table operator == dense operator on small lattices
+  nonlinear trajectory on config 1: PARITY UNPINNED beyond oracle-internal cross checks (no printed
+                     worked example exists for the config laws; SURVEY.md §8(c) pins table).
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+import scipy.linalg
+import scipy.special
+
+MU0 = 4.0e-7 * math.pi
+
+# event flag bits (PAPER.md:105 |J/Jc|>1, PAPER.md:119 rho>0.95 rho_n)
+FJ_T, FJ_E, FJ_J, Q_T, Q_RHO = 1, 2, 4, 8, 16
+# qs_step return bits
+RET_FLUXJUMP, RET_QUENCH, RET_CG_MAXIT = 1, 2, 4
+
+
+# --------------------------------------------------------------------------------------
+# C2: ring-to-ring mutual inductance (Maxwell's formula for two coaxial filaments)
+# --------------------------------------------------------------------------------------
+def elliptic_KE(kp2):
+    """K(k), E(k) from the complementary parameter kp2 = 1 - k^2 = B2/A2 (library routines)."""
+    K = scipy.special.ellipkm1(kp2)
+    E = scipy.special.ellipe(1.0 - kp2)
+    return K, E
+
+
+def mutual_pair(ri, zi, rj, zj, soft2=0.0):
+    """M_ij [H] between coaxial filaments; ``soft2`` = g^2 added to dz^2.
+
+    A2 = (ri+rj)^2 + dz^2, B2 = (ri-rj)^2 + dz^2, k^2 = 4 ri rj / A2 = 1 - B2/A2
+    M = mu0 sqrt(ri rj) [ (2/k - k) K(k) - (2/k) E(k) ]
+    """
+    dz2 = (zi - zj) ** 2 + soft2
+    A2 = (ri + rj) ** 2 + dz2
+    B2 = (ri - rj) ** 2 + dz2
+    kp2 = B2 / A2
+    k = np.sqrt(1.0 - kp2)
+    K, E = elliptic_KE(kp2)
+    return MU0 * np.sqrt(ri * rj) * ((2.0 / k - k) * K - (2.0 / k) * E)
+
+
+def mutual_rows(geo, rows):
+    """Rows ``rows`` of the symmetric matrix M: [len(rows), N].
+
+    lattice: filament formula off the diagonal, M_ii = M(r_i, r_i, dz = g) (Maxwell's GMD rule);
+    free rings: dz^2 + g^2 for every pair (softened Neumann kernel, SPD by construction).
+    """
+    rows = np.asarray(rows, dtype=np.int64)
+    g2 = float(geo.softening) ** 2
+    ri, zi = geo.r[rows, None], geo.z[rows, None]
+    rj, zj = geo.r[None, :], geo.z[None, :]
+    if geo.lattice:
+        soft = np.zeros((rows.size, geo.n_rings))
+        soft[np.arange(rows.size), rows] = g2          # i == j only
+        return mutual_pair(ri, zi, rj, zj, soft)
+    return mutual_pair(ri, zi, rj, zj, g2)
+
+
+def dense_M(geo, chunk=512):
+    N = geo.n_rings
+    M = np.empty((N, N))
+    for s in range(0, N, chunk):
+        e = min(N, s + chunk)
+        M[s:e] = mutual_rows(geo, np.arange(s, e))
+    return M
+
+
+def matvec_rows(geo, x, rows, chunk=256):
+    """y_i = sum_j M_ij x_j for the listed target rows, evaluated pair by pair."""
+    rows = np.asarray(rows, dtype=np.int64)
+    y = np.empty(rows.size)
+    for s in range(0, rows.size, chunk):
+        e = min(rows.size, s + chunk)
+        y[s:e] = mutual_rows(geo, rows[s:e]) @ x
+    return y
+
+
+def matvec(geo, x, chunk=256):
+    return matvec_rows(geo, x, np.arange(geo.n_rings), chunk)
+
+
+# --------------------------------------------------------------------------------------
+# C3: field of a unit-current loop
+# --------------------------------------------------------------------------------------
+def field_pair(ri, zi, rj, zj):
+    """(Br, Bz) [T/A] at (ri, zi) of a unit-current filament loop of radius rj at height zj.
+
+    Bz = mu0/(2 pi sqrt(A2)) [ K + (rj^2 - ri^2 - dz^2)/B2 E ]
+    Br = mu0/(2 pi sqrt(A2)) (dz/ri) [ -K + (rj^2 + ri^2 + dz^2)/B2 E ],   dz = zi - zj
+    """
+    dz = zi - zj
+    A2 = (ri + rj) ** 2 + dz ** 2
+    B2 = (ri - rj) ** 2 + dz ** 2
+    K, E = elliptic_KE(B2 / A2)
+    pref = MU0 / (2.0 * math.pi * np.sqrt(A2))
+    Bz = pref * (K + (rj ** 2 - ri ** 2 - dz ** 2) / B2 * E)
+    Br = pref * (dz / ri) * (-K + (rj ** 2 + ri ** 2 + dz ** 2) / B2 * E)
+    return Br, Bz
+
+
+def self_field_coef(geo):
+    """Bz_self,i / I_i = mu0 [ln(8 r_i / g) - 1] / (4 pi r_i); Br_self = 0."""
+    return MU0 * (np.log(8.0 * geo.r / geo.softening) - 1.0) / (4.0 * math.pi * geo.r)
+
+
+def field_rows(geo, rows):
+    """Rows of the dense field matrices (GBr, GBz): B_i = sum_j GB_ij I_j, self term on the diagonal."""
+    rows = np.asarray(rows, dtype=np.int64)
+    ri, zi = geo.r[rows, None], geo.z[rows, None]
+    rj = np.broadcast_to(geo.r[None, :], (rows.size, geo.n_rings)).copy()
+    zj = np.broadcast_to(geo.z[None, :], (rows.size, geo.n_rings)).copy()
+    idx = np.arange(rows.size)
+    zj[idx, rows] += 1.0                      # keep the i == j entry finite; overwritten below
+    Br, Bz = field_pair(ri, zi, rj, zj)
+    Br[idx, rows] = 0.0
+    Bz[idx, rows] = self_field_coef(geo)[rows]
+    return Br, Bz
+
+
+def dense_GB(geo, chunk=512):
+    N = geo.n_rings
+    GBr, GBz = np.empty((N, N)), np.empty((N, N))
+    for s in range(0, N, chunk):
+        e = min(N, s + chunk)
+        GBr[s:e], GBz[s:e] = field_rows(geo, np.arange(s, e))
+    return GBr, GBz
+
+
+def field_eval_rows(geo, I, rows, chunk=256):
+    """(Br_i, Bz_i) of ring currents I [A] at the listed rows, without B_ext."""
+    rows = np.asarray(rows, dtype=np.int64)
+    Br, Bz = np.empty(rows.size), np.empty(rows.size)
+    for s in range(0, rows.size, chunk):
+        e = min(rows.size, s + chunk)
+        gr, gz = field_rows(geo, rows[s:e])
+        Br[s:e], Bz[s:e] = gr @ I, gz @ I
+    return Br, Bz
+
+
+# --------------------------------------------------------------------------------------
+# Lattice tables (SURVEY.md §8(d) "Oracle timing"): on a regular lattice M and G_B depend only
+# on (ir, jr, iz - jz).  Used for lattices too large for dense matrices; checked against the
+# dense operators on small lattices (tests/test_oracle_lattice.py).
+# --------------------------------------------------------------------------------------
+class LatticeTables:
+    def __init__(self, geo, with_field=True):
+        assert geo.lattice
+        Nr, Nz, h = geo.Nr, geo.Nz, geo.h
+        self.Nr, self.Nz = Nr, Nz
+        rr = geo.r.reshape(Nr, Nz)[:, 0]
+        d = np.arange(Nz) * h                                   # |iz - jz| * h
+        ri, rj, dz = rr[:, None, None], rr[None, :, None], d[None, None, :]
+        soft = np.zeros((Nr, Nr, Nz))
+        soft[np.arange(Nr), np.arange(Nr), 0] = float(geo.softening) ** 2
+        self.M = np.empty((Nr, Nr, Nz))
+        for a in range(Nr):                                     # row by row: bounded memory
+            self.M[a] = mutual_pair(ri[a], 0.0, rj[0], dz[0], soft[a])
+        self.with_field = with_field
+        if with_field:
+            self.Br = np.empty((Nr, Nr, Nz))                    # for dz = +d (target above source)
+            self.Bz = np.empty((Nr, Nr, Nz))
+            selfc = self_field_coef(geo).reshape(Nr, Nz)[:, 0]
+            for a in range(Nr):
+                dzz = np.broadcast_to(dz[0], (Nr, Nz)).copy()
+                dzz[a, 0] = 1.0
+                br, bz = field_pair(ri[a], dzz, rj[0], 0.0)
+                br[a, 0], bz[a, 0] = 0.0, selfc[a]
+                self.Br[a], self.Bz[a] = br, bz
+
+    def _apply(self, tab, X, odd):
+        """Y[ir, iz] = sum_{jr, jz} tab[ir, jr, |iz-jz|] * sgn * X[jr, jz], offset by offset."""
+        Nz = self.Nz
+        Y = tab[:, :, 0] @ X
+        for d in range(1, Nz):
+            T = tab[:, :, d]
+            Y[:, d:] += T @ X[:, : Nz - d]                       # targets above sources: dz = +d h
+            Y[:, : Nz - d] += (-1.0 if odd else 1.0) * (T @ X[:, d:])   # dz = -d h
+        return Y
+
+    def matvec(self, x):
+        return self._apply(self.M, x.reshape(self.Nr, self.Nz), False).reshape(-1)
+
+    def field(self, I):
+        X = I.reshape(self.Nr, self.Nz)
+        return (self._apply(self.Br, X, True).reshape(-1), self._apply(self.Bz, X, False).reshape(-1))
+
+
+# --------------------------------------------------------------------------------------
+# C5: material law (BASELINE.json configs[0]; PAPER.md:79 E-J law spanning creep -> normal)
+# --------------------------------------------------------------------------------------
+def ipow(x, n):
+    """x**n for a non-negative integer n by repeated multiplication (SURVEY.md C5 guard note)."""
+    out = np.ones_like(x)
+    with np.errstate(over="ignore"):
+        for _ in range(int(n)):
+            out = out * x
+    return out
+
+
+def material_law(mat, J, T, Br, Bz, r, jc0_scale):
+    """Returns dict(eps, Jc, rho, E, dEdJ, Q) per cell.
+
+    eps = J Bz r / Y ; |B| = sqrt(Br^2+Bz^2)
+    Jc  = Jc0 s max(1-T/Tc,0)^2 / (1+|B|/B0) max(1-eps_coef |eps|^eps_exp, 0)
+    rho_sc = (Ec/Jc)(|J|/Jc)^(n-1) ; rho = rho_sc rho_n/(rho_sc+rho_n)
+    E = rho J ; Q = E J ; dE/dJ = rho (1 + (n-1) rho_n/(rho_sc+rho_n))
+    Guards: Jc <= 0 -> rho = dE/dJ = rho_n ; J == 0 -> rho = dE/dJ = 0.
+    """
+    n = mat.n_exp
+    eps = J * Bz * r / mat.Y
+    Bmag = np.sqrt(Br * Br + Bz * Bz)
+    fT = np.maximum(1.0 - T / mat.Tc, 0.0)
+    fe = np.maximum(1.0 - mat.eps_coef * np.abs(eps) ** mat.eps_exp, 0.0)
+    Jc = mat.Jc0 * jc0_scale * fT * fT / (1.0 + Bmag / mat.B0) * fe
+    rho = np.empty_like(J)
+    dEdJ = np.empty_like(J)
+    normal = Jc <= 0.0
+    zero = (J == 0.0) & ~normal
+    sc = ~normal & ~zero
+    rho[normal] = mat.rho_n
+    dEdJ[normal] = mat.rho_n
+    rho[zero] = 0.0
+    dEdJ[zero] = 0.0
+    if np.any(sc):
+        x = np.abs(J[sc]) / Jc[sc]
+        if float(n) == int(n):
+            xp = ipow(x, int(n) - 1)
+        else:
+            xp = x ** (n - 1.0)
+        with np.errstate(over="ignore", invalid="ignore", divide="ignore"):
+            rho_sc = (mat.Ec / Jc[sc]) * xp
+            big = rho_sc >= mat.rho_n
+            u = np.where(big, mat.rho_n / rho_sc, rho_sc / mat.rho_n)   # always in [0, 1]
+        # rho = rho_sc rho_n/(rho_sc + rho_n), w = rho_n/(rho_sc + rho_n), overflow-free forms
+        rho_s = np.where(big, mat.rho_n / (1.0 + u), np.where(np.isfinite(rho_sc), rho_sc, 0.0) / (1.0 + u))
+        w = np.where(big, u / (1.0 + u), 1.0 / (1.0 + u))
+        rho[sc] = rho_s
+        dEdJ[sc] = rho_s * (1.0 + (n - 1.0) * w)
+    E = rho * J
+    return dict(eps=eps, Jc=Jc, rho=rho, E=E, dEdJ=dEdJ, Q=E * J)
+
+
+# --------------------------------------------------------------------------------------
+# C9: explicit finite-volume heat sub-steps in enthalpy form (PAPER.md:75 heat equation + Robin BC)
+# --------------------------------------------------------------------------------------
+def enthalpy(mat, T):
+    """H(T) = int_0^T C dT = C3/4 T^4 + C1/2 T^2,  C(T) = C3 T^3 + C1 T."""
+    return 0.25 * mat.C3 * T ** 4 + 0.5 * mat.C1 * T ** 2
+
+
+def temperature(mat, H):
+    """Inverse of enthalpy(): T^2 = (-C1/2 + sqrt(C1^2/4 + C3 H)) / (C3/2)."""
+    return np.sqrt((-0.5 * mat.C1 + np.sqrt(0.25 * mat.C1 ** 2 + mat.C3 * H)) / (0.5 * mat.C3))
+
+
+def heat_substeps_count(geo, mat, dt):
+    """m = ceil(dt / (0.8 h^2/(4 alpha0))), alpha0 = k_in/(C3 T_bath^2 + C1)."""
+    alpha0 = mat.k_in / (mat.C3 * geo.T_bath * geo.T_bath + mat.C1)
+    limit = 0.8 * geo.h * geo.h / (4.0 * alpha0)
+    return max(1, int(math.ceil(dt / limit)))
+
+
+def heat_flux_divergence(geo, mat, T2d):
+    """sum_f F_f [W] per cell and the boundary loss [W] summed over the pack.
+
+    interior face c|c': F = kappa_f (T_c'^2 - T_c^2)/(2h) A_f, kappa_f = k_in if same turn else k_between
+    boundary face:      F = -h_conv,side (T_c - T_bath) A_f
+    radial face area 2 pi (r_c +- h/2) h, axial face area 2 pi r_c h.
+    """
+    Nr, Nz, n, h = geo.Nr, geo.Nz, geo.cells_per_side, geo.h
+    r2d = geo.r.reshape(Nr, Nz)
+    T2 = T2d * T2d
+    F = np.zeros((Nr, Nz))
+    # radial faces between ir and ir+1
+    same = ((np.arange(Nr - 1) // n) == (np.arange(1, Nr) // n))
+    kap = np.where(same, mat.k_in, mat.k_between)[:, None]
+    area = 2.0 * math.pi * (r2d[:-1] + 0.5 * h) * h
+    flow = kap * (T2[1:] - T2[:-1]) / (2.0 * h) * area          # into cell ir from ir+1
+    F[:-1] += flow
+    F[1:] -= flow
+    # axial faces between iz and iz+1
+    same = ((np.arange(Nz - 1) // n) == (np.arange(1, Nz) // n))
+    kap = np.where(same, mat.k_in, mat.k_between)[None, :]
+    area = 2.0 * math.pi * r2d[:, :-1] * h
+    flow = kap * (T2[:, 1:] - T2[:, :-1]) / (2.0 * h) * area
+    F[:, :-1] += flow
+    F[:, 1:] -= flow
+    # four borders of the winding pack ("four borders on the cross-section")
+    hc = geo.h_conv
+    loss = np.zeros((Nr, Nz))
+    loss[0] += hc[0] * (T2d[0] - geo.T_bath) * 2.0 * math.pi * (r2d[0] - 0.5 * h) * h
+    loss[-1] += hc[1] * (T2d[-1] - geo.T_bath) * 2.0 * math.pi * (r2d[-1] + 0.5 * h) * h
+    loss[:, 0] += hc[2] * (T2d[:, 0] - geo.T_bath) * 2.0 * math.pi * r2d[:, 0] * h
+    loss[:, -1] += hc[3] * (T2d[:, -1] - geo.T_bath) * 2.0 * math.pi * r2d[:, -1] * h
+    return F - loss, float(loss.sum())
+
+
+def heat_substeps(geo, mat, H, Q, dt, m):
+    """m explicit sub-steps of dH/dt = sum_f F_f / V + Q with Q frozen; returns (H, boundary energy [J])."""
+    Nr, Nz, h = geo.Nr, geo.Nz, geo.h
+    vol = (2.0 * math.pi * geo.r * h * h).reshape(Nr, Nz)
+    H2 = H.reshape(Nr, Nz).copy()
+    Q2 = Q.reshape(Nr, Nz)
+    sub = dt / m
+    lost = 0.0
+    for _ in range(m):
+        T2d = temperature(mat, H2)
+        div, loss = heat_flux_divergence(geo, mat, T2d)
+        H2 = H2 + sub * (div / vol + Q2)
+        lost += sub * loss
+    return H2.reshape(-1), lost
+
+
+# --------------------------------------------------------------------------------------
+# C4 / C8: circuit equations.   [A C; C^T 0] [I'; V] = [b; d],  A = M + theta dt D
+# --------------------------------------------------------------------------------------
+def constraint_matrix(geo):
+    C = np.zeros((geo.n_rings, geo.n_turns))
+    if geo.n_turns:
+        C[np.arange(geo.n_rings), geo.turn_id] = 1.0
+    return C
+
+
+def kkt_dense(A, C, b, d):
+    """Unique solution of the KKT system by dense Cholesky + Schur complement (SURVEY.md C8 brute force).
+
+    S = C^T A^-1 C ; V = S^-1 (C^T A^-1 b - d) ; I' = A^-1 (b - C V)
+    """
+    cf = scipy.linalg.cho_factor(A, lower=True)
+    Ainv_b = scipy.linalg.cho_solve(cf, b)
+    if C.shape[1] == 0:
+        return Ainv_b, np.zeros(0)
+    Ainv_C = scipy.linalg.cho_solve(cf, C)
+    S = C.T @ Ainv_C
+    V = np.linalg.solve(S, C.T @ Ainv_b - d)
+    return Ainv_b - Ainv_C @ V, V
+
+
+def pcg(apply_A, diagA, turn_id, n_turns, b, d, tol, maxit, x0=None):
+    """Projected CG with per-turn Schur complement, SURVEY.md C8 step by step.
+
+    Returns (x, V, iterations, sqrt(r^T g) / nu).  nu = sqrt(r^T g) of the cold start x_p
+    (reference norm: b can be exactly 0, so "relative to |b|" is undefined).
+    """
+    N = b.size
+    Hd = diagA
+    if n_turns:
+        s = np.bincount(turn_id, weights=1.0 / Hd, minlength=n_turns)
+
+    def project(r):
+        if not n_turns:
+            return r / Hd, np.zeros(0)
+        v = np.bincount(turn_id, weights=r / Hd, minlength=n_turns) / s
+        return (r - v[turn_id]) / Hd, v
+
+    # cold start x_p = H^-1 C (d/s): satisfies C^T x = d; its projected residual is the reference norm nu
+    x = np.zeros(N)
+    if n_turns:
+        x = (d / s)[turn_id] / Hd
+    vsum = np.zeros(n_turns)
+    r = apply_A(x) - b
+    g, v = project(r)
+    if n_turns:
+        r = r - v[turn_id]
+    nu = math.sqrt(max(float(r @ g), 0.0))
+    if nu == 0.0:
+        return x, -v, 0, 0.0
+    if x0 is not None:                       # warm start, moved onto the constraint
+        x = x0.copy()
+        if n_turns:
+            cur = np.bincount(turn_id, weights=x, minlength=n_turns)
+            x = x + ((d - cur) / s)[turn_id] / Hd
+        r = apply_A(x) - b
+        g, v = project(r)
+        if n_turns:
+            r = r - v[turn_id]
+    if n_turns:
+        vsum += v
+    p = -g
+    rg = float(r @ g)
+    it = 0
+    while it < maxit and math.sqrt(max(rg, 0.0)) > tol * nu:
+        q = apply_A(p)
+        alpha = rg / float(p @ q)
+        x = x + alpha * p
+        r = r + alpha * q
+        g, v = project(r)
+        if n_turns:
+            r = r - v[turn_id]
+            vsum += v
+        rg_new = float(r @ g)
+        p = -g + (rg_new / rg) * p
+        rg = rg_new
+        it += 1
+    return x, -vsum, it, math.sqrt(max(rg, 0.0)) / nu
+
+
+# --------------------------------------------------------------------------------------
+# C10: events
+# --------------------------------------------------------------------------------------
+def turn_observables(geo, mat, T, E, J, Jc, rho):
+    """Per turn: Tmax, mean|E|, max|J|/Jc, min rho/rho_n."""
+    nt, tid = geo.n_turns, geo.turn_id
+    Tmax = np.full(nt, -np.inf)
+    np.maximum.at(Tmax, tid, T)
+    Ebar = np.bincount(tid, weights=np.abs(E), minlength=nt) / np.bincount(tid, minlength=nt)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        ratio = np.where(Jc > 0.0, np.abs(J) / np.where(Jc > 0.0, Jc, 1.0), np.where(J != 0.0, np.inf, 0.0))
+    xmax = np.zeros(nt)
+    np.maximum.at(xmax, tid, ratio)
+    rmin = np.full(nt, np.inf)
+    np.minimum.at(rmin, tid, rho / mat.rho_n)
+    return Tmax, Ebar, xmax, rmin
+
+
+# --------------------------------------------------------------------------------------
+# The stepper: same calls as include/qs.h (qs_init / qs_step / qs_read / qs_write / ...)
+# --------------------------------------------------------------------------------------
+class Oracle:
+    """operator = 'dense' (N <= ~8k), 'tables' (regular lattices of any size)."""
+
+    def __init__(self, geo, mat, operator="dense", solver="cholesky"):
+        self.geo, self.mat = geo, mat
+        N = geo.n_rings
+        self.N = N
+        self.scale = np.ones(N) if mat.jc0_scale is None else np.asarray(mat.jc0_scale, dtype=np.float64)
+        self.operator, self.solver = operator, solver
+        self.tables = None
+        self.M = self.GBr = self.GBz = None
+        if operator == "dense":
+            self.M = dense_M(geo)
+            if geo.lattice:
+                self.GBr, self.GBz = dense_GB(geo)
+            self.diagM = np.diag(self.M).copy()
+        elif operator == "tables":
+            self.tables = LatticeTables(geo)
+            rr = np.arange(geo.Nr)
+            self.diagM = np.repeat(self.tables.M[rr, rr, 0], geo.Nz)
+        else:
+            raise ValueError(operator)
+        self.C = constraint_matrix(geo) if (solver == "cholesky" and operator == "dense") else None
+        self.J = np.zeros(N)
+        self.T = np.full(N, geo.T_bath)
+        self.H = enthalpy(mat, self.T)
+        self.t, self.I = 0.0, 0.0
+        self.Br, self.Bz, self.E = np.zeros(N), np.zeros(N), np.zeros(N)
+        self.Idot = np.zeros(N)
+        nt = max(geo.n_turns, 0)
+        self.flags = np.zeros(nt, dtype=np.int32)
+        self.t_first = np.full(nt, -1.0)
+        self.count = np.zeros(nt, dtype=np.int32)
+        self.Ebar_prev = None
+        self.stats = dict(cg_iters=0, cg_relres=0.0, U_terminal=0.0, Tmax=geo.T_bath, joule_power=0.0,
+                          boundary_energy=0.0, heat_substeps=0)
+
+    # -- operators ----------------------------------------------------------------
+    def apply_M(self, x):
+        return self.M @ x if self.M is not None else self.tables.matvec(x)
+
+    def field(self, Icur):
+        if self.M is not None:
+            return self.GBr @ Icur, self.GBz @ Icur
+        return self.tables.field(Icur)
+
+    def Bext(self, t):
+        g = self.geo
+        if g.Bext_rate == 0.0:
+            return g.Bext0
+        return min(g.Bext0 + g.Bext_rate * t, g.Bext_max)
+
+    # -- state --------------------------------------------------------------------
+    def write(self, J, T, t, I):
+        self.J, self.T = np.array(J, dtype=np.float64), np.array(T, dtype=np.float64)
+        self.H = enthalpy(self.mat, self.T)
+        self.t, self.I = float(t), float(I)
+        self.Ebar_prev = None
+        self.Idot = np.zeros(self.N)
+
+    def read(self):
+        return self.J.copy(), self.T.copy(), np.concatenate([self.Br, self.Bz]), self.E.copy()
+
+    # -- one step (order of C6: everything on the rhs at t^k) ----------
+    def step(self, dt, I_ramp):
+        geo, mat = self.geo, self.mat
+        if not geo.lattice:
+            raise ValueError("qs_step needs a lattice geometry")
+        if dt <= 0.0:
+            return -5
+        a = geo.area
+        # S1 field of the ring currents I = a J plus the background field at t^k
+        B0, B1 = self.Bext(self.t), self.Bext(self.t + dt)
+        Bdot = (B1 - B0) / dt
+        Br, Bz = self.field(a * self.J)
+        Bz = Bz + B0
+        # S2 material law at (J^k, T^k, B^k); rhs b = -2 pi r (E + r Bdot / 2)   (C4)
+        ml = material_law(mat, self.J, self.T, Br, Bz, geo.r, self.scale)
+        b = -2.0 * math.pi * geo.r * (ml["E"] + 0.5 * geo.r * Bdot)
+        D = 2.0 * math.pi * geo.r * ml["dEdJ"] / a
+        shift = mat.theta * dt * D
+        d = np.full(geo.n_turns, float(I_ramp))
+        # S3/S4 constrained solve (C7: linearly implicit theta step)
+        if self.solver == "cholesky":
+            A = self.M + np.diag(shift)
+            Idot, V = kkt_dense(A, self.C, b, d)
+            iters, relres = 0, 0.0
+        else:
+            Idot, V, iters, relres = pcg(lambda x: self.apply_M(x) + shift * x, self.diagM + shift,
+                                         geo.turn_id, geo.n_turns, b, d, mat.cg_tol, mat.cg_maxit, self.Idot)
+        # S5 update
+        self.Idot = Idot
+        Jold = self.J
+        self.J = self.J + dt * Idot / a
+        self.I += dt * I_ramp
+        self.t += dt
+        # S6 heat with the Joule source of step k frozen over the sub-steps
+        m = heat_substeps_count(geo, mat, dt)
+        self.H, lost = heat_substeps(geo, mat, self.H, ml["Q"], dt, m)
+        self.T = temperature(mat, self.H)
+        self.Br, self.Bz, self.E = Br, Bz, ml["E"]
+        # S7 events: T^{k+1}; E, |J|/Jc, rho of the material evaluation of this step
+        ret = self._events(dt, Jold, ml) if geo.n_turns else 0
+        self.stats = dict(cg_iters=iters, cg_relres=relres, U_terminal=float(-V.sum()),
+                          Tmax=float(self.T.max()),
+                          joule_power=float(np.sum(ml["Q"] * 2.0 * math.pi * geo.r * a)),
+                          boundary_energy=lost, heat_substeps=m)
+        if not (np.all(np.isfinite(self.J)) and np.all(np.isfinite(self.T))):
+            return -3
+        return ret
+
+    def _events(self, dt, Jold, ml):
+        geo, mat = self.geo, self.mat
+        Tmax, Ebar, xmax, rmin = turn_observables(geo, mat, self.T, ml["E"], Jold, ml["Jc"], ml["rho"])
+        fl = np.zeros(geo.n_turns, dtype=np.int32)
+        fl |= np.where(Tmax > mat.T_fluxjump, FJ_T, 0).astype(np.int32)
+        if self.Ebar_prev is not None:
+            fl |= np.where((Ebar - self.Ebar_prev) / dt > mat.dEdt_spike, FJ_E, 0).astype(np.int32)
+        fl |= np.where(xmax > 1.0, FJ_J, 0).astype(np.int32)
+        fl |= np.where(Tmax > mat.Tc, Q_T, 0).astype(np.int32)
+        fl |= np.where(rmin > 0.95, Q_RHO, 0).astype(np.int32)
+        fj_mask = FJ_T | FJ_E
+        rising = ((fl & fj_mask) != 0) & ((self.flags & fj_mask) == 0)
+        self.count += rising.astype(np.int32)
+        first = (fl != 0) & (self.t_first < 0.0)
+        self.t_first[first] = self.t
+        fj_all = FJ_T | FJ_E | FJ_J
+        started = ((fl & fj_all) != 0) & ((self.flags & fj_all) == 0)
+        ret = (RET_FLUXJUMP if np.any(started) else 0) | (RET_QUENCH if np.any(fl & (Q_T | Q_RHO)) else 0)
+        self.flags = fl
+        self.Ebar_prev = Ebar
+        return int(ret)
+
+    # -- config 4 ---------------------------------------------------------------------
+    def solve(self, b, tol=None, maxit=None, dense=False):
+        """M x = b with no constraint (free rings) or with the geometry's turns and d = 0."""
+        geo, mat = self.geo, self.mat
+        d = np.zeros(geo.n_turns)
+        if dense:
+            x, _ = kkt_dense(self.M, constraint_matrix(geo), b, d)
+            return x, 0, 0.0
+        x, _, it, rel = pcg(self.apply_M, self.diagM, geo.turn_id, geo.n_turns, b, d,
+                            mat.cg_tol if tol is None else tol, mat.cg_maxit if maxit is None else maxit)
+        return x, it, rel

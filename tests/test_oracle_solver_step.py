@@ -1,0 +1,195 @@
+"""Pins of the oracle's constrained solve, lattice tables and whole step (C6, C7, C10)."""
+import dataclasses
+import math
+
+import numpy as np
+import pytest
+
+import workloads as wl
+from oracle import qs_oracle as qo
+
+MU0 = 4e-7 * math.pi
+
+
+def small_lattice():
+    return wl.lattice_geometry(2, 3, 4, 1e-3, 30e-3)
+
+
+def test_kkt_dense_satisfies_the_kkt_system():
+    geo = small_lattice()
+    g = np.random.default_rng(1)
+    M = qo.dense_M(geo)
+    A = M + np.diag(g.random(geo.n_rings) * 1e-8)
+    C = qo.constraint_matrix(geo)
+    assert C.shape == (96, 6) and np.all(C.sum(axis=1) == 1) and np.all(C.sum(axis=0) == 16)
+    b = g.standard_normal(geo.n_rings) * 1e-6
+    d = g.standard_normal(geo.n_turns) * 10
+    x, V = qo.kkt_dense(A, C, b, d)
+    # brute force: the full (N + Nw) KKT matrix solved by LU
+    KKT = np.block([[A / MU0, C], [C.T, np.zeros((6, 6))]])
+    sol = np.linalg.solve(KKT, np.concatenate([b / MU0, d]))
+    assert np.max(np.abs(x - sol[:96])) < 1e-9 * np.max(np.abs(x))
+    assert np.max(np.abs(V - sol[96:] * MU0)) < 1e-9 * np.max(np.abs(V))
+    assert np.max(np.abs(C.T @ x - d)) < 1e-10 * np.max(np.abs(d))
+    assert np.max(np.abs(A @ x + C @ V - b)) < 1e-9 * np.max(np.abs(b))
+
+
+def test_projected_cg_equals_dense_kkt_and_keeps_the_constraint():
+    geo = small_lattice()
+    g = np.random.default_rng(2)
+    M = qo.dense_M(geo)
+    shift = g.random(geo.n_rings) * 1e-8
+    A = M + np.diag(shift)
+    b = g.standard_normal(geo.n_rings) * 1e-6
+    d = np.full(geo.n_turns, 50.0)
+    xd, Vd = qo.kkt_dense(A, qo.constraint_matrix(geo), b, d)
+    x, V, it, rel = qo.pcg(lambda v: A @ v, np.diag(A).copy(), geo.turn_id, geo.n_turns, b, d, 1e-13, 500)
+    assert 0 < it < 200 and rel <= 1e-13
+    assert np.max(np.abs(x - xd)) < 1e-9 * np.max(np.abs(xd))
+    assert np.max(np.abs(V - Vd)) < 1e-8 * np.max(np.abs(Vd))
+    cur = np.bincount(geo.turn_id, weights=x)
+    assert np.max(np.abs(cur - d)) < 1e-10 * 50
+    # warm start from the solution: converged at once; from a perturbed solution: same answer
+    x2, V2, it2, _ = qo.pcg(lambda v: A @ v, np.diag(A).copy(), geo.turn_id, geo.n_turns, b, d, 1e-10, 500, x0=xd)
+    assert it2 == 0 and np.max(np.abs(V2 - Vd)) < 1e-8 * np.max(np.abs(Vd))
+    x3, _, it3, _ = qo.pcg(lambda v: A @ v, np.diag(A).copy(), geo.turn_id, geo.n_turns, b, d, 1e-13, 500,
+                           x0=xd * (1 + 0.1 * g.standard_normal(96)))
+    assert np.max(np.abs(x3 - xd)) < 1e-9 * np.max(np.abs(xd))
+
+
+def test_unconstrained_cg_on_free_rings():
+    geo, x = wl.free_rings(256)
+    o = qo.Oracle(geo, wl.Material(cg_tol=1e-13, cg_maxit=5000))
+    b = o.apply_M(x)
+    assert np.max(np.abs(b - qo.matvec(geo, x))) == 0.0
+    xd, _, _ = o.solve(b, dense=True)
+    xc, it, rel = o.solve(b)
+    assert np.linalg.norm(xd - x) < 1e-6 * np.linalg.norm(x)              # cond ~ 1e6
+    assert np.linalg.norm(o.apply_M(xc) - b) < 1e-11 * np.linalg.norm(b)
+
+
+def test_lattice_tables_equal_dense_operators():
+    geo = wl.lattice_geometry(3, 2, 3, 0.8e-3, 40e-3)
+    g = np.random.default_rng(3)
+    x = g.standard_normal(geo.n_rings)
+    tab = qo.LatticeTables(geo)
+    M = qo.dense_M(geo)
+    GBr, GBz = qo.dense_GB(geo)
+    assert np.max(np.abs(tab.matvec(x) - M @ x)) < 1e-14 * np.max(np.abs(M @ x))
+    br, bz = tab.field(x)
+    assert np.max(np.abs(br - GBr @ x)) < 1e-13 * np.max(np.abs(GBr @ x))
+    assert np.max(np.abs(bz - GBz @ x)) < 1e-13 * np.max(np.abs(GBz @ x))
+
+
+def test_single_ring_is_an_LR_circuit():
+    # one normal-state ring (T > Tc: rho = rho_n) in a ramped axial field, no current constraint:
+    # L I' + R I = -pi r^2 Bdot,  L = mu0 r [ln(8r/g) - 2],  R = rho_n 2 pi r / a;  I(t) = I_inf (1 - exp(-t/tau))
+    base = wl.lattice_geometry(1, 1, 1, 1e-3, 30e-3, h_conv=0.0, Bext_rate=10.0, Bext_max=100.0)
+    geo = dataclasses.replace(base, n_turns=0, turn_id=None)
+    mat = wl.Material()
+    r, a = geo.r[0], geo.area[0]
+    L = MU0 * r * (math.log(8 * r / geo.softening) - 2.0)
+    R = mat.rho_n * 2 * math.pi * r / a
+    tau, I_inf = L / R, -math.pi * r * r * 10.0 / R
+    t_end = 2.0 * tau
+    errs = []
+    for steps in (200, 400):
+        o = qo.Oracle(geo, mat)
+        o.write(np.zeros(1), np.full(1, 20.0), 0.0, 0.0)
+        for _ in range(steps):
+            assert o.step(t_end / steps, 0.0) >= 0
+        assert o.T[0] >= 20.0
+        exact = I_inf * (1 - math.exp(-o.t / tau))
+        errs.append(abs(o.J[0] * a - exact) / abs(exact))
+    assert errs[1] < 2e-3 and 1.8 < errs[0] / errs[1] < 2.2                # first order in dt, right limit
+
+
+def test_step_keeps_turn_currents_and_inductance_in_linear_regime():
+    w = wl.shrunk(0, 2, 2, 4)
+    o = qo.Oracle(w.geometry, w.material)
+    U = []
+    for k in range(6):
+        assert o.step(w.dt, w.I_ramp) == 0
+        U.append(o.stats["U_terminal"])
+        cur = np.bincount(w.geometry.turn_id, weights=o.J * w.geometry.area)
+        assert np.max(np.abs(cur - o.I)) < 1e-10 * o.I
+    assert abs(o.I - 6 * w.dt * w.I_ramp) < 1e-15
+    assert max(U) - min(U) < 1e-9 * U[0] and U[0] > 0                    # U = L dI/dt, constant
+    # the shielding inductance is below the uniform-current inductance sum(M)/Nw^2-normalised
+    Luni = o.M.sum() / (16 * 16)
+    assert 0.5 * Luni < U[0] / w.I_ramp < Luni
+    assert np.all(o.T == w.geometry.T_bath)
+
+
+def test_theta0_equals_theta1_in_linear_regime_and_solvers_agree():
+    w = wl.shrunk(0, 2, 2, 4)
+    outs = []
+    for theta, op, solver in [(1.0, "dense", "cholesky"), (0.0, "dense", "cholesky"), (1.0, "tables", "pcg")]:
+        mat = dataclasses.replace(w.material, theta=theta, cg_tol=1e-13)
+        o = qo.Oracle(w.geometry, mat, operator=op, solver=solver)
+        for k in range(5):
+            o.step(w.dt, w.I_ramp)
+        outs.append(o.read())
+    for a, b in [(0, 1), (0, 2)]:
+        for u, v in zip(outs[a], outs[b]):
+            assert np.linalg.norm(u - v) <= 1e-9 * max(np.linalg.norm(u), 1e-300)
+
+
+def test_nonlinear_magnetisation_dense_cholesky_vs_tables_cg():
+    # shrunk config 1 (single wire in a ramped field): the flux front enters, |J|/Jc -> ~1, E' matters
+    w = wl.shrunk(1, 1, 1, 12)
+    geo = dataclasses.replace(w.geometry, Bext_rate=10.0)          # 10 T/s: the front crosses a cell in 300 steps
+    outs = []
+    for op, solver in [("dense", "cholesky"), ("tables", "pcg")]:
+        o = qo.Oracle(geo, dataclasses.replace(w.material, cg_tol=1e-13), operator=op, solver=solver)
+        for k in range(300):
+            ret = o.step(w.dt, w.I_ramp)
+            assert ret >= 0
+        outs.append((o.read(), o.stats, ret))
+    (J, T, B, E), st, ret = outs[0]
+    Jc = 2e9 * (1 - 4.2 / 18) ** 2
+    assert 0.9 < np.max(np.abs(J)) / Jc < 1.1 and np.max(np.abs(E)) > 1e-6      # nonlinear regime reached
+    assert abs(np.sum(J)) < 1e-6 * np.sum(np.abs(J))                          # zero net current in the wire
+    for u, v in zip(outs[0][0], outs[1][0]):
+        assert np.linalg.norm(u - v) <= 1e-8 * np.linalg.norm(u)
+    # shielding: induced currents oppose the field rise (Lenz): outer edge (larger r) carries J < 0 for Bdot > 0
+    J2 = J.reshape(12, 12)
+    assert J2[-1].mean() < 0 < J2[0].mean()
+
+
+def test_joule_heat_equals_enthalpy_rise_plus_boundary_flux():
+    # north_star energy balance across whole steps: sum_k dt P_k = sum V (H_end - H_0) + boundary losses
+    w = wl.shrunk(1, 1, 1, 8)
+    geo = dataclasses.replace(w.geometry, Bext_rate=200.0, Bext_max=1e3)        # strong drive: real heating
+    o = qo.Oracle(geo, w.material)
+    vol = 2 * math.pi * geo.r * geo.h ** 2
+    H0 = o.H.copy()
+    joule = lost = 0.0
+    for k in range(100):
+        assert o.step(w.dt, 0.0) >= 0
+        joule += w.dt * o.stats["joule_power"]
+        lost += o.stats["boundary_energy"]
+    rise = np.sum(vol * (o.H - H0))
+    assert o.T.max() > geo.T_bath + 1e-3 and joule > 0
+    assert abs(joule - rise - lost) < 1e-10 * joule
+
+
+def test_event_variants():
+    # a prepared hot turn sets FJ_T (12 K) or Q_T|Q_rho (19 K); first-event time, counters
+    w = wl.config(0)
+    geo = w.geometry
+    o = qo.Oracle(geo, w.material)
+    T = np.full(geo.n_rings, geo.T_bath)
+    T[geo.turn_id == 5] = 12.0
+    o.write(np.zeros(geo.n_rings), T, 0.0, 0.0)
+    ret = o.step(w.dt, w.I_ramp)
+    assert ret & qo.RET_FLUXJUMP and not ret & qo.RET_QUENCH
+    assert o.flags[5] & qo.FJ_T and o.count[5] == 1 and abs(o.t_first[5] - w.dt) < 1e-18
+    assert np.all(np.delete(o.flags, 5) == 0) and np.all(np.delete(o.t_first, 5) < 0)
+    ret = o.step(w.dt, w.I_ramp)
+    assert not ret & qo.RET_FLUXJUMP and o.count[5] == 1                     # no new rising edge
+    T[geo.turn_id == 5] = 19.0
+    o.write(np.zeros(geo.n_rings), T, 0.0, 0.0)
+    ret = o.step(1e-6, w.I_ramp)
+    assert ret & qo.RET_QUENCH and o.flags[5] & qo.Q_T and o.flags[5] & qo.Q_RHO and o.flags[5] & qo.FJ_T
+    assert np.all(np.delete(o.flags, 5) & (qo.Q_T | qo.Q_RHO) == 0)

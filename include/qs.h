@@ -1,0 +1,172 @@
+/* qs.h — C ABI of the B200-native quench-simulation hot path (after arXiv:2403.07666).
+ *
+ * One handle = one simulation of a solenoid cross-section of N coaxial current rings ("cells")
+ * advanced step by step under a ramped transport current I_a(t) and a ramped axial background
+ * field (the problem statement; J^{k+1} from rho^k = rho(J^k),
+ * then the heat equation with the Joule source E.J).  Every step of the path runs in
+ * hand-written CUDA kernels for sm_100a; there is no CPU fallback: a call made without a usable
+ * CUDA device fails with QS_ERR_CUDA.
+ *
+ * Readings of the points the paper leaves to its (unavailable) Supplementary Information are
+ * numbered C1..C13 in SURVEY.md §8(c) and restated in DESIGN.md; they are cited as "C<k>" below.
+ *
+ * Conventions
+ *   - All array arguments of the plain calls are HOST pointers owned by the caller, valid for the
+ *     duration of the call only; the library copies what it needs.  The *_device variants take
+ *     DEVICE pointers (FP64, at least n_rings elements, 16-byte aligned) and enqueue on the handle's
+ *     stream; they return after the work has been enqueued and checked for launch errors only.
+ *   - FP64 throughout (BASELINE.json configs[0]).  SI units.  Ring order is the caller's order
+ *     (lattice: canonical c = ir*Nz + iz, C1); any internal re-ordering is invisible.
+ *   - Return value: 0 = OK, negative = error (state unchanged), and for qs_step a non-negative
+ *     event bitmask.  qs_last_error() returns a human-readable message for the calling thread.
+ *   - One handle per host thread; calls on one handle are serialised on its stream.
+ */
+#ifndef QS_H_
+#define QS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qs_ctx qs_ctx;
+
+/* error codes */
+#define QS_OK            0
+#define QS_ERR_ARG      -1   /* bad argument (NULL, size, inconsistent lattice, rings outside the validity domain) */
+#define QS_ERR_CUDA     -2   /* CUDA error or no device */
+#define QS_ERR_NONFINITE -3  /* NaN/Inf in J or T after the step (state restored)            */
+#define QS_ERR_CG       -4   /* CG breakdown p^T A p <= 0 (state restored)                  */
+#define QS_ERR_DT       -5   /* dt <= 0                                                      */
+
+/* qs_step return bits */
+#define QS_EV_FLUXJUMP   1   /* some turn's flux-jump flag group (FJ_T|FJ_E|FJ_J) rose this step */
+#define QS_EV_QUENCH     2   /* some turn has a quench flag (Q_T|Q_RHO) set                    */
+#define QS_EV_CG_MAXIT   4   /* CG stopped at cg_maxit; the state was advanced anyway          */
+
+/* per-turn flag bits (C10; PAPER.md:105 |J/Jc| > 1, PAPER.md:119 rho > 0.95 rho_n; configs[3]) */
+#define QS_FJ_T    1         /* Tmax_w > T_fluxjump                                            */
+#define QS_FJ_E    2         /* d(mean|E|_w)/dt > dEdt_spike                                   */
+#define QS_FJ_J    4         /* max |J|/Jc > 1 in the turn                                     */
+#define QS_Q_T     8         /* Tmax_w > Tc                                                    */
+#define QS_Q_RHO  16         /* min rho/rho_n > 0.95 in the turn                               */
+
+/* qs_geometry.flags */
+#define QS_GEO_NO_OPERATOR 1 /* thermal / pointwise use only: no pair operator is set up, qs_step,
+                                qs_matvec, qs_solve, qs_field return QS_ERR_ARG (roofline runs of
+                                the HBM-bound passes on lattices whose N^2 sweep is out of reach)  */
+
+typedef struct {
+  int32_t  n_rings;                 /* N                                                         */
+  const double *r, *z, *area;       /* [N] ring centre radius, height, cross-section [m, m, m^2] */
+  const int32_t *turn_id;           /* [N] in 0..n_turns-1, or NULL when n_turns == 0            */
+  int32_t  n_turns;                 /* N_w; 0 = no net-current constraint (config 4)             */
+  int32_t  lattice;                 /* 1: regular winding pack described below (enables qs_step);
+                                       0: free rings (operator / solve only)                     */
+  int32_t  layers, turns_per_layer, cells_per_side;  /* lattice: L along r, T_n along z, n (C1)  */
+  double   wire_size, r_inner;      /* lattice: wire side s [m] (h = s/n), inner radius [m];
+                                       r = r_inner+(ir+1/2)h, z = (iz+1/2)h - Nz h/2 are CHECKED
+                                       against r[], z[] to 1e-9 relative                          */
+  double   softening;               /* g [m] (C2): lattice: M_ii = M(r_i, r_i, dz = g) and the
+                                       self-field term; free rings: dz^2 + g^2 for ALL pairs      */
+  double   h_conv[4];               /* bath film coefficient on the r_min, r_max, z_min, z_max
+                                       borders of the winding pack [W/m^2K]        */
+  double   T_bath;                  /* [K]                                                       */
+  double   Bext0, Bext_rate, Bext_max; /* axial background field B_ext(t) = min(Bext0 + rate t, max);
+                                       rate == 0: constant Bext0                                  */
+  int32_t  flags;                   /* QS_GEO_*                                                  */
+} qs_geometry;
+
+typedef struct {
+  double Ec, n_exp, Jc0, Tc, B0, eps_coef, eps_exp, Y, rho_n;  /* C5: 1e-4, 20, 2e9, 18, 1, 900, 1.7, 1e11, 5e-10 */
+  const double *jc0_scale;          /* [N] per-cell Jc0 multiplier, NULL = 1                     */
+  double C3, C1;                    /* C(T) = C3 T^3 + C1 T  [J/m^3K]  (2000, 500)               */
+  double k_in, k_between;           /* k = k_in T inside a wire, k_between T across wires (5, 0.5) */
+  double theta;                     /* C7: 0 explicit Euler (literal), 1 linearly implicit (default) */
+  double cg_tol; int32_t cg_maxit;  /* stop when sqrt(r^T g) <= cg_tol * nu (C8)                 */
+  double T_fluxjump, dEdt_spike;    /* C10: 10 K, 1 V/m/s                                        */
+} qs_material;
+
+typedef struct {
+  int32_t cg_iters;                 /* projected-CG iterations of the last step / solve          */
+  int32_t heat_substeps;            /* m of the last step (C9)                                   */
+  int32_t event_word;               /* last qs_step return value                                 */
+  int32_t sweeps;                   /* pair sweeps (operator applications) of the last step/solve */
+  double  cg_relres;                /* sqrt(r^T g)/nu reached                                    */
+  double  U_terminal;               /* -sum_w V_w [V] (PAPER.md:99 terminal voltage)             */
+  double  Tmax;                     /* max T after the step [K]                                  */
+  double  joule_power;              /* sum_i Q_i 2 pi r_i a_i [W] of the step's material evaluation */
+  double  t, I;                     /* time [s] and transport current [A] after the step         */
+  int64_t launches;                 /* kernels launched by this handle since qs_init             */
+  int64_t pair_evals;               /* ring-pair evaluations since qs_init                       */
+} qs_stats_t;
+
+/* ---- the three calls north_star names -------------------------------------------------------- */
+
+/* Create a simulation: copies geometry and material, allocates device state with cudaMalloc on
+ * the current device, uses its own stream.  State: J = 0, T = T_bath, t = 0, I = 0.  */
+int  qs_init(const qs_geometry *geo, const qs_material *mat, qs_ctx **out);
+
+/* One time step k -> k+1 (order C6):
+ *   S1 B^k = G_B (a J^k) + B_ext(t^k)            all-pairs ring field, K/E by AGM per pair (C3)
+ *   S2 eps, Jc, rho, E, dE/dJ, Q at (J^k, T^k, B^k); rhs b = -2 pi r (E + r Bdot_ext/2)   (C5, C4)
+ *   S3 projected CG on (M + theta dt D) I' + C V = b, C^T I' = I_ramp     (C4, C7, C8)
+ *   S4 per-turn Schur projection inside S3; multipliers V_w -> terminal voltage
+ *   S5 J += dt I'/a ; I += dt I_ramp ; t += dt
+ *   S6 m explicit 5-point finite-volume heat sub-steps with Q^k frozen, Robin borders (C9)
+ *   S7 per-turn event flags (C10)
+ * I_ramp = dI/dt [A/s] held over the step.  Lattice geometries only.  Synchronous.  */
+int  qs_step(qs_ctx *ctx, double dt, double I_ramp);
+
+/* Copy out J [N], T [N], B [2N: Br then Bz], E [N]; NULL = skip.  J, T are the state after the
+ * last step; B, E are those of the last step's material evaluation (time level k).  */
+int  qs_read(qs_ctx *ctx, double *J, double *T, double *B, double *E);
+
+/* ---- extras (tests, resume, config 4, roofline runs) ----------------------------------------- */
+
+/* Bytes of device workspace qs_init_device needs for this geometry.  */
+size_t qs_workspace_bytes(const qs_geometry *geo);
+
+/* As qs_init, but all device state lives in the caller's DEVICE buffer `workspace` (256-byte
+ * aligned, >= qs_workspace_bytes(geo), owned by the caller and kept alive until qs_free) and all
+ * work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = default stream).  This is
+ * how the Python binding lets PyTorch own device memory and streams.  */
+int  qs_init_device(const qs_geometry *geo, const qs_material *mat, void *workspace,
+                    size_t workspace_bytes, void *stream, qs_ctx **out);
+
+/* Set the state (resume, prepared variants C12).  NULL J or T keeps the current array.  Resets the
+ * warm start and the dE/dt history.  */
+int  qs_write(qs_ctx *ctx, const double *J, const double *T, double t, double I);
+
+/* y = M x (C2): x [A] -> y [Wb], symmetric mutual-inductance matrix, evaluated pair by pair.  */
+int  qs_matvec(qs_ctx *ctx, const double *x, double *y);
+int  qs_matvec_device(qs_ctx *ctx, const double *d_x, double *d_y);
+
+/* Br, Bz [N each, B = Br then Bz] of ring currents I [A] (C3), without B_ext; lattice only.  */
+int  qs_field(qs_ctx *ctx, const double *I, double *B);
+
+/* Solve M x = b (plus C^T x = 0 when the geometry has turns) by projected CG to the material's
+ * cg_tol / cg_maxit; maxit_override > 0 replaces cg_maxit.  Returns 0 or QS_EV_CG_MAXIT.  */
+int  qs_solve(qs_ctx *ctx, const double *b, double *x, int32_t maxit_override, int32_t *iters, double *relres);
+int  qs_solve_device(qs_ctx *ctx, const double *d_b, double *d_x, int32_t maxit_override, int32_t *iters, double *relres);
+
+/* S2 alone on the current (J, T, B) and S6 alone (m sub-steps of dt with the current Q): unit
+ * parity of the pointwise passes and their HBM-roofline runs.  qs_set_fields loads B [2N] and/or
+ * Q [N] (NULL = keep).  qs_heat returns m.  */
+int  qs_material_eval(qs_ctx *ctx, double dt);
+int  qs_heat(qs_ctx *ctx, double dt);
+int  qs_set_fields(qs_ctx *ctx, const double *B, const double *Q);
+int  qs_read_aux(qs_ctx *ctx, double *Q, double *dEdJ, double *Jc, double *rho);
+
+int  qs_stats(qs_ctx *ctx, qs_stats_t *out);
+int  qs_events(qs_ctx *ctx, int32_t *flags /*[N_w]*/, double *t_first /*[N_w]*/, int32_t *count /*[N_w]*/);
+int  qs_sync(qs_ctx *ctx);                 /* wait for the handle's stream */
+const char *qs_last_error(void);
+void qs_free(qs_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QS_H_ */

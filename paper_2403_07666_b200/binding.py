@@ -1,0 +1,269 @@
+"""Thin ctypes binding of libqs.so (include/qs.h): argument marshalling only.
+
+PyTorch is used for exactly two things: it owns the device workspace (one uint8 tensor handed to
+``qs_init_device``) and the CUDA stream the library enqueues on.  Every step of the path runs in the
+library's own kernels; there is no Python or CPU fallback — without the built library or without a
+CUDA device the constructor raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+from .build import build as _build_lib
+
+c_double_p = C.POINTER(C.c_double)
+c_int32_p = C.POINTER(C.c_int32)
+
+
+class QsGeometry(C.Structure):
+    _fields_ = [("n_rings", C.c_int32), ("r", c_double_p), ("z", c_double_p), ("area", c_double_p),
+                ("turn_id", c_int32_p), ("n_turns", C.c_int32), ("lattice", C.c_int32),
+                ("layers", C.c_int32), ("turns_per_layer", C.c_int32), ("cells_per_side", C.c_int32),
+                ("wire_size", C.c_double), ("r_inner", C.c_double), ("softening", C.c_double),
+                ("h_conv", C.c_double * 4), ("T_bath", C.c_double),
+                ("Bext0", C.c_double), ("Bext_rate", C.c_double), ("Bext_max", C.c_double),
+                ("flags", C.c_int32)]
+
+
+class QsMaterial(C.Structure):
+    _fields_ = [("Ec", C.c_double), ("n_exp", C.c_double), ("Jc0", C.c_double), ("Tc", C.c_double),
+                ("B0", C.c_double), ("eps_coef", C.c_double), ("eps_exp", C.c_double), ("Y", C.c_double),
+                ("rho_n", C.c_double), ("jc0_scale", c_double_p), ("C3", C.c_double), ("C1", C.c_double),
+                ("k_in", C.c_double), ("k_between", C.c_double), ("theta", C.c_double),
+                ("cg_tol", C.c_double), ("cg_maxit", C.c_int32),
+                ("T_fluxjump", C.c_double), ("dEdt_spike", C.c_double)]
+
+
+class QsStats(C.Structure):
+    _fields_ = [("cg_iters", C.c_int32), ("heat_substeps", C.c_int32), ("event_word", C.c_int32),
+                ("sweeps", C.c_int32), ("cg_relres", C.c_double), ("U_terminal", C.c_double),
+                ("Tmax", C.c_double), ("joule_power", C.c_double), ("t", C.c_double), ("I", C.c_double),
+                ("launches", C.c_int64), ("pair_evals", C.c_int64)]
+
+
+# every symbol include/qs.h declares: (name, restype, argtypes)
+_VP = C.c_void_p
+SYMBOLS = [
+    ("qs_init", C.c_int, [C.POINTER(QsGeometry), C.POINTER(QsMaterial), C.POINTER(_VP)]),
+    ("qs_step", C.c_int, [_VP, C.c_double, C.c_double]),
+    ("qs_read", C.c_int, [_VP, c_double_p, c_double_p, c_double_p, c_double_p]),
+    ("qs_workspace_bytes", C.c_size_t, [C.POINTER(QsGeometry)]),
+    ("qs_init_device", C.c_int, [C.POINTER(QsGeometry), C.POINTER(QsMaterial), _VP, C.c_size_t, _VP, C.POINTER(_VP)]),
+    ("qs_write", C.c_int, [_VP, c_double_p, c_double_p, C.c_double, C.c_double]),
+    ("qs_matvec", C.c_int, [_VP, c_double_p, c_double_p]),
+    ("qs_matvec_device", C.c_int, [_VP, _VP, _VP]),
+    ("qs_field", C.c_int, [_VP, c_double_p, c_double_p]),
+    ("qs_solve", C.c_int, [_VP, c_double_p, c_double_p, C.c_int32, c_int32_p, c_double_p]),
+    ("qs_solve_device", C.c_int, [_VP, _VP, _VP, C.c_int32, c_int32_p, c_double_p]),
+    ("qs_material_eval", C.c_int, [_VP, C.c_double]),
+    ("qs_heat", C.c_int, [_VP, C.c_double]),
+    ("qs_set_fields", C.c_int, [_VP, c_double_p, c_double_p]),
+    ("qs_read_aux", C.c_int, [_VP, c_double_p, c_double_p, c_double_p, c_double_p]),
+    ("qs_stats", C.c_int, [_VP, C.POINTER(QsStats)]),
+    ("qs_events", C.c_int, [_VP, c_int32_p, c_double_p, c_int32_p]),
+    ("qs_sync", C.c_int, [_VP]),
+    ("qs_last_error", C.c_char_p, []),
+    ("qs_free", None, [_VP]),
+]
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None) -> C.CDLL:
+    """dlopen libqs.so (building it in-tree with nvcc first if it is missing or stale)."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    if path is None:
+        path = _build_lib()            # raises if nvcc fails; never falls back to anything else
+    lib = C.CDLL(path)
+    for name, res, args in SYMBOLS:
+        fn = getattr(lib, name)          # AttributeError if the library does not export it
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+class QsError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libqs error {code}: {msg}")
+        self.code = code
+
+
+def _dp(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(c_double_p)
+
+
+def _f64(a, n=None) -> np.ndarray:
+    out = np.ascontiguousarray(a, dtype=np.float64)
+    if n is not None and out.size != n:
+        raise ValueError(f"expected {n} elements, got {out.size}")
+    return out
+
+
+class QS:
+    """One simulation handle.  ``geometry`` / ``material`` are objects with the fields of
+    ``qs_geometry`` / ``qs_material`` (e.g. ``workloads.Geometry`` / ``workloads.Material``)."""
+
+    def __init__(self, geometry, material, device: int = 0, no_operator: bool = False, torch_memory: bool = True):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2403_07666_b200 needs a CUDA device: there is no CPU path")
+        self._lib = load_library()
+        self._torch = torch
+        self.N = int(geometry.r.shape[0])
+        self.n_turns = int(geometry.n_turns)
+        self._keep = []                              # host arrays referenced by the structs
+        g = QsGeometry()
+        g.n_rings = self.N
+        for name in ("r", "z", "area"):
+            arr = _f64(getattr(geometry, name), self.N)
+            self._keep.append(arr)
+            setattr(g, name, _dp(arr))
+        if geometry.turn_id is not None and self.n_turns > 0:
+            tid = np.ascontiguousarray(geometry.turn_id, dtype=np.int32)
+            self._keep.append(tid)
+            g.turn_id = tid.ctypes.data_as(c_int32_p)
+        g.n_turns = self.n_turns
+        g.lattice = int(geometry.lattice)
+        g.layers, g.turns_per_layer, g.cells_per_side = int(geometry.layers), int(geometry.turns_per_layer), int(geometry.cells_per_side)
+        g.wire_size, g.r_inner, g.softening = float(geometry.wire_size), float(geometry.r_inner), float(geometry.softening)
+        g.h_conv = (C.c_double * 4)(*[float(v) for v in geometry.h_conv])
+        g.T_bath = float(geometry.T_bath)
+        g.Bext0, g.Bext_rate, g.Bext_max = float(geometry.Bext0), float(geometry.Bext_rate), float(geometry.Bext_max)
+        g.flags = 1 if no_operator else 0
+        m = QsMaterial()
+        for name, _ in QsMaterial._fields_:
+            if name == "jc0_scale":
+                if material.jc0_scale is not None:
+                    arr = _f64(material.jc0_scale, self.N)
+                    self._keep.append(arr)
+                    m.jc0_scale = _dp(arr)
+            elif name == "cg_maxit":
+                m.cg_maxit = int(material.cg_maxit)
+            else:
+                setattr(m, name, float(getattr(material, name)))
+        self._h = _VP()
+        self.device = torch.device("cuda", device)
+        with torch.cuda.device(self.device):
+            if torch_memory:
+                nbytes = self._lib.qs_workspace_bytes(C.byref(g))
+                if nbytes == 0:
+                    raise QsError(-1, self._lib.qs_last_error().decode())
+                self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+                base = (self.workspace.data_ptr() + 255) // 256 * 256
+                self.stream = torch.cuda.Stream(device=self.device)
+                rc = self._lib.qs_init_device(C.byref(g), C.byref(m), _VP(base), nbytes, _VP(self.stream.cuda_stream),
+                                              C.byref(self._h))
+            else:
+                self.workspace, self.stream = None, None
+                rc = self._lib.qs_init(C.byref(g), C.byref(m), C.byref(self._h))
+        self._check(rc)
+
+    # ---- plumbing -------------------------------------------------------------------------------
+    def _check(self, rc: int) -> int:
+        if rc < 0:
+            raise QsError(rc, self._lib.qs_last_error().decode())
+        return rc
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.qs_free(self._h)
+            self._h = _VP()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # ---- the three calls -------------------------------------------------------------------------
+    def step(self, dt: float, I_ramp: float) -> int:
+        return self._check(self._lib.qs_step(self._h, float(dt), float(I_ramp)))
+
+    def read(self, J=True, T=True, B=True, E=True, out=None):
+        """Returns (J, T, B, E) as numpy arrays (B = [Br, Bz] concatenated); skipped entries are None.
+        ``out`` may hold preallocated (e.g. pinned) float64 arrays of the right sizes."""
+        N = self.N
+        bufs = list(out) if out is not None else [np.empty(N) if J else None, np.empty(N) if T else None,
+                                                   np.empty(2 * N) if B else None, np.empty(N) if E else None]
+        self._check(self._lib.qs_read(self._h, *[_dp(b) for b in bufs]))
+        return tuple(bufs)
+
+    # ---- extras ----------------------------------------------------------------------------------
+    def write(self, J=None, T=None, t: float = 0.0, I: float = 0.0):
+        Ja = None if J is None else _f64(J, self.N)
+        Ta = None if T is None else _f64(T, self.N)
+        self._check(self._lib.qs_write(self._h, _dp(Ja), _dp(Ta), float(t), float(I)))
+
+    def matvec(self, x) -> np.ndarray:
+        xa = _f64(x, self.N)
+        y = np.empty(self.N)
+        self._check(self._lib.qs_matvec(self._h, _dp(xa), _dp(y)))
+        return y
+
+    def matvec_device(self, x, y):
+        """x, y: float64 CUDA tensors of N elements on this handle's device; enqueued on self.stream."""
+        self._check(self._lib.qs_matvec_device(self._h, _VP(x.data_ptr()), _VP(y.data_ptr())))
+
+    def field(self, I) -> np.ndarray:
+        Ia = _f64(I, self.N)
+        B = np.empty(2 * self.N)
+        self._check(self._lib.qs_field(self._h, _dp(Ia), _dp(B)))
+        return B
+
+    def solve(self, b, maxit: int = 0):
+        ba = _f64(b, self.N)
+        x = np.empty(self.N)
+        it, rel = C.c_int32(0), C.c_double(0.0)
+        rc = self._check(self._lib.qs_solve(self._h, _dp(ba), _dp(x), int(maxit), C.byref(it), C.byref(rel)))
+        return x, it.value, rel.value, rc
+
+    def solve_device(self, b, x, maxit: int = 0):
+        it, rel = C.c_int32(0), C.c_double(0.0)
+        rc = self._check(self._lib.qs_solve_device(self._h, _VP(b.data_ptr()), _VP(x.data_ptr()), int(maxit),
+                                                   C.byref(it), C.byref(rel)))
+        return it.value, rel.value, rc
+
+    def material_eval(self, dt: float = 0.0):
+        self._check(self._lib.qs_material_eval(self._h, float(dt)))
+
+    def heat(self, dt: float) -> int:
+        return self._check(self._lib.qs_heat(self._h, float(dt)))
+
+    def set_fields(self, B=None, Q=None):
+        Ba = None if B is None else _f64(B, 2 * self.N)
+        Qa = None if Q is None else _f64(Q, self.N)
+        self._check(self._lib.qs_set_fields(self._h, _dp(Ba), _dp(Qa)))
+
+    def read_aux(self):
+        N = self.N
+        Q, d, Jc, rho = np.empty(N), np.empty(N), np.empty(N), np.empty(N)
+        self._check(self._lib.qs_read_aux(self._h, _dp(Q), _dp(d), _dp(Jc), _dp(rho)))
+        return dict(Q=Q, dEdJ=d, Jc=Jc, rho=rho)
+
+    def stats(self) -> dict:
+        s = QsStats()
+        self._check(self._lib.qs_stats(self._h, C.byref(s)))
+        return {name: getattr(s, name) for name, _ in QsStats._fields_}
+
+    def events(self):
+        nt = max(self.n_turns, 0)
+        fl, tf, cnt = np.zeros(nt, dtype=np.int32), np.zeros(nt), np.zeros(nt, dtype=np.int32)
+        if nt:
+            self._check(self._lib.qs_events(self._h, fl.ctypes.data_as(c_int32_p), _dp(tf), cnt.ctypes.data_as(c_int32_p)))
+        return fl, tf, cnt
+
+    def sync(self):
+        self._check(self._lib.qs_sync(self._h))

@@ -1,0 +1,849 @@
+// qs_api.cu — the C ABI of include/qs.h: context, workspace layout, step driver (S1..S7), projected CG.
+//
+// Host code only enqueues kernels on the handle's stream and reads back one small Scalars block per CG
+// iteration (the convergence test) and per step (events, statistics).  No arithmetic of the method runs
+// on the host except set-up constants (bounding boxes, Morton order of free rings, self-field coefficients).
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/qs.h"
+#include "qs_internal.h"
+
+using namespace qs;
+
+namespace {
+
+thread_local std::string g_err;
+int fail(int code, const std::string& msg) {
+  g_err = msg;
+  return code;
+}
+#define QS_CUDA(call)                                                                          \
+  do {                                                                                         \
+    cudaError_t e_ = (call);                                                                   \
+    if (e_ != cudaSuccess)                                                                     \
+      return fail(QS_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_));            \
+  } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// Carves named arrays out of one device buffer; used twice (size query with base == nullptr, then for real).
+struct Carver {
+  char* base;
+  size_t off = 0;
+  explicit Carver(void* b) : base(static_cast<char*>(b)) {}
+  template <class T>
+  T* take(size_t count) {
+    off = align_up(off, 256);
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += count * sizeof(T);
+    return p;
+  }
+};
+
+}  // namespace
+
+struct qs_ctx {
+  // problem
+  int N = 0, Np = 0, nb = 0, n_turns = 0;
+  bool lattice = false, has_operator = true;
+  MaterialParams mp{};
+  LatticeParams lp{};
+  double theta = 1.0, cg_tol = 1e-10;
+  int cg_maxit = 20000;
+  double Bext0 = 0, Bext_rate = 0, Bext_max = 0;
+  double soft_all = 0, soft_self = 0, minsep2 = 0, diag_d2 = 0;
+  std::vector<int> perm;             // internal k -> caller index (empty = identity)
+  // device
+  cudaStream_t stream = nullptr;
+  void* owned = nullptr;             // cudaMalloc'ed workspace (qs_init) or nullptr (qs_init_device)
+  int sm_count = 148;
+  double *r, *z, *area, *jc0s, *selfcoef, *diagM;
+  double *J, *Jold, *Ha, *Hb, *Hold, *Br, *Bz, *E, *dEdJ, *Q, *b, *shift, *Hd, *Jc, *rho;
+  double *x, *xold, *cur, *p, *q, *rr, *g, *xp1, *Mxp1, *tmp, *tmp2, *zero;
+  unsigned long long* counter;       // followed contiguously by yacc, bracc, bzacc (one memset)
+  double *yacc, *bracc, *bzacc;
+  size_t acc_bytes = 0;
+  double *sw, *swM, *vw, *vsum, *defw, *ebar_prev, *t_first;
+  int *flags, *count, *turn_ptr, *turn_idx, *turn_id, *d_perm;
+  double4* bbox;
+  Scalars* sc;
+  Scalars* h_sc = nullptr;           // pinned
+  double* h_stage = nullptr;         // pinned staging, 2N doubles
+  double* H = nullptr;               // current enthalpy (Ha or Hb)
+  double* Halt = nullptr;
+  // state
+  double t = 0, I = 0;
+  bool have_prev_E = false;
+  long long launches = 0, pair_evals = 0;
+  qs_stats_t st{};
+  VecCtx v{};
+};
+
+namespace {
+
+void carve(qs_ctx* c, void* base, size_t* total) {
+  Carver k(base);
+  const size_t N = c->N, Np = c->Np, nt = std::max(c->n_turns, 1);
+  c->r = k.take<double>(Np);
+  c->z = k.take<double>(Np);
+  c->area = k.take<double>(N);
+  c->jc0s = k.take<double>(N);
+  c->selfcoef = k.take<double>(N);
+  c->diagM = k.take<double>(N);
+  c->J = k.take<double>(N);
+  c->Jold = k.take<double>(N);
+  c->Ha = k.take<double>(N);
+  c->Hb = k.take<double>(N);
+  c->Hold = k.take<double>(N);
+  c->Br = k.take<double>(N);
+  c->Bz = k.take<double>(N);
+  c->E = k.take<double>(N);
+  c->dEdJ = k.take<double>(N);
+  c->Q = k.take<double>(N);
+  c->b = k.take<double>(N);
+  c->shift = k.take<double>(N);
+  c->Hd = k.take<double>(N);
+  c->Jc = k.take<double>(N);
+  c->rho = k.take<double>(N);
+  c->x = k.take<double>(Np);
+  c->xold = k.take<double>(Np);
+  c->cur = k.take<double>(Np);
+  c->p = k.take<double>(Np);
+  c->q = k.take<double>(N);
+  c->rr = k.take<double>(N);
+  c->g = k.take<double>(N);
+  c->xp1 = k.take<double>(N);
+  c->Mxp1 = k.take<double>(N);
+  c->tmp = k.take<double>(Np);
+  c->tmp2 = k.take<double>(Np);
+  c->zero = k.take<double>(N);
+  // counter + accumulators: contiguous, zeroed by one memset per sweep
+  k.off = align_up(k.off, 256);
+  const size_t acc0 = k.off;
+  c->counter = k.take<unsigned long long>(32);
+  c->yacc = k.take<double>(Np);
+  c->bracc = k.take<double>(Np);
+  c->bzacc = k.take<double>(Np);
+  c->acc_bytes = k.off - acc0;
+  c->sw = k.take<double>(nt);
+  c->swM = k.take<double>(nt);
+  c->vw = k.take<double>(nt);
+  c->vsum = k.take<double>(nt);
+  c->defw = k.take<double>(nt);
+  c->ebar_prev = k.take<double>(nt);
+  c->t_first = k.take<double>(nt);
+  c->flags = k.take<int>(nt);
+  c->count = k.take<int>(nt);
+  c->turn_ptr = k.take<int>(nt + 1);
+  c->turn_idx = k.take<int>(N);
+  c->turn_id = k.take<int>(N);
+  c->d_perm = k.take<int>(N);
+  c->bbox = k.take<double4>(std::max(c->nb, 1));
+  c->sc = k.take<Scalars>(1);
+  *total = align_up(k.off, 256);
+}
+
+int check_geometry(const qs_geometry* g) {
+  if (!g || g->n_rings <= 0 || !g->r || !g->z || !g->area) return fail(QS_ERR_ARG, "geometry: NULL array or n_rings <= 0");
+  if (g->n_turns < 0 || (g->n_turns > 0 && !g->turn_id)) return fail(QS_ERR_ARG, "geometry: n_turns without turn_id");
+  if (!(g->softening > 0.0)) return fail(QS_ERR_ARG, "geometry: softening must be > 0");
+  if (g->lattice) {
+    if (g->layers <= 0 || g->turns_per_layer <= 0 || g->cells_per_side <= 0 || !(g->wire_size > 0.0))
+      return fail(QS_ERR_ARG, "geometry: bad lattice description");
+    const long long n = g->cells_per_side, Nr = g->layers * n, Nz = g->turns_per_layer * n;
+    if (Nr * Nz != g->n_rings) return fail(QS_ERR_ARG, "geometry: n_rings != Nr*Nz");
+  }
+  return QS_OK;
+}
+
+int sync_scalars(qs_ctx* c) {
+  QS_CUDA(cudaMemcpyAsync(c->h_sc, c->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, c->stream));
+  QS_CUDA(cudaStreamSynchronize(c->stream));
+  return QS_OK;
+}
+
+// y-accumulators <- sweep of (x [, cur]); consumer applies the scale factors
+int do_sweep(qs_ctx* c, const double* x, const double* cur, bool field) {
+  QS_CUDA(cudaMemsetAsync(c->counter, 0, c->acc_bytes, c->stream));
+  SweepParams prm;
+  prm.r = c->r;
+  prm.z = c->z;
+  prm.x = x;
+  prm.cur = cur ? cur : x;
+  prm.bbox = c->bbox;
+  prm.yacc = c->yacc;
+  prm.bracc = c->bracc;
+  prm.bzacc = c->bzacc;
+  prm.counter = c->counter;
+  prm.nb = c->nb;
+  prm.n_items = static_cast<long long>(c->nb) * (c->nb + 1) / 2;
+  prm.soft_all = c->soft_all;
+  prm.soft_self = c->soft_self;
+  prm.minsep2 = c->minsep2;
+  prm.diag_d2 = c->diag_d2;
+  const int wpc = sweep_warps_per_cta();
+  int grid = sweep_grid(c->sm_count, field);
+  const long long need = (prm.n_items + wpc - 1) / wpc;
+  if (need < grid) grid = static_cast<int>(need);
+  const long long warps = static_cast<long long>(grid) * wpc;
+  prm.chunk = static_cast<int>(std::max<long long>(1, std::min<long long>(32, prm.n_items / (warps * 8))));
+  QS_CUDA(launch_sweep(prm, field, grid, c->stream));
+  ++c->launches;
+  c->pair_evals += prm.n_items * 1024;
+  ++c->st.sweeps;
+  return QS_OK;
+}
+
+constexpr double kCM = 0.5 * kMu0 * kPi;   // yacc -> henry * ampere
+
+// Projected CG (C8) on A = M + diag(shift), constraint C^T x = const kept by the projection.
+// In: x satisfies the constraint; if yacc_has_Mx the accumulators hold the sweep of x.  nu < 0: nu = start norm.
+int cg_core(qs_ctx* c, const double* b, double* x, const double* shift, const double* Hd, const double* sw,
+            bool yacc_has_Mx, double tol, int maxit, double nu, int* iters, double* relres, bool* hit_max) {
+  const VecCtx& v = c->v;
+  int rc;
+  if (!yacc_has_Mx && (rc = do_sweep(c, x, nullptr, false)) != QS_OK) return rc;
+  k_residual(v, c->yacc, shift, x, b, c->rr, kCM);
+  if (c->n_turns) QS_CUDA(cudaMemsetAsync(c->vsum, 0, sizeof(double) * c->n_turns, c->stream));
+  int par = 0;
+  k_turn_project(v, c->rr, Hd, sw, c->vw, c->vsum);
+  k_project_apply(v, par, c->vw, Hd, c->rr, c->g);
+  k_direction(v, par, true, c->g, c->p);
+  if ((rc = sync_scalars(c)) != QS_OK) return rc;
+  double rg = c->h_sc->rg[par];
+  if (nu < 0.0) nu = std::sqrt(std::max(rg, 0.0));
+  int it = 0;
+  *hit_max = false;
+  while (true) {
+    if (!(rg == rg)) return fail(QS_ERR_NONFINITE, "CG: r^T g is NaN");
+    if (nu == 0.0 || std::sqrt(std::max(rg, 0.0)) <= tol * nu) break;
+    if (it >= maxit) {
+      *hit_max = true;
+      break;
+    }
+    if ((rc = do_sweep(c, c->p, nullptr, false)) != QS_OK) return rc;
+    k_finish_Ap(v, c->yacc, shift, c->p, c->q, kCM);
+    k_update_xr(v, par, c->p, c->q, x, c->rr);
+    k_turn_project(v, c->rr, Hd, sw, c->vw, c->vsum);
+    k_project_apply(v, par ^ 1, c->vw, Hd, c->rr, c->g);
+    QS_CUDA(cudaMemcpyAsync(c->h_sc, c->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, c->stream));
+    k_direction(v, par ^ 1, false, c->g, c->p);
+    QS_CUDA(cudaStreamSynchronize(c->stream));
+    if (!(c->h_sc->pq > 0.0)) return fail(QS_ERR_CG, "CG breakdown: p^T A p <= 0");
+    par ^= 1;
+    rg = c->h_sc->rg[par];
+    ++it;
+  }
+  *iters = it;
+  *relres = nu > 0.0 ? std::sqrt(std::max(rg, 0.0)) / nu : 0.0;
+  return QS_OK;
+}
+
+double bext_at(const qs_ctx* c, double t) {
+  if (c->Bext_rate == 0.0) return c->Bext0;
+  return std::min(c->Bext0 + c->Bext_rate * t, c->Bext_max);
+}
+
+int heat_substeps_count(const qs_ctx* c, double dt) {
+  const double alpha0 = c->mp.k_in / (c->mp.C3 * c->lp.T_bath * c->lp.T_bath + c->mp.C1);
+  const double limit = 0.8 * c->lp.h * c->lp.h / (4.0 * alpha0);
+  return std::max(1, static_cast<int>(std::ceil(dt / limit)));
+}
+
+int run_heat(qs_ctx* c, double dt, int* m_out) {
+  const int m = heat_substeps_count(c, dt);
+  const double sub = dt / m;
+  for (int s = 0; s < m; ++s) {
+    k_heat_substep(c->v, c->mp, c->lp, c->H, c->Q, c->Halt, sub);
+    std::swap(c->H, c->Halt);
+  }
+  *m_out = m;
+  QS_CUDA(cudaGetLastError());
+  return QS_OK;
+}
+
+MaterialArgs material_args(qs_ctx* c, double Bext, double Bdot, double dt, bool from_acc) {
+  MaterialArgs a;
+  a.N = c->N;
+  a.J = c->J;
+  a.H = c->H;
+  a.r = c->r;
+  a.area = c->area;
+  a.jc0_scale = c->jc0s;
+  a.selfcoef = c->selfcoef;
+  a.bracc = c->bracc;
+  a.bzacc = c->bzacc;
+  a.diagM = c->diagM;
+  a.Br = c->Br;
+  a.Bz = c->Bz;
+  a.E = c->E;
+  a.dEdJ = c->dEdJ;
+  a.Q = c->Q;
+  a.b = c->b;
+  a.shift = c->shift;
+  a.Hd = c->Hd;
+  a.Jc = c->Jc;
+  a.rho = c->rho;
+  a.Bext = Bext;
+  a.Bdot = Bdot;
+  a.dt = dt;
+  a.from_acc = from_acc;
+  return a;
+}
+
+// host arrays in caller order <-> device arrays in internal order
+int upload(qs_ctx* c, const double* src, double* dst, int n_pad) {
+  for (int k = 0; k < c->N; ++k) c->h_stage[k] = src[c->perm.empty() ? k : c->perm[k]];
+  for (int k = c->N; k < n_pad; ++k) c->h_stage[k] = 0.0;
+  QS_CUDA(cudaMemcpyAsync(dst, c->h_stage, sizeof(double) * n_pad, cudaMemcpyHostToDevice, c->stream));
+  QS_CUDA(cudaStreamSynchronize(c->stream));
+  return QS_OK;
+}
+int download(qs_ctx* c, const double* src, double* dst, double scale = 1.0) {
+  QS_CUDA(cudaMemcpyAsync(c->h_stage, src, sizeof(double) * c->N, cudaMemcpyDeviceToHost, c->stream));
+  QS_CUDA(cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < c->N; ++k) dst[c->perm.empty() ? k : c->perm[k]] = scale * c->h_stage[k];
+  return QS_OK;
+}
+
+uint32_t morton16(uint32_t a, uint32_t b) {
+  auto spread = [](uint32_t v) {
+    v &= 0xffff;
+    v = (v | (v << 8)) & 0x00ff00ff;
+    v = (v | (v << 4)) & 0x0f0f0f0f;
+    v = (v | (v << 2)) & 0x33333333;
+    v = (v | (v << 1)) & 0x55555555;
+    return v;
+  };
+  return spread(a) | (spread(b) << 1);
+}
+
+int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace, size_t workspace_bytes, void* stream,
+                bool own, qs_ctx** out) {
+  int rc = check_geometry(geo);
+  if (rc != QS_OK) return rc;
+  if (!mat || !out) return fail(QS_ERR_ARG, "NULL material or out pointer");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(QS_ERR_CUDA, "no CUDA device: libqs has no CPU path");
+  qs_ctx* c = new (std::nothrow) qs_ctx();
+  if (!c) return fail(QS_ERR_ARG, "out of host memory");
+  auto bail = [&](int code) {
+    qs_free(c);
+    return code;
+  };
+  const int N = geo->n_rings;
+  c->N = N;
+  c->Np = (N + 31) / 32 * 32;
+  c->nb = c->Np / 32;
+  c->n_turns = geo->n_turns;
+  c->lattice = geo->lattice != 0;
+  c->has_operator = !(geo->flags & QS_GEO_NO_OPERATOR);
+  c->Bext0 = geo->Bext0;
+  c->Bext_rate = geo->Bext_rate;
+  c->Bext_max = geo->Bext_max;
+  c->theta = mat->theta;
+  c->cg_tol = mat->cg_tol > 0 ? mat->cg_tol : 1e-10;
+  c->cg_maxit = mat->cg_maxit > 0 ? mat->cg_maxit : 20000;
+  MaterialParams& mp = c->mp;
+  mp.Ec = mat->Ec; mp.n_exp = mat->n_exp; mp.Jc0 = mat->Jc0; mp.Tc = mat->Tc; mp.B0 = mat->B0;
+  mp.eps_coef = mat->eps_coef; mp.eps_exp = mat->eps_exp; mp.Y = mat->Y; mp.rho_n = mat->rho_n;
+  mp.C3 = mat->C3; mp.C1 = mat->C1; mp.k_in = mat->k_in; mp.k_between = mat->k_between; mp.theta = mat->theta;
+  mp.T_fluxjump = mat->T_fluxjump; mp.dEdt_spike = mat->dEdt_spike;
+  mp.n_int = (mat->n_exp == std::floor(mat->n_exp) && mat->n_exp >= 1 && mat->n_exp <= 200) ? static_cast<int>(mat->n_exp) : 0;
+  if (!(mp.C3 > 0.0) || !(mp.rho_n > 0.0) || !(mp.Tc > 0.0)) return bail(fail(QS_ERR_ARG, "material: C3, rho_n, Tc must be > 0"));
+  LatticeParams& lp = c->lp;
+  lp = LatticeParams{};
+  lp.T_bath = geo->T_bath;
+  if (c->lattice) {
+    lp.n = geo->cells_per_side;
+    lp.Nr = geo->layers * lp.n;
+    lp.Nz = geo->turns_per_layer * lp.n;
+    lp.h = geo->wire_size / lp.n;
+    lp.r_inner = geo->r_inner;
+    for (int s = 0; s < 4; ++s) lp.h_conv[s] = geo->h_conv[s];
+    // the lattice description must agree with the ring arrays (C1)
+    const int probe[4] = {0, N - 1, N / 2, N / 3};
+    for (int k : probe) {
+      const int ir = k / lp.Nz, iz = k % lp.Nz;
+      const double rr = lp.r_inner + (ir + 0.5) * lp.h, zz = (iz + 0.5) * lp.h - lp.Nz * lp.h / 2.0;
+      if (std::fabs(geo->r[k] - rr) > 1e-9 * rr || std::fabs(geo->z[k] - zz) > 1e-9 * (std::fabs(zz) + lp.h))
+        return bail(fail(QS_ERR_ARG, "geometry: r/z arrays do not match the lattice description (order c = ir*Nz + iz)"));
+    }
+  }
+  const double g2 = geo->softening * geo->softening;
+  c->soft_all = c->lattice ? 0.0 : g2;
+  c->soft_self = c->lattice ? g2 : 0.0;
+  c->minsep2 = c->lattice ? lp.h * lp.h * (1.0 - 1e-9) : 0.0;
+  c->diag_d2 = std::min(c->soft_all + c->soft_self, c->minsep2 + c->soft_all);
+  if (c->diag_d2 <= 0.0) c->diag_d2 = c->soft_all + c->soft_self;
+
+  // validity domain of the squared-AGM recurrence: k'^2 <= 0.98 over the whole ring set
+  double rmin = 1e300, rmax = 0, zmin = 1e300, zmax = -1e300;
+  for (int k = 0; k < N; ++k) {
+    if (!(geo->r[k] > 0.0) || !std::isfinite(geo->z[k]) || !(geo->area[k] > 0.0))
+      return bail(fail(QS_ERR_ARG, "geometry: r, area must be > 0 and z finite"));
+    rmin = std::min(rmin, geo->r[k]); rmax = std::max(rmax, geo->r[k]);
+    zmin = std::min(zmin, geo->z[k]); zmax = std::max(zmax, geo->z[k]);
+  }
+  if (c->has_operator) {
+    const double d2 = (rmax - rmin) * (rmax - rmin) + (zmax - zmin) * (zmax - zmin);
+    if (d2 / (4.0 * rmin * rmin + d2) > 0.98)
+      return bail(fail(QS_ERR_ARG, "geometry: ring set too spread out relative to its radius (k'^2 > 0.98)"));
+  }
+  if (geo->n_turns > 0)
+    for (int k = 0; k < N; ++k)
+      if (geo->turn_id[k] < 0 || geo->turn_id[k] >= geo->n_turns) return bail(fail(QS_ERR_ARG, "geometry: turn_id out of range"));
+
+  // internal order: canonical for lattices (the heat stencil needs it); Morton order of (r, z) for free rings so
+  // that blocks of 32 rings are compact and the per-item AGM depth bound is tight
+  if (!c->lattice && c->has_operator) {
+    std::vector<std::pair<uint32_t, int>> key(N);
+    const double sr = rmax > rmin ? 65535.0 / (rmax - rmin) : 0.0, sz = zmax > zmin ? 65535.0 / (zmax - zmin) : 0.0;
+    for (int k = 0; k < N; ++k)
+      key[k] = {morton16(static_cast<uint32_t>((geo->r[k] - rmin) * sr), static_cast<uint32_t>((geo->z[k] - zmin) * sz)), k};
+    std::sort(key.begin(), key.end());
+    c->perm.resize(N);
+    for (int k = 0; k < N; ++k) c->perm[k] = key[k].second;
+  }
+  const bool has_perm = !c->perm.empty();
+
+  // device set-up
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return bail(fail(QS_ERR_CUDA, "cudaGetDevice failed"));
+  cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  size_t need = 0;
+  carve(c, nullptr, &need);
+  if (own) {
+    if (cudaMalloc(&c->owned, need) != cudaSuccess) return bail(fail(QS_ERR_CUDA, "cudaMalloc of the workspace failed"));
+    workspace = c->owned;
+    if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) return bail(fail(QS_ERR_CUDA, "stream"));
+  } else {
+    if (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 255))
+      return bail(fail(QS_ERR_ARG, "workspace NULL, too small or not 256-byte aligned"));
+    c->stream = static_cast<cudaStream_t>(stream);
+  }
+  carve(c, workspace, &need);
+  if (cudaMallocHost(&c->h_sc, sizeof(Scalars)) != cudaSuccess ||
+      cudaMallocHost(&c->h_stage, sizeof(double) * 2 * c->Np) != cudaSuccess)
+    return bail(fail(QS_ERR_CUDA, "cudaMallocHost failed"));
+  if (cudaMemsetAsync(workspace, 0, need, c->stream) != cudaSuccess) return bail(fail(QS_ERR_CUDA, "memset"));
+  c->H = c->Ha;
+  c->Halt = c->Hb;
+  VecCtx& v = c->v;
+  v.N = N; v.Np = c->Np; v.n_turns = c->n_turns;
+  v.turn_id = c->turn_id; v.turn_ptr = c->turn_ptr; v.turn_idx = c->turn_idx;
+  v.stream = c->stream; v.sc = c->sc; v.launches = &c->launches;
+
+  // geometry arrays in internal order, padded with far-away dummy rings that carry no current
+  std::vector<double> hr(c->Np), hz(c->Np), tmp(N);
+  for (int k = 0; k < N; ++k) {
+    const int o = c->perm.empty() ? k : c->perm[k];
+    hr[k] = geo->r[o];
+    hz[k] = geo->z[o];
+  }
+  for (int k = N; k < c->Np; ++k) {
+    hr[k] = hr[0];
+    hz[k] = zmax + 1.0 + 0.01 * (k - N);
+  }
+  auto put = [&](double* dst, const std::vector<double>& src, size_t n) {
+    return cudaMemcpyAsync(dst, src.data(), sizeof(double) * n, cudaMemcpyHostToDevice, c->stream) == cudaSuccess &&
+           cudaStreamSynchronize(c->stream) == cudaSuccess;
+  };
+  bool ok = put(c->r, hr, c->Np) && put(c->z, hz, c->Np);
+  for (int k = 0; k < N; ++k) tmp[k] = geo->area[c->perm.empty() ? k : c->perm[k]];
+  ok = ok && put(c->area, tmp, N);
+  for (int k = 0; k < N; ++k) tmp[k] = mat->jc0_scale ? mat->jc0_scale[c->perm.empty() ? k : c->perm[k]] : 1.0;
+  ok = ok && put(c->jc0s, tmp, N);
+  for (int k = 0; k < N; ++k)   // C3 self field: mu0 [ln(8 r/g) - 1] / (4 pi r)
+    tmp[k] = kMu0 * (std::log(8.0 * hr[k] / geo->softening) - 1.0) / (4.0 * kPi * hr[k]);
+  ok = ok && put(c->selfcoef, tmp, N);
+  if (!ok) return bail(fail(QS_ERR_CUDA, "upload of the geometry failed"));
+  if (has_perm && (cudaMemcpyAsync(c->d_perm, c->perm.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+                   cudaStreamSynchronize(c->stream) != cudaSuccess))
+    return bail(fail(QS_ERR_CUDA, "upload of the permutation failed"));
+  // bounding boxes of the blocks of 32
+  {
+    std::vector<double4> bb(c->nb);
+    for (int bidx = 0; bidx < c->nb; ++bidx) {
+      double4 q = make_double4(1e300, -1e300, 1e300, -1e300);
+      for (int l = 0; l < 32; ++l) {
+        const int k = bidx * 32 + l;
+        q.x = std::min(q.x, hr[k]); q.y = std::max(q.y, hr[k]);
+        q.z = std::min(q.z, hz[k]); q.w = std::max(q.w, hz[k]);
+      }
+      bb[bidx] = q;
+    }
+    if (cudaMemcpyAsync(c->bbox, bb.data(), sizeof(double4) * c->nb, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess)
+      return bail(fail(QS_ERR_CUDA, "upload of the block boxes failed"));
+  }
+  // turns: ids in internal order + CSR
+  if (c->n_turns) {
+    std::vector<int> tid(N), ptr(c->n_turns + 1, 0), idx(N);
+    for (int k = 0; k < N; ++k) tid[k] = geo->turn_id[c->perm.empty() ? k : c->perm[k]];
+    for (int k = 0; k < N; ++k) ++ptr[tid[k] + 1];
+    for (int w = 0; w < c->n_turns; ++w) {
+      if (ptr[w + 1] == 0) return bail(fail(QS_ERR_ARG, "geometry: a turn has no cells"));
+      ptr[w + 1] += ptr[w];
+    }
+    std::vector<int> fill(ptr.begin(), ptr.end() - 1);
+    for (int k = 0; k < N; ++k) idx[fill[tid[k]]++] = k;
+    std::vector<double> tf(c->n_turns, -1.0);
+    if (cudaMemcpyAsync(c->turn_id, tid.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+        cudaMemcpyAsync(c->turn_ptr, ptr.data(), sizeof(int) * (c->n_turns + 1), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+        cudaMemcpyAsync(c->turn_idx, idx.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+        cudaMemcpyAsync(c->t_first, tf.data(), sizeof(double) * c->n_turns, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess)
+      return bail(fail(QS_ERR_CUDA, "upload of the turn tables failed"));
+  }
+  // initial state: J = 0 (memset), T = T_bath
+  {
+    std::vector<double> T0(N, geo->T_bath);
+    if (!put(c->tmp, T0, N)) return bail(fail(QS_ERR_CUDA, "upload"));
+    k_enthalpy_from_T(v, mp, c->tmp, c->H, N);
+  }
+  k_set_scalars(v);
+  if (c->has_operator) {
+    if (launch_diag(N, c->r, c->soft_all + c->soft_self, c->diagM, c->stream) != cudaSuccess)
+      return bail(fail(QS_ERR_CUDA, "diag kernel launch failed"));
+    ++c->launches;
+    if (cudaMemcpyAsync(c->Hd, c->diagM, sizeof(double) * N, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
+      return bail(fail(QS_ERR_CUDA, "copy"));
+    if (c->n_turns) {
+      // unit-ramp particular solution x_p1 = H_M^-1 C (1/s_M) and M x_p1 (reference norm of the CG, C8)
+      k_turn_schur(v, c->diagM, c->swM);
+      std::vector<double> ones(c->n_turns, 1.0);
+      if (cudaMemcpyAsync(c->defw, ones.data(), sizeof(double) * c->n_turns, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+          cudaStreamSynchronize(c->stream) != cudaSuccess)
+        return bail(fail(QS_ERR_CUDA, "upload"));
+      k_apply_deficit(v, c->defw, c->diagM, c->swM, c->xp1);
+      if (cudaMemcpyAsync(c->p, c->xp1, sizeof(double) * N, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
+        return bail(fail(QS_ERR_CUDA, "copy"));
+      if ((rc = do_sweep(c, c->p, nullptr, false)) != QS_OK) return bail(rc);
+      k_scatter_scaled(v, c->yacc, nullptr, c->Mxp1, N, kCM);
+    }
+  }
+  if (cudaStreamSynchronize(c->stream) != cudaSuccess || cudaGetLastError() != cudaSuccess)
+    return bail(fail(QS_ERR_CUDA, std::string("initialisation kernels failed: ") + cudaGetErrorString(cudaGetLastError())));
+  c->st = qs_stats_t{};
+  c->st.Tmax = geo->T_bath;
+  *out = c;
+  return QS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* qs_last_error(void) { return g_err.c_str(); }
+
+size_t qs_workspace_bytes(const qs_geometry* geo) {
+  if (check_geometry(geo) != QS_OK) return 0;
+  qs_ctx tmp;
+  tmp.N = geo->n_rings;
+  tmp.Np = (tmp.N + 31) / 32 * 32;
+  tmp.nb = tmp.Np / 32;
+  tmp.n_turns = geo->n_turns;
+  size_t need = 0;
+  carve(&tmp, nullptr, &need);
+  return need;
+}
+
+int qs_init(const qs_geometry* geo, const qs_material* mat, qs_ctx** out) {
+  return init_common(geo, mat, nullptr, 0, nullptr, true, out);
+}
+int qs_init_device(const qs_geometry* geo, const qs_material* mat, void* workspace, size_t workspace_bytes, void* stream,
+                   qs_ctx** out) {
+  return init_common(geo, mat, workspace, workspace_bytes, stream, false, out);
+}
+
+void qs_free(qs_ctx* c) {
+  if (!c) return;
+  if (c->stream) cudaStreamSynchronize(c->stream);
+  if (c->h_sc) cudaFreeHost(c->h_sc);
+  if (c->h_stage) cudaFreeHost(c->h_stage);
+  if (c->owned) {
+    cudaFree(c->owned);
+    if (c->stream) cudaStreamDestroy(c->stream);
+  }
+  delete c;
+}
+
+int qs_sync(qs_ctx* c) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  QS_CUDA(cudaStreamSynchronize(c->stream));
+  return QS_OK;
+}
+
+int qs_step(qs_ctx* c, double dt, double I_ramp) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  if (!c->lattice || !c->has_operator) return fail(QS_ERR_ARG, "qs_step needs a lattice geometry with the operator set up");
+  if (!(dt > 0.0)) return fail(QS_ERR_DT, "dt <= 0");
+  const VecCtx& v = c->v;
+  const int N = c->N;
+  int rc;
+  c->st.sweeps = 0;
+  const size_t nb8 = sizeof(double) * N;
+  // backups: the step is transactional
+  QS_CUDA(cudaMemcpyAsync(c->Jold, c->J, nb8, cudaMemcpyDeviceToDevice, c->stream));
+  QS_CUDA(cudaMemcpyAsync(c->Hold, c->H, nb8, cudaMemcpyDeviceToDevice, c->stream));
+  QS_CUDA(cudaMemcpyAsync(c->xold, c->x, nb8, cudaMemcpyDeviceToDevice, c->stream));
+  k_set_scalars(v);
+  // warm start I'_prev moved onto the constraint C^T x = I_ramp with the static diagonal of M
+  k_turn_deficit(v, c->x, I_ramp, c->defw);
+  k_apply_deficit(v, c->defw, c->diagM, c->swM, c->x);
+  // S1 (+ M x0 in the same sweep): ring currents I = a J
+  k_mul(v, c->area, c->J, c->cur);
+  if ((rc = do_sweep(c, c->x, c->cur, true)) != QS_OK) return rc;
+  // S2
+  const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
+  k_material(v, c->mp, material_args(c, B0, (B1 - B0) / dt, dt, true));
+  // S3/S4
+  double nu = -1.0;
+  if (c->n_turns) {
+    k_turn_schur(v, c->Hd, c->sw);
+    k_nu_residual(v, I_ramp, c->Mxp1, c->shift, c->xp1, c->b, c->rr);
+    k_turn_project(v, c->rr, c->Hd, c->sw, c->vw, nullptr);
+    k_project_apply(v, 0, c->vw, c->Hd, c->rr, c->g);
+    k_copy_rg_to_nu2(v, 0);
+  } else {  // no constraint: nu^2 = b^T H^-1 b
+    QS_CUDA(cudaMemcpyAsync(c->rr, c->b, nb8, cudaMemcpyDeviceToDevice, c->stream));
+    k_project_apply(v, 0, nullptr, c->Hd, c->rr, c->g);
+    k_copy_rg_to_nu2(v, 0);
+  }
+  if ((rc = sync_scalars(c)) != QS_OK) return rc;
+  nu = std::sqrt(std::max(c->h_sc->nu2, 0.0));
+  int iters = 0;
+  double relres = 0.0;
+  bool hit_max = false;
+  auto restore = [&]() {
+    cudaMemcpyAsync(c->x, c->xold, nb8, cudaMemcpyDeviceToDevice, c->stream);
+    cudaStreamSynchronize(c->stream);
+  };
+  if (nu > 0.0) {
+    rc = cg_core(c, c->b, c->x, c->shift, c->Hd, c->sw, true, c->cg_tol, c->cg_maxit, nu, &iters, &relres, &hit_max);
+    if (rc != QS_OK) {
+      restore();
+      return rc;
+    }
+  } else {
+    QS_CUDA(cudaMemsetAsync(c->x, 0, nb8, c->stream));
+    if (c->n_turns) QS_CUDA(cudaMemsetAsync(c->vsum, 0, sizeof(double) * c->n_turns, c->stream));
+  }
+  k_sum_uterm(v, c->vsum);
+  // S5
+  k_scale_div(v, dt, c->x, c->area, c->J);
+  // S6
+  int m = 0;
+  if ((rc = run_heat(c, dt, &m)) != QS_OK) return rc;
+  // S7 + statistics
+  EventArgs ev;
+  ev.H = c->H; ev.E = c->E; ev.J = c->Jold; ev.Jc = c->Jc; ev.rho = c->rho;
+  ev.ebar_prev = c->ebar_prev; ev.flags = c->flags; ev.t_first = c->t_first; ev.count = c->count;
+  ev.dt = dt; ev.t_new = c->t + dt; ev.have_prev = c->have_prev_E;
+  k_events(v, c->mp, ev);
+  k_step_stats(v, c->mp, c->J, c->H, c->Q, c->r, c->area);
+  if ((rc = sync_scalars(c)) != QS_OK) return rc;
+  if (c->h_sc->nonfinite) {
+    cudaMemcpyAsync(c->J, c->Jold, nb8, cudaMemcpyDeviceToDevice, c->stream);
+    cudaMemcpyAsync(c->H, c->Hold, nb8, cudaMemcpyDeviceToDevice, c->stream);
+    restore();
+    return fail(QS_ERR_NONFINITE, "NaN/Inf in J or T after the step; state restored");
+  }
+  c->t += dt;
+  c->I += dt * I_ramp;
+  c->have_prev_E = true;
+  int ret = c->h_sc->event_or | (hit_max ? QS_EV_CG_MAXIT : 0);
+  c->st.cg_iters = iters;
+  c->st.cg_relres = relres;
+  c->st.heat_substeps = m;
+  c->st.event_word = ret;
+  c->st.U_terminal = c->h_sc->uterm;
+  c->st.Tmax = c->h_sc->tmax;
+  c->st.joule_power = c->h_sc->joule;
+  c->st.t = c->t;
+  c->st.I = c->I;
+  return ret;
+}
+
+int qs_read(qs_ctx* c, double* J, double* T, double* B, double* E) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  int rc;
+  if (J && (rc = download(c, c->J, J)) != QS_OK) return rc;
+  if (T) {
+    k_T_from_enthalpy(c->v, c->mp, c->H, c->tmp, c->N);
+    if ((rc = download(c, c->tmp, T)) != QS_OK) return rc;
+  }
+  if (B) {
+    if ((rc = download(c, c->Br, B)) != QS_OK) return rc;
+    if ((rc = download(c, c->Bz, B + c->N)) != QS_OK) return rc;
+  }
+  if (E && (rc = download(c, c->E, E)) != QS_OK) return rc;
+  return QS_OK;
+}
+
+int qs_read_aux(qs_ctx* c, double* Q, double* dEdJ, double* Jc, double* rho) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  int rc;
+  if (Q && (rc = download(c, c->Q, Q)) != QS_OK) return rc;
+  if (dEdJ && (rc = download(c, c->dEdJ, dEdJ)) != QS_OK) return rc;
+  if (Jc && (rc = download(c, c->Jc, Jc)) != QS_OK) return rc;
+  if (rho && (rc = download(c, c->rho, rho)) != QS_OK) return rc;
+  return QS_OK;
+}
+
+int qs_write(qs_ctx* c, const double* J, const double* T, double t, double I) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  int rc;
+  if (J && (rc = upload(c, J, c->J, c->N)) != QS_OK) return rc;
+  if (T) {
+    for (int k = 0; k < c->N; ++k)
+      if (!(T[k] > 0.0)) return fail(QS_ERR_ARG, "qs_write: T must be > 0");
+    if ((rc = upload(c, T, c->tmp, c->N)) != QS_OK) return rc;
+    k_enthalpy_from_T(c->v, c->mp, c->tmp, c->H, c->N);
+  }
+  QS_CUDA(cudaMemsetAsync(c->x, 0, sizeof(double) * c->Np, c->stream));
+  QS_CUDA(cudaStreamSynchronize(c->stream));
+  c->t = t;
+  c->I = I;
+  c->have_prev_E = false;
+  return QS_OK;
+}
+
+int qs_matvec_device(qs_ctx* c, const double* d_x, double* d_y) {
+  if (!c || !d_x || !d_y) return fail(QS_ERR_ARG, "NULL argument");
+  if (!c->has_operator) return fail(QS_ERR_ARG, "operator not set up (QS_GEO_NO_OPERATOR)");
+  c->st.sweeps = 0;
+  k_gather(c->v, d_x, c->perm.empty() ? nullptr : c->d_perm, c->p, c->N, c->Np);
+  int rc = do_sweep(c, c->p, nullptr, false);
+  if (rc != QS_OK) return rc;
+  k_scatter_scaled(c->v, c->yacc, c->perm.empty() ? nullptr : c->d_perm, d_y, c->N, kCM);
+  QS_CUDA(cudaGetLastError());
+  return QS_OK;
+}
+
+int qs_matvec(qs_ctx* c, const double* x, double* y) {
+  if (!c || !x || !y) return fail(QS_ERR_ARG, "NULL argument");
+  if (!c->has_operator) return fail(QS_ERR_ARG, "operator not set up (QS_GEO_NO_OPERATOR)");
+  int rc;
+  c->st.sweeps = 0;
+  if ((rc = upload(c, x, c->p, c->Np)) != QS_OK) return rc;
+  if ((rc = do_sweep(c, c->p, nullptr, false)) != QS_OK) return rc;
+  return download(c, c->yacc, y, kCM);
+}
+
+int qs_field(qs_ctx* c, const double* I, double* B) {
+  if (!c || !I || !B) return fail(QS_ERR_ARG, "NULL argument");
+  if (!c->lattice || !c->has_operator) return fail(QS_ERR_ARG, "qs_field needs a lattice geometry with the operator set up");
+  int rc;
+  c->st.sweeps = 0;
+  if ((rc = upload(c, I, c->cur, c->Np)) != QS_OK) return rc;
+  QS_CUDA(cudaMemsetAsync(c->p, 0, sizeof(double) * c->Np, c->stream));
+  if ((rc = do_sweep(c, c->p, c->cur, true)) != QS_OK) return rc;
+  // Br = mu0/(4 r) bracc ; Bz = mu0/4 bzacc + selfcoef I
+  QS_CUDA(cudaMemcpyAsync(c->h_stage, c->bracc, sizeof(double) * c->N, cudaMemcpyDeviceToHost, c->stream));
+  QS_CUDA(cudaMemcpyAsync(c->h_stage + c->Np, c->bzacc, sizeof(double) * c->N, cudaMemcpyDeviceToHost, c->stream));
+  std::vector<double> hr(c->N), hs(c->N);
+  QS_CUDA(cudaMemcpyAsync(hr.data(), c->r, sizeof(double) * c->N, cudaMemcpyDeviceToHost, c->stream));
+  QS_CUDA(cudaMemcpyAsync(hs.data(), c->selfcoef, sizeof(double) * c->N, cudaMemcpyDeviceToHost, c->stream));
+  QS_CUDA(cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < c->N; ++k) {   // output scaling of the accumulators (same as the material kernel applies)
+    B[k] = (0.25 * kMu0) * c->h_stage[k] / hr[k];
+    B[c->N + k] = (0.25 * kMu0) * c->h_stage[c->Np + k] + hs[k] * I[k];
+  }
+  return QS_OK;
+}
+
+int qs_solve_device(qs_ctx* c, const double* d_b, double* d_x, int32_t maxit_override, int32_t* iters, double* relres) {
+  if (!c || !d_b || !d_x) return fail(QS_ERR_ARG, "NULL argument");
+  if (!c->has_operator) return fail(QS_ERR_ARG, "operator not set up (QS_GEO_NO_OPERATOR)");
+  const int* perm = c->perm.empty() ? nullptr : c->d_perm;
+  c->st.sweeps = 0;
+  k_set_scalars(c->v);
+  k_gather(c->v, d_b, perm, c->b, c->N, c->N);
+  QS_CUDA(cudaMemsetAsync(c->tmp, 0, sizeof(double) * c->Np, c->stream));   // x0 = 0 satisfies C^T x = 0
+  QS_CUDA(cudaMemsetAsync(c->yacc, 0, sizeof(double) * c->Np, c->stream));  // M x0 = 0
+  int it = 0;
+  double rel = 0.0;
+  bool hit = false;
+  int rc = cg_core(c, c->b, c->tmp, c->zero, c->diagM, c->swM, true, c->cg_tol, maxit_override > 0 ? maxit_override : c->cg_maxit,
+                   -1.0, &it, &rel, &hit);
+  if (rc != QS_OK) return rc;
+  k_scatter_scaled(c->v, c->tmp, perm, d_x, c->N, 1.0);
+  QS_CUDA(cudaStreamSynchronize(c->stream));
+  if (iters) *iters = it;
+  if (relres) *relres = rel;
+  c->st.cg_iters = it;
+  c->st.cg_relres = rel;
+  return hit ? QS_EV_CG_MAXIT : QS_OK;
+}
+
+int qs_solve(qs_ctx* c, const double* b, double* x, int32_t maxit_override, int32_t* iters, double* relres) {
+  if (!c || !b || !x) return fail(QS_ERR_ARG, "NULL argument");
+  if (!c->has_operator) return fail(QS_ERR_ARG, "operator not set up (QS_GEO_NO_OPERATOR)");
+  // stage through tmp2 (caller order on the device), then the device variant
+  QS_CUDA(cudaMemcpyAsync(c->tmp2, b, sizeof(double) * c->N, cudaMemcpyHostToDevice, c->stream));
+  QS_CUDA(cudaStreamSynchronize(c->stream));
+  int rc = qs_solve_device(c, c->tmp2, c->tmp2, maxit_override, iters, relres);
+  if (rc < 0) return rc;
+  QS_CUDA(cudaMemcpyAsync(x, c->tmp2, sizeof(double) * c->N, cudaMemcpyDeviceToHost, c->stream));
+  QS_CUDA(cudaStreamSynchronize(c->stream));
+  return rc;
+}
+
+int qs_set_fields(qs_ctx* c, const double* B, const double* Q) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  int rc;
+  if (B) {
+    if ((rc = upload(c, B, c->Br, c->N)) != QS_OK) return rc;
+    if ((rc = upload(c, B + c->N, c->Bz, c->N)) != QS_OK) return rc;
+  }
+  if (Q && (rc = upload(c, Q, c->Q, c->N)) != QS_OK) return rc;
+  return QS_OK;
+}
+
+int qs_material_eval(qs_ctx* c, double dt) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
+  k_material(c->v, c->mp, material_args(c, B0, dt > 0 ? (B1 - B0) / dt : 0.0, dt, false));
+  QS_CUDA(cudaGetLastError());
+  return QS_OK;
+}
+
+int qs_heat(qs_ctx* c, double dt) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  if (!c->lattice) return fail(QS_ERR_ARG, "qs_heat needs a lattice geometry");
+  if (!(dt > 0.0)) return fail(QS_ERR_DT, "dt <= 0");
+  int m = 0;
+  int rc = run_heat(c, dt, &m);
+  return rc != QS_OK ? rc : m;
+}
+
+int qs_stats(qs_ctx* c, qs_stats_t* out) {
+  if (!c || !out) return fail(QS_ERR_ARG, "NULL argument");
+  *out = c->st;
+  out->launches = c->launches;
+  out->pair_evals = c->pair_evals;
+  out->t = c->t;
+  out->I = c->I;
+  return QS_OK;
+}
+
+int qs_events(qs_ctx* c, int32_t* flags, double* t_first, int32_t* count) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  if (!c->n_turns) return QS_OK;
+  const size_t nt = c->n_turns;
+  if (flags) QS_CUDA(cudaMemcpyAsync(flags, c->flags, sizeof(int) * nt, cudaMemcpyDeviceToHost, c->stream));
+  if (t_first) QS_CUDA(cudaMemcpyAsync(t_first, c->t_first, sizeof(double) * nt, cudaMemcpyDeviceToHost, c->stream));
+  if (count) QS_CUDA(cudaMemcpyAsync(count, c->count, sizeof(int) * nt, cudaMemcpyDeviceToHost, c->stream));
+  QS_CUDA(cudaStreamSynchronize(c->stream));
+  return QS_OK;
+}
+
+}  // extern "C"

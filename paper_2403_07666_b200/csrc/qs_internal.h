@@ -1,0 +1,129 @@
+// qs_internal.h — declarations shared by the CUDA translation units of libqs (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace qs {
+
+constexpr double kMu0 = 1.2566370614359172953850573533118e-6;   // 4 pi 1e-7
+constexpr double kPi = 3.1415926535897932384626433832795;
+
+// ---- pair sweeps (qs_operator.cu) -------------------------------------------------------------
+struct SweepParams {
+  const double* r;        // [Np] ring radius, padded to a multiple of 32
+  const double* z;        // [Np]
+  const double* x;        // [Np] vector multiplied by M (padding = 0)
+  const double* cur;      // [Np] ring currents whose field is wanted (FIELD sweeps; padding = 0)
+  const double4* bbox;    // [nb] (rmin, rmax, zmin, zmax) of each block of 32 rings
+  double* yacc;           // [Np] += sum_j S/a_inf x_j        (scale mu0 pi/2 applied by the consumer)
+  double* bracc;          // [Np] += sum_j dz(-Kt + mid Qt) I_j   (scale mu0/(4 r_i) by the consumer)
+  double* bzacc;          // [Np] += sum_j (Kt + c_ij Qt) I_j     (scale mu0/4 by the consumer)
+  unsigned long long* counter;
+  long long n_items;      // nb (nb + 1) / 2
+  int nb;
+  int chunk;
+  double soft_all;        // g^2 added to dz^2 of every pair (free rings) or 0 (lattice)
+  double soft_self;       // extra dz^2 of the self pair (lattice: g^2)
+  double minsep2;         // lower bound on the squared centre distance of two distinct rings
+  double diag_d2;         // smallest B2 inside a diagonal item (self pair included)
+};
+int sweep_grid(int sm_count, bool field);
+int sweep_warps_per_cta();
+cudaError_t launch_sweep(const SweepParams& prm, bool field, int grid, cudaStream_t stream);
+// diagM_i = M(r_i, r_i, dz^2 = d2self) in henry
+cudaError_t launch_diag(int n, const double* r, double d2self, double* diagM, cudaStream_t stream);
+
+// ---- vector / CG kernels (qs_vector.cu) -------------------------------------------------------
+// Device scalars of the solver; all reductions land here (no host round trip inside an iteration).
+struct Scalars {
+  double rg[2];          // r^T g, double buffered by iteration parity
+  double pq;             // p^T A p
+  double nu2;            // reference norm squared
+  double uterm;          // sum_w vsum_w = terminal voltage
+  double tmax, joule;    // step statistics
+  int nonfinite;         // set when J or T is NaN/Inf
+  int event_or;          // OR of per-turn return bits
+  int pad[2];
+};
+
+struct VecCtx {
+  int N;                 // rings
+  int Np;                // padded
+  int n_turns;
+  const int* turn_id;    // [N] (internal order)
+  const int* turn_ptr;   // [n_turns+1] CSR of cells per turn
+  const int* turn_idx;   // [N]
+  cudaStream_t stream;
+  Scalars* sc;
+  long long* launches;   // host counter
+};
+
+// q = cM*yacc + shift*p ; pq = p.q
+void k_finish_Ap(const VecCtx& v, const double* yacc, const double* shift, const double* p, double* q, double cM);
+// r = cM*yacc + shift*x - b
+void k_residual(const VecCtx& v, const double* yacc, const double* shift, const double* x, const double* b, double* r,
+                double cM);
+// alpha = rg[par]/pq ; x += alpha p ; r += alpha q
+void k_update_xr(const VecCtx& v, int par, const double* p, const double* q, double* x, double* r);
+// tw = sum_{i in w} r_i/H_i ; vw = tw/s_w ; vsum += vw      (one warp per turn)
+void k_turn_project(const VecCtx& v, const double* r, const double* Hd, const double* sw, double* vw, double* vsum);
+// s_w = sum_{i in w} 1/H_i
+void k_turn_schur(const VecCtx& v, const double* Hd, double* sw);
+// r -= v[turn] ; g = r/H ; rg[par] = r.g
+void k_project_apply(const VecCtx& v, int par, const double* vw, const double* Hd, double* r, double* g);
+// first direction p = -g ; later p = -g + (rg[par]/rg[par^1]) p ; also zeroes rg[par^1], pq for the next iteration
+void k_direction(const VecCtx& v, int par, bool first, const double* g, double* p);
+// deficit_w = d - sum_{i in w} x_i ; x_i += deficit_w / (H_i s_w)   (moves a warm start onto the constraint)
+void k_turn_deficit(const VecCtx& v, const double* x, double d, double* defw);
+void k_apply_deficit(const VecCtx& v, const double* defw, const double* Hd, const double* sw, double* x);
+void k_axpy(const VecCtx& v, double a, const double* x, double* y);                     // y += a x
+void k_scale_div(const VecCtx& v, double a, const double* x, const double* d, double* y);   // y += a x / d
+void k_mul(const VecCtx& v, const double* a, const double* b, double* y);               // y = a b
+void k_set_scalars(const VecCtx& v);                                                    // zero the Scalars block
+void k_copy_rg_to_nu2(const VecCtx& v, int par);
+// r = I_ramp (Mxp1 + shift xp1) - b : residual of the cold start x_p = I_ramp xp1 (reference norm, C8)
+void k_nu_residual(const VecCtx& v, double I_ramp, const double* Mxp1, const double* shift, const double* xp1,
+                   const double* b, double* r);
+void k_sum_uterm(const VecCtx& v, const double* vsum);                                  // sc->uterm = sum vsum
+void k_gather(const VecCtx& v, const double* src, const int* perm, double* dst, int n, int npad);   // dst[k] = src[perm[k]], pad 0
+void k_scatter_scaled(const VecCtx& v, const double* src, const int* perm, double* dst, int n, double scale);  // dst[perm[k]] = scale*src[k]
+
+// ---- pointwise passes (qs_pointwise.cu) ---------------------------------------------------------
+struct MaterialParams {
+  double Ec, n_exp, Jc0, Tc, B0, eps_coef, eps_exp, Y, rho_n;
+  double C3, C1, k_in, k_between, theta;
+  double T_fluxjump, dEdt_spike;
+  int n_int;             // n_exp when it is a small integer, else 0
+};
+struct LatticeParams {
+  int Nr, Nz, n;         // cells along r, along z, per wire side
+  double h, r_inner;
+  double h_conv[4];
+  double T_bath;
+};
+struct MaterialArgs {
+  int N;
+  const double *J, *H, *r, *area, *jc0_scale, *selfcoef, *bracc, *bzacc, *diagM;
+  double *Br, *Bz, *E, *dEdJ, *Q, *b, *shift, *Hd, *Jc, *rho;
+  double Bext, Bdot, dt;
+  bool from_acc;         // true: B from the sweep accumulators (+ self + Bext); false: B arrays given
+};
+void k_material(const VecCtx& v, const MaterialParams& mp, const MaterialArgs& a);
+void k_enthalpy_from_T(const VecCtx& v, const MaterialParams& mp, const double* T, double* H, int n);
+void k_T_from_enthalpy(const VecCtx& v, const MaterialParams& mp, const double* H, double* T, int n);
+void k_heat_substep(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, const double* Hin,
+                    const double* Q, double* Hout, double dtsub);
+struct EventArgs {
+  const double *H, *E, *J, *Jc, *rho;
+  double* ebar_prev;     // [n_turns]
+  int* flags;            // [n_turns]
+  double* t_first;       // [n_turns]
+  int* count;            // [n_turns]
+  double dt, t_new;
+  bool have_prev;
+};
+void k_events(const VecCtx& v, const MaterialParams& mp, const EventArgs& e);
+void k_step_stats(const VecCtx& v, const MaterialParams& mp, const double* J, const double* H, const double* Q,
+                  const double* r, const double* area);
+
+}  // namespace qs

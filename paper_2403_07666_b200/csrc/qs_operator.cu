@@ -1,0 +1,297 @@
+// qs_operator.cu — the all-pairs ring operator sweeps K1 (y = M x) and K2 (y = M x fused with Br, Bz = G_B I).
+//
+// Decomposition (B200-first, not the paper's): rings are grouped in blocks of 32 (one per lane).  The
+// symmetric kernel is evaluated ONCE per unordered pair: a work item is a pair of ring blocks
+// (bi <= bj); lane l owns target i = 32 bi + l and walks the 32 sources of block bj in a rotated order
+// j = 32 bj + ((l + s) & 31), s = 0..31.  The contribution to y_i stays in a register; the
+// contribution to y_j rides in a register that is passed to the neighbouring lane after every step
+// (one 64-bit shuffle), so that after 32 steps lane l holds the finished partial sum for source
+// 32 bj + l.  Partial sums go to FP64 accumulators in L2 with RED.ADD.F64 (256-byte coalesced).
+// Source blocks (r, z, x[, I]: 3-4 x 256 B) are staged in per-warp shared memory with TMA bulk copies
+// (cp.async.bulk + mbarrier), double buffered one item ahead.  Items are handed out in contiguous
+// chunks from an atomic counter to a persistent grid (a multiple of the SM count).
+// The AGM depth is chosen per item from the bounding boxes of the two blocks (a lower bound on
+// k'^2 over the 1024 pairs), so the 32-step loops are branch-free and fully unrolled in the depth.
+#include "qs_internal.h"
+#include "qs_pair.cuh"
+
+namespace qs {
+
+// smallest k'^2 for which NIT iterations (+ the closed-form last step) are exact to < 1e-16
+// (60-digit evaluation of the truncated recurrence against K, E).
+__device__ __constant__ double kKp2Min[8] = {1e300, 0.9995, 0.9030, 0.2754, 6.46e-3, 2.62e-6, 4.3e-13, 0.0};
+
+constexpr int kWarpsPerCta = 8;
+constexpr int kThreads = kWarpsPerCta * 32;
+constexpr int kMaxArrays = 4;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+// TMA 1-D bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP)
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+__device__ __forceinline__ void red_add(double* addr, double v) {
+  asm volatile("red.global.add.f64 [%0], %1;" ::"l"(addr), "d"(v) : "memory");
+}
+
+struct TargetRegs {
+  double r, z, x, cur;
+};
+struct Accum {
+  double y, br, bz;
+};
+
+// ---- one off-diagonal item: all 32 x 32 pairs, both directions -----------------------------------
+template <int NIT, bool FIELD>
+__device__ __forceinline__ void item_offdiag(const TargetRegs& t, const double* __restrict__ sr,
+                                             const double* __restrict__ sz, const double* __restrict__ sx,
+                                             const double* __restrict__ sc, double soft_all, int lane, Accum& acc,
+                                             Accum& trav) {
+  const unsigned full = 0xffffffffu;
+  const int next = (lane + 1) & 31;
+  const double ri2 = t.r * t.r;
+#pragma unroll 1
+  for (int s = 0; s < 32; ++s) {
+    const int jl = (lane + s) & 31;
+    const double rj = sr[jl], zj = sz[jl], xj = sx[jl];
+    const double dz = t.z - zj;
+    const double dz2 = fma(dz, dz, soft_all);
+    const double sum = t.r + rj, dif = t.r - rj;
+    const double A2 = fma(sum, sum, dz2), B2 = fma(dif, dif, dz2);
+    const PairAGM a = agm_pair<NIT, FIELD>(A2, B2);
+    const double mt = a.S * a.yinf;
+    acc.y = fma(mt, xj, acc.y);
+    trav.y = fma(mt, t.x, trav.y);
+    if (FIELD) {
+      const double cj = sc[jl];
+      const double qt = a.yinf * (a.mid - a.S) * a.y0sq;
+      const double e = fma(rj, rj, -ri2);                  // rj^2 - ri^2
+      const double bz_ij = fma(e - dz2, qt, a.yinf);       // Kt + (rj^2 - ri^2 - dz^2) Qt
+      const double bz_ji = fma(-e - dz2, qt, a.yinf);
+      const double ur = dz * fma(a.mid, qt, -a.yinf);      // dz (-Kt + (ri^2 + rj^2 + dz^2) Qt)
+      acc.bz = fma(bz_ij, cj, acc.bz);
+      acc.br = fma(ur, cj, acc.br);
+      trav.bz = fma(bz_ji, t.cur, trav.bz);
+      trav.br = fma(-ur, t.cur, trav.br);
+      trav.bz = __shfl_sync(full, trav.bz, next);
+      trav.br = __shfl_sync(full, trav.br, next);
+    }
+    trav.y = __shfl_sync(full, trav.y, next);
+  }
+}
+
+// ---- one diagonal item (bi == bj): every ordered pair appears once in the rotation -----------------
+template <int NIT, bool FIELD>
+__device__ __forceinline__ void item_diag(const TargetRegs& t, const double* __restrict__ sr,
+                                          const double* __restrict__ sz, const double* __restrict__ sx,
+                                          const double* __restrict__ sc, double soft_all, double soft_self, int lane,
+                                          Accum& acc) {
+  const double ri2 = t.r * t.r;
+  {  // s = 0: the self pair; M_ii = M(ri, ri, dz^2 = soft_all + soft_self); no field term (C3 self field is analytic)
+    const double dz2 = soft_all + soft_self;
+    const double sum = t.r + t.r;
+    const PairAGM a = agm_pair<NIT, false>(fma(sum, sum, dz2), dz2);
+    acc.y = fma(a.S * a.yinf, t.x, acc.y);
+  }
+#pragma unroll 1
+  for (int s = 1; s < 32; ++s) {
+    const int jl = (lane + s) & 31;
+    const double rj = sr[jl], zj = sz[jl], xj = sx[jl];
+    const double dz = t.z - zj;
+    const double dz2 = fma(dz, dz, soft_all);
+    const double sum = t.r + rj, dif = t.r - rj;
+    const PairAGM a = agm_pair<NIT, FIELD>(fma(sum, sum, dz2), fma(dif, dif, dz2));
+    acc.y = fma(a.S * a.yinf, xj, acc.y);
+    if (FIELD) {
+      const double cj = sc[jl];
+      const double qt = a.yinf * (a.mid - a.S) * a.y0sq;
+      const double e = fma(rj, rj, -ri2);
+      acc.bz = fma(fma(e - dz2, qt, a.yinf), cj, acc.bz);
+      acc.br = fma(dz * fma(a.mid, qt, -a.yinf), cj, acc.br);
+    }
+  }
+}
+
+__device__ __forceinline__ int classify(const double4& bi, const double4& bj, bool diag, const SweepParams& prm) {
+  // double4 = (rmin, rmax, zmin, zmax) of the ring centres of a block
+  const double dr = fmax(0.0, fmax(bi.x - bj.y, bj.x - bi.y));
+  const double dzg = fmax(0.0, fmax(bi.z - bj.w, bj.z - bi.w));
+  const double smax = bi.y + bj.y;
+  const double d2 = diag ? prm.diag_d2 : fmax(fma(dr, dr, dzg * dzg), prm.minsep2) + prm.soft_all;
+  const double kp2 = d2 / (fma(smax, smax, d2));
+  int n = 7;
+#pragma unroll
+  for (int k = 6; k >= 2; --k)
+    if (kp2 >= kKp2Min[k]) n = k;
+  return n;
+}
+
+// row-major enumeration of the upper triangle (bi <= bj) of an nb x nb block matrix
+__device__ __forceinline__ void unrank(long long k, int nb, int& bi, int& bj) {
+  const double t = 2.0 * nb + 1.0;
+  int i = static_cast<int>(floor(0.5 * (t - sqrt(t * t - 8.0 * static_cast<double>(k)))));
+  i = max(0, min(i, nb - 1));
+  auto row_start = [nb](int r) { return static_cast<long long>(r) * nb - static_cast<long long>(r) * (r - 1) / 2; };
+  while (i > 0 && row_start(i) > k) --i;
+  while (i + 1 < nb && row_start(i + 1) <= k) ++i;
+  bi = i;
+  bj = i + static_cast<int>(k - row_start(i));
+}
+
+template <bool FIELD>
+__global__ void __launch_bounds__(kThreads, FIELD ? 2 : 3) sweep_kernel(SweepParams prm) {
+  constexpr int NA = FIELD ? 4 : 3;
+  __shared__ __align__(128) double sbuf[kWarpsPerCta][2][kMaxArrays][32];
+  __shared__ __align__(8) uint64_t sbar[kWarpsPerCta][2];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const unsigned full = 0xffffffffu;
+  if (threadIdx.x < kWarpsPerCta * 2) mbar_init(&sbar[threadIdx.x >> 1][threadIdx.x & 1], 1);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  __syncthreads();
+
+  uint32_t phase = 0u;   // bit b = parity to wait for on buffer b
+  const double* src[kMaxArrays] = {prm.r, prm.z, prm.x, prm.cur};
+
+  auto issue = [&](int buf, int bj) {
+    if (lane == 0) {
+      mbar_expect_tx(&sbar[warp][buf], NA * 256u);
+#pragma unroll
+      for (int a = 0; a < NA; ++a) bulk_g2s(&sbuf[warp][buf][a][0], src[a] + 32ll * bj, 256u, &sbar[warp][buf]);
+    }
+  };
+
+  for (;;) {
+    long long k0 = 0;
+    if (lane == 0) k0 = static_cast<long long>(atomicAdd(prm.counter, static_cast<unsigned long long>(prm.chunk)));
+    k0 = __shfl_sync(full, k0, 0);
+    if (k0 >= prm.n_items) break;
+    const int cnt = static_cast<int>(min(static_cast<long long>(prm.chunk), prm.n_items - k0));
+    int bi, bj;
+    unrank(k0, prm.nb, bi, bj);
+    issue(0, bj);
+
+    TargetRegs t;
+    Accum acc = {0.0, 0.0, 0.0};
+    double4 bbi;
+    int cur_bi = -1;
+    for (int it = 0; it < cnt; ++it) {
+      const int buf = it & 1;
+      if (bi != cur_bi) {  // new target block: flush the old accumulators, load the new targets
+        if (cur_bi >= 0) {
+          red_add(prm.yacc + 32ll * cur_bi + lane, acc.y);
+          if (FIELD) {
+            red_add(prm.bracc + 32ll * cur_bi + lane, acc.br);
+            red_add(prm.bzacc + 32ll * cur_bi + lane, acc.bz);
+          }
+        }
+        acc = {0.0, 0.0, 0.0};
+        cur_bi = bi;
+        const long long i = 32ll * bi + lane;
+        t.r = prm.r[i];
+        t.z = prm.z[i];
+        t.x = prm.x[i];
+        t.cur = FIELD ? prm.cur[i] : 0.0;
+        bbi = prm.bbox[bi];
+      }
+      // next item of this chunk (row-major walk), prefetched into the other buffer
+      int nbi = bi, nbj = bj + 1;
+      if (nbj == prm.nb) {
+        nbi = bi + 1;
+        nbj = nbi;
+      }
+      if (it + 1 < cnt) issue(buf ^ 1, nbj);
+
+      const int nit = classify(bbi, prm.bbox[bj], bi == bj, prm);
+      mbar_wait(&sbar[warp][buf], (phase >> buf) & 1u);
+      phase ^= 1u << buf;
+      const double* sr = sbuf[warp][buf][0];
+      const double* sz = sbuf[warp][buf][1];
+      const double* sx = sbuf[warp][buf][2];
+      const double* sc = sbuf[warp][buf][3];
+      if (bi == bj) {
+        switch (nit) {
+          case 2: case 3: case 4:
+            item_diag<4, FIELD>(t, sr, sz, sx, sc, prm.soft_all, prm.soft_self, lane, acc); break;
+          case 5: item_diag<5, FIELD>(t, sr, sz, sx, sc, prm.soft_all, prm.soft_self, lane, acc); break;
+          case 6: item_diag<6, FIELD>(t, sr, sz, sx, sc, prm.soft_all, prm.soft_self, lane, acc); break;
+          default: item_diag<7, FIELD>(t, sr, sz, sx, sc, prm.soft_all, prm.soft_self, lane, acc); break;
+        }
+      } else {
+        Accum trav = {0.0, 0.0, 0.0};
+        switch (nit) {
+          case 2: item_offdiag<2, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break;
+          case 3: item_offdiag<3, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break;
+          case 4: item_offdiag<4, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break;
+          case 5: item_offdiag<5, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break;
+          case 6: item_offdiag<6, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break;
+          default: item_offdiag<7, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break;
+        }
+        red_add(prm.yacc + 32ll * bj + lane, trav.y);
+        if (FIELD) {
+          red_add(prm.bracc + 32ll * bj + lane, trav.br);
+          red_add(prm.bzacc + 32ll * bj + lane, trav.bz);
+        }
+      }
+      __syncwarp();  // every lane is done reading sbuf[buf] before it is refilled two items later
+      bi = nbi;
+      bj = nbj;
+    }
+    red_add(prm.yacc + 32ll * cur_bi + lane, acc.y);
+    if (FIELD) {
+      red_add(prm.bracc + 32ll * cur_bi + lane, acc.br);
+      red_add(prm.bzacc + 32ll * cur_bi + lane, acc.bz);
+    }
+  }
+}
+
+__global__ void diag_kernel(int n, const double* __restrict__ r, double d2self, double* __restrict__ diagM) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double s = r[i] + r[i];
+  const PairAGM a = agm_pair<7, false>(fma(s, s, d2self), d2self);
+  diagM[i] = (0.5 * kMu0 * kPi) * a.S * a.yinf;
+}
+cudaError_t launch_diag(int n, const double* r, double d2self, double* diagM, cudaStream_t stream) {
+  diag_kernel<<<(n + 255) / 256, 256, 0, stream>>>(n, r, d2self, diagM);
+  return cudaGetLastError();
+}
+
+int sweep_grid(int sm_count, bool field) { return sm_count * (field ? 2 : 3); }
+
+cudaError_t launch_sweep(const SweepParams& prm, bool field, int grid, cudaStream_t stream) {
+  if (field)
+    sweep_kernel<true><<<grid, kThreads, 0, stream>>>(prm);
+  else
+    sweep_kernel<false><<<grid, kThreads, 0, stream>>>(prm);
+  return cudaGetLastError();
+}
+
+int sweep_warps_per_cta() { return kWarpsPerCta; }
+
+}  // namespace qs

@@ -1,0 +1,286 @@
+// qs_vector.cu — K3 (CG vector kernels: fused axpy / dot) and K4 (per-turn segmented reductions, Schur scalars).
+//
+// Projected CG with a per-turn constraint, SURVEY.md §8(c) C8.  All scalars (r^T g, p^T A p, alpha, beta) stay
+// on the device in a Scalars block: a kernel reads the dot products its predecessor reduced, so an iteration
+// needs no host round trip.  Reductions: warp shuffles -> one shared-memory stage -> one FP64 atomic per CTA.
+// Streaming kernels use grid-stride loops over a grid that is a multiple of the SM count.
+#include "qs_internal.h"
+
+namespace qs {
+
+namespace {
+constexpr int kBlock = 256;
+int g_sm_count = 0;
+
+inline int grid_for(int n) {
+  if (g_sm_count == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (g_sm_count <= 0) g_sm_count = 148;
+  }
+  const int need = (n + kBlock - 1) / kBlock;
+  const int cap = g_sm_count * 8;
+  return need < cap ? (need > 0 ? need : 1) : cap;
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ void block_atomic_sum(double v, double* dst) {
+  __shared__ double part[kBlock / 32];
+  v = warp_sum(v);
+  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    double s = threadIdx.x < kBlock / 32 ? part[threadIdx.x] : 0.0;
+    s = warp_sum(s);
+    if (threadIdx.x == 0) atomicAdd(dst, s);
+  }
+}
+
+__global__ void finish_Ap_kernel(int n, const double* __restrict__ yacc, const double* __restrict__ shift,
+                                 const double* __restrict__ p, double* __restrict__ q, double cM, Scalars* sc) {
+  double acc = 0.0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const double pi = p[i];
+    const double qi = fma(shift[i], pi, cM * yacc[i]);
+    q[i] = qi;
+    acc = fma(pi, qi, acc);
+  }
+  block_atomic_sum(acc, &sc->pq);
+}
+
+__global__ void residual_kernel(int n, const double* __restrict__ yacc, const double* __restrict__ shift,
+                                const double* __restrict__ x, const double* __restrict__ b, double* __restrict__ r,
+                                double cM) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+    r[i] = fma(shift[i], x[i], cM * yacc[i]) - b[i];
+}
+
+__global__ void update_xr_kernel(int n, int par, const double* __restrict__ p, const double* __restrict__ q,
+                                 double* __restrict__ x, double* __restrict__ r, const Scalars* sc) {
+  const double alpha = sc->rg[par] / sc->pq;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    x[i] = fma(alpha, p[i], x[i]);
+    r[i] = fma(alpha, q[i], r[i]);
+  }
+}
+
+// one warp per turn: CSR gather of the turn's cells
+__global__ void turn_project_kernel(int n_turns, const int* __restrict__ ptr, const int* __restrict__ idx,
+                                    const double* __restrict__ r, const double* __restrict__ Hd,
+                                    const double* __restrict__ sw, double* __restrict__ vw, double* __restrict__ vsum) {
+  const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (w >= n_turns) return;
+  double acc = 0.0;
+  for (int k = ptr[w] + lane; k < ptr[w + 1]; k += 32) {
+    const int i = idx[k];
+    acc += r[i] / Hd[i];
+  }
+  acc = warp_sum(acc);
+  if (lane == 0) {
+    const double v = acc / sw[w];
+    vw[w] = v;
+    if (vsum) vsum[w] += v;
+  }
+}
+
+__global__ void turn_schur_kernel(int n_turns, const int* __restrict__ ptr, const int* __restrict__ idx,
+                                  const double* __restrict__ Hd, double* __restrict__ sw) {
+  const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (w >= n_turns) return;
+  double acc = 0.0;
+  for (int k = ptr[w] + lane; k < ptr[w + 1]; k += 32) acc += 1.0 / Hd[idx[k]];
+  acc = warp_sum(acc);
+  if (lane == 0) sw[w] = acc;
+}
+
+__global__ void turn_deficit_kernel(int n_turns, const int* __restrict__ ptr, const int* __restrict__ idx,
+                                    const double* __restrict__ x, double d, double* __restrict__ defw, Scalars* sc) {
+  const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (w >= n_turns) return;
+  double acc = 0.0;
+  for (int k = ptr[w] + lane; k < ptr[w + 1]; k += 32) acc += x[idx[k]];
+  acc = warp_sum(acc);
+  if (lane == 0) defw[w] = d - acc;
+}
+
+__global__ void apply_deficit_kernel(int n, const int* __restrict__ turn, const double* __restrict__ defw,
+                                     const double* __restrict__ Hd, const double* __restrict__ sw,
+                                     double* __restrict__ x) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const int w = turn[i];
+    x[i] += defw[w] / (Hd[i] * sw[w]);
+  }
+}
+
+__global__ void project_apply_kernel(int n, int par, const int* __restrict__ turn, const double* __restrict__ vw,
+                                     const double* __restrict__ Hd, double* __restrict__ r, double* __restrict__ g,
+                                     Scalars* sc) {
+  double acc = 0.0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    double ri = r[i];
+    if (turn) {
+      ri -= vw[turn[i]];
+      r[i] = ri;
+    }
+    const double gi = ri / Hd[i];
+    g[i] = gi;
+    acc = fma(ri, gi, acc);
+  }
+  block_atomic_sum(acc, &sc->rg[par]);
+}
+
+__global__ void direction_kernel(int n, int par, int first, const double* __restrict__ g, double* __restrict__ p,
+                                 Scalars* sc) {
+  const double beta = first ? 0.0 : sc->rg[par] / sc->rg[par ^ 1];
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+    p[i] = first ? -g[i] : fma(beta, p[i], -g[i]);
+}
+// runs after direction_kernel (stream order): the scalars of the finished iteration are no longer needed
+__global__ void recycle_scalars_kernel(int par, Scalars* sc) {
+  sc->rg[par ^ 1] = 0.0;
+  sc->pq = 0.0;
+}
+
+__global__ void axpy_kernel(int n, double a, const double* __restrict__ x, double* __restrict__ y) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) y[i] = fma(a, x[i], y[i]);
+}
+__global__ void scale_div_kernel(int n, double a, const double* __restrict__ x, const double* __restrict__ d,
+                                 double* __restrict__ y) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) y[i] += a * x[i] / d[i];
+}
+__global__ void mul_kernel(int n, const double* __restrict__ a, const double* __restrict__ b, double* __restrict__ y) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) y[i] = a[i] * b[i];
+}
+__global__ void set_scalars_kernel(Scalars* sc) {
+  sc->rg[0] = sc->rg[1] = sc->pq = sc->nu2 = 0.0;
+  sc->uterm = sc->joule = 0.0;
+  sc->tmax = 0.0;
+  sc->nonfinite = 0;
+  sc->event_or = 0;
+}
+__global__ void copy_rg_to_nu2_kernel(int par, Scalars* sc) {
+  sc->nu2 = sc->rg[par];
+  sc->rg[par] = 0.0;
+}
+__global__ void nu_residual_kernel(int n, double I_ramp, const double* __restrict__ Mxp1,
+                                   const double* __restrict__ shift, const double* __restrict__ xp1,
+                                   const double* __restrict__ b, double* __restrict__ r) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+    r[i] = I_ramp * fma(shift[i], xp1[i], Mxp1[i]) - b[i];
+}
+__global__ void sum_uterm_kernel(int n, const double* __restrict__ vsum, Scalars* sc) {
+  double acc = 0.0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) acc += vsum[i];
+  block_atomic_sum(acc, &sc->uterm);
+}
+__global__ void gather_kernel(int n, int npad, const double* __restrict__ src, const int* __restrict__ perm,
+                              double* __restrict__ dst) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < npad; i += gridDim.x * blockDim.x)
+    dst[i] = i < n ? src[perm ? perm[i] : i] : 0.0;
+}
+__global__ void scatter_scaled_kernel(int n, const double* __restrict__ src, const int* __restrict__ perm,
+                                      double* __restrict__ dst, double scale) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+    dst[perm ? perm[i] : i] = scale * src[i];
+}
+}  // namespace
+
+#define QS_LAUNCH(v) (++*(v).launches)
+
+void k_finish_Ap(const VecCtx& v, const double* yacc, const double* shift, const double* p, double* q, double cM) {
+  QS_LAUNCH(v);
+  finish_Ap_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, yacc, shift, p, q, cM, v.sc);
+}
+void k_residual(const VecCtx& v, const double* yacc, const double* shift, const double* x, const double* b, double* r,
+                double cM) {
+  QS_LAUNCH(v);
+  residual_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, yacc, shift, x, b, r, cM);
+}
+void k_update_xr(const VecCtx& v, int par, const double* p, const double* q, double* x, double* r) {
+  QS_LAUNCH(v);
+  update_xr_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, par, p, q, x, r, v.sc);
+}
+void k_turn_project(const VecCtx& v, const double* r, const double* Hd, const double* sw, double* vw, double* vsum) {
+  if (!v.n_turns) return;
+  QS_LAUNCH(v);
+  turn_project_kernel<<<(v.n_turns * 32 + kBlock - 1) / kBlock, kBlock, 0, v.stream>>>(v.n_turns, v.turn_ptr,
+                                                                                      v.turn_idx, r, Hd, sw, vw, vsum);
+}
+void k_turn_schur(const VecCtx& v, const double* Hd, double* sw) {
+  if (!v.n_turns) return;
+  QS_LAUNCH(v);
+  turn_schur_kernel<<<(v.n_turns * 32 + kBlock - 1) / kBlock, kBlock, 0, v.stream>>>(v.n_turns, v.turn_ptr, v.turn_idx,
+                                                                                    Hd, sw);
+}
+void k_turn_deficit(const VecCtx& v, const double* x, double d, double* defw) {
+  if (!v.n_turns) return;
+  QS_LAUNCH(v);
+  turn_deficit_kernel<<<(v.n_turns * 32 + kBlock - 1) / kBlock, kBlock, 0, v.stream>>>(v.n_turns, v.turn_ptr,
+                                                                                      v.turn_idx, x, d, defw, v.sc);
+}
+void k_apply_deficit(const VecCtx& v, const double* defw, const double* Hd, const double* sw, double* x) {
+  if (!v.n_turns) return;
+  QS_LAUNCH(v);
+  apply_deficit_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, v.turn_id, defw, Hd, sw, x);
+}
+void k_project_apply(const VecCtx& v, int par, const double* vw, const double* Hd, double* r, double* g) {
+  QS_LAUNCH(v);
+  project_apply_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, par, v.n_turns ? v.turn_id : nullptr, vw, Hd, r, g,
+                                                              v.sc);
+}
+void k_direction(const VecCtx& v, int par, bool first, const double* g, double* p) {
+  QS_LAUNCH(v);
+  direction_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, par, first ? 1 : 0, g, p, v.sc);
+  QS_LAUNCH(v);
+  recycle_scalars_kernel<<<1, 1, 0, v.stream>>>(par, v.sc);
+}
+void k_axpy(const VecCtx& v, double a, const double* x, double* y) {
+  QS_LAUNCH(v);
+  axpy_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, a, x, y);
+}
+void k_scale_div(const VecCtx& v, double a, const double* x, const double* d, double* y) {
+  QS_LAUNCH(v);
+  scale_div_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, a, x, d, y);
+}
+void k_mul(const VecCtx& v, const double* a, const double* b, double* y) {
+  QS_LAUNCH(v);
+  mul_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, a, b, y);
+}
+void k_set_scalars(const VecCtx& v) {
+  QS_LAUNCH(v);
+  set_scalars_kernel<<<1, 1, 0, v.stream>>>(v.sc);
+}
+void k_copy_rg_to_nu2(const VecCtx& v, int par) {
+  QS_LAUNCH(v);
+  copy_rg_to_nu2_kernel<<<1, 1, 0, v.stream>>>(par, v.sc);
+}
+void k_nu_residual(const VecCtx& v, double I_ramp, const double* Mxp1, const double* shift, const double* xp1,
+                   const double* b, double* r) {
+  QS_LAUNCH(v);
+  nu_residual_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, I_ramp, Mxp1, shift, xp1, b, r);
+}
+void k_sum_uterm(const VecCtx& v, const double* vsum) {
+  if (!v.n_turns) return;
+  QS_LAUNCH(v);
+  sum_uterm_kernel<<<1, kBlock, 0, v.stream>>>(v.n_turns, vsum, v.sc);
+}
+void k_gather(const VecCtx& v, const double* src, const int* perm, double* dst, int n, int npad) {
+  QS_LAUNCH(v);
+  gather_kernel<<<grid_for(npad), kBlock, 0, v.stream>>>(n, npad, src, perm, dst);
+}
+void k_scatter_scaled(const VecCtx& v, const double* src, const int* perm, double* dst, int n, double scale) {
+  QS_LAUNCH(v);
+  scatter_scaled_kernel<<<grid_for(n), kBlock, 0, v.stream>>>(n, src, perm, dst, scale);
+}
+
+}  // namespace qs

@@ -1,0 +1,210 @@
+"""GPU parity of the pair operator K1/K2, the CG solve and the pointwise passes against the CPU oracle.
+
+All calls go through the C ABI (paper_2403_07666_b200.QS -> libqs.so).  Tolerances: north_star
+(rel-L2 <= 1e-9 for the G matvec); the pointwise passes are compared far tighter (same formulas in FP64,
+differences come from FMA contraction and libm-vs-CUDA pow only).
+"""
+import dataclasses
+import math
+
+import numpy as np
+import pytest
+
+import workloads as wl
+from oracle import qs_oracle as qo
+
+pytestmark = pytest.mark.gpu
+
+
+def rel(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import paper_2403_07666_b200 as p
+    return p
+
+
+@pytest.mark.parametrize("n", [1, 31, 33, 1000, 4096])
+def test_matvec_free_rings_full(pkg, n):
+    geo, x = wl.free_rings(n, seed=4000 + n)
+    with pkg.QS(geo, wl.Material()) as sim:
+        y = sim.matvec(x)
+        st = sim.stats()
+    yo = qo.matvec(geo, x)
+    assert rel(y, yo) <= 1e-9
+    assert np.max(np.abs(y - yo)) <= 1e-9 * np.max(np.abs(yo))
+    nb = (n + 31) // 32
+    assert st["pair_evals"] >= nb * (nb + 1) // 2 * 1024 and st["launches"] > 0
+
+
+@pytest.mark.parametrize("n,rows", [(65536, 256), (262144, 128), (1048576, 64)])
+def test_matvec_free_rings_sampled_rows(pkg, n, rows):
+    # BASELINE.json configs[4] sizes; the oracle evaluates exact rows sum_j M_ij x_j on a seeded row sample
+    geo, x = wl.free_rings(n)
+    idx = wl.sample_rows(n, rows, seed=n)
+    with pkg.QS(geo, wl.Material()) as sim:
+        y = sim.matvec(x)
+    yo = qo.matvec_rows(geo, x, idx, chunk=16)
+    assert rel(y[idx], yo) <= 1e-9
+    assert np.all(np.isfinite(y))
+
+
+def test_matvec_device_variant_and_symmetry(pkg):
+    import torch
+    geo, x = wl.free_rings(2048)
+    g = np.random.default_rng(11)
+    w = g.standard_normal(2048)
+    with pkg.QS(geo, wl.Material()) as sim:
+        y = sim.matvec(x)
+        with torch.cuda.stream(sim.stream):
+            xd = torch.from_numpy(x).to(sim.device)
+            yd = torch.empty_like(xd)
+        sim.stream.synchronize()
+        sim.matvec_device(xd, yd)
+        sim.sync()
+        assert rel(yd.cpu().numpy(), y) <= 1e-13
+        Mw = sim.matvec(w)
+    # x^T M w == w^T M x (one evaluation per unordered pair makes this exact up to summation order); SPD
+    assert abs(x @ Mw - w @ y) <= 1e-12 * abs(w @ y)
+    assert x @ y > 0 and w @ Mw > 0
+
+
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_matvec_and_field_lattice_configs(pkg, cfg):
+    w = wl.config(cfg)
+    geo = w.geometry
+    g = np.random.default_rng(20 + cfg)
+    x = g.standard_normal(geo.n_rings)
+    with pkg.QS(geo, w.material) as sim:
+        y = sim.matvec(x)
+        B = sim.field(x)
+    M = qo.dense_M(geo)
+    assert rel(y, M @ x) <= 1e-9
+    del M
+    GBr, GBz = qo.dense_GB(geo)
+    N = geo.n_rings
+    assert rel(B[:N], GBr @ x) <= 1e-9 and rel(B[N:], GBz @ x) <= 1e-9
+
+
+def test_matvec_ragged_lattice(pkg):
+    # Nz = 18 is not a multiple of 32: blocks straddle rows, last block is padded (N = 12*18 = 216)
+    geo = wl.lattice_geometry(2, 3, 6, 0.9e-3, 35e-3)
+    x = np.random.default_rng(3).standard_normal(geo.n_rings)
+    with pkg.QS(geo, wl.Material()) as sim:
+        y, B = sim.matvec(x), sim.field(x)
+    GBr, GBz = qo.dense_GB(geo)
+    assert rel(y, qo.dense_M(geo) @ x) <= 1e-9
+    assert rel(B[:216], GBr @ x) <= 1e-9 and rel(B[216:], GBz @ x) <= 1e-9
+
+
+@pytest.mark.parametrize("cfg,rows", [(2, 96), (3, 32)])
+def test_matvec_full_size_coils_sampled_rows(pkg, cfg, rows):
+    w = wl.config(cfg)
+    geo = w.geometry
+    x = np.random.default_rng(30 + cfg).standard_normal(geo.n_rings)
+    idx = wl.sample_rows(geo.n_rings, rows, seed=cfg)
+    with pkg.QS(geo, w.material) as sim:
+        y = sim.matvec(x)
+    assert rel(y[idx], qo.matvec_rows(geo, x, idx, chunk=16)) <= 1e-9
+
+
+def test_solve_free_rings_and_constrained_lattice(pkg):
+    geo, x = wl.free_rings(1024)
+    mat = wl.Material(cg_tol=1e-10, cg_maxit=20000)
+    M = qo.dense_M(geo)
+    b = M @ x
+    with pkg.QS(geo, mat) as sim:
+        xs, it, relres, rc = sim.solve(b)
+    assert rc == 0 and 0 < it < 20000 and relres <= 1e-10
+    assert rel(M @ xs, b) <= 1e-8
+    xd = np.linalg.solve(M, b)
+    assert rel(xs, xd) <= 1e-4                                   # cond(M) ~ 1e6
+    # lattice with turns: M x + C V = b, C^T x = 0 against the dense KKT solve
+    geo = wl.lattice_geometry(2, 2, 8, 1e-3, 30e-3)
+    b = np.random.default_rng(5).standard_normal(geo.n_rings) * 1e-6
+    xk, _ = qo.kkt_dense(qo.dense_M(geo), qo.constraint_matrix(geo), b, np.zeros(geo.n_turns))
+    with pkg.QS(geo, wl.Material(cg_tol=1e-12)) as sim:
+        xs, it, relres, rc = sim.solve(b)
+    assert rc == 0 and rel(xs, xk) <= 1e-8
+    assert np.max(np.abs(np.bincount(geo.turn_id, weights=xs))) <= 1e-10 * np.max(np.abs(xs)) * 64
+
+
+def test_solve_maxit_is_reported(pkg):
+    geo, x = wl.free_rings(512)
+    with pkg.QS(geo, wl.Material(cg_tol=1e-14)) as sim:
+        _, it, relres, rc = sim.solve(sim.matvec(x), maxit=5)
+    assert rc == 4 and it == 5 and relres > 1e-14
+
+
+def test_material_law_pointwise(pkg):
+    w = wl.shrunk(0, 3, 2, 8)
+    geo, mat = w.geometry, w.material
+    N = geo.n_rings
+    g = np.random.default_rng(8)
+    Jc0 = 2e9 * (1 - 4.2 / 18) ** 2
+    J = Jc0 * g.uniform(-1.3, 1.3, N)
+    J[:7] = 0.0
+    J[7:12] = 1e3 * Jc0                                          # deep normal state / overflow guard
+    T = g.uniform(4.2, 17.0, N)
+    T[20:30] = 19.0                                              # above Tc
+    B = np.concatenate([g.uniform(-2, 2, N), g.uniform(-12, 12, N)])
+    dt = 1e-4
+    with pkg.QS(geo, mat) as sim:
+        sim.write(J, T, 0.0, 0.0)
+        sim.set_fields(B=B)
+        sim.material_eval(dt)
+        _, Tg, Bg, E = sim.read()
+        aux = sim.read_aux()
+    ml = qo.material_law(mat, J, T, B[:N], B[N:], geo.r, mat.jc0_scale)
+    assert np.max(np.abs(Tg - T)) <= 1e-13 * 19 and np.array_equal(Bg, B)
+    assert np.any(ml["Jc"] == 0.0) and np.any(ml["rho"] == mat.rho_n) and np.any(ml["rho"] == 0.0)
+    for key, got in [("E", E), ("Q", aux["Q"]), ("dEdJ", aux["dEdJ"]), ("Jc", aux["Jc"]), ("rho", aux["rho"])]:
+        ref = ml[key]
+        assert np.max(np.abs(got - ref)) <= 1e-11 * np.max(np.abs(ref)), key
+        assert rel(got, ref) <= 1e-12, key
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 8), (3, 2, 4), (2, 5, 13), (5, 3, 24)])
+def test_heat_substeps_pointwise(pkg, shape):
+    L, Tn, n = shape
+    geo = wl.lattice_geometry(L, Tn, n, 1e-3, 30e-3)
+    geo = dataclasses.replace(geo, h_conv=(500.0, 300.0, 200.0, 100.0))
+    mat = wl.Material()
+    N = geo.n_rings
+    g = np.random.default_rng(9)
+    T = g.uniform(4.2, 12.0, N)
+    Q = g.uniform(0, 5e6, N)
+    dt = 1e-4
+    with pkg.QS(geo, mat, no_operator=True) as sim:
+        sim.write(np.zeros(N), T, 0.0, 0.0)
+        sim.set_fields(Q=Q)
+        m = sim.heat(dt)
+        _, Tg, _, _ = sim.read(J=False, B=False, E=False)
+    mo = qo.heat_substeps_count(geo, mat, dt)
+    Ho, _ = qo.heat_substeps(geo, mat, qo.enthalpy(mat, T), Q, dt, mo)
+    assert m == mo
+    assert np.max(np.abs(Tg - qo.temperature(mat, Ho))) <= 1e-12 * 12.0
+
+
+def test_errors_and_no_operator_mode(pkg):
+    geo, x = wl.free_rings(64)
+    with pkg.QS(geo, wl.Material()) as sim:
+        with pytest.raises(pkg.QsError) as e:
+            sim.step(1e-4, 0.0)                                  # free rings cannot step
+        assert e.value.code == -1
+    w = wl.shrunk(0, 1, 1, 4)
+    with pkg.QS(w.geometry, w.material) as sim:
+        with pytest.raises(pkg.QsError) as e:
+            sim.step(0.0, 1.0)
+        assert e.value.code == -5
+    with pkg.QS(w.geometry, w.material, no_operator=True) as sim:
+        with pytest.raises(pkg.QsError):
+            sim.matvec(np.ones(16))
+    bad = dataclasses.replace(w.geometry, r=w.geometry.r[::-1].copy())
+    with pytest.raises(pkg.QsError):
+        pkg.QS(bad, w.material)                                  # r/z arrays contradict the lattice description
+    with pkg.QS(w.geometry, w.material, torch_memory=False) as sim:   # plain-C path: cudaMalloc + own stream
+        y = sim.matvec(np.ones(16))
+    assert rel(y, qo.dense_M(w.geometry) @ np.ones(16)) <= 1e-9

@@ -137,7 +137,8 @@ int  qs_init_device(const qs_geometry *geo, const qs_material *mat, void *worksp
                     size_t workspace_bytes, void *stream, qs_ctx **out);
 
 /* Set the state (resume, prepared variants C12).  NULL J or T keeps the current array.  Resets the
- * warm start and the dE/dt history.  */
+ * dE/dt history of the event detector; the previous I' is kept as the CG's initial guess (the
+ * solution of the step does not depend on it beyond cg_tol).  */
 int  qs_write(qs_ctx *ctx, const double *J, const double *T, double t, double I);
 
 /* y = M x (C2): x [A] -> y [Wb], symmetric mutual-inductance matrix, evaluated pair by pair.  */
@@ -161,6 +162,32 @@ int  qs_set_fields(qs_ctx *ctx, const double *B, const double *Q);
 int  qs_read_aux(qs_ctx *ctx, double *Q, double *dEdJ, double *Jc, double *rho);
 
 int  qs_stats(qs_ctx *ctx, qs_stats_t *out);
+
+/* ---- measurement (bench.py) ---------------------------------------------------
+ * Device-side timing of the library's own kernels with cudaEvent pairs recorded on the handle's
+ * stream around the launches of each kernel class.  Off by default (no events are recorded).
+ * qs_profile_read waits for the stream, writes the totals accumulated since the last read (or since
+ * qs_profile_enable) and resets them.  ms[k] = summed launch durations of class k, launches[k] =
+ * kernels launched in class k.  A class that launches m kernels back to back (the heat sub-steps of
+ * one step) is bracketed once and counts m launches.  */
+#define QS_PROF_SWEEP_M      0   /* K1: y = M x pair sweep                                          */
+#define QS_PROF_SWEEP_FIELD  1   /* K2: fused M x + Br, Bz pair sweep                               */
+#define QS_PROF_MATERIAL     2   /* K5                                                              */
+#define QS_PROF_HEAT         3   /* K6 (all sub-steps of a step)                                    */
+#define QS_PROF_EVENTS       4   /* K7 + step statistics                                            */
+#define QS_PROF_CG_VECTOR    5   /* K3/K4 kernels of one projected-CG iteration                     */
+#define QS_PROF_CLASSES      8
+typedef struct {
+  double  ms[QS_PROF_CLASSES];
+  int64_t launches[QS_PROF_CLASSES];
+} qs_profile_t;
+int  qs_profile_enable(qs_ctx *ctx, int32_t on);
+int  qs_profile_read(qs_ctx *ctx, qs_profile_t *out);
+
+/* FP64 FMA throughput of the current device [TFLOP/s, FMA = 2 flop]: 16 independent DFMA chains per
+ * thread on every SM, timed with CUDA events (best of 5).  The denominator of the operator's
+ * roofline ("bound": "alu"); needs no handle.  Returns 0 or QS_ERR_CUDA.  */
+int  qs_fp64_peak(double *tflops, double *sm_clock_mhz_effective);
 int  qs_events(qs_ctx *ctx, int32_t *flags /*[N_w]*/, double *t_first /*[N_w]*/, int32_t *count /*[N_w]*/);
 int  qs_sync(qs_ctx *ctx);                 /* wait for the handle's stream */
 const char *qs_last_error(void);

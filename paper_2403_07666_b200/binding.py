@@ -45,6 +45,12 @@ class QsStats(C.Structure):
                 ("launches", C.c_int64), ("pair_evals", C.c_int64)]
 
 
+class QsProfile(C.Structure):
+    _fields_ = [("ms", C.c_double * 8), ("launches", C.c_int64 * 8)]
+
+
+PROFILE_CLASSES = ["sweep_M", "sweep_field", "material", "heat", "events", "cg_vector"]
+
 # every symbol include/qs.h declares: (name, restype, argtypes)
 _VP = C.c_void_p
 SYMBOLS = [
@@ -64,6 +70,9 @@ SYMBOLS = [
     ("qs_set_fields", C.c_int, [_VP, c_double_p, c_double_p]),
     ("qs_read_aux", C.c_int, [_VP, c_double_p, c_double_p, c_double_p, c_double_p]),
     ("qs_stats", C.c_int, [_VP, C.POINTER(QsStats)]),
+    ("qs_profile_enable", C.c_int, [_VP, C.c_int32]),
+    ("qs_profile_read", C.c_int, [_VP, C.POINTER(QsProfile)]),
+    ("qs_fp64_peak", C.c_int, [c_double_p, c_double_p]),
     ("qs_events", C.c_int, [_VP, c_int32_p, c_double_p, c_int32_p]),
     ("qs_sync", C.c_int, [_VP]),
     ("qs_last_error", C.c_char_p, []),
@@ -104,6 +113,16 @@ def _f64(a, n=None) -> np.ndarray:
     if n is not None and out.size != n:
         raise ValueError(f"expected {n} elements, got {out.size}")
     return out
+
+
+def fp64_peak():
+    """(TFLOP/s, effective SM MHz) of the DFMA probe kernel on the current CUDA device."""
+    lib = load_library()
+    tf, mhz = C.c_double(0.0), C.c_double(0.0)
+    rc = lib.qs_fp64_peak(C.byref(tf), C.byref(mhz))
+    if rc < 0:
+        raise QsError(rc, lib.qs_last_error().decode())
+    return tf.value, mhz.value
 
 
 class QS:
@@ -257,6 +276,15 @@ class QS:
         s = QsStats()
         self._check(self._lib.qs_stats(self._h, C.byref(s)))
         return {name: getattr(s, name) for name, _ in QsStats._fields_}
+
+    def profile_enable(self, on: bool = True):
+        self._check(self._lib.qs_profile_enable(self._h, 1 if on else 0))
+
+    def profile_read(self) -> dict:
+        """{class name: (summed ms, launches)} since the last read; resets the totals."""
+        p = QsProfile()
+        self._check(self._lib.qs_profile_read(self._h, C.byref(p)))
+        return {name: (p.ms[k], int(p.launches[k])) for k, name in enumerate(PROFILE_CLASSES)}
 
     def events(self):
         nt = max(self.n_turns, 0)

@@ -48,7 +48,61 @@ struct Carver {
 
 }  // namespace
 
+// cudaEvent pairs around kernel classes (qs_profile_*): recorded only while enabled
+struct Profiler {
+  struct Rec { int cls; int n; cudaEvent_t a, b; };
+  bool on = false;
+  std::vector<Rec> pending;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> pool;
+  double ms[QS_PROF_CLASSES] = {};
+  long long launches[QS_PROF_CLASSES] = {};
+  cudaEvent_t cur_a = nullptr, cur_b = nullptr;
+  void begin(cudaStream_t st) {
+    if (!on) return;
+    if (pool.empty()) {
+      cudaEvent_t a, b;
+      cudaEventCreate(&a);
+      cudaEventCreate(&b);
+      pool.emplace_back(a, b);
+    }
+    cur_a = pool.back().first;
+    cur_b = pool.back().second;
+    pool.pop_back();
+    cudaEventRecord(cur_a, st);
+  }
+  void end(cudaStream_t st, int cls, int n) {
+    if (!on) return;
+    cudaEventRecord(cur_b, st);
+    pending.push_back({cls, n, cur_a, cur_b});
+    if (pending.size() >= 4096) fold(st);
+  }
+  void fold(cudaStream_t st) {
+    if (pending.empty()) return;
+    cudaStreamSynchronize(st);
+    for (const Rec& r : pending) {
+      float t = 0.f;
+      if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess) ms[r.cls] += t;
+      launches[r.cls] += r.n;
+      pool.emplace_back(r.a, r.b);
+    }
+    pending.clear();
+  }
+  void reset() {
+    for (int k = 0; k < QS_PROF_CLASSES; ++k) ms[k] = 0.0, launches[k] = 0;
+  }
+  void destroy() {
+    for (const Rec& r : pending) pool.emplace_back(r.a, r.b);
+    pending.clear();
+    for (auto& e : pool) {
+      cudaEventDestroy(e.first);
+      cudaEventDestroy(e.second);
+    }
+    pool.clear();
+  }
+};
+
 struct qs_ctx {
+  Profiler prof;
   // problem
   int N = 0, Np = 0, nb = 0, n_turns = 0;
   bool lattice = false, has_operator = true;
@@ -193,7 +247,9 @@ int do_sweep(qs_ctx* c, const double* x, const double* cur, bool field) {
   if (need < grid) grid = static_cast<int>(need);
   const long long warps = static_cast<long long>(grid) * wpc;
   prm.chunk = static_cast<int>(std::max<long long>(1, std::min<long long>(32, prm.n_items / (warps * 8))));
+  c->prof.begin(c->stream);
   QS_CUDA(launch_sweep(prm, field, grid, c->stream));
+  c->prof.end(c->stream, field ? QS_PROF_SWEEP_FIELD : QS_PROF_SWEEP_M, 1);
   ++c->launches;
   c->pair_evals += prm.n_items * 1024;
   ++c->st.sweeps;
@@ -228,12 +284,14 @@ int cg_core(qs_ctx* c, const double* b, double* x, const double* shift, const do
       break;
     }
     if ((rc = do_sweep(c, c->p, nullptr, false)) != QS_OK) return rc;
+    c->prof.begin(c->stream);
     k_finish_Ap(v, c->yacc, shift, c->p, c->q, kCM);
     k_update_xr(v, par, c->p, c->q, x, c->rr);
     k_turn_project(v, c->rr, Hd, sw, c->vw, c->vsum);
     k_project_apply(v, par ^ 1, c->vw, Hd, c->rr, c->g);
     QS_CUDA(cudaMemcpyAsync(c->h_sc, c->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, c->stream));
     k_direction(v, par ^ 1, false, c->g, c->p);
+    c->prof.end(c->stream, QS_PROF_CG_VECTOR, c->n_turns ? 6 : 5);
     QS_CUDA(cudaStreamSynchronize(c->stream));
     if (!(c->h_sc->pq > 0.0)) return fail(QS_ERR_CG, "CG breakdown: p^T A p <= 0");
     par ^= 1;
@@ -259,10 +317,12 @@ int heat_substeps_count(const qs_ctx* c, double dt) {
 int run_heat(qs_ctx* c, double dt, int* m_out) {
   const int m = heat_substeps_count(c, dt);
   const double sub = dt / m;
+  c->prof.begin(c->stream);
   for (int s = 0; s < m; ++s) {
     k_heat_substep(c->v, c->mp, c->lp, c->H, c->Q, c->Halt, sub);
     std::swap(c->H, c->Halt);
   }
+  c->prof.end(c->stream, QS_PROF_HEAT, m);
   *m_out = m;
   QS_CUDA(cudaGetLastError());
   return QS_OK;
@@ -566,6 +626,7 @@ int qs_init_device(const qs_geometry* geo, const qs_material* mat, void* workspa
 void qs_free(qs_ctx* c) {
   if (!c) return;
   if (c->stream) cudaStreamSynchronize(c->stream);
+  c->prof.destroy();
   if (c->h_sc) cudaFreeHost(c->h_sc);
   if (c->h_stage) cudaFreeHost(c->h_stage);
   if (c->owned) {
@@ -603,7 +664,9 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
   if ((rc = do_sweep(c, c->x, c->cur, true)) != QS_OK) return rc;
   // S2
   const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
+  c->prof.begin(c->stream);
   k_material(v, c->mp, material_args(c, B0, (B1 - B0) / dt, dt, true));
+  c->prof.end(c->stream, QS_PROF_MATERIAL, 1);
   // S3/S4
   double nu = -1.0;
   if (c->n_turns) {
@@ -647,8 +710,10 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
   ev.H = c->H; ev.E = c->E; ev.J = c->Jold; ev.Jc = c->Jc; ev.rho = c->rho;
   ev.ebar_prev = c->ebar_prev; ev.flags = c->flags; ev.t_first = c->t_first; ev.count = c->count;
   ev.dt = dt; ev.t_new = c->t + dt; ev.have_prev = c->have_prev_E;
+  c->prof.begin(c->stream);
   k_events(v, c->mp, ev);
   k_step_stats(v, c->mp, c->J, c->H, c->Q, c->r, c->area);
+  c->prof.end(c->stream, QS_PROF_EVENTS, c->n_turns ? 2 : 1);
   if ((rc = sync_scalars(c)) != QS_OK) return rc;
   if (c->h_sc->nonfinite) {
     cudaMemcpyAsync(c->J, c->Jold, nb8, cudaMemcpyDeviceToDevice, c->stream);
@@ -708,7 +773,7 @@ int qs_write(qs_ctx* c, const double* J, const double* T, double t, double I) {
     if ((rc = upload(c, T, c->tmp, c->N)) != QS_OK) return rc;
     k_enthalpy_from_T(c->v, c->mp, c->tmp, c->H, c->N);
   }
-  QS_CUDA(cudaMemsetAsync(c->x, 0, sizeof(double) * c->Np, c->stream));
+  // the previous I' stays as the CG's initial guess (a guess only: the solution does not depend on it)
   QS_CUDA(cudaStreamSynchronize(c->stream));
   c->t = t;
   c->I = I;
@@ -811,7 +876,9 @@ int qs_set_fields(qs_ctx* c, const double* B, const double* Q) {
 int qs_material_eval(qs_ctx* c, double dt) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
   const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
+  c->prof.begin(c->stream);
   k_material(c->v, c->mp, material_args(c, B0, dt > 0 ? (B1 - B0) / dt : 0.0, dt, false));
+  c->prof.end(c->stream, QS_PROF_MATERIAL, 1);
   QS_CUDA(cudaGetLastError());
   return QS_OK;
 }
@@ -832,6 +899,36 @@ int qs_stats(qs_ctx* c, qs_stats_t* out) {
   out->pair_evals = c->pair_evals;
   out->t = c->t;
   out->I = c->I;
+  return QS_OK;
+}
+
+int qs_profile_enable(qs_ctx* c, int32_t on) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  c->prof.fold(c->stream);
+  c->prof.reset();
+  c->prof.on = on != 0;
+  return QS_OK;
+}
+
+int qs_profile_read(qs_ctx* c, qs_profile_t* out) {
+  if (!c || !out) return fail(QS_ERR_ARG, "NULL argument");
+  QS_CUDA(cudaStreamSynchronize(c->stream));
+  c->prof.fold(c->stream);
+  for (int k = 0; k < QS_PROF_CLASSES; ++k) {
+    out->ms[k] = c->prof.ms[k];
+    out->launches[k] = c->prof.launches[k];
+  }
+  c->prof.reset();
+  return QS_OK;
+}
+
+int qs_fp64_peak(double* tflops, double* sm_clock_mhz_effective) {
+  if (!tflops) return fail(QS_ERR_ARG, "NULL argument");
+  double tf = 0.0, mhz = 0.0;
+  const cudaError_t e = fp64_peak_probe(&tf, &mhz);
+  if (e != cudaSuccess) return fail(QS_ERR_CUDA, std::string("fp64 probe: ") + cudaGetErrorString(e));
+  *tflops = tf;
+  if (sm_clock_mhz_effective) *sm_clock_mhz_effective = mhz;
   return QS_OK;
 }
 

@@ -33,6 +33,9 @@ cudaError_t launch_sweep(const SweepParams& prm, bool field, int grid, cudaStrea
 // diagM_i = M(r_i, r_i, dz^2 = d2self) in henry
 cudaError_t launch_diag(int n, const double* r, double d2self, double* diagM, cudaStream_t stream);
 
+// FP64 FMA throughput probe (qs_operator.cu): TFLOP/s and the SM clock seen by the kernel
+cudaError_t fp64_peak_probe(double* tflops, double* sm_mhz);
+
 // ---- vector / CG kernels (qs_vector.cu) -------------------------------------------------------
 // Device scalars of the solver; all reductions land here (no host round trip inside an iteration).
 struct Scalars {

@@ -282,6 +282,63 @@ cudaError_t launch_diag(int n, const double* r, double d2self, double* diagM, cu
   return cudaGetLastError();
 }
 
+// ---- FP64 FMA roofline probe: 16 independent chains per thread, 1024 threads x 2 CTAs per SM ----------------
+__global__ void __launch_bounds__(512) dfma_probe_kernel(int iters, double seed, double* sink, long long* cycles) {
+  double a[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) a[k] = seed + 1e-3 * (threadIdx.x + k);
+  const double m = 1.0 - 1e-9 * seed, c = 1e-9;
+  const long long t0 = clock64();
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int k = 0; k < 16; ++k) a[k] = fma(a[k], m, c);
+  }
+  const long long t1 = clock64();
+  double s = 0.0;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) s += a[k];
+  if (s == 123.456) sink[0] = s;   // keeps the chains alive
+  if (threadIdx.x == 0 && blockIdx.x == 0) cycles[0] = t1 - t0;
+}
+
+cudaError_t fp64_peak_probe(double* tflops, double* sm_mhz) {
+  int dev = 0, sms = 0;
+  cudaError_t e;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  double* sink = nullptr;
+  long long* cyc = nullptr;
+  if ((e = cudaMalloc(&sink, 64)) != cudaSuccess) return e;
+  cyc = reinterpret_cast<long long*>(sink + 1);
+  cudaEvent_t a, b;
+  cudaEventCreate(&a);
+  cudaEventCreate(&b);
+  const int iters = 20000, grid = sms * 4, threads = 512;
+  double best_ms = 1e300, best_mhz = 0.0;
+  for (int rep = 0; rep < 6; ++rep) {
+    cudaEventRecord(a, 0);
+    dfma_probe_kernel<<<grid, threads>>>(iters, 1.0 + rep, sink, cyc);
+    cudaEventRecord(b, 0);
+    if ((e = cudaEventSynchronize(b)) != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    long long hc = 0;
+    cudaMemcpy(&hc, cyc, sizeof(hc), cudaMemcpyDeviceToHost);
+    if (rep > 0 && ms < best_ms) {   // rep 0 warms up
+      best_ms = ms;
+      best_mhz = static_cast<double>(hc) / (ms * 1e-3) / 1e6;
+    }
+  }
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  cudaFree(sink);
+  if (e != cudaSuccess) return e;
+  *tflops = 2.0 * 16.0 * iters * static_cast<double>(grid) * threads / (best_ms * 1e-3) / 1e12;
+  *sm_mhz = best_mhz;
+  return cudaSuccess;
+}
+
 int sweep_grid(int sm_count, bool field) { return sm_count * (field ? 2 : 3); }
 
 cudaError_t launch_sweep(const SweepParams& prm, bool field, int grid, cudaStream_t stream) {

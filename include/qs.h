@@ -184,6 +184,13 @@ typedef struct {
 int  qs_profile_enable(qs_ctx *ctx, int32_t on);
 int  qs_profile_read(qs_ctx *ctx, qs_profile_t *out);
 
+/* Test hook for the per-pair arithmetic of the sweeps (C2, C3): for each i, with A2 = (ri+rj)^2 + dz^2 and
+ * B2 = (ri-rj)^2 + dz^2 given (host arrays [n], A2 >= B2 > 0), evaluates through evaluation class `cls`
+ * (0..9, cheapest first; < 0: the class the sweep would choose from k'^2 = B2/A2) and returns
+ * M = mu0 sqrt(ri rj)[(2/k - k)K - (2/k)E] [H], K(k), E(k) and the class used.  Needs no handle.  */
+int  qs_pair_eval(int32_t n, const double *A2, const double *B2, int32_t cls,
+                  double *M, double *K, double *E, int32_t *used);
+
 /* FP64 FMA throughput of the current device [TFLOP/s, FMA = 2 flop]: 16 independent DFMA chains per
  * thread on every SM, timed with CUDA events (best of 5).  The denominator of the operator's
  * roofline ("bound": "alu"); needs no handle.  Returns 0 or QS_ERR_CUDA.  */

@@ -73,6 +73,7 @@ SYMBOLS = [
     ("qs_profile_enable", C.c_int, [_VP, C.c_int32]),
     ("qs_profile_read", C.c_int, [_VP, C.POINTER(QsProfile)]),
     ("qs_fp64_peak", C.c_int, [c_double_p, c_double_p]),
+    ("qs_pair_eval", C.c_int, [C.c_int32, c_double_p, c_double_p, C.c_int32, c_double_p, c_double_p, c_double_p, c_int32_p]),
     ("qs_events", C.c_int, [_VP, c_int32_p, c_double_p, c_int32_p]),
     ("qs_sync", C.c_int, [_VP]),
     ("qs_last_error", C.c_char_p, []),
@@ -123,6 +124,19 @@ def fp64_peak():
     if rc < 0:
         raise QsError(rc, lib.qs_last_error().decode())
     return tf.value, mhz.value
+
+
+def pair_eval(A2, B2, cls: int = -1):
+    """(M, K, E, class used) of the sweeps' per-pair arithmetic for given A2, B2 arrays (test hook)."""
+    lib = load_library()
+    a, b = _f64(A2), _f64(B2, None)
+    n = a.size
+    M, K, E = np.empty(n), np.empty(n), np.empty(n)
+    used = np.empty(n, dtype=np.int32)
+    rc = lib.qs_pair_eval(n, _dp(a), _dp(b), int(cls), _dp(M), _dp(K), _dp(E), used.ctypes.data_as(c_int32_p))
+    if rc < 0:
+        raise QsError(rc, lib.qs_last_error().decode())
+    return M, K, E, used
 
 
 class QS:

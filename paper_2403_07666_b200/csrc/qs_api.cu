@@ -922,6 +922,27 @@ int qs_profile_read(qs_ctx* c, qs_profile_t* out) {
   return QS_OK;
 }
 
+int qs_pair_eval(int32_t n, const double* A2, const double* B2, int32_t cls, double* M, double* K, double* E, int32_t* used) {
+  if (n <= 0 || !A2 || !B2 || !M || !K || !E || !used) return fail(QS_ERR_ARG, "qs_pair_eval: bad argument");
+  if (cls >= pair_num_classes()) return fail(QS_ERR_ARG, "qs_pair_eval: class out of range");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(QS_ERR_CUDA, "no CUDA device: libqs has no CPU path");
+  double* d = nullptr;
+  const size_t nb8 = sizeof(double) * n;
+  QS_CUDA(cudaMalloc(&d, 5 * nb8 + sizeof(int) * n));
+  int* du = reinterpret_cast<int*>(d + 5 * static_cast<size_t>(n));
+  cudaError_t e = cudaMemcpy(d, A2, nb8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(d + n, B2, nb8, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = launch_pair_eval(n, d, d + n, cls, d + 2 * n, d + 3 * n, d + 4 * n, du, nullptr);
+  if (e == cudaSuccess) e = cudaMemcpy(M, d + 2 * n, nb8, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(K, d + 3 * n, nb8, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(E, d + 4 * n, nb8, cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemcpy(used, du, sizeof(int) * n, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (e != cudaSuccess) return fail(QS_ERR_CUDA, std::string("qs_pair_eval: ") + cudaGetErrorString(e));
+  return QS_OK;
+}
+
 int qs_fp64_peak(double* tflops, double* sm_clock_mhz_effective) {
   if (!tflops) return fail(QS_ERR_ARG, "NULL argument");
   double tf = 0.0, mhz = 0.0;

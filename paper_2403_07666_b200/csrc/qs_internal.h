@@ -33,6 +33,10 @@ cudaError_t launch_sweep(const SweepParams& prm, bool field, int grid, cudaStrea
 // diagM_i = M(r_i, r_i, dz^2 = d2self) in henry
 cudaError_t launch_diag(int n, const double* r, double d2self, double* diagM, cudaStream_t stream);
 
+// test hook: per-pair evaluation through evaluation class cls (or the class the sweep would pick when cls < 0)
+cudaError_t launch_pair_eval(int n, const double* A2, const double* B2, int cls, double* M, double* K, double* E,
+                             int* used, cudaStream_t stream);
+int pair_num_classes();
 // FP64 FMA throughput probe (qs_operator.cu): TFLOP/s and the SM clock seen by the kernel
 cudaError_t fp64_peak_probe(double* tflops, double* sm_mhz);
 

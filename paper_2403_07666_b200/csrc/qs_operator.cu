@@ -17,9 +17,15 @@
 
 namespace qs {
 
-// smallest k'^2 for which NIT iterations (+ the closed-form last step) are exact to < 1e-16
-// (60-digit evaluation of the truncated recurrence against K, E).
-__device__ __constant__ double kKp2Min[8] = {1e300, 0.9995, 0.9030, 0.2754, 6.46e-3, 2.62e-6, 4.3e-13, 0.0};
+// Evaluation classes, cheapest first: (AGM iterations NIT, series order HI) and the smallest k'^2 = B2/A2 for which
+// the truncated evaluation is exact to < 1e-16 relative in M, K and E (60-digit evaluation of the truncated
+// recurrence against K, E, plus 2 % margin).  FP64 operations per pair:
+// 8 + 10 NIT + 16 (lo) or 20 (hi).
+constexpr int kNumClasses = 10;
+__device__ __constant__ double kClassKp2Min[kNumClasses] = {0.3965,   0.1394,   0.01529,   1.374e-3, 1.453e-5,
+                                                            1.157e-7, 1.293e-11, 8.2e-16,  1.03e-23, 0.0};
+//                                                class:      0       1       2       3       4       5       6       7       8       9
+//                                                (NIT,HI): (2,lo)  (2,hi)  (3,lo)  (3,hi)  (4,lo)  (4,hi)  (5,lo)  (5,hi)  (6,lo)  (7,lo)
 
 constexpr int kWarpsPerCta = 8;
 constexpr int kThreads = kWarpsPerCta * 32;
@@ -68,23 +74,23 @@ struct Accum {
 };
 
 // ---- one off-diagonal item: all 32 x 32 pairs, both directions -----------------------------------
-template <int NIT, bool FIELD>
+template <int NIT, bool HI, bool FIELD>
 __device__ __forceinline__ void item_offdiag(const TargetRegs& t, const double* __restrict__ sr,
                                              const double* __restrict__ sz, const double* __restrict__ sx,
                                              const double* __restrict__ sc, double soft_all, int lane, Accum& acc,
                                              Accum& trav) {
   const unsigned full = 0xffffffffu;
   const int next = (lane + 1) & 31;
-  const double ri2 = t.r * t.r;
+  const double ri2 = t.r * t.r, ri4 = 4.0 * t.r;
 #pragma unroll 1
   for (int s = 0; s < 32; ++s) {
     const int jl = (lane + s) & 31;
     const double rj = sr[jl], zj = sz[jl], xj = sx[jl];
     const double dz = t.z - zj;
     const double dz2 = fma(dz, dz, soft_all);
-    const double sum = t.r + rj, dif = t.r - rj;
-    const double A2 = fma(sum, sum, dz2), B2 = fma(dif, dif, dz2);
-    const PairAGM a = agm_pair<NIT, FIELD>(A2, B2);
+    const double dif = t.r - rj;
+    const double B2 = fma(dif, dif, dz2), A2 = fma(ri4, rj, B2);   // (ri+rj)^2 = (ri-rj)^2 + 4 ri rj
+    const PairAGM a = agm_pair<NIT, HI, FIELD>(A2, B2);
     const double mt = a.S * a.yinf;
     acc.y = fma(mt, xj, acc.y);
     trav.y = fma(mt, t.x, trav.y);
@@ -107,7 +113,7 @@ __device__ __forceinline__ void item_offdiag(const TargetRegs& t, const double* 
 }
 
 // ---- one diagonal item (bi == bj): every ordered pair appears once in the rotation -----------------
-template <int NIT, bool FIELD>
+template <int NIT, bool HI, bool FIELD>
 __device__ __forceinline__ void item_diag(const TargetRegs& t, const double* __restrict__ sr,
                                           const double* __restrict__ sz, const double* __restrict__ sx,
                                           const double* __restrict__ sc, double soft_all, double soft_self, int lane,
@@ -116,7 +122,7 @@ __device__ __forceinline__ void item_diag(const TargetRegs& t, const double* __r
   {  // s = 0: the self pair; M_ii = M(ri, ri, dz^2 = soft_all + soft_self); no field term (C3 self field is analytic)
     const double dz2 = soft_all + soft_self;
     const double sum = t.r + t.r;
-    const PairAGM a = agm_pair<NIT, false>(fma(sum, sum, dz2), dz2);
+    const PairAGM a = agm_pair<NIT, HI, false>(fma(sum, sum, dz2), dz2);
     acc.y = fma(a.S * a.yinf, t.x, acc.y);
   }
 #pragma unroll 1
@@ -126,7 +132,7 @@ __device__ __forceinline__ void item_diag(const TargetRegs& t, const double* __r
     const double dz = t.z - zj;
     const double dz2 = fma(dz, dz, soft_all);
     const double sum = t.r + rj, dif = t.r - rj;
-    const PairAGM a = agm_pair<NIT, FIELD>(fma(sum, sum, dz2), fma(dif, dif, dz2));
+    const PairAGM a = agm_pair<NIT, HI, FIELD>(fma(sum, sum, dz2), fma(dif, dif, dz2));
     acc.y = fma(a.S * a.yinf, xj, acc.y);
     if (FIELD) {
       const double cj = sc[jl];
@@ -145,11 +151,11 @@ __device__ __forceinline__ int classify(const double4& bi, const double4& bj, bo
   const double smax = bi.y + bj.y;
   const double d2 = diag ? prm.diag_d2 : fmax(fma(dr, dr, dzg * dzg), prm.minsep2) + prm.soft_all;
   const double kp2 = d2 / (fma(smax, smax, d2));
-  int n = 7;
+  int cls = kNumClasses - 1;
 #pragma unroll
-  for (int k = 6; k >= 2; --k)
-    if (kp2 >= kKp2Min[k]) n = k;
-  return n;
+  for (int k = kNumClasses - 2; k >= 0; --k)
+    if (kp2 >= kClassKp2Min[k]) cls = k;
+  return cls;
 }
 
 // row-major enumeration of the upper triangle (bi <= bj) of an nb x nb block matrix
@@ -235,23 +241,32 @@ __global__ void __launch_bounds__(kThreads, FIELD ? 2 : 3) sweep_kernel(SweepPar
       const double* sx = sbuf[warp][buf][2];
       const double* sc = sbuf[warp][buf][3];
       if (bi == bj) {
-        switch (nit) {
-          case 2: case 3: case 4:
-            item_diag<4, FIELD>(t, sr, sz, sx, sc, prm.soft_all, prm.soft_self, lane, acc); break;
-          case 5: item_diag<5, FIELD>(t, sr, sz, sx, sc, prm.soft_all, prm.soft_self, lane, acc); break;
-          case 6: item_diag<6, FIELD>(t, sr, sz, sx, sc, prm.soft_all, prm.soft_self, lane, acc); break;
-          default: item_diag<7, FIELD>(t, sr, sz, sx, sc, prm.soft_all, prm.soft_self, lane, acc); break;
+#define QS_DIAG(N_, HI_) item_diag<N_, HI_, FIELD>(t, sr, sz, sx, sc, prm.soft_all, prm.soft_self, lane, acc); break
+        switch (nit) {   // diagonal items are rare: the four cheapest classes share (4, lo)
+          case 0: case 1: case 2: case 3: case 4: QS_DIAG(4, false);
+          case 5: QS_DIAG(4, true);
+          case 6: QS_DIAG(5, false);
+          case 7: QS_DIAG(5, true);
+          case 8: QS_DIAG(6, false);
+          default: QS_DIAG(7, false);
         }
+#undef QS_DIAG
       } else {
         Accum trav = {0.0, 0.0, 0.0};
+#define QS_OFF(N_, HI_) item_offdiag<N_, HI_, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break
         switch (nit) {
-          case 2: item_offdiag<2, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break;
-          case 3: item_offdiag<3, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break;
-          case 4: item_offdiag<4, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break;
-          case 5: item_offdiag<5, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break;
-          case 6: item_offdiag<6, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break;
-          default: item_offdiag<7, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break;
+          case 0: QS_OFF(2, false);
+          case 1: QS_OFF(2, true);
+          case 2: QS_OFF(3, false);
+          case 3: QS_OFF(3, true);
+          case 4: QS_OFF(4, false);
+          case 5: QS_OFF(4, true);
+          case 6: QS_OFF(5, false);
+          case 7: QS_OFF(5, true);
+          case 8: QS_OFF(6, false);
+          default: QS_OFF(7, false);
         }
+#undef QS_OFF
         red_add(prm.yacc + 32ll * bj + lane, trav.y);
         if (FIELD) {
           red_add(prm.bracc + 32ll * bj + lane, trav.br);
@@ -274,9 +289,51 @@ __global__ void diag_kernel(int n, const double* __restrict__ r, double d2self, 
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const double s = r[i] + r[i];
-  const PairAGM a = agm_pair<7, false>(fma(s, s, d2self), d2self);
+  const PairAGM a = agm_pair<7, false, false>(fma(s, s, d2self), d2self);
   diagM[i] = (0.5 * kMu0 * kPi) * a.S * a.yinf;
 }
+// ---- test hook: one pair per thread through a chosen evaluation class (cls < 0: chosen from k'^2 like the sweep) ----
+template <int NIT, bool HI>
+__device__ __forceinline__ void pair_out(double A2, double B2, double* M, double* K, double* E) {
+  const PairAGM a = agm_pair<NIT, HI, true>(A2, B2);
+  *M = (0.5 * kMu0 * kPi) * a.S * a.yinf;
+  const double sa = sqrt(A2);
+  *K = (0.5 * kPi) * a.yinf * sa;
+  *E = (0.5 * kPi) * a.yinf * (a.mid - a.S) / sa;
+}
+__global__ void pair_eval_kernel(int n, const double* __restrict__ A2, const double* __restrict__ B2, int cls,
+                                 double* __restrict__ M, double* __restrict__ K, double* __restrict__ E,
+                                 int* __restrict__ used) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int c = cls;
+  if (c < 0) {
+    const double kp2 = B2[i] / A2[i];
+    c = kNumClasses - 1;
+    for (int k = kNumClasses - 2; k >= 0; --k)
+      if (kp2 >= kClassKp2Min[k]) c = k;
+  }
+  used[i] = c;
+  switch (c) {
+    case 0: pair_out<2, false>(A2[i], B2[i], M + i, K + i, E + i); break;
+    case 1: pair_out<2, true>(A2[i], B2[i], M + i, K + i, E + i); break;
+    case 2: pair_out<3, false>(A2[i], B2[i], M + i, K + i, E + i); break;
+    case 3: pair_out<3, true>(A2[i], B2[i], M + i, K + i, E + i); break;
+    case 4: pair_out<4, false>(A2[i], B2[i], M + i, K + i, E + i); break;
+    case 5: pair_out<4, true>(A2[i], B2[i], M + i, K + i, E + i); break;
+    case 6: pair_out<5, false>(A2[i], B2[i], M + i, K + i, E + i); break;
+    case 7: pair_out<5, true>(A2[i], B2[i], M + i, K + i, E + i); break;
+    case 8: pair_out<6, false>(A2[i], B2[i], M + i, K + i, E + i); break;
+    default: pair_out<7, false>(A2[i], B2[i], M + i, K + i, E + i); break;
+  }
+}
+cudaError_t launch_pair_eval(int n, const double* A2, const double* B2, int cls, double* M, double* K, double* E,
+                             int* used, cudaStream_t stream) {
+  pair_eval_kernel<<<(n + 127) / 128, 128, 0, stream>>>(n, A2, B2, cls, M, K, E, used);
+  return cudaGetLastError();
+}
+int pair_num_classes() { return kNumClasses; }
+
 cudaError_t launch_diag(int n, const double* r, double d2self, double* diagM, cudaStream_t stream) {
   diag_kernel<<<(n + 255) / 256, 256, 0, stream>>>(n, r, d2self, diagM);
   return cudaGetLastError();

@@ -208,3 +208,34 @@ def test_errors_and_no_operator_mode(pkg):
     with pkg.QS(w.geometry, w.material, torch_memory=False) as sim:   # plain-C path: cudaMalloc + own stream
         y = sim.matvec(np.ones(16))
     assert rel(y, qo.dense_M(w.geometry) @ np.ones(16)) <= 1e-9
+
+
+def test_pair_arithmetic_every_class_at_its_threshold(pkg):
+    # per-pair K, E, M of the sweeps against the oracle's library route (scipy Cephes K/E + Maxwell bracket),
+    # each evaluation class probed from its own k'^2 threshold upwards (where its truncation error is largest)
+    from paper_2403_07666_b200 import pair_eval
+    thr = [0.3965, 0.1394, 0.01529, 1.374e-3, 1.453e-5, 1.157e-7, 1.293e-11, 8.2e-16, 1.03e-23, 1e-27]
+    ri = 0.05
+    for cls, t in enumerate(thr):
+        kp2 = t * np.logspace(0.0, 1.0, 64) if t < 0.09 else np.linspace(t, 0.98, 64)
+        kp2 = np.minimum(kp2, 0.98)
+        # coaxial pair with ri = rj: A2 = 4 ri^2 + dz^2, B2 = dz^2  ->  dz^2 = 4 ri^2 kp2/(1-kp2)
+        dz2 = 4 * ri * ri * kp2 / (1.0 - kp2)
+        A2, B2 = 4 * ri * ri + dz2, dz2
+        M, K, E, used = pair_eval(A2, B2, cls)
+        assert np.all(used == cls)
+        Ko, Eo = qo.elliptic_KE(B2 / A2)
+        Mo = qo.mutual_pair(ri, 0.0, ri, 0.0, soft2=dz2)
+        assert np.max(np.abs(K / Ko - 1)) <= 4e-15, (cls, np.max(np.abs(K / Ko - 1)))
+        assert np.max(np.abs(E / Eo - 1)) <= 2e-14, (cls, np.max(np.abs(E / Eo - 1)))
+        # Maxwell's bracket loses digits to cancellation at small k (far pairs): compare M where it is well conditioned
+        ok = kp2 <= 0.5
+        if np.any(ok):
+            assert np.max(np.abs(M[ok] / Mo[ok] - 1)) <= 2e-14, (cls, np.max(np.abs(M[ok] / Mo[ok] - 1)))
+    # automatic class choice is monotone in k'^2 and never cheaper than the threshold table allows
+    kp2 = np.logspace(-26, np.log10(0.98), 400)
+    dz2 = 4 * ri * ri * kp2 / (1.0 - kp2)
+    M, K, E, used = pair_eval(4 * ri * ri + dz2, dz2, -1)
+    assert np.all(np.diff(used) <= 0)
+    Ko, Eo = qo.elliptic_KE(dz2 / (4 * ri * ri + dz2))
+    assert np.max(np.abs(K / Ko - 1)) <= 4e-15 and np.max(np.abs(E / Eo - 1)) <= 2e-14

@@ -82,9 +82,10 @@ __device__ __forceinline__ void item_offdiag(const TargetRegs& t, const double* 
   const unsigned full = 0xffffffffu;
   const int next = (lane + 1) & 31;
   const double ri2 = t.r * t.r, ri4 = 4.0 * t.r;
-#pragma unroll 1
+  sr += lane, sz += lane, sx += lane, sc += lane;   // arrays are stored twice: entry lane + s = source (lane + s) & 31
+#pragma unroll 2
   for (int s = 0; s < 32; ++s) {
-    const int jl = (lane + s) & 31;
+    const int jl = s;
     const double rj = sr[jl], zj = sz[jl], xj = sx[jl];
     const double dz = t.z - zj;
     const double dz2 = fma(dz, dz, soft_all);
@@ -125,9 +126,10 @@ __device__ __forceinline__ void item_diag(const TargetRegs& t, const double* __r
     const PairAGM a = agm_pair<NIT, HI, false>(fma(sum, sum, dz2), dz2);
     acc.y = fma(a.S * a.yinf, t.x, acc.y);
   }
+  sr += lane, sz += lane, sx += lane, sc += lane;
 #pragma unroll 1
   for (int s = 1; s < 32; ++s) {
-    const int jl = (lane + s) & 31;
+    const int jl = s;
     const double rj = sr[jl], zj = sz[jl], xj = sx[jl];
     const double dz = t.z - zj;
     const double dz2 = fma(dz, dz, soft_all);
@@ -173,7 +175,7 @@ __device__ __forceinline__ void unrank(long long k, int nb, int& bi, int& bj) {
 template <bool FIELD>
 __global__ void __launch_bounds__(kThreads, FIELD ? 2 : 3) sweep_kernel(SweepParams prm) {
   constexpr int NA = FIELD ? 4 : 3;
-  __shared__ __align__(128) double sbuf[kWarpsPerCta][2][kMaxArrays][32];
+  __shared__ __align__(128) double sbuf[kWarpsPerCta][2][kMaxArrays][64];   // every array twice: no wrap of lane + s
   __shared__ __align__(8) uint64_t sbar[kWarpsPerCta][2];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const unsigned full = 0xffffffffu;
@@ -186,9 +188,12 @@ __global__ void __launch_bounds__(kThreads, FIELD ? 2 : 3) sweep_kernel(SweepPar
 
   auto issue = [&](int buf, int bj) {
     if (lane == 0) {
-      mbar_expect_tx(&sbar[warp][buf], NA * 256u);
+      mbar_expect_tx(&sbar[warp][buf], NA * 512u);
 #pragma unroll
-      for (int a = 0; a < NA; ++a) bulk_g2s(&sbuf[warp][buf][a][0], src[a] + 32ll * bj, 256u, &sbar[warp][buf]);
+      for (int a = 0; a < NA; ++a) {
+        bulk_g2s(&sbuf[warp][buf][a][0], src[a] + 32ll * bj, 256u, &sbar[warp][buf]);
+        bulk_g2s(&sbuf[warp][buf][a][32], src[a] + 32ll * bj, 256u, &sbar[warp][buf]);
+      }
     }
   };
 

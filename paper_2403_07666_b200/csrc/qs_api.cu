@@ -125,6 +125,8 @@ struct qs_ctx {
   size_t acc_bytes = 0;
   double *sw, *swM, *vw, *vsum, *defw, *ebar_prev, *t_first;
   int *flags, *count, *turn_ptr, *turn_idx, *turn_id, *d_perm;
+  double* heat_tab = nullptr;        // hr_p, hr_m, rb_r [Nr each], hz_p, hz_m, rb_z [Nz each]
+  int tabNr = 0, tabNz = 0;
   double4* bbox;
   Scalars* sc;
   Scalars* h_sc = nullptr;           // pinned
@@ -199,6 +201,7 @@ void carve(qs_ctx* c, void* base, size_t* total) {
   c->turn_id = k.take<int>(N);
   c->d_perm = k.take<int>(N);
   c->bbox = k.take<double4>(std::max(c->nb, 1));
+  c->heat_tab = k.take<double>(3 * static_cast<size_t>(c->tabNr + c->tabNz) + 1);
   c->sc = k.take<Scalars>(1);
   *total = align_up(k.off, 256);
 }
@@ -427,6 +430,8 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
     lp.h = geo->wire_size / lp.n;
     lp.r_inner = geo->r_inner;
     for (int s = 0; s < 4; ++s) lp.h_conv[s] = geo->h_conv[s];
+    c->tabNr = lp.Nr;
+    c->tabNz = lp.Nz;
     // the lattice description must agree with the ring arrays (C1)
     const int probe[4] = {0, N - 1, N / 2, N / 3};
     for (int k : probe) {
@@ -562,6 +567,33 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
         cudaStreamSynchronize(c->stream) != cudaSuccess)
       return bail(fail(QS_ERR_CUDA, "upload of the turn tables failed"));
   }
+  // heat-step coefficient tables (C9): conductivities, face areas and the cell volume folded per row / column
+  if (c->lattice) {
+    const int Nr = lp.Nr, Nz = lp.Nz, n = lp.n;
+    const double h = lp.h;
+    std::vector<double> tab(3 * static_cast<size_t>(Nr + Nz), 0.0);
+    double *hr_p = tab.data(), *hr_m = hr_p + Nr, *rb_r = hr_m + Nr, *hz_p = rb_r + Nr, *hz_m = hz_p + Nz, *rb_z = hz_m + Nz;
+    for (int ir = 0; ir < Nr; ++ir) {
+      const double rc = lp.r_inner + (ir + 0.5) * h;
+      if (ir + 1 < Nr) hr_p[ir] = ((ir / n == (ir + 1) / n) ? mp.k_in : mp.k_between) * (rc + 0.5 * h) / (2.0 * h * h * rc);
+      if (ir > 0) hr_m[ir] = (((ir - 1) / n == ir / n) ? mp.k_in : mp.k_between) * (rc - 0.5 * h) / (2.0 * h * h * rc);
+      if (ir == 0) rb_r[ir] += lp.h_conv[0] * (rc - 0.5 * h) / (rc * h);
+      if (ir == Nr - 1) rb_r[ir] += lp.h_conv[1] * (rc + 0.5 * h) / (rc * h);
+    }
+    for (int iz = 0; iz < Nz; ++iz) {
+      if (iz + 1 < Nz) hz_p[iz] = ((iz / n == (iz + 1) / n) ? mp.k_in : mp.k_between) / (2.0 * h * h);
+      if (iz > 0) hz_m[iz] = (((iz - 1) / n == iz / n) ? mp.k_in : mp.k_between) / (2.0 * h * h);
+      if (iz == 0) rb_z[iz] += lp.h_conv[2] / h;
+      if (iz == Nz - 1) rb_z[iz] += lp.h_conv[3] / h;
+    }
+    if (!put(c->heat_tab, tab, tab.size())) return bail(fail(QS_ERR_CUDA, "upload of the heat tables failed"));
+    lp.hr_p = c->heat_tab;
+    lp.hr_m = lp.hr_p + Nr;
+    lp.rb_r = lp.hr_m + Nr;
+    lp.hz_p = lp.rb_r + Nr;
+    lp.hz_m = lp.hz_p + Nz;
+    lp.rb_z = lp.hz_m + Nz;
+  }
   // initial state: J = 0 (memset), T = T_bath
   {
     std::vector<double> T0(N, geo->T_bath);
@@ -610,6 +642,10 @@ size_t qs_workspace_bytes(const qs_geometry* geo) {
   tmp.Np = (tmp.N + 31) / 32 * 32;
   tmp.nb = tmp.Np / 32;
   tmp.n_turns = geo->n_turns;
+  if (geo->lattice) {
+    tmp.tabNr = geo->layers * geo->cells_per_side;
+    tmp.tabNz = geo->turns_per_layer * geo->cells_per_side;
+  }
   size_t need = 0;
   carve(&tmp, nullptr, &need);
   return need;

@@ -107,6 +107,12 @@ struct LatticeParams {
   double h, r_inner;
   double h_conv[4];
   double T_bath;
+  // face and border coefficients of the finite-volume heat step divided by the cell volume (C9), set up at init:
+  //   hr_p[ir] = kappa(ir|ir+1) (r_c + h/2) / (2 h^2 r_c)   (0 on the outer border)     hr_m likewise for ir-1|ir
+  //   hz_p[iz] = kappa(iz|iz+1) / (2 h^2)                    (0 on the border)           hz_m likewise
+  //   rb_r[ir], rb_z[iz] = Robin film coefficient x border face area / cell volume (0 for interior rows / columns)
+  const double *hr_p, *hr_m, *rb_r;   // [Nr]
+  const double *hz_p, *hz_m, *rb_z;   // [Nz]
 };
 struct MaterialArgs {
   int N;

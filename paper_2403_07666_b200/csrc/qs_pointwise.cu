@@ -8,6 +8,7 @@
 //      algorithmic traffic is read H, Q + write H = 24 B per cell per sub-step.
 //   K7 one warp per turn over the CSR cell list: Tmax, mean|E|, max|J|/Jc, min rho/rho_n -> flags (C10).
 #include "qs_internal.h"
+#include "qs_pair.cuh"
 
 namespace qs {
 
@@ -117,62 +118,123 @@ __global__ void temperature_kernel(int n, double C3, double C1, const double* __
     T[i] = sqrt(tsq_of_H(H[i], C3, C1));
 }
 
-// ---- K6: one explicit sub-step.  Tile = kTz cells along z (contiguous) x kTr cells along r. ------------------
-constexpr int kTz = 64, kTr = 8;   // 512 cells per CTA, 256 threads -> 2 cells per thread along r
-__global__ void __launch_bounds__(256) heat_kernel(MaterialParams mp, LatticeParams lp, const double* __restrict__ Hin,
-                                                   const double* __restrict__ Q, double* __restrict__ Hout,
-                                                   double dtsub) {
-  __shared__ double U[kTr + 2][kTz + 2];          // T^2 of the tile and its halo
-  const int tz0 = blockIdx.x * kTz, tr0 = blockIdx.y * kTr;
-  // stage: (kTr+2) x (kTz+2) entries, out-of-pack entries are never read
-  for (int e = threadIdx.x; e < (kTr + 2) * (kTz + 2); e += blockDim.x) {
-    const int lr = e / (kTz + 2), lz = e - lr * (kTz + 2);
-    const int ir = tr0 + lr - 1, iz = tz0 + lz - 1;
-    double u = 0.0;
-    if (ir >= 0 && ir < lp.Nr && iz >= 0 && iz < lp.Nz) u = tsq_of_H(Hin[(long long)ir * lp.Nz + iz], mp.C3, mp.C1);
-    U[lr][lz] = u;
-  }
+// ---- K6: one explicit sub-step (C9) -----------------------------------------------------------------------------
+// Marching stencil without shared-memory tiles: a warp owns 30 consecutive columns (iz) plus one halo lane on each
+// side and marches along r over a strip of rows, keeping T^2 of the previous, current and next row in registers
+// (one square root per cell and row; the Kirchhoff flux needs only T^2); the z-neighbours come from the adjacent
+// lanes by shuffles.  Conductivities, face areas and the cell volume are folded into per-row / per-column
+// coefficient tables (LatticeParams), so a cell update is 4 differences, 4 multiply-adds, the source and the
+// update: read H, Q and write H = 24 B per cell.
+constexpr int kHeatLanes = 30;           // owner lanes per warp (lanes 0 and 31 carry the halo columns)
+constexpr int kHeatCols = 2 * kHeatLanes; // useful columns per warp: every lane holds two adjacent columns
+constexpr int kHeatWarps = 8;
+constexpr int kHeatMaxRows = 32;
+
+// T^2 from H with the fast reciprocal square root (MUFU seed + one Halley step): argument > 0 always (H >= 0)
+__device__ __forceinline__ double tsq_fast(double H, double C3, double qC1sq, double hC1, double inv_hC3) {
+  const double a = fma(C3, H, qC1sq);                 // C1^2/4 + C3 H
+  const double y0 = rsqrt_seed(a);
+  const double g = a * y0;
+  const double e = fma(-g, y0, 1.0);
+  const double s = fma(g * e, fma(0.375, e, 0.5), g); // sqrt(a)
+  return (s - hC1) * inv_hC3;
+}
+
+// T from T^2 (border cells only), same fast root
+__device__ __forceinline__ double sqrt_fast(double a) {
+  const double y0 = rsqrt_seed(a);
+  const double g = a * y0;
+  const double e = fma(-g, y0, 1.0);
+  return fma(g * e, fma(0.375, e, 0.5), g);
+}
+
+template <bool VEC>   // VEC: Nz even, so that the column pair of a lane is 16-byte aligned in every row
+__global__ void __launch_bounds__(kHeatWarps * 32, 3) heat_kernel(MaterialParams mp, LatticeParams lp, int rows_per_cta,
+                                                               const double* __restrict__ Hin,
+                                                               const double* __restrict__ Q, double* __restrict__ Hout,
+                                                               double dtsub) {
+  __shared__ double4 srow[kHeatMaxRows];               // (hr_p, hr_m, rb_r, -) of the rows of this strip
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int iz0 = 2 * ((blockIdx.x * kHeatWarps + warp) * kHeatLanes + lane - 1);
+  const int r0 = blockIdx.y * rows_per_cta, r1 = min(r0 + rows_per_cta, lp.Nr);
+  if (threadIdx.x < r1 - r0)
+    srow[threadIdx.x] = make_double4(lp.hr_p[r0 + threadIdx.x], lp.hr_m[r0 + threadIdx.x], lp.rb_r[r0 + threadIdx.x], 0.0);
   __syncthreads();
-  const int lz = threadIdx.x & (kTz - 1);
-  const int iz = tz0 + lz;
-  const double two_pi = 2.0 * kPi, h = lp.h;
-#pragma unroll
-  for (int sub = 0; sub < kTr * kTz / 256; ++sub) {
-    const int lr = (threadIdx.x >> 6) + sub * (256 / kTz);
-    const int ir = tr0 + lr;
-    if (ir >= lp.Nr || iz >= lp.Nz) continue;
-    const long long c = (long long)ir * lp.Nz + iz;
-    const double rc = lp.r_inner + (ir + 0.5) * h;
-    const double u = U[lr + 1][lz + 1];
-    double F = 0.0;
-    if (ir + 1 < lp.Nr) {   // radial face ir | ir+1, area 2 pi (r_c + h/2) h
-      const double kap = (ir / lp.n == (ir + 1) / lp.n) ? mp.k_in : mp.k_between;
-      F += kap * (U[lr + 2][lz + 1] - u) / (2.0 * h) * (two_pi * (rc + 0.5 * h) * h);
+  const bool in0 = iz0 >= 0 && iz0 < lp.Nz, in1 = iz0 + 1 >= 0 && iz0 + 1 < lp.Nz;
+  const bool own = lane >= 1 && lane <= kHeatLanes;
+  const bool own0 = own && in0, own1 = own && in1;
+  const double C3 = mp.C3, qC1sq = 0.25 * mp.C1 * mp.C1, hC1 = 0.5 * mp.C1, inv_hC3 = 2.0 / mp.C3;
+  const double zp0 = in0 ? lp.hz_p[iz0] : 0.0, zm0 = in0 ? lp.hz_m[iz0] : 0.0, zb0 = in0 ? lp.rb_z[iz0] : 0.0;
+  const double zp1 = in1 ? lp.hz_p[iz0 + 1] : 0.0, zm1 = in1 ? lp.hz_m[iz0 + 1] : 0.0, zb1 = in1 ? lp.rb_z[iz0 + 1] : 0.0;
+  // lanes (partly) outside the pack read a clamped column pair and are ignored
+  const int izc = max(0, min(iz0, lp.Nz - 2 + (lp.Nz & 1)));
+  const bool pair_ok = in0 && in1;
+  const long long Nz = lp.Nz;
+  const double* hn = Hin + static_cast<long long>(r0) * Nz + izc;     // walks one row ahead of the update
+  const double* q = Q + static_cast<long long>(r0) * Nz + izc;
+  double* o = Hout + static_cast<long long>(r0) * Nz + izc;
+  auto load2 = [&](const double* ptr) -> double2 {
+    if (VEC) return *reinterpret_cast<const double2*>(ptr);
+    double2 v;
+    v.x = ptr[0];
+    v.y = pair_ok ? ptr[1] : ptr[0];
+    return v;
+  };
+  double2 Up = make_double2(0.0, 0.0);
+  if (r0 > 0) {
+    const double2 h = load2(hn - Nz);
+    Up = make_double2(tsq_fast(h.x, C3, qC1sq, hC1, inv_hC3), tsq_fast(h.y, C3, qC1sq, hC1, inv_hC3));
+  }
+  double2 Hc = load2(hn);
+  double2 Uc = make_double2(tsq_fast(Hc.x, C3, qC1sq, hC1, inv_hC3), tsq_fast(Hc.y, C3, qC1sq, hC1, inv_hC3));
+  const int last = lp.Nr - 1;
+  // software pipeline: the enthalpy row two ahead and the source row one ahead are in flight while a row is updated
+  // (past the last row of the pack the pointer stays on the last row: its coefficient is 0)
+  if (r0 < last) hn += Nz;
+  double2 Hn = load2(hn);
+  if (r0 + 1 < last) hn += Nz;
+  double2 Hn2 = load2(hn);
+  double2 qc = load2(q);
+  if (r0 + 1 < r1) q += Nz;
+  double2 qn = load2(q);
+  const bool zborder = (zb0 != 0.0) || (zb1 != 0.0);
+  for (int ir = r0; ir < r1; ++ir) {
+    if (ir + 2 < last) hn += Nz;
+    const double2 Hn3 = load2(hn);                     // enthalpy row ir + 3 (clamped to the last row)
+    if (ir + 2 < r1) q += Nz;
+    const double2 qn2 = load2(q);                      // source row ir + 2 (clamped to the strip)
+    const double2 Un = make_double2(tsq_fast(Hn.x, C3, qC1sq, hC1, inv_hC3), tsq_fast(Hn.y, C3, qC1sq, hC1, inv_hC3));
+    const double Ul = __shfl_up_sync(0xffffffffu, Uc.y, 1), Ur = __shfl_down_sync(0xffffffffu, Uc.x, 1);
+    if (own0) {
+      const double4 rc = srow[ir - r0];
+      double a0 = fma(rc.x, Un.x - Uc.x, qc.x), a1 = fma(rc.x, Un.y - Uc.y, qc.y);
+      a0 = fma(rc.y, Up.x - Uc.x, a0);
+      a1 = fma(rc.y, Up.y - Uc.y, a1);
+      const double dzc = Uc.y - Uc.x;
+      a0 = fma(zp0, dzc, a0);
+      a1 = fma(-zm1, dzc, a1);
+      a0 = fma(zm0, Ul - Uc.x, a0);
+      a1 = fma(zp1, Ur - Uc.y, a1);
+      if (rc.z != 0.0 || zborder) {                    // Robin borders of the winding pack (rare: rb = 0 inside)
+        a0 = fma(-(rc.z + zb0), sqrt_fast(Uc.x) - lp.T_bath, a0);
+        a1 = fma(-(rc.z + zb1), sqrt_fast(Uc.y) - lp.T_bath, a1);
+      }
+      const double2 out = make_double2(fma(dtsub, a0, Hc.x), fma(dtsub, a1, Hc.y));
+      if (VEC) {
+        *reinterpret_cast<double2*>(o) = out;
+      } else {
+        o[0] = out.x;
+        if (own1) o[1] = out.y;
+      }
     }
-    if (ir > 0) {           // radial face ir-1 | ir, area 2 pi (r_{c-1} + h/2) h
-      const double kap = ((ir - 1) / lp.n == ir / lp.n) ? mp.k_in : mp.k_between;
-      const double rm = lp.r_inner + (ir - 0.5) * h;
-      F -= kap * (u - U[lr][lz + 1]) / (2.0 * h) * (two_pi * (rm + 0.5 * h) * h);
-    }
-    if (iz + 1 < lp.Nz) {   // axial faces, area 2 pi r_c h
-      const double kap = (iz / lp.n == (iz + 1) / lp.n) ? mp.k_in : mp.k_between;
-      F += kap * (U[lr + 1][lz + 2] - u) / (2.0 * h) * (two_pi * rc * h);
-    }
-    if (iz > 0) {
-      const double kap = ((iz - 1) / lp.n == iz / lp.n) ? mp.k_in : mp.k_between;
-      F -= kap * (u - U[lr + 1][lz]) / (2.0 * h) * (two_pi * rc * h);
-    }
-    if (ir == 0 || ir == lp.Nr - 1 || iz == 0 || iz == lp.Nz - 1) {   // Robin borders of the winding pack
-      const double dT = sqrt(u) - lp.T_bath;
-      double loss = 0.0;
-      if (ir == 0) loss += lp.h_conv[0] * dT * two_pi * (rc - 0.5 * h) * h;
-      if (ir == lp.Nr - 1) loss += lp.h_conv[1] * dT * two_pi * (rc + 0.5 * h) * h;
-      if (iz == 0) loss += lp.h_conv[2] * dT * two_pi * rc * h;
-      if (iz == lp.Nz - 1) loss += lp.h_conv[3] * dT * two_pi * rc * h;
-      F -= loss;
-    }
-    const double vol = two_pi * rc * h * h;
-    Hout[c] = Hin[c] + dtsub * (F / vol + Q[c]);
+    Up = Uc;
+    Uc = Un;
+    Hc = Hn;
+    Hn = Hn2;
+    Hn2 = Hn3;
+    qc = qn;
+    qn = qn2;
+    o += Nz;
   }
 }
 
@@ -254,8 +316,16 @@ void k_T_from_enthalpy(const VecCtx& v, const MaterialParams& mp, const double* 
 void k_heat_substep(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, const double* Hin,
                     const double* Q, double* Hout, double dtsub) {
   QS_LAUNCH(v);
-  dim3 grid((lp.Nz + kTz - 1) / kTz, (lp.Nr + kTr - 1) / kTr);
-  heat_kernel<<<grid, 256, 0, v.stream>>>(mp, lp, Hin, Q, Hout, dtsub);
+  const int gx = (lp.Nz + kHeatWarps * kHeatCols - 1) / (kHeatWarps * kHeatCols);
+  // strips of rows: long enough to amortise the two halo rows, short enough to fill the GPU (>= 4 CTAs per SM)
+  if (g_sm_count == 0) grid_for(1);
+  int rows = kHeatMaxRows;
+  while (rows > 4 && static_cast<long long>(gx) * ((lp.Nr + rows - 1) / rows) < 4ll * g_sm_count) rows >>= 1;
+  dim3 grid(gx, (lp.Nr + rows - 1) / rows);
+  if (lp.Nz % 2 == 0)
+    heat_kernel<true><<<grid, kHeatWarps * 32, 0, v.stream>>>(mp, lp, rows, Hin, Q, Hout, dtsub);
+  else
+    heat_kernel<false><<<grid, kHeatWarps * 32, 0, v.stream>>>(mp, lp, rows, Hin, Q, Hout, dtsub);
 }
 void k_events(const VecCtx& v, const MaterialParams& mp, const EventArgs& e) {
   if (!v.n_turns) return;

@@ -123,7 +123,7 @@ struct qs_ctx {
   unsigned long long* counter;       // followed contiguously by yacc, bracc, bzacc (one memset)
   double *yacc, *bracc, *bzacc;
   size_t acc_bytes = 0;
-  double *sw, *swM, *vw, *vsum, *defw, *ebar_prev, *t_first;
+  double *sw, *swM, *vw, *vsum, *tw, *defw, *ebar_prev, *t_first;
   int *flags, *count, *turn_ptr, *turn_idx, *turn_id, *d_perm;
   double* heat_tab = nullptr;        // hr_p, hr_m, rb_r [Nr each], hz_p, hz_m, rb_z [Nz each]
   int tabNr = 0, tabNz = 0;
@@ -191,6 +191,7 @@ void carve(qs_ctx* c, void* base, size_t* total) {
   c->swM = k.take<double>(nt);
   c->vw = k.take<double>(nt);
   c->vsum = k.take<double>(nt);
+  c->tw = k.take<double>(nt);
   c->defw = k.take<double>(nt);
   c->ebar_prev = k.take<double>(nt);
   c->t_first = k.take<double>(nt);
@@ -225,9 +226,10 @@ int sync_scalars(qs_ctx* c) {
   return QS_OK;
 }
 
-// y-accumulators <- sweep of (x [, cur]); consumer applies the scale factors
-int do_sweep(qs_ctx* c, const double* x, const double* cur, bool field) {
-  QS_CUDA(cudaMemsetAsync(c->counter, 0, c->acc_bytes, c->stream));
+// y-accumulators <- sweep of (x [, cur]); consumer applies the scale factors.  prezeroed: the accumulators and the
+// work counter were cleared by the previous CG iteration (fused path), no memset is enqueued.
+int do_sweep(qs_ctx* c, const double* x, const double* cur, bool field, bool prezeroed = false, bool cg_guard = false) {
+  if (!prezeroed) QS_CUDA(cudaMemsetAsync(c->counter, 0, c->acc_bytes, c->stream));
   SweepParams prm;
   prm.r = c->r;
   prm.z = c->z;
@@ -238,6 +240,7 @@ int do_sweep(qs_ctx* c, const double* x, const double* cur, bool field) {
   prm.bracc = c->bracc;
   prm.bzacc = c->bzacc;
   prm.counter = c->counter;
+  prm.done = cg_guard ? &c->sc->done : nullptr;
   prm.nb = c->nb;
   prm.n_items = static_cast<long long>(c->nb) * (c->nb + 1) / 2;
   prm.soft_all = c->soft_all;
@@ -263,6 +266,8 @@ constexpr double kCM = 0.5 * kMu0 * kPi;   // yacc -> henry * ampere
 
 // Projected CG (C8) on A = M + diag(shift), constraint C^T x = const kept by the projection.
 // In: x satisfies the constraint; if yacc_has_Mx the accumulators hold the sweep of x.  nu < 0: nu = start norm.
+// Iterations are enqueued in batches without a host round trip: the kernels stop themselves (Scalars::done) at the
+// iteration where sqrt(r^T g) <= tol nu, so the result is the one of the iteration-by-iteration loop.
 int cg_core(qs_ctx* c, const double* b, double* x, const double* shift, const double* Hd, const double* sw,
             bool yacc_has_Mx, double tol, int maxit, double nu, int* iters, double* relres, bool* hit_max) {
   const VecCtx& v = c->v;
@@ -270,39 +275,69 @@ int cg_core(qs_ctx* c, const double* b, double* x, const double* shift, const do
   if (!yacc_has_Mx && (rc = do_sweep(c, x, nullptr, false)) != QS_OK) return rc;
   k_residual(v, c->yacc, shift, x, b, c->rr, kCM);
   if (c->n_turns) QS_CUDA(cudaMemsetAsync(c->vsum, 0, sizeof(double) * c->n_turns, c->stream));
-  int par = 0;
   k_turn_project(v, c->rr, Hd, sw, c->vw, c->vsum);
-  k_project_apply(v, par, c->vw, Hd, c->rr, c->g);
-  k_direction(v, par, true, c->g, c->p);
+  k_project_apply(v, 0, c->vw, Hd, c->rr, c->g);
+  k_direction(v, 0, true, c->g, c->p);
   if ((rc = sync_scalars(c)) != QS_OK) return rc;
-  double rg = c->h_sc->rg[par];
+  double rg = c->h_sc->rg[0];
   if (nu < 0.0) nu = std::sqrt(std::max(rg, 0.0));
-  int it = 0;
   *hit_max = false;
-  while (true) {
-    if (!(rg == rg)) return fail(QS_ERR_NONFINITE, "CG: r^T g is NaN");
-    if (nu == 0.0 || std::sqrt(std::max(rg, 0.0)) <= tol * nu) break;
-    if (it >= maxit) {
-      *hit_max = true;
-      break;
-    }
-    if ((rc = do_sweep(c, c->p, nullptr, false)) != QS_OK) return rc;
-    c->prof.begin(c->stream);
-    k_finish_Ap(v, c->yacc, shift, c->p, c->q, kCM);
-    k_update_xr(v, par, c->p, c->q, x, c->rr);
-    k_turn_project(v, c->rr, Hd, sw, c->vw, c->vsum);
-    k_project_apply(v, par ^ 1, c->vw, Hd, c->rr, c->g);
-    QS_CUDA(cudaMemcpyAsync(c->h_sc, c->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, c->stream));
-    k_direction(v, par ^ 1, false, c->g, c->p);
-    c->prof.end(c->stream, QS_PROF_CG_VECTOR, c->n_turns ? 6 : 5);
-    QS_CUDA(cudaStreamSynchronize(c->stream));
-    if (!(c->h_sc->pq > 0.0)) return fail(QS_ERR_CG, "CG breakdown: p^T A p <= 0");
-    par ^= 1;
-    rg = c->h_sc->rg[par];
-    ++it;
+  *iters = 0;
+  if (!(rg == rg)) return fail(QS_ERR_NONFINITE, "CG: r^T g is NaN");
+  if (nu == 0.0 || std::sqrt(std::max(rg, 0.0)) <= tol * nu) {
+    *relres = nu > 0.0 ? std::sqrt(std::max(rg, 0.0)) / nu : 0.0;
+    return QS_OK;
   }
-  *iters = it;
-  *relres = nu > 0.0 ? std::sqrt(std::max(rg, 0.0)) / nu : 0.0;
+  if (maxit <= 0) {
+    *hit_max = true;
+    *relres = std::sqrt(std::max(rg, 0.0)) / nu;
+    return QS_OK;
+  }
+  // fused iterations
+  QS_CUDA(cudaMemsetAsync(c->counter, 0, c->acc_bytes, c->stream));
+  if (c->n_turns) QS_CUDA(cudaMemsetAsync(c->tw, 0, sizeof(double) * c->n_turns, c->stream));
+  k_cg_begin(v, (tol * nu) * (tol * nu));
+  CgIter it;
+  it.yacc_in = c->yacc;
+  it.shift = shift;
+  it.Hd = Hd;
+  it.sw = sw;
+  it.x = x;
+  it.r = c->rr;
+  it.g = c->g;
+  it.p = c->p;
+  it.q = c->q;
+  it.tw = c->tw;
+  it.vsum = c->vsum;
+  it.yacc_zero = c->yacc;
+  it.counter = c->counter;
+  it.cM = kCM;
+  int enq = 0, batch = 2;
+  for (;;) {
+    const int todo = std::min(batch, maxit - enq);
+    for (int k = 0; k < todo; ++k, ++enq) {
+      it.par = enq & 1;
+      if ((rc = do_sweep(c, c->p, nullptr, false, true, true)) != QS_OK) return rc;
+      c->prof.begin(c->stream);
+      k_cg_Ap(v, it);
+      k_cg_update(v, it);
+      k_cg_project(v, it);
+      k_cg_direction(v, it);
+      c->prof.end(c->stream, QS_PROF_CG_VECTOR, 4);
+    }
+    if ((rc = sync_scalars(c)) != QS_OK) return rc;
+    if (c->h_sc->done == 2) return fail(QS_ERR_CG, "CG breakdown: p^T A p <= 0 or NaN");
+    if (c->h_sc->done == 1 || enq >= maxit) break;
+    batch = std::min(16, batch * 2);
+  }
+  const int done_it = c->h_sc->iters;
+  rg = c->h_sc->rg[done_it & 1];
+  *iters = done_it;
+  *hit_max = c->h_sc->done != 1;
+  *relres = std::sqrt(std::max(rg, 0.0)) / nu;
+  // no-op launches after convergence did not run; the sweep count reflects the enqueued ones: correct it
+  c->st.sweeps -= (enq - done_it);
+  c->pair_evals -= static_cast<long long>(enq - done_it) * (static_cast<long long>(c->nb) * (c->nb + 1) / 2) * 1024;
   return QS_OK;
 }
 

@@ -19,6 +19,7 @@ struct SweepParams {
   double* bracc;          // [Np] += sum_j dz(-Kt + mid Qt) I_j   (scale mu0/(4 r_i) by the consumer)
   double* bzacc;          // [Np] += sum_j (Kt + c_ij Qt) I_j     (scale mu0/4 by the consumer)
   unsigned long long* counter;
+  const int* done;        // fused CG: the sweep returns at once when *done != 0 (nullptr: always run)
   long long n_items;      // nb (nb + 1) / 2
   int nb;
   int chunk;
@@ -44,13 +45,17 @@ cudaError_t fp64_peak_probe(double* tflops, double* sm_mhz);
 // Device scalars of the solver; all reductions land here (no host round trip inside an iteration).
 struct Scalars {
   double rg[2];          // r^T g, double buffered by iteration parity
-  double pq;             // p^T A p
+  double pq[2];          // p^T A p, double buffered by iteration parity
   double nu2;            // reference norm squared
   double uterm;          // sum_w vsum_w = terminal voltage
   double tmax, joule;    // step statistics
+  double thresh2;        // (cg_tol * nu)^2: the fused CG iterations stop themselves when rg <= thresh2
   int nonfinite;         // set when J or T is NaN/Inf
   int event_or;          // OR of per-turn return bits
-  int pad[2];
+  int done;              // fused CG: 0 running, 1 converged, 2 breakdown (p^T A p <= 0 or NaN); later launches no-op
+  int iters;             // fused CG: completed iterations
+  unsigned int blocks_done;   // last-block-done counter of the direction kernel
+  int pad;
 };
 
 struct VecCtx {
@@ -64,6 +69,27 @@ struct VecCtx {
   Scalars* sc;
   long long* launches;   // host counter
 };
+
+// ---- fused projected-CG iteration (C8): four launches after the sweep, no host round trip; every kernel returns at
+// once when sc->done is set, so a batch of iterations can be enqueued blind -----------------------------------------
+struct CgIter {
+  int par;                   // parity of this iteration: rg[par] old, rg[par^1] new, pq[par]
+  const double* yacc_in;     // sweep accumulators of p
+  const double* shift;       // diagonal shift theta dt D (zeros for the plain operator)
+  const double* Hd;          // diag(M) + shift
+  const double* sw;          // per-turn Schur scalars
+  double *x, *r, *g, *p, *q;
+  double* tw;                // [n_turns] per-turn sums of r/H (zero on entry, zero on exit)
+  double* vsum;              // [n_turns] accumulated multipliers
+  double* yacc_zero;         // accumulators to clear for the next sweep (Np doubles) ...
+  unsigned long long* counter;   // ... and its work counter
+  double cM;
+};
+void k_cg_Ap(const VecCtx& v, const CgIter& it);          // q = shift p + cM yacc ; pq[par] += p.q
+void k_cg_update(const VecCtx& v, const CgIter& it);      // alpha = rg[par]/pq[par]; x += alpha p; r += alpha q; tw += r/H
+void k_cg_project(const VecCtx& v, const CgIter& it);     // r -= tw/sw; g = r/H; rg[par^1] += r.g
+void k_cg_direction(const VecCtx& v, const CgIter& it);   // p = -g + beta p; clears accumulators; last block: bookkeeping
+void k_cg_begin(const VecCtx& v, double thresh2);         // done = 0, iters = 0, pq = 0, blocks_done = 0
 
 // q = cM*yacc + shift*p ; pq = p.q
 void k_finish_Ap(const VecCtx& v, const double* yacc, const double* shift, const double* p, double* q, double cM);

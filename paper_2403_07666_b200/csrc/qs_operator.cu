@@ -179,6 +179,7 @@ __global__ void __launch_bounds__(kThreads, FIELD ? 2 : 3) sweep_kernel(SweepPar
   __shared__ __align__(8) uint64_t sbar[kWarpsPerCta][2];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const unsigned full = 0xffffffffu;
+  if (prm.done != nullptr && *prm.done != 0) return;   // a converged CG batch: nothing left to do
   if (threadIdx.x < kWarpsPerCta * 2) mbar_init(&sbar[threadIdx.x >> 1][threadIdx.x & 1], 1);
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   __syncthreads();

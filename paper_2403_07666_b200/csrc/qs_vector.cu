@@ -55,7 +55,7 @@ __global__ void finish_Ap_kernel(int n, const double* __restrict__ yacc, const d
     q[i] = qi;
     acc = fma(pi, qi, acc);
   }
-  block_atomic_sum(acc, &sc->pq);
+  block_atomic_sum(acc, &sc->pq[0]);
 }
 
 __global__ void residual_kernel(int n, const double* __restrict__ yacc, const double* __restrict__ shift,
@@ -67,7 +67,7 @@ __global__ void residual_kernel(int n, const double* __restrict__ yacc, const do
 
 __global__ void update_xr_kernel(int n, int par, const double* __restrict__ p, const double* __restrict__ q,
                                  double* __restrict__ x, double* __restrict__ r, const Scalars* sc) {
-  const double alpha = sc->rg[par] / sc->pq;
+  const double alpha = sc->rg[par] / sc->pq[0];
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     x[i] = fma(alpha, p[i], x[i]);
     r[i] = fma(alpha, q[i], r[i]);
@@ -148,7 +148,7 @@ __global__ void direction_kernel(int n, int par, int first, const double* __rest
 // runs after direction_kernel (stream order): the scalars of the finished iteration are no longer needed
 __global__ void recycle_scalars_kernel(int par, Scalars* sc) {
   sc->rg[par ^ 1] = 0.0;
-  sc->pq = 0.0;
+  sc->pq[0] = 0.0;
 }
 
 __global__ void axpy_kernel(int n, double a, const double* __restrict__ x, double* __restrict__ y) {
@@ -162,7 +162,11 @@ __global__ void mul_kernel(int n, const double* __restrict__ a, const double* __
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) y[i] = a[i] * b[i];
 }
 __global__ void set_scalars_kernel(Scalars* sc) {
-  sc->rg[0] = sc->rg[1] = sc->pq = sc->nu2 = 0.0;
+  sc->rg[0] = sc->rg[1] = sc->pq[0] = sc->pq[1] = sc->nu2 = 0.0;
+  sc->done = 0;
+  sc->iters = 0;
+  sc->blocks_done = 0u;
+  sc->thresh2 = 0.0;
   sc->uterm = sc->joule = 0.0;
   sc->tmax = 0.0;
   sc->nonfinite = 0;
@@ -192,6 +196,108 @@ __global__ void scatter_scaled_kernel(int n, const double* __restrict__ src, con
                                       double* __restrict__ dst, double scale) {
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
     dst[perm ? perm[i] : i] = scale * src[i];
+}
+
+// ---- fused CG iteration ---------------------------------------------------------------------------------------------
+__global__ void cg_begin_kernel(Scalars* sc, double thresh2) {
+  sc->done = 0;
+  sc->iters = 0;
+  sc->pq[0] = sc->pq[1] = 0.0;
+  sc->blocks_done = 0u;
+  sc->thresh2 = thresh2;
+}
+
+__global__ void cg_Ap_kernel(int n, CgIter it, Scalars* sc) {
+  if (sc->done) return;
+  double acc = 0.0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const double pi = it.p[i];
+    const double qi = fma(it.shift[i], pi, it.cM * it.yacc_in[i]);
+    it.q[i] = qi;
+    acc = fma(pi, qi, acc);
+  }
+  block_atomic_sum(acc, &sc->pq[it.par]);
+}
+
+__global__ void cg_update_kernel(int n, CgIter it, const int* __restrict__ turn, Scalars* sc) {
+  if (sc->done) return;
+  const double pq = sc->pq[it.par];
+  if (!(pq > 0.0)) {   // breakdown: every thread sees the same pq and leaves the state alone
+    if (blockIdx.x == 0 && threadIdx.x == 0) sc->done = 2;
+    return;
+  }
+  const double alpha = sc->rg[it.par] / pq;
+  for (int base = blockIdx.x * blockDim.x; base < n; base += gridDim.x * blockDim.x) {
+    const int i = base + threadIdx.x;
+    const bool ok = i < n;
+    double t = 0.0;
+    int w = -1;
+    if (ok) {
+      it.x[i] = fma(alpha, it.p[i], it.x[i]);
+      const double ri = fma(alpha, it.q[i], it.r[i]);
+      it.r[i] = ri;
+      if (turn) {
+        t = ri / it.Hd[i];
+        w = turn[i];
+      }
+    }
+    if (turn) {   // per-turn sums: one atomic per warp when the warp lies inside one turn, else one per lane
+      const int w0 = __shfl_sync(0xffffffffu, w, 0);
+      if (__all_sync(0xffffffffu, w == w0 || !ok)) {
+        t = warp_sum(t);
+        if ((threadIdx.x & 31) == 0 && w0 >= 0) atomicAdd(it.tw + w0, t);
+      } else if (ok) {
+        atomicAdd(it.tw + w, t);
+      }
+    }
+  }
+}
+
+__global__ void cg_project_kernel(int n, CgIter it, const int* __restrict__ turn, Scalars* sc) {
+  if (sc->done) return;
+  double acc = 0.0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    double ri = it.r[i];
+    if (turn) {
+      const int w = turn[i];
+      ri -= it.tw[w] / it.sw[w];
+      it.r[i] = ri;
+    }
+    const double gi = ri / it.Hd[i];
+    it.g[i] = gi;
+    acc = fma(ri, gi, acc);
+  }
+  block_atomic_sum(acc, &sc->rg[it.par ^ 1]);
+}
+
+__global__ void cg_direction_kernel(int n, int npad, int n_turns, CgIter it, Scalars* sc) {
+  if (sc->done) return;
+  const double rg_new = sc->rg[it.par ^ 1];
+  const double beta = rg_new / sc->rg[it.par];
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < npad; i += gridDim.x * blockDim.x) {
+    if (i < n) it.p[i] = fma(beta, it.p[i], -it.g[i]);
+    it.yacc_zero[i] = 0.0;
+  }
+  // the last block to finish does the bookkeeping of the iteration: every block has read the scalars by then
+  __shared__ bool last;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) last = atomicAdd(&sc->blocks_done, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!last) return;
+  for (int w = threadIdx.x; w < n_turns; w += blockDim.x) {   // multipliers (C8): V = -sum of the subtracted v
+    it.vsum[w] += it.tw[w] / it.sw[w];
+    it.tw[w] = 0.0;
+  }
+  if (threadIdx.x == 0) {
+    sc->rg[it.par] = 0.0;
+    sc->pq[it.par] = 0.0;
+    sc->blocks_done = 0u;
+    *it.counter = 0ull;
+    sc->iters += 1;
+    if (!(rg_new == rg_new)) sc->done = 2;
+    else if (rg_new <= sc->thresh2) sc->done = 1;
+  }
 }
 }  // namespace
 
@@ -243,6 +349,26 @@ void k_direction(const VecCtx& v, int par, bool first, const double* g, double* 
   direction_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, par, first ? 1 : 0, g, p, v.sc);
   QS_LAUNCH(v);
   recycle_scalars_kernel<<<1, 1, 0, v.stream>>>(par, v.sc);
+}
+void k_cg_begin(const VecCtx& v, double thresh2) {
+  QS_LAUNCH(v);
+  cg_begin_kernel<<<1, 1, 0, v.stream>>>(v.sc, thresh2);
+}
+void k_cg_Ap(const VecCtx& v, const CgIter& it) {
+  QS_LAUNCH(v);
+  cg_Ap_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.sc);
+}
+void k_cg_update(const VecCtx& v, const CgIter& it) {
+  QS_LAUNCH(v);
+  cg_update_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.n_turns ? v.turn_id : nullptr, v.sc);
+}
+void k_cg_project(const VecCtx& v, const CgIter& it) {
+  QS_LAUNCH(v);
+  cg_project_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.n_turns ? v.turn_id : nullptr, v.sc);
+}
+void k_cg_direction(const VecCtx& v, const CgIter& it) {
+  QS_LAUNCH(v);
+  cg_direction_kernel<<<grid_for(v.Np), kBlock, 0, v.stream>>>(v.N, v.Np, v.n_turns, it, v.sc);
 }
 void k_axpy(const VecCtx& v, double a, const double* x, double* y) {
   QS_LAUNCH(v);

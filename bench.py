@@ -252,11 +252,11 @@ def hbm_roofline_leg(torch, pkg, hbm_peak):
         sim.set_fields(B=0.1 * g.standard_normal(2 * N), Q=1e3 * g.random(N))
         sub_dt = 1e-9
         for _ in range(3):
-            sim.material_eval(1e-4)
+            sim.material_eval(1e-4, aux=False)
             sim.heat(sub_dt)
         sim.profile_enable(True)
         for _ in range(10):
-            sim.material_eval(1e-4)
+            sim.material_eval(1e-4, aux=False)
         for _ in range(20):
             sim.heat(sub_dt)
         pr = sim.profile_read()

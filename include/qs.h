@@ -157,9 +157,11 @@ int  qs_solve_device(qs_ctx *ctx, const double *d_b, double *d_x, int32_t maxit_
  * parity of the pointwise passes and their HBM-roofline runs.  qs_set_fields loads B [2N] and/or
  * Q [N] (NULL = keep).  qs_heat returns m.  */
 int  qs_material_eval(qs_ctx *ctx, double dt);
+int  qs_set_aux(qs_ctx *ctx, int32_t on);   /* on: qs_material_eval also stores dE/dJ for qs_read_aux (off by default:
+                                               the step itself never needs the array) */
 int  qs_heat(qs_ctx *ctx, double dt);
 int  qs_set_fields(qs_ctx *ctx, const double *B, const double *Q);
-int  qs_read_aux(qs_ctx *ctx, double *Q, double *dEdJ, double *Jc, double *rho);
+int  qs_read_aux(qs_ctx *ctx, double *Q, double *dEdJ, double *Jc, double *rho);   /* dEdJ: see qs_set_aux */
 
 int  qs_stats(qs_ctx *ctx, qs_stats_t *out);
 

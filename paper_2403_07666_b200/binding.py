@@ -66,6 +66,7 @@ SYMBOLS = [
     ("qs_solve", C.c_int, [_VP, c_double_p, c_double_p, C.c_int32, c_int32_p, c_double_p]),
     ("qs_solve_device", C.c_int, [_VP, _VP, _VP, C.c_int32, c_int32_p, c_double_p]),
     ("qs_material_eval", C.c_int, [_VP, C.c_double]),
+    ("qs_set_aux", C.c_int, [_VP, C.c_int32]),
     ("qs_heat", C.c_int, [_VP, C.c_double]),
     ("qs_set_fields", C.c_int, [_VP, c_double_p, c_double_p]),
     ("qs_read_aux", C.c_int, [_VP, c_double_p, c_double_p, c_double_p, c_double_p]),
@@ -269,7 +270,9 @@ class QS:
                                                    C.byref(it), C.byref(rel)))
         return it.value, rel.value, rc
 
-    def material_eval(self, dt: float = 0.0):
+    def material_eval(self, dt: float = 0.0, aux: bool = True):
+        """S2 alone on the current (J, T, B); aux: also store dE/dJ for read_aux (the step never does)."""
+        self._check(self._lib.qs_set_aux(self._h, 1 if aux else 0))
         self._check(self._lib.qs_material_eval(self._h, float(dt)))
 
     def heat(self, dt: float) -> int:

@@ -125,6 +125,9 @@ struct qs_ctx {
   size_t acc_bytes = 0;
   double *sw, *swM, *vw, *vsum, *tw, *defw, *ebar_prev, *t_first;
   int *flags, *count, *turn_ptr, *turn_idx, *turn_id, *d_perm;
+  double4* rowtab = nullptr;         // [Nr] (r, selfcoef, diagM, area) per radial row of a lattice
+  bool aux_on = false;               // qs_material_eval also writes dE/dJ (after the first qs_read_aux)
+  double last_eval_dt = 0.0;
   double* heat_tab = nullptr;        // hr_p, hr_m, rb_r [Nr each], hz_p, hz_m, rb_z [Nz each]
   int tabNr = 0, tabNz = 0;
   double4* bbox;
@@ -203,6 +206,7 @@ void carve(qs_ctx* c, void* base, size_t* total) {
   c->d_perm = k.take<int>(N);
   c->bbox = k.take<double4>(std::max(c->nb, 1));
   c->heat_tab = k.take<double>(3 * static_cast<size_t>(c->tabNr + c->tabNz) + 1);
+  c->rowtab = k.take<double4>(static_cast<size_t>(c->tabNr) + 1);
   c->sc = k.take<Scalars>(1);
   *total = align_up(k.off, 256);
 }
@@ -268,7 +272,7 @@ constexpr double kCM = 0.5 * kMu0 * kPi;   // yacc -> henry * ampere
 // In: x satisfies the constraint; if yacc_has_Mx the accumulators hold the sweep of x.  nu < 0: nu = start norm.
 // Iterations are enqueued in batches without a host round trip: the kernels stop themselves (Scalars::done) at the
 // iteration where sqrt(r^T g) <= tol nu, so the result is the one of the iteration-by-iteration loop.
-int cg_core(qs_ctx* c, const double* b, double* x, const double* shift, const double* Hd, const double* sw,
+int cg_core(qs_ctx* c, const Rhs& b, double* x, const double* shift, const double* Hd, const double* sw,
             bool yacc_has_Mx, double tol, int maxit, double nu, int* iters, double* relres, bool* hit_max) {
   const VecCtx& v = c->v;
   int rc;
@@ -366,28 +370,29 @@ int run_heat(qs_ctx* c, double dt, int* m_out) {
   return QS_OK;
 }
 
-MaterialArgs material_args(qs_ctx* c, double Bext, double Bdot, double dt, bool from_acc) {
+MaterialArgs material_args(qs_ctx* c, double Bext, double Bdot, double dt, bool from_acc, bool aux) {
   MaterialArgs a;
   a.N = c->N;
+  a.Nz = c->lattice ? c->lp.Nz : 0;
   a.J = c->J;
   a.H = c->H;
-  a.r = c->r;
-  a.area = c->area;
   a.jc0_scale = c->jc0s;
-  a.selfcoef = c->selfcoef;
   a.bracc = c->bracc;
   a.bzacc = c->bzacc;
+  a.rowtab = c->rowtab;
+  a.r = c->r;
+  a.area = c->area;
+  a.selfcoef = c->selfcoef;
   a.diagM = c->diagM;
   a.Br = c->Br;
   a.Bz = c->Bz;
   a.E = c->E;
-  a.dEdJ = c->dEdJ;
   a.Q = c->Q;
-  a.b = c->b;
   a.shift = c->shift;
   a.Hd = c->Hd;
   a.Jc = c->Jc;
   a.rho = c->rho;
+  a.dEdJ = aux ? c->dEdJ : nullptr;
   a.Bext = Bext;
   a.Bdot = Bdot;
   a.dt = dt;
@@ -642,6 +647,7 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
     ++c->launches;
     if (cudaMemcpyAsync(c->Hd, c->diagM, sizeof(double) * N, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
       return bail(fail(QS_ERR_CUDA, "copy"));
+    if (c->lattice) k_build_rowtab(v, lp.Nr, lp.Nz, c->r, c->selfcoef, c->diagM, c->area, c->rowtab);
     if (c->n_turns) {
       // unit-ramp particular solution x_p1 = H_M^-1 C (1/s_M) and M x_p1 (reference norm of the CG, C8)
       k_turn_schur(v, c->diagM, c->swM);
@@ -656,6 +662,7 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
       k_scatter_scaled(v, c->yacc, nullptr, c->Mxp1, N, kCM);
     }
   }
+  if (c->lattice && !c->has_operator) k_build_rowtab(v, lp.Nr, lp.Nz, c->r, c->selfcoef, c->diagM, c->area, c->rowtab);
   if (cudaStreamSynchronize(c->stream) != cudaSuccess || cudaGetLastError() != cudaSuccess)
     return bail(fail(QS_ERR_CUDA, std::string("initialisation kernels failed: ") + cudaGetErrorString(cudaGetLastError())));
   c->st = qs_stats_t{};
@@ -736,18 +743,19 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
   // S2
   const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
   c->prof.begin(c->stream);
-  k_material(v, c->mp, material_args(c, B0, (B1 - B0) / dt, dt, true));
+  k_material(v, c->mp, material_args(c, B0, (B1 - B0) / dt, dt, true, false));
   c->prof.end(c->stream, QS_PROF_MATERIAL, 1);
-  // S3/S4
+  // S3/S4: the right-hand side b = -2 pi r (E + r Bdot / 2) is evaluated on the fly from E (C4)
+  const Rhs rhs{nullptr, c->E, c->r, (B1 - B0) / dt};
   double nu = -1.0;
   if (c->n_turns) {
     k_turn_schur(v, c->Hd, c->sw);
-    k_nu_residual(v, I_ramp, c->Mxp1, c->shift, c->xp1, c->b, c->rr);
+    k_nu_residual(v, I_ramp, c->Mxp1, c->shift, c->xp1, rhs, c->rr);
     k_turn_project(v, c->rr, c->Hd, c->sw, c->vw, nullptr);
     k_project_apply(v, 0, c->vw, c->Hd, c->rr, c->g);
     k_copy_rg_to_nu2(v, 0);
   } else {  // no constraint: nu^2 = b^T H^-1 b
-    QS_CUDA(cudaMemcpyAsync(c->rr, c->b, nb8, cudaMemcpyDeviceToDevice, c->stream));
+    k_rhs_fill(v, rhs, c->rr);
     k_project_apply(v, 0, nullptr, c->Hd, c->rr, c->g);
     k_copy_rg_to_nu2(v, 0);
   }
@@ -761,7 +769,7 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
     cudaStreamSynchronize(c->stream);
   };
   if (nu > 0.0) {
-    rc = cg_core(c, c->b, c->x, c->shift, c->Hd, c->sw, true, c->cg_tol, c->cg_maxit, nu, &iters, &relres, &hit_max);
+    rc = cg_core(c, rhs, c->x, c->shift, c->Hd, c->sw, true, c->cg_tol, c->cg_maxit, nu, &iters, &relres, &hit_max);
     if (rc != QS_OK) {
       restore();
       return rc;
@@ -908,7 +916,8 @@ int qs_solve_device(qs_ctx* c, const double* d_b, double* d_x, int32_t maxit_ove
   int it = 0;
   double rel = 0.0;
   bool hit = false;
-  int rc = cg_core(c, c->b, c->tmp, c->zero, c->diagM, c->swM, true, c->cg_tol, maxit_override > 0 ? maxit_override : c->cg_maxit,
+  const Rhs rhs{c->b, nullptr, nullptr, 0.0};
+  int rc = cg_core(c, rhs, c->tmp, c->zero, c->diagM, c->swM, true, c->cg_tol, maxit_override > 0 ? maxit_override : c->cg_maxit,
                    -1.0, &it, &rel, &hit);
   if (rc != QS_OK) return rc;
   k_scatter_scaled(c->v, c->tmp, perm, d_x, c->N, 1.0);
@@ -948,9 +957,15 @@ int qs_material_eval(qs_ctx* c, double dt) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
   const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
   c->prof.begin(c->stream);
-  k_material(c->v, c->mp, material_args(c, B0, dt > 0 ? (B1 - B0) / dt : 0.0, dt, false));
+  k_material(c->v, c->mp, material_args(c, B0, dt > 0 ? (B1 - B0) / dt : 0.0, dt, false, c->aux_on));
   c->prof.end(c->stream, QS_PROF_MATERIAL, 1);
   QS_CUDA(cudaGetLastError());
+  return QS_OK;
+}
+
+int qs_set_aux(qs_ctx* c, int32_t on) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  c->aux_on = on != 0;
   return QS_OK;
 }
 

@@ -91,11 +91,21 @@ void k_cg_project(const VecCtx& v, const CgIter& it);     // r -= tw/sw; g = r/H
 void k_cg_direction(const VecCtx& v, const CgIter& it);   // p = -g + beta p; clears accumulators; last block: bookkeeping
 void k_cg_begin(const VecCtx& v, double thresh2);         // done = 0, iters = 0, pq = 0, blocks_done = 0
 
+// Right-hand side of the circuit equations: a given array, or (inside qs_step) evaluated on the fly from the
+// material law's E as b_i = -2 pi r_i (E_i + r_i Bdot_ext / 2)   (C4)
+struct Rhs {
+  const double* b;       // non-null: use this array
+  const double* E;       // else: E [V/m] ...
+  const double* radius;  // ... ring radius [m] ...
+  double Bdot;           // ... and the background-field slope [T/s]
+};
+
 // q = cM*yacc + shift*p ; pq = p.q
 void k_finish_Ap(const VecCtx& v, const double* yacc, const double* shift, const double* p, double* q, double cM);
 // r = cM*yacc + shift*x - b
-void k_residual(const VecCtx& v, const double* yacc, const double* shift, const double* x, const double* b, double* r,
+void k_residual(const VecCtx& v, const double* yacc, const double* shift, const double* x, const Rhs& b, double* r,
                 double cM);
+void k_rhs_fill(const VecCtx& v, const Rhs& b, double* r);      // r = b
 // alpha = rg[par]/pq ; x += alpha p ; r += alpha q
 void k_update_xr(const VecCtx& v, int par, const double* p, const double* q, double* x, double* r);
 // tw = sum_{i in w} r_i/H_i ; vw = tw/s_w ; vsum += vw      (one warp per turn)
@@ -116,7 +126,7 @@ void k_set_scalars(const VecCtx& v);                                            
 void k_copy_rg_to_nu2(const VecCtx& v, int par);
 // r = I_ramp (Mxp1 + shift xp1) - b : residual of the cold start x_p = I_ramp xp1 (reference norm, C8)
 void k_nu_residual(const VecCtx& v, double I_ramp, const double* Mxp1, const double* shift, const double* xp1,
-                   const double* b, double* r);
+                   const Rhs& b, double* r);
 void k_sum_uterm(const VecCtx& v, const double* vsum);                                  // sc->uterm = sum vsum
 void k_gather(const VecCtx& v, const double* src, const int* perm, double* dst, int n, int npad);   // dst[k] = src[perm[k]], pad 0
 void k_scatter_scaled(const VecCtx& v, const double* src, const int* perm, double* dst, int n, double scale);  // dst[perm[k]] = scale*src[k]
@@ -142,11 +152,18 @@ struct LatticeParams {
 };
 struct MaterialArgs {
   int N;
-  const double *J, *H, *r, *area, *jc0_scale, *selfcoef, *bracc, *bzacc, *diagM;
-  double *Br, *Bz, *E, *dEdJ, *Q, *b, *shift, *Hd, *Jc, *rho;
+  int Nz;                // > 0: lattice, per-row geometry from rowtab[i / Nz]; 0: per-cell arrays r, area, selfcoef, diagM
+  const double *J, *H, *jc0_scale, *bracc, *bzacc;
+  const double4* rowtab; // [Nr] (r, selfcoef, diagM, area) of the cells of radial row ir
+  const double *r, *area, *selfcoef, *diagM;
+  double *Br, *Bz;       // read when !from_acc, written when from_acc
+  double *E, *Q, *shift, *Hd, *Jc, *rho;
+  double* dEdJ;          // optional (test hook), may be null
   double Bext, Bdot, dt;
   bool from_acc;         // true: B from the sweep accumulators (+ self + Bext); false: B arrays given
 };
+void k_build_rowtab(const VecCtx& v, int Nr, int Nz, const double* r, const double* selfcoef, const double* diagM,
+                    const double* area, double4* rowtab);
 void k_material(const VecCtx& v, const MaterialParams& mp, const MaterialArgs& a);
 void k_enthalpy_from_T(const VecCtx& v, const MaterialParams& mp, const double* T, double* H, int n);
 void k_T_from_enthalpy(const VecCtx& v, const MaterialParams& mp, const double* H, double* T, int n);

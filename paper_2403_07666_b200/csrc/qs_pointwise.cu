@@ -51,25 +51,78 @@ __device__ __forceinline__ double tsq_of_H(double H, double C3, double C1) {
   return (-0.5 * C1 + sqrt(0.25 * C1 * C1 + C3 * H)) / (0.5 * C3);
 }
 
-__global__ void material_kernel(MaterialParams mp, MaterialArgs a) {
+// T^2 from H with the fast reciprocal square root (MUFU seed + one Halley step): argument > 0 always (H >= 0)
+__device__ __forceinline__ double tsq_fast(double H, double C3, double qC1sq, double hC1, double inv_hC3) {
+  const double a = fma(C3, H, qC1sq);                 // C1^2/4 + C3 H
+  const double y0 = rsqrt_seed(a);
+  const double g = a * y0;
+  const double e = fma(-g, y0, 1.0);
+  const double s = fma(g * e, fma(0.375, e, 0.5), g); // sqrt(a)
+  return (s - hC1) * inv_hC3;
+}
+
+// 1/x for a positive normal x: MUFU seed + two Newton steps (relative error ~ 1 ulp)
+__device__ __forceinline__ double rcp_fast(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-x, y, 1.0);
+  return fma(y, e, y);
+}
+// sqrt(a), a >= 0: MUFU seed + one Halley step; exact zero for a == 0
+__device__ __forceinline__ double sqrt_pos(double a) {
+  const double y0 = rsqrt_seed(fmax(a, 1e-300));
+  const double g = a * y0;
+  const double e = fma(-g, y0, 1.0);
+  return fma(g * e, fma(0.375, e, 0.5), g);
+}
+// x^k, k >= 0 integer, by binary powering
+__device__ __forceinline__ double ipow_bin(double x, int k) {
+  double r = 1.0;
+  while (k) {
+    if (k & 1) r *= x;
+    x *= x;
+    k >>= 1;
+  }
+  return r;
+}
+
+struct MaterialConsts {   // host-side reciprocals of the constant divisors (qs_material)
+  double inv_Tc, inv_B0, inv_Y, inv_rho_n, hC1, qC1sq, inv_hC3;
+};
+
+__global__ void __launch_bounds__(256) material_kernel(MaterialParams mp, MaterialConsts k, MaterialArgs a) {
   const double two_pi = 2.0 * kPi;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < a.N; i += gridDim.x * blockDim.x) {
-    const double J = a.J[i], r = a.r[i], area = a.area[i];
-    const double T = sqrt(tsq_of_H(a.H[i], mp.C3, mp.C1));
+    double r, area, selfc, dM;
+    if (a.Nz > 0) {
+      const double4 t = a.rowtab[i / a.Nz];
+      r = t.x, selfc = t.y, dM = t.z, area = t.w;
+    } else {
+      r = a.r[i], area = a.area[i], selfc = a.selfcoef[i], dM = a.diagM[i];
+    }
+    const double J = a.J[i];
+    const double U = tsq_fast(a.H[i], mp.C3, k.qC1sq, k.hC1, k.inv_hC3);
+    const double T = sqrt_pos(U);
     double Br, Bz;
     if (a.from_acc) {
-      Br = (0.25 * kMu0) * a.bracc[i] / r;
-      Bz = (0.25 * kMu0) * a.bzacc[i] + a.selfcoef[i] * (area * J) + a.Bext;
+      Br = (0.25 * kMu0) * a.bracc[i] * rcp_fast(r);
+      Bz = (0.25 * kMu0) * a.bzacc[i] + selfc * (area * J) + a.Bext;
+      a.Br[i] = Br;
+      a.Bz[i] = Bz;
     } else {
       Br = a.Br[i];
       Bz = a.Bz[i];
     }
-    const double eps = J * Bz * r / mp.Y;
-    const double Bmag = sqrt(Br * Br + Bz * Bz);
-    const double fT = fmax(1.0 - T / mp.Tc, 0.0);
-    const double fe = fmax(1.0 - mp.eps_coef * pow(fabs(eps), mp.eps_exp), 0.0);
+    const double eps = J * Bz * r * k.inv_Y;
+    const double Bmag = sqrt_pos(fma(Br, Br, Bz * Bz));
+    const double fT = fmax(fma(-T, k.inv_Tc, 1.0), 0.0);
+    const double ae = fabs(eps);
+    const double pw = ae > 0.0 ? exp(mp.eps_exp * log(ae)) : 0.0;       // |eps|^eps_exp
+    const double fe = fmax(fma(-mp.eps_coef, pw, 1.0), 0.0);
     const double s = a.jc0_scale ? a.jc0_scale[i] : 1.0;
-    const double Jc = mp.Jc0 * s * fT * fT / (1.0 + Bmag / mp.B0) * fe;
+    const double Jc = mp.Jc0 * s * fT * fT * rcp_fast(fma(Bmag, k.inv_B0, 1.0)) * fe;
     double rho, dEdJ;
     if (Jc <= 0.0) {
       rho = mp.rho_n;
@@ -78,33 +131,35 @@ __global__ void material_kernel(MaterialParams mp, MaterialArgs a) {
       rho = 0.0;
       dEdJ = 0.0;
     } else {
-      const double x = fabs(J) / Jc;
-      double xp = 1.0;
-      if (mp.n_int > 0) {
-        for (int k = 1; k < mp.n_int; ++k) xp *= x;          // x^(n-1), same multiplication chain as the oracle
-      } else {
-        xp = pow(x, mp.n_exp - 1.0);
-      }
-      const double rho_sc = (mp.Ec / Jc) * xp;
+      const double invJc = rcp_fast(Jc);
+      const double x = fabs(J) * invJc;
+      const double xp = mp.n_int > 0 ? ipow_bin(x, mp.n_int - 1) : exp((mp.n_exp - 1.0) * log(x));
+      const double rho_sc = (mp.Ec * invJc) * xp;
       const bool big = rho_sc >= mp.rho_n;
-      const double u = big ? mp.rho_n / rho_sc : rho_sc / mp.rho_n;     // in [0, 1], no inf/inf
-      rho = (big ? mp.rho_n : rho_sc) / (1.0 + u);
-      const double w = (big ? u : 1.0) / (1.0 + u);
-      dEdJ = rho * (1.0 + (mp.n_exp - 1.0) * w);
+      const double u = big ? mp.rho_n / rho_sc : rho_sc * k.inv_rho_n;    // in [0, 1], no inf/inf (rho_sc may be inf)
+      const double inv1u = rcp_fast(1.0 + u);
+      rho = (big ? mp.rho_n : rho_sc) * inv1u;
+      dEdJ = rho * fma(mp.n_exp - 1.0, (big ? u : 1.0) * inv1u, 1.0);
     }
     const double E = rho * J;
-    a.Br[i] = Br;
-    a.Bz[i] = Bz;
     a.E[i] = E;
-    a.dEdJ[i] = dEdJ;
     a.Q[i] = E * J;
     a.Jc[i] = Jc;
     a.rho[i] = rho;
-    a.b[i] = -two_pi * r * (E + 0.5 * r * a.Bdot);
-    const double shift = mp.theta * a.dt * (two_pi * r * dEdJ / area);
+    if (a.dEdJ) a.dEdJ[i] = dEdJ;
+    const double shift = mp.theta * a.dt * (two_pi * r * dEdJ * rcp_fast(area));
     a.shift[i] = shift;
-    a.Hd[i] = a.diagM[i] + shift;
+    a.Hd[i] = dM + shift;
   }
+}
+
+__global__ void rowtab_kernel(int Nr, int Nz, const double* __restrict__ r, const double* __restrict__ selfcoef,
+                              const double* __restrict__ diagM, const double* __restrict__ area,
+                              double4* __restrict__ rowtab) {
+  const int ir = blockIdx.x * blockDim.x + threadIdx.x;
+  if (ir >= Nr) return;
+  const long long c = static_cast<long long>(ir) * Nz;
+  rowtab[ir] = make_double4(r[c], selfcoef[c], diagM[c], area[c]);
 }
 
 __global__ void enthalpy_kernel(int n, double C3, double C1, const double* __restrict__ T, double* __restrict__ H) {
@@ -129,16 +184,6 @@ constexpr int kHeatLanes = 30;           // owner lanes per warp (lanes 0 and 31
 constexpr int kHeatCols = 2 * kHeatLanes; // useful columns per warp: every lane holds two adjacent columns
 constexpr int kHeatWarps = 8;
 constexpr int kHeatMaxRows = 32;
-
-// T^2 from H with the fast reciprocal square root (MUFU seed + one Halley step): argument > 0 always (H >= 0)
-__device__ __forceinline__ double tsq_fast(double H, double C3, double qC1sq, double hC1, double inv_hC3) {
-  const double a = fma(C3, H, qC1sq);                 // C1^2/4 + C3 H
-  const double y0 = rsqrt_seed(a);
-  const double g = a * y0;
-  const double e = fma(-g, y0, 1.0);
-  const double s = fma(g * e, fma(0.375, e, 0.5), g); // sqrt(a)
-  return (s - hC1) * inv_hC3;
-}
 
 // T from T^2 (border cells only), same fast root
 __device__ __forceinline__ double sqrt_fast(double a) {
@@ -303,7 +348,20 @@ __global__ void stats_kernel(int n, double C3, double C1, const double* __restri
 
 void k_material(const VecCtx& v, const MaterialParams& mp, const MaterialArgs& a) {
   QS_LAUNCH(v);
-  material_kernel<<<grid_for(a.N), kBlock, 0, v.stream>>>(mp, a);
+  MaterialConsts k;
+  k.inv_Tc = 1.0 / mp.Tc;
+  k.inv_B0 = 1.0 / mp.B0;
+  k.inv_Y = 1.0 / mp.Y;
+  k.inv_rho_n = 1.0 / mp.rho_n;
+  k.hC1 = 0.5 * mp.C1;
+  k.qC1sq = 0.25 * mp.C1 * mp.C1;
+  k.inv_hC3 = 2.0 / mp.C3;
+  material_kernel<<<grid_for(a.N), kBlock, 0, v.stream>>>(mp, k, a);
+}
+void k_build_rowtab(const VecCtx& v, int Nr, int Nz, const double* r, const double* selfcoef, const double* diagM,
+                    const double* area, double4* rowtab) {
+  QS_LAUNCH(v);
+  rowtab_kernel<<<(Nr + 127) / 128, 128, 0, v.stream>>>(Nr, Nz, r, selfcoef, diagM, area, rowtab);
 }
 void k_enthalpy_from_T(const VecCtx& v, const MaterialParams& mp, const double* T, double* H, int n) {
   QS_LAUNCH(v);

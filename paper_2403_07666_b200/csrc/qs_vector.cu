@@ -58,11 +58,19 @@ __global__ void finish_Ap_kernel(int n, const double* __restrict__ yacc, const d
   block_atomic_sum(acc, &sc->pq[0]);
 }
 
+__device__ __forceinline__ double rhs_at(const Rhs& b, int i) {
+  if (b.b) return b.b[i];
+  const double r = b.radius[i];
+  return -2.0 * kPi * r * (b.E[i] + 0.5 * r * b.Bdot);
+}
+
 __global__ void residual_kernel(int n, const double* __restrict__ yacc, const double* __restrict__ shift,
-                                const double* __restrict__ x, const double* __restrict__ b, double* __restrict__ r,
-                                double cM) {
+                                const double* __restrict__ x, Rhs b, double* __restrict__ r, double cM) {
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
-    r[i] = fma(shift[i], x[i], cM * yacc[i]) - b[i];
+    r[i] = fma(shift[i], x[i], cM * yacc[i]) - rhs_at(b, i);
+}
+__global__ void rhs_fill_kernel(int n, Rhs b, double* __restrict__ r) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) r[i] = rhs_at(b, i);
 }
 
 __global__ void update_xr_kernel(int n, int par, const double* __restrict__ p, const double* __restrict__ q,
@@ -177,10 +185,10 @@ __global__ void copy_rg_to_nu2_kernel(int par, Scalars* sc) {
   sc->rg[par] = 0.0;
 }
 __global__ void nu_residual_kernel(int n, double I_ramp, const double* __restrict__ Mxp1,
-                                   const double* __restrict__ shift, const double* __restrict__ xp1,
-                                   const double* __restrict__ b, double* __restrict__ r) {
+                                   const double* __restrict__ shift, const double* __restrict__ xp1, Rhs b,
+                                   double* __restrict__ r) {
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
-    r[i] = I_ramp * fma(shift[i], xp1[i], Mxp1[i]) - b[i];
+    r[i] = I_ramp * fma(shift[i], xp1[i], Mxp1[i]) - rhs_at(b, i);
 }
 __global__ void sum_uterm_kernel(int n, const double* __restrict__ vsum, Scalars* sc) {
   double acc = 0.0;
@@ -307,7 +315,11 @@ void k_finish_Ap(const VecCtx& v, const double* yacc, const double* shift, const
   QS_LAUNCH(v);
   finish_Ap_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, yacc, shift, p, q, cM, v.sc);
 }
-void k_residual(const VecCtx& v, const double* yacc, const double* shift, const double* x, const double* b, double* r,
+void k_rhs_fill(const VecCtx& v, const Rhs& b, double* r) {
+  QS_LAUNCH(v);
+  rhs_fill_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, b, r);
+}
+void k_residual(const VecCtx& v, const double* yacc, const double* shift, const double* x, const Rhs& b, double* r,
                 double cM) {
   QS_LAUNCH(v);
   residual_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, yacc, shift, x, b, r, cM);
@@ -391,7 +403,7 @@ void k_copy_rg_to_nu2(const VecCtx& v, int par) {
   copy_rg_to_nu2_kernel<<<1, 1, 0, v.stream>>>(par, v.sc);
 }
 void k_nu_residual(const VecCtx& v, double I_ramp, const double* Mxp1, const double* shift, const double* xp1,
-                   const double* b, double* r) {
+                   const Rhs& b, double* r) {
   QS_LAUNCH(v);
   nu_residual_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, I_ramp, Mxp1, shift, xp1, b, r);
 }

@@ -396,6 +396,7 @@ MaterialArgs material_args(qs_ctx* c, double Bext, double Bdot, double dt, bool 
   a.Bext = Bext;
   a.Bdot = Bdot;
   a.dt = dt;
+  a.inv_area = c->lattice ? 1.0 / (c->lp.h * c->lp.h) : 0.0;
   a.from_acc = from_acc;
   return a;
 }

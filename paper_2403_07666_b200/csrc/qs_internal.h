@@ -160,6 +160,7 @@ struct MaterialArgs {
   double *E, *Q, *shift, *Hd, *Jc, *rho;
   double* dEdJ;          // optional (test hook), may be null
   double Bext, Bdot, dt;
+  double inv_area;       // lattice: 1 / (h h)
   bool from_acc;         // true: B from the sweep accumulators (+ self + Bext); false: B arrays given
 };
 void k_build_rowtab(const VecCtx& v, int Nr, int Nz, const double* r, const double* selfcoef, const double* diagM,

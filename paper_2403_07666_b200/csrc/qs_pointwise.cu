@@ -11,6 +11,7 @@
 
 #include "qs_internal.h"
 #include "qs_pair.cuh"
+#include "qs_tma.cuh"
 
 namespace qs {
 
@@ -327,6 +328,119 @@ __global__ void __launch_bounds__(kHeatWarps * 32, 3) heat_kernel(MaterialParams
   }
 }
 
+// ---- K6, TMA-pipelined variant (Nz even): same marching scheme, but every warp streams its 512-byte row segments
+// of H and Q through a ring of kHeatStages shared-memory stages with TMA bulk copies (cp.async.bulk + mbarrier,
+// issued by lane 0), so that kHeatStages rows per warp are in flight whatever the register budget.
+constexpr int kHeatStages = 6;
+struct HeatStage {
+  double h[64];
+  double q[64];
+};
+struct HeatSmem {
+  HeatStage st[kHeatWarps][kHeatStages];
+  double4 srow[kHeatMaxRows];
+  uint64_t bar[kHeatWarps][kHeatStages];
+};
+
+__global__ void __launch_bounds__(kHeatWarps * 32, 3) heat_tma_kernel(MaterialParams mp, LatticeParams lp,
+                                                                      int rows_per_cta, const double* __restrict__ Hin,
+                                                                      const double* __restrict__ Q,
+                                                                      double* __restrict__ Hout, double dtsub) {
+  extern __shared__ __align__(128) unsigned char heat_smem_raw[];
+  HeatSmem& sm = *reinterpret_cast<HeatSmem*>(heat_smem_raw);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int r0 = blockIdx.y * rows_per_cta, r1 = min(r0 + rows_per_cta, lp.Nr), nrows = r1 - r0;
+  if (threadIdx.x < nrows)
+    sm.srow[threadIdx.x] = make_double4(lp.hr_p[r0 + threadIdx.x], lp.hr_m[r0 + threadIdx.x], lp.rb_r[r0 + threadIdx.x], 0.0);
+  if (threadIdx.x < kHeatWarps * kHeatStages) mbar_init(&sm.bar[threadIdx.x / kHeatStages][threadIdx.x % kHeatStages], 1);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  __syncthreads();
+  const int col_lo = (blockIdx.x * kHeatWarps + warp) * kHeatCols - 2;      // first column of the warp's 64-wide window
+  const int cs = max(col_lo, 0), ce = min(col_lo + 64, lp.Nz);             // clipped to the pack
+  if (col_lo + 2 >= lp.Nz) return;                                          // no owned column in this warp
+  const uint32_t seg_bytes = static_cast<uint32_t>(ce - cs) * 8u;
+  const int soff = cs - col_lo;
+  const int iz0 = col_lo + 2 * lane;
+  const bool in0 = iz0 >= 0 && iz0 < lp.Nz, in1 = iz0 + 1 >= 0 && iz0 + 1 < lp.Nz;
+  const bool own0 = lane >= 1 && lane <= kHeatLanes && in0;
+  const double C3 = mp.C3, qC1sq = 0.25 * mp.C1 * mp.C1, hC1 = 0.5 * mp.C1, inv_hC3 = 2.0 / mp.C3;
+  const double zp0 = in0 ? lp.hz_p[iz0] : 0.0, zm0 = in0 ? lp.hz_m[iz0] : 0.0, zb0 = in0 ? lp.rb_z[iz0] : 0.0;
+  const double zp1 = in1 ? lp.hz_p[iz0 + 1] : 0.0, zm1 = in1 ? lp.hz_m[iz0 + 1] : 0.0, zb1 = in1 ? lp.rb_z[iz0 + 1] : 0.0;
+  const bool zborder = (zb0 != 0.0) || (zb1 != 0.0);
+  const long long Nz = lp.Nz;
+  // stage t holds row g = r0 - 1 + t of H (0 <= t <= nrows + 1) and, for 1 <= t <= nrows, of Q
+  const int T_last = nrows + 1;
+  auto row_ok = [&](int t) { const int g = r0 - 1 + t; return g >= 0 && g < lp.Nr; };
+  auto fill = [&](int t) {
+    if (lane != 0 || t > T_last) return;
+    HeatStage& s = sm.st[warp][t % kHeatStages];
+    uint64_t* b = &sm.bar[warp][t % kHeatStages];
+    if (!row_ok(t)) {          // a row outside the pack: complete the phase empty, the parity sequence stays regular
+      mbar_arrive(b);
+      return;
+    }
+    const bool needq = t >= 1 && t <= nrows;
+    const long long off = static_cast<long long>(r0 - 1 + t) * Nz + cs;
+    mbar_expect_tx(b, needq ? 2u * seg_bytes : seg_bytes);
+    bulk_g2s(&s.h[soff], Hin + off, seg_bytes, b);
+    if (needq) bulk_g2s(&s.q[soff], Q + off, seg_bytes, b);
+  };
+  auto take = [&](int t, double2& h, double2& q) {   // waits for stage t and copies this lane's column pair out
+    h = make_double2(0.0, 0.0);
+    q = h;
+    const HeatStage& s = sm.st[warp][t % kHeatStages];
+    mbar_wait(&sm.bar[warp][t % kHeatStages], (t / kHeatStages) & 1);
+    if (!row_ok(t)) {
+      __syncwarp();
+      fill(t + kHeatStages);
+      return;
+    }
+    const double2 hv = *reinterpret_cast<const double2*>(&s.h[2 * lane]);
+    const double2 qv = *reinterpret_cast<const double2*>(&s.q[2 * lane]);
+    h = make_double2(in0 ? hv.x : 0.0, in1 ? hv.y : 0.0);
+    if (t >= 1 && t <= nrows) q = make_double2(in0 ? qv.x : 0.0, in1 ? qv.y : 0.0);
+    __syncwarp();
+    fill(t + kHeatStages);
+  };
+#pragma unroll
+  for (int t = 0; t < kHeatStages; ++t) fill(t);
+  double2 h, qc, qn;
+  take(0, h, qc);
+  double2 Up = make_double2(0.0, 0.0);
+  if (r0 > 0) Up = make_double2(tsq_fast(h.x, C3, qC1sq, hC1, inv_hC3), tsq_fast(h.y, C3, qC1sq, hC1, inv_hC3));
+  double2 Hc;
+  take(1, Hc, qc);
+  double2 Uc = make_double2(tsq_fast(Hc.x, C3, qC1sq, hC1, inv_hC3), tsq_fast(Hc.y, C3, qC1sq, hC1, inv_hC3));
+  double* o = Hout + static_cast<long long>(r0) * Nz + max(iz0, 0);
+  for (int k = 0; k < nrows; ++k) {
+    double2 Hn;
+    take(k + 2, Hn, qn);
+    const double2 Un = make_double2(tsq_fast(Hn.x, C3, qC1sq, hC1, inv_hC3), tsq_fast(Hn.y, C3, qC1sq, hC1, inv_hC3));
+    const double Ul = __shfl_up_sync(0xffffffffu, Uc.y, 1), Ur = __shfl_down_sync(0xffffffffu, Uc.x, 1);
+    if (own0) {
+      const double4 rc = sm.srow[k];
+      double a0 = fma(rc.x, Un.x - Uc.x, qc.x), a1 = fma(rc.x, Un.y - Uc.y, qc.y);
+      a0 = fma(rc.y, Up.x - Uc.x, a0);
+      a1 = fma(rc.y, Up.y - Uc.y, a1);
+      const double dzc = Uc.y - Uc.x;
+      a0 = fma(zp0, dzc, a0);
+      a1 = fma(-zm1, dzc, a1);
+      a0 = fma(zm0, Ul - Uc.x, a0);
+      a1 = fma(zp1, Ur - Uc.y, a1);
+      if (rc.z != 0.0 || zborder) {                    // Robin borders of the winding pack (rare: rb = 0 inside)
+        a0 = fma(-(rc.z + zb0), sqrt_fast(Uc.x) - lp.T_bath, a0);
+        a1 = fma(-(rc.z + zb1), sqrt_fast(Uc.y) - lp.T_bath, a1);
+      }
+      *reinterpret_cast<double2*>(o) = make_double2(fma(dtsub, a0, Hc.x), fma(dtsub, a1, Hc.y));
+    }
+    Up = Uc;
+    Uc = Un;
+    Hc = Hn;
+    qc = qn;
+    o += Nz;
+  }
+}
+
 // ---- K7 ---------------------------------------------------------------------------------------------------
 __global__ void events_kernel(int n_turns, const int* __restrict__ ptr, const int* __restrict__ idx,
                               MaterialParams mp, EventArgs e, Scalars* sc) {
@@ -439,9 +553,14 @@ void k_heat_substep(const VecCtx& v, const MaterialParams& mp, const LatticePara
     if (eff > best + 1e-9) best = eff, rows = cand;
   }
   dim3 grid(gx, (lp.Nr + rows - 1) / rows);
-  if (lp.Nz % 2 == 0)
-    heat_kernel<true><<<grid, kHeatWarps * 32, 0, v.stream>>>(mp, lp, rows, Hin, Q, Hout, dtsub);
-  else
+  if (lp.Nz % 2 == 0) {
+    static bool attr_set = false;
+    if (!attr_set) {
+      cudaFuncSetAttribute(heat_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(sizeof(HeatSmem)));
+      attr_set = true;
+    }
+    heat_tma_kernel<<<grid, kHeatWarps * 32, sizeof(HeatSmem), v.stream>>>(mp, lp, rows, Hin, Q, Hout, dtsub);
+  } else
     heat_kernel<false><<<grid, kHeatWarps * 32, 0, v.stream>>>(mp, lp, rows, Hin, Q, Hout, dtsub);
 }
 void k_events(const VecCtx& v, const MaterialParams& mp, const EventArgs& e) {

@@ -125,7 +125,10 @@ struct qs_ctx {
   size_t acc_bytes = 0;
   double *sw, *swM, *vw, *vsum, *tw, *defw, *ebar_prev, *t_first;
   int *flags, *count, *turn_ptr, *turn_idx, *turn_id, *d_perm;
+  int* rowturn = nullptr;            // [Nr] (ir / n) * turns_per_layer
+  unsigned long long *xmax_bits = nullptr, *rmin_bits = nullptr;   // [n_turns] event observables of the material pass
   double4* rowtab = nullptr;         // [Nr] (r, selfcoef, diagM, area) per radial row of a lattice
+  bool canonical_turns = false;      // turn_id[c] == (ir / n) * turns_per_layer + iz / n for every cell
   bool aux_on = false;               // qs_material_eval also writes dE/dJ (after the first qs_read_aux)
   double last_eval_dt = 0.0;
   double* heat_tab = nullptr;        // hr_p, hr_m, rb_r [Nr each], hz_p, hz_m, rb_z [Nz each]
@@ -207,6 +210,9 @@ void carve(qs_ctx* c, void* base, size_t* total) {
   c->bbox = k.take<double4>(std::max(c->nb, 1));
   c->heat_tab = k.take<double>(3 * static_cast<size_t>(c->tabNr + c->tabNz) + 1);
   c->rowtab = k.take<double4>(static_cast<size_t>(c->tabNr) + 1);
+  c->rowturn = k.take<int>(static_cast<size_t>(c->tabNr) + 1);
+  c->xmax_bits = k.take<unsigned long long>(nt);   // xmax_bits and rmin_bits are contiguous: one reset
+  c->rmin_bits = k.take<unsigned long long>(nt);
   c->sc = k.take<Scalars>(1);
   *total = align_up(k.off, 256);
 }
@@ -370,6 +376,14 @@ int run_heat(qs_ctx* c, double dt, int* m_out) {
   return QS_OK;
 }
 
+// presets of the per-turn event observables the material pass reduces into: max -> 0, min -> all ones
+int reset_event_bits(qs_ctx* c) {
+  if (!c->lattice || c->n_turns <= 0) return QS_OK;
+  QS_CUDA(cudaMemsetAsync(c->xmax_bits, 0, sizeof(unsigned long long) * c->n_turns, c->stream));
+  QS_CUDA(cudaMemsetAsync(c->rmin_bits, 0xff, sizeof(unsigned long long) * c->n_turns, c->stream));
+  return QS_OK;
+}
+
 MaterialArgs material_args(qs_ctx* c, double Bext, double Bdot, double dt, bool from_acc, bool aux) {
   MaterialArgs a;
   a.N = c->N;
@@ -390,9 +404,15 @@ MaterialArgs material_args(qs_ctx* c, double Bext, double Bdot, double dt, bool 
   a.Q = c->Q;
   a.shift = c->shift;
   a.Hd = c->Hd;
-  a.Jc = c->Jc;
-  a.rho = c->rho;
   a.dEdJ = aux ? c->dEdJ : nullptr;
+  a.Jc = aux ? c->Jc : nullptr;
+  a.rho = aux ? c->rho : nullptr;
+  const bool ev = c->lattice && c->n_turns > 0;
+  a.rowturn = ev && c->canonical_turns ? c->rowturn : nullptr;
+  a.turn_id = c->turn_id;
+  a.cells_per_side = c->lp.n;
+  a.xmax_bits = ev ? c->xmax_bits : nullptr;
+  a.rmin_bits = ev ? c->rmin_bits : nullptr;
   a.Bext = Bext;
   a.Bdot = Bdot;
   a.dt = dt;
@@ -628,6 +648,14 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
       if (iz == Nz - 1) rb_z[iz] += lp.h_conv[3] / h;
     }
     if (!put(c->heat_tab, tab, tab.size())) return bail(fail(QS_ERR_CUDA, "upload of the heat tables failed"));
+    std::vector<int> rt(Nr);
+    for (int ir = 0; ir < Nr; ++ir) rt[ir] = (ir / n) * geo->turns_per_layer;
+    c->canonical_turns = geo->n_turns == geo->layers * geo->turns_per_layer;
+    for (int k = 0; k < N && c->canonical_turns; ++k)
+      c->canonical_turns = geo->turn_id[k] == rt[k / Nz] + (k % Nz) / n;
+    if (cudaMemcpyAsync(c->rowturn, rt.data(), sizeof(int) * Nr, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess)
+      return bail(fail(QS_ERR_CUDA, "upload of the row turn table failed"));
     lp.hr_p = c->heat_tab;
     lp.hr_m = lp.hr_p + Nr;
     lp.rb_r = lp.hr_m + Nr;
@@ -743,6 +771,7 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
   if ((rc = do_sweep(c, c->x, c->cur, true)) != QS_OK) return rc;
   // S2
   const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
+  if ((rc = reset_event_bits(c)) != QS_OK) return rc;
   c->prof.begin(c->stream);
   k_material(v, c->mp, material_args(c, B0, (B1 - B0) / dt, dt, true, false));
   c->prof.end(c->stream, QS_PROF_MATERIAL, 1);
@@ -787,7 +816,7 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
   if ((rc = run_heat(c, dt, &m)) != QS_OK) return rc;
   // S7 + statistics
   EventArgs ev;
-  ev.H = c->H; ev.E = c->E; ev.J = c->Jold; ev.Jc = c->Jc; ev.rho = c->rho;
+  ev.H = c->H; ev.E = c->E; ev.xmax_bits = c->xmax_bits; ev.rmin_bits = c->rmin_bits;
   ev.ebar_prev = c->ebar_prev; ev.flags = c->flags; ev.t_first = c->t_first; ev.count = c->count;
   ev.dt = dt; ev.t_new = c->t + dt; ev.have_prev = c->have_prev_E;
   c->prof.begin(c->stream);
@@ -957,6 +986,8 @@ int qs_set_fields(qs_ctx* c, const double* B, const double* Q) {
 int qs_material_eval(qs_ctx* c, double dt) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
   const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
+  int rc = reset_event_bits(c);
+  if (rc != QS_OK) return rc;
   c->prof.begin(c->stream);
   k_material(c->v, c->mp, material_args(c, B0, dt > 0 ? (B1 - B0) / dt : 0.0, dt, false, c->aux_on));
   c->prof.end(c->stream, QS_PROF_MATERIAL, 1);

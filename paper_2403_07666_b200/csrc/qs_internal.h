@@ -157,8 +157,14 @@ struct MaterialArgs {
   const double4* rowtab; // [Nr] (r, selfcoef, diagM, area) of the cells of radial row ir
   const double *r, *area, *selfcoef, *diagM;
   double *Br, *Bz;       // read when !from_acc, written when from_acc
-  double *E, *Q, *shift, *Hd, *Jc, *rho;
-  double* dEdJ;          // optional (test hook), may be null
+  double *E, *Q, *shift, *Hd;
+  double *dEdJ, *Jc, *rho;   // optional (test hook qs_read_aux), may be null: the step itself never stores them
+  // per-turn event observables folded into this pass (C10; lattice with turns only, else null):
+  // bit patterns of max |J|/Jc and min rho over the cells of each turn, combined with 64-bit atomics
+  const int* rowturn;    // [Nr] (ir / n) * turns_per_layer, when the caller's turn ids are the canonical l*Tn + tau
+  const int* turn_id;    // else: per-cell turn ids
+  int cells_per_side;    // n
+  unsigned long long *xmax_bits, *rmin_bits;   // [n_turns], preset to 0 and ~0
   double Bext, Bdot, dt;
   double inv_area;       // lattice: 1 / (h h)
   bool from_acc;         // true: B from the sweep accumulators (+ self + Bext); false: B arrays given
@@ -171,7 +177,8 @@ void k_T_from_enthalpy(const VecCtx& v, const MaterialParams& mp, const double* 
 void k_heat_substep(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, const double* Hin,
                     const double* Q, double* Hout, double dtsub);
 struct EventArgs {
-  const double *H, *E, *J, *Jc, *rho;
+  const double *H, *E;
+  const unsigned long long *xmax_bits, *rmin_bits;   // per turn, from the material pass
   double* ebar_prev;     // [n_turns]
   int* flags;            // [n_turns]
   double* t_first;       // [n_turns]

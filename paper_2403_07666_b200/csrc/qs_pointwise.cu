@@ -80,6 +80,41 @@ __device__ __forceinline__ double sqrt_pos(double a) {
   const double e = fma(-g, y0, 1.0);
   return fma(g * e, fma(0.375, e, 0.5), g);
 }
+// x^e for 0 < x < ~1 (the strain term |eps|^1.7): exp(e log x) with both series written out against coefficient
+// tables in constant memory (the FMA takes them as constant-bank operands: no register or move traffic, which is
+// what makes the library log/exp expensive here).  log m = 2 atanh((m-1)/(m+1)) to z^15 on m in [1/sqrt2, sqrt2),
+// exp r to r^11 on |r| <= ln2/2: absolute error of the exponent < 2e-14, relative error of the power likewise.
+__device__ __constant__ double kLogC[7] = {2.0 / 3.0, 2.0 / 5.0, 2.0 / 7.0, 2.0 / 9.0, 2.0 / 11.0, 2.0 / 13.0, 2.0 / 15.0};
+__device__ __constant__ double kExpC[10] = {1.0 / 2.0,       1.0 / 6.0,        1.0 / 24.0,        1.0 / 120.0,        1.0 / 720.0,
+                                            1.0 / 5040.0,    1.0 / 40320.0,    1.0 / 362880.0,    1.0 / 3628800.0,    1.0 / 39916800.0};
+__device__ __forceinline__ double pow_small(double x, double e) {
+  int hi = __double2hiint(x);
+  const int lo = __double2loint(x);
+  int k = (hi >> 20) - 1023;
+  hi = (hi & 0x000fffff) | 0x3ff00000;                 // mantissa in [1, 2)
+  if (hi >= 0x3ff6a09f) hi -= 0x00100000, k += 1;      // > sqrt(2): halve
+  const double m = __hiloint2double(hi, lo);
+  const double z = (m - 1.0) * rcp_fast(m + 1.0);
+  const double z2 = z * z;
+  double p = kLogC[6];
+#pragma unroll
+  for (int j = 5; j >= 0; --j) p = fma(p, z2, kLogC[j]);
+  const double logm = fma(z * z2, p, z + z);           // 2 z + 2 z^3/3 + ...
+  const double t = e * fma(static_cast<double>(k), 0.69314718055994530942, logm);
+  if (t < -700.0) return 0.0;
+  const double shifter = 6755399441055744.0;           // 1.5 * 2^52: rounds to nearest integer in the low word
+  const double nf = fma(t, 1.4426950408889634074, shifter);
+  const int n = __double2loint(nf);
+  const double nr = nf - shifter;
+  double r = fma(-nr, 0.693147180369123816490, t);     // ln2 high part (33 bits)
+  r = fma(-nr, 1.90821492927058770002e-10, r);         // ln2 low part
+  double q = kExpC[9];
+#pragma unroll
+  for (int j = 8; j >= 0; --j) q = fma(q, r, kExpC[j]);
+  q = fma(q * r, r, r) + 1.0;                          // 1 + r + r^2 (1/2 + r/6 + ...)
+  return __hiloint2double(__double2hiint(q) + (n << 20), __double2loint(q));
+}
+
 // x^k, k >= 0 integer, by binary powering
 __device__ __forceinline__ double ipow_bin(double x, int k) {
   double r = 1.0;
@@ -96,19 +131,23 @@ struct MaterialConsts {   // host-side reciprocals of the constant divisors (qs_
 };
 
 // Lattice: blockIdx.y strides over radial rows (per-row geometry from rowtab), threads over iz.  Free rings: flat.
-__global__ void __launch_bounds__(256) material_kernel(MaterialParams mp, MaterialConsts k, MaterialArgs a) {
+template <bool FROM_ACC, bool AUX, bool EVENTS>
+__global__ void __launch_bounds__(256, 4) material_kernel(MaterialParams mp, MaterialConsts k, MaterialArgs a) {
   const double two_pi = 2.0 * kPi;
   const int ncol = a.Nz > 0 ? a.Nz : a.N, nrow = a.Nz > 0 ? a.N / a.Nz : 1;
   const int col0 = blockIdx.x * blockDim.x + threadIdx.x, dcol = gridDim.x * blockDim.x;
+  const unsigned wmask = __ballot_sync(0xffffffffu, col0 < ncol);   // lanes of this warp that own a column
   if (col0 >= ncol) return;
+  constexpr bool ev_on = EVENTS;                        // lattice launches: dcol >= ncol, uniform trips
+  const int tcol = ev_on ? col0 / a.cells_per_side : 0;
   // software pipeline: the five inputs of the next cell are in flight while the current one is evaluated
   struct In { double J, H, b0, b1, s; };
   auto load = [&](int i) {
     In v;
     v.J = a.J[i];
     v.H = a.H[i];
-    v.b0 = a.from_acc ? a.bracc[i] : a.Br[i];
-    v.b1 = a.from_acc ? a.bzacc[i] : a.Bz[i];
+    v.b0 = FROM_ACC ? a.bracc[i] : a.Br[i];
+    v.b1 = FROM_ACC ? a.bzacc[i] : a.Bz[i];
     v.s = a.jc0_scale ? a.jc0_scale[i] : 1.0;
     return v;
   };
@@ -141,7 +180,7 @@ __global__ void __launch_bounds__(256) material_kernel(MaterialParams mp, Materi
     const double U = tsq_fast(cur.H, mp.C3, k.qC1sq, k.hC1, k.inv_hC3);
     const double T = sqrt_pos(U);
     double Br, Bz;
-    if (a.from_acc) {
+    if (FROM_ACC) {
       Br = (0.25 * kMu0) * cur.b0 * rcp_fast(r);
       Bz = (0.25 * kMu0) * cur.b1 + selfc * (area * J) + a.Bext;
       a.Br[i] = Br;
@@ -154,15 +193,17 @@ __global__ void __launch_bounds__(256) material_kernel(MaterialParams mp, Materi
     const double Bmag = sqrt_pos(fma(Br, Br, Bz * Bz));
     const double fT = fmax(fma(-T, k.inv_Tc, 1.0), 0.0);
     const double ae = fabs(eps);
-    const double pw = ae > 0.0 ? exp(mp.eps_exp * log(ae)) : 0.0;       // |eps|^eps_exp
+    const double pw = ae > 1e-290 ? pow_small(ae, mp.eps_exp) : 0.0;    // |eps|^eps_exp
     const double fe = fmax(fma(-mp.eps_coef, pw, 1.0), 0.0);
     const double s = cur.s;
     // Jc = num/den and 1/Jc = den/num from one reciprocal of num den
     const double num = mp.Jc0 * s * fT * fT * fe, den = fma(Bmag, k.inv_B0, 1.0);
     double Jc = 0.0, rho, dEdJ;
+    double xr = 0.0;                               // |J| / Jc of this cell (C10)
     if (num <= 0.0) {
       rho = mp.rho_n;
       dEdJ = mp.rho_n;
+      if (J != 0.0) xr = __longlong_as_double(0x7ff0000000000000LL);
     } else {
       const double R = rcp_fast(num * den);
       Jc = num * num * R;
@@ -172,6 +213,7 @@ __global__ void __launch_bounds__(256) material_kernel(MaterialParams mp, Materi
       } else {
       const double invJc = den * den * R;
       const double x = fabs(J) * invJc;
+      xr = x;
       double xp;
       if (mp.n_int == 20) {                       // the configs' n = 20: x^19 = x^16 x^2 x
         const double x2 = x * x, x4 = x2 * x2, x8 = x4 * x4;
@@ -189,9 +231,27 @@ __global__ void __launch_bounds__(256) material_kernel(MaterialParams mp, Materi
     const double E = rho * J;
     a.E[i] = E;
     a.Q[i] = E * J;
-    a.Jc[i] = Jc;
-    a.rho[i] = rho;
-    if (a.dEdJ) a.dEdJ[i] = dEdJ;
+    if (AUX) {
+      a.dEdJ[i] = dEdJ;
+      a.Jc[i] = Jc;
+      a.rho[i] = rho;
+    }
+    if (ev_on) {   // per-turn max |J|/Jc and min rho: group the lanes of a turn, two 32-bit reductions per 64-bit key
+      const int turn = a.rowturn ? a.rowturn[row_i] + tcol : a.turn_id[i];
+      // common case: the whole warp lies in one turn (n >= 32 or aligned); else group the lanes by turn
+      const int t0 = __shfl_sync(wmask, turn, __ffs(wmask) - 1);
+      const unsigned grp = __all_sync(wmask, turn == t0) ? wmask : __match_any_sync(wmask, turn);
+      const unsigned long long xb = static_cast<unsigned long long>(__double_as_longlong(xr));
+      const unsigned long long rb = ~static_cast<unsigned long long>(__double_as_longlong(rho));   // min -> max of the complement
+      const unsigned xh = __reduce_max_sync(grp, static_cast<unsigned>(xb >> 32));
+      const unsigned xl = __reduce_max_sync(grp, static_cast<unsigned>(xb >> 32) == xh ? static_cast<unsigned>(xb) : 0u);
+      const unsigned rh = __reduce_max_sync(grp, static_cast<unsigned>(rb >> 32));
+      const unsigned rl = __reduce_max_sync(grp, static_cast<unsigned>(rb >> 32) == rh ? static_cast<unsigned>(rb) : 0u);
+      if ((threadIdx.x & 31) == __ffs(grp) - 1) {
+        atomicMax(a.xmax_bits + turn, (static_cast<unsigned long long>(xh) << 32) | xl);
+        atomicMin(a.rmin_bits + turn, ~((static_cast<unsigned long long>(rh) << 32) | rl));
+      }
+    }
     const double shift = mp.theta * a.dt * (two_pi * r * dEdJ * inv_area);
     a.shift[i] = shift;
     a.Hd[i] = dM + shift;
@@ -446,20 +506,16 @@ __global__ void events_kernel(int n_turns, const int* __restrict__ ptr, const in
                               MaterialParams mp, EventArgs e, Scalars* sc) {
   const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (w >= n_turns) return;
-  double tsq = 0.0, esum = 0.0, xmax = 0.0, rmin = 1e300;
+  double tsq = 0.0, esum = 0.0;
   for (int k = ptr[w] + lane; k < ptr[w + 1]; k += 32) {
     const int i = idx[k];
     tsq = fmax(tsq, tsq_of_H(e.H[i], mp.C3, mp.C1));
     esum += fabs(e.E[i]);
-    const double J = e.J[i], Jc = e.Jc[i];
-    const double ratio = Jc > 0.0 ? fabs(J) / Jc : (J != 0.0 ? __longlong_as_double(0x7ff0000000000000LL) : 0.0);
-    xmax = fmax(xmax, ratio);
-    rmin = fmin(rmin, e.rho[i] / mp.rho_n);
   }
   tsq = warp_max(tsq);
   esum = warp_sum(esum);
-  xmax = warp_max(xmax);
-  rmin = warp_min(rmin);
+  const double xmax = __longlong_as_double(static_cast<long long>(e.xmax_bits[w]));
+  const double rmin = __longlong_as_double(static_cast<long long>(e.rmin_bits[w])) / mp.rho_n;
   if (lane != 0) return;
   const double Tmax = sqrt(tsq);
   const double ebar = esum / static_cast<double>(ptr[w + 1] - ptr[w]);
@@ -520,7 +576,16 @@ void k_material(const VecCtx& v, const MaterialParams& mp, const MaterialArgs& a
     grid.x = (a.Nz + kBlock - 1) / kBlock;
     grid.y = std::min(nrow, std::max(1, 8 * g_sm_count / static_cast<int>(grid.x)));
   }
-  material_kernel<<<grid, kBlock, 0, v.stream>>>(mp, k, a);
+  const bool ev = a.xmax_bits != nullptr, aux = a.dEdJ != nullptr;
+#define QS_MAT(F_, A_, E_) material_kernel<F_, A_, E_><<<grid, kBlock, 0, v.stream>>>(mp, k, a)
+  if (a.from_acc) {
+    if (ev) QS_MAT(true, false, true); else QS_MAT(true, false, false);
+  } else if (aux) {
+    if (ev) QS_MAT(false, true, true); else QS_MAT(false, true, false);
+  } else {
+    if (ev) QS_MAT(false, false, true); else QS_MAT(false, false, false);
+  }
+#undef QS_MAT
 }
 void k_build_rowtab(const VecCtx& v, int Nr, int Nz, const double* r, const double* selfcoef, const double* diagM,
                     const double* area, double4* rowtab) {

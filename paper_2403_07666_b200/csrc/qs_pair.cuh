@@ -11,7 +11,7 @@
 // u_n = a_n^2, v_n = b_n^2, so that one iteration needs exactly one square root (MUFU seed + one cubic
 // correction, 5 FP64 operations) and the two start-up roots sqrt(A2), sqrt(B2) are never taken:
 //   p = sqrt(u v) (= a_n b_n);  4 c_{n+1}^2 = u + v - 2p;  u' = (u + v + 2p)/4;  v' = p
-// (10 FP64 operations per iteration; the division by 4 is an exponent decrement on the integer pipe).
+// (10 FP64 operations per iteration: u' is formed as p + c_{n+1}^2, which needs no separate division by 4).
 // After NIT iterations the rest of the AGM is summed in closed form as a power series in
 // delta = 1 - v/u = k_NIT^2 (the modulus at level NIT), from the identities
 //   1/agm(a, b)                       = (1/a) F(delta),  F = (2/pi) K = sum_j ((2j-1)!!/(2j)!!)^2 delta^j
@@ -38,11 +38,6 @@ __device__ __forceinline__ double rsqrt_fast(double x) {
   const double q = fma(0.375, e, 0.5);
   const double ye = y * e;
   return fma(ye, q, y);
-}
-
-// x / 4 for a positive normal x well above the underflow range: exponent field minus 2 (integer pipe)
-__device__ __forceinline__ double quarter(double x) {
-  return __hiloint2double(__double2hiint(x) - 0x00200000, __double2loint(x));
 }
 
 struct PairAGM {
@@ -74,8 +69,9 @@ __device__ __forceinline__ PairAGM agm_pair(double A2, double B2) {
       o.y0sq = y * y;
       o.mid = 0.5 * s;
     }
-    S = fma(coef, fma(-2.0, p, s), S);
-    u = fma(0.5, p, quarter(s));
+    const double t = fma(-2.0, p, s);         // 4 c_{n+1}^2 = u + v - 2p
+    S = fma(coef, t, S);
+    u = fma(0.25, t, p);                      // (u + v + 2p)/4 = p + c_{n+1}^2
     v = p;
     coef *= 2.0;
   }

@@ -35,6 +35,9 @@ UNIT = "cell-steps/s"
 FLOP_K1, FLOP_K2 = 76.0, 100.0
 # FP64 peak derived from unit counts: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9 / 1e12
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the ncu --set full captures summarised
+# under profiles/ (r01_sweep_field_cfg2.md, r01_hbm_passes.md); None where no capture of that workload exists
+NCU_TRAFFIC = {"sweep_field:cfg2_mid_solenoid_20x40x16": 11.8e6, "material_K5": 671.6e6 + 492.5e6, "heat_K6": 275.9e6 + 102.7e6}
 DEFAULTS = {"cfg0": (50, 5), "cfg1": (100, 5), "cfg2": (10, 3), "cfg3": (3, 3)}
 
 
@@ -266,7 +269,8 @@ def hbm_roofline_leg(torch, pkg, hbm_peak):
     # writes E, dE/dJ, Q, b (32) = 72; K6 reads H, Q and writes H = 24 per sub-step
     for name, ms, bpc in (("material_K5", ms_mat, 72.0), ("heat_K6", ms_heat, 24.0)):
         gbs = bpc * N / (ms * 1e-3) / 1e9
-        out[name] = {"ms": ms, "bytes_per_cell": bpc, "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak}
+        out[name] = {"bound": "hbm", "ms": ms, "bytes_per_cell": bpc, "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
+                     "frac": gbs / hbm_peak, "traffic": NCU_TRAFFIC.get(name)}
     return out
 
 
@@ -311,33 +315,23 @@ def gpu_arm(args):
     import torch
     import paper_2403_07666_b200 as pkg
 
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    from paper_2403_07666_b200.replicas import Group, env_rank, replica_seed
+    rank, local, world = env_rank()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product has no CPU path (use --impl reference for the oracle)")
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    group = Group("nccl", torch.device("cuda", local))   # no-op for world == 1; replicas only: barrier + max reduce
 
     def barrier():
-        if dist is not None:
-            dist.barrier()
+        group.barrier()
         torch.cuda.synchronize()
 
-    def max_over_ranks(v):
-        if dist is None:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    max_over_ranks = group.max_over_ranks
 
     cfg = int(args.workload[3])
     w = wl.config(cfg)
     if rank > 0:   # replicas: same coil, another seeded Jc0 perturbation (a parameter study)
-        w.material.jc0_scale = wl.jc0_scale(w.seed + 100 * rank, w.geometry.n_rings, 0.02 if cfg == 2 else 0.01)
+        w.material.jc0_scale = wl.jc0_scale(replica_seed(w.seed, rank), w.geometry.n_rings, 0.02 if cfg == 2 else 0.01)
     N = w.geometry.n_rings
     hbm_peak, hbm_src = load_measured_peaks()
     fp64_tf, fp64_mhz = pkg.fp64_peak()
@@ -386,7 +380,8 @@ def gpu_arm(args):
     flop = (FLOP_K2 if dom == "sweep_field" else FLOP_K1) * pe
     ach = flop / (d_ms / max(d_n, 1) * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": f"qs::sweep_kernel<{'true' if dom == 'sweep_field' else 'false'}> ({dom})",
-                "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s", "frac": ach / fp64_tf, "traffic": None,
+                "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s", "frac": ach / fp64_tf,
+                "traffic": NCU_TRAFFIC.get(f"{dom}:{w.name}"),
                 "peak_source": "measured in this run: DFMA-chain probe qs_fp64_peak; "
                                f"unit-count peak 148 SM x 64 lanes x 2 x 1.965 GHz = {FP64_PEAK_NOMINAL:.2f}",
                 "frac_of_nominal_peak": ach / FP64_PEAK_NOMINAL,
@@ -403,6 +398,9 @@ def gpu_arm(args):
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()}}
     if rank == 0 and world == 1 and not args.no_extras:
+        line["issue_model"] = dict(pkg.issue_probe(), unit="SM cycles per DFMA warp-instruction per sub-partition",
+                                   note="FP64 pipe rate is 2; a third register operand costs a cycle, and so does every "
+                                        "non-FP64 instruction issued beside the DFMAs (DESIGN.md section 6)")
         line["roofline_hbm"] = hbm_roofline_leg(torch, pkg, hbm_peak)
         line["roofline_hbm"]["peak_source"] = f"MEASURED_PEAKS.json hbm_gbs ({hbm_src})"
         line["operator_cfg4"] = operator_leg(torch, pkg, fp64_tf)
@@ -416,8 +414,7 @@ def gpu_arm(args):
                                 "seconds": total}
     if rank == 0:
         print(json.dumps(line), flush=True)
-    if dist is not None:
-        dist.destroy_process_group()
+    group.close()
 
 
 if __name__ == "__main__":

@@ -197,6 +197,12 @@ int  qs_pair_eval(int32_t n, const double *A2, const double *B2, int32_t cls,
  * thread on every SM, timed with CUDA events (best of 5).  The denominator of the operator's
  * roofline ("bound": "alu"); needs no handle.  Returns 0 or QS_ERR_CUDA.  */
 int  qs_fp64_peak(double *tflops, double *sm_clock_mhz_effective);
+
+/* Issue-model probes behind the sweeps' roofline: SM cycles (at the maximum SM clock) per DFMA
+ * warp-instruction per SM sub-partition for 8 independent chains per thread with mode 1: three distinct register
+ * operands; mode 2: two register operands and an immediate; mode 3: mode 2 plus one integer ALU instruction per
+ * DFMA.  Needs no handle.  */
+int  qs_issue_probe(int32_t mode, double *cycles_per_dfma);
 int  qs_events(qs_ctx *ctx, int32_t *flags /*[N_w]*/, double *t_first /*[N_w]*/, int32_t *count /*[N_w]*/);
 int  qs_sync(qs_ctx *ctx);                 /* wait for the handle's stream */
 const char *qs_last_error(void);

@@ -74,6 +74,7 @@ SYMBOLS = [
     ("qs_profile_enable", C.c_int, [_VP, C.c_int32]),
     ("qs_profile_read", C.c_int, [_VP, C.POINTER(QsProfile)]),
     ("qs_fp64_peak", C.c_int, [c_double_p, c_double_p]),
+    ("qs_issue_probe", C.c_int, [C.c_int32, c_double_p]),
     ("qs_pair_eval", C.c_int, [C.c_int32, c_double_p, c_double_p, C.c_int32, c_double_p, c_double_p, c_double_p, c_int32_p]),
     ("qs_events", C.c_int, [_VP, c_int32_p, c_double_p, c_int32_p]),
     ("qs_sync", C.c_int, [_VP]),
@@ -125,6 +126,19 @@ def fp64_peak():
     if rc < 0:
         raise QsError(rc, lib.qs_last_error().decode())
     return tf.value, mhz.value
+
+
+def issue_probe() -> dict:
+    """SM cycles per DFMA warp-instruction per sub-partition: 3 register operands / 2 + immediate / + integer ALU."""
+    lib = load_library()
+    out = {}
+    for mode, name in ((1, "dfma_3reg"), (2, "dfma_2reg_imm"), (3, "dfma_2reg_imm_plus_1_alu")):
+        v = C.c_double(0.0)
+        rc = lib.qs_issue_probe(mode, C.byref(v))
+        if rc < 0:
+            raise QsError(rc, lib.qs_last_error().decode())
+        out[name] = v.value
+    return out
 
 
 def pair_eval(A2, B2, cls: int = -1):

@@ -1040,6 +1040,13 @@ int qs_profile_read(qs_ctx* c, qs_profile_t* out) {
   return QS_OK;
 }
 
+int qs_issue_probe(int32_t mode, double* cycles_per_dfma) {
+  if (!cycles_per_dfma || mode < 1 || mode > 3) return fail(QS_ERR_ARG, "qs_issue_probe: mode 1..3 and a result pointer");
+  const cudaError_t e = issue_probe(mode, cycles_per_dfma);
+  if (e != cudaSuccess) return fail(QS_ERR_CUDA, std::string("issue probe: ") + cudaGetErrorString(e));
+  return QS_OK;
+}
+
 int qs_pair_eval(int32_t n, const double* A2, const double* B2, int32_t cls, double* M, double* K, double* E, int32_t* used) {
   if (n <= 0 || !A2 || !B2 || !M || !K || !E || !used) return fail(QS_ERR_ARG, "qs_pair_eval: bad argument");
   if (cls >= pair_num_classes()) return fail(QS_ERR_ARG, "qs_pair_eval: class out of range");

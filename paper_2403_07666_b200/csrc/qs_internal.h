@@ -40,6 +40,7 @@ cudaError_t launch_pair_eval(int n, const double* A2, const double* B2, int cls,
 int pair_num_classes();
 // FP64 FMA throughput probe (qs_operator.cu): TFLOP/s and the SM clock seen by the kernel
 cudaError_t fp64_peak_probe(double* tflops, double* sm_mhz);
+cudaError_t issue_probe(int mode, double* cycles_per_dfma);
 
 // ---- vector / CG kernels (qs_vector.cu) -------------------------------------------------------
 // Device scalars of the solver; all reductions land here (no host round trip inside an iteration).

@@ -372,6 +372,73 @@ cudaError_t fp64_peak_probe(double* tflops, double* sm_mhz) {
   return cudaSuccess;
 }
 
+// Issue-model probes behind DESIGN.md §6 (what bounds the sweeps): 8 independent DFMA chains per thread with
+//   mode 1: three distinct register operands per DFMA            (register-file read port: 3 cycles per warp-instr)
+//   mode 2: two register operands + immediate                     (2 cycles per warp-instr: the pipe rate)
+//   mode 3: mode 2 plus 8 integer ALU instructions per 8 DFMAs    (an FP64 instruction holds the issue port: the
+//                                                                   integer work does not co-issue for free)
+template <int MODE>
+__global__ void __launch_bounds__(256) issue_probe_kernel(int iters, const double* __restrict__ in, double* __restrict__ out,
+                                                          int sh) {
+  double a[8], b[8], c[8];
+  int q[4] = {static_cast<int>(threadIdx.x), static_cast<int>(threadIdx.x) * 3, static_cast<int>(threadIdx.x) * 5,
+              static_cast<int>(threadIdx.x) * 7};
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    a[i] = in[threadIdx.x + 32 * i];
+    b[i] = in[threadIdx.x + 32 * i + 1000];
+    c[i] = in[threadIdx.x + 32 * i + 2000];
+  }
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = MODE == 1 ? fma(a[i], b[i], c[i]) : fma(a[i], b[i], 0.5);
+    if (MODE == 3) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) q[j] = (q[j] + sh) ^ it;
+    }
+  }
+  double s = q[0] + q[1] + q[2] + q[3];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += a[i] + b[i] + c[i];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+cudaError_t issue_probe(int mode, double* cycles_per_dfma) {
+  int dev = 0, sms = 0, khz = 0;
+  cudaError_t e;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev);
+  const int iters = 20000, grid = sms * 4, threads = 256;
+  double* buf = nullptr;
+  if ((e = cudaMalloc(&buf, sizeof(double) * (4096 + static_cast<size_t>(grid) * threads))) != cudaSuccess) return e;
+  cudaMemset(buf, 0, sizeof(double) * 4096);
+  cudaEvent_t a, b;
+  cudaEventCreate(&a);
+  cudaEventCreate(&b);
+  float best = 1e30f;
+  for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {
+    cudaEventRecord(a, 0);
+    if (mode == 1) issue_probe_kernel<1><<<grid, threads>>>(iters, buf, buf + 4096, 3);
+    else if (mode == 2) issue_probe_kernel<2><<<grid, threads>>>(iters, buf, buf + 4096, 3);
+    else issue_probe_kernel<3><<<grid, threads>>>(iters, buf, buf + 4096, 3);
+    cudaEventRecord(b, 0);
+    e = cudaEventSynchronize(b);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  cudaFree(buf);
+  if (e != cudaSuccess) return e;
+  // cycles per DFMA warp-instruction per SM sub-partition at the maximum SM clock: 8 warps x 8 DFMA x iters per SMSP... per CTA
+  const double warp_instr_per_smsp = static_cast<double>(iters) * 8.0 * (static_cast<double>(grid) * threads / 32.0) / (sms * 4.0);
+  *cycles_per_dfma = best * 1e-3 * (khz * 1e3) / warp_instr_per_smsp;
+  return cudaSuccess;
+}
+
 int sweep_grid(int sm_count, bool field) { return sm_count * (field ? 2 : 3); }
 
 cudaError_t launch_sweep(const SweepParams& prm, bool field, int grid, cudaStream_t stream) {

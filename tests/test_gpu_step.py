@@ -157,3 +157,35 @@ def test_step_is_transactional_and_write_resumes(pkg):
         b.step(w.dt, w.I_ramp)
         for u, v in zip(a.read(), b.read()):
             assert rel(u, v) <= 1e-9 or np.linalg.norm(v) < 1e-30
+
+
+@pytest.mark.parametrize("cfg,rows", [(2, 24), (3, 8)])
+def test_full_size_step_sampled_outputs_and_invariants(pkg, cfg, rows):
+    # BASELINE.json configs[2], [3] at FULL size, in the launch configuration bench.py times.  The oracle cannot
+    # step these, but every output of the step that has a row-by-row definition can be sampled:
+    #   B^k = G_B (a J^k) + B_ext and E^k = E(J^k, T^k, B^k) on seeded cells (pair by pair against all N sources),
+    # and the properties that hold at any size: the turn currents advance by dt*I_ramp exactly (every CG iterate
+    # keeps the constraint, so two iterations suffice), T stays at the bath while Q ~ 0, no event fires.
+    w = wl.config(cfg)
+    geo = w.geometry
+    mat = dataclasses.replace(w.material, cg_maxit=2)
+    N = geo.n_rings
+    g = np.random.default_rng(50 + cfg)
+    Jc0 = 2e9 * (1 - 4.2 / 18) ** 2
+    J0 = 0.7 * Jc0 * g.uniform(-1.0, 1.0, N)
+    T0 = g.uniform(4.2, 6.0, N)
+    idx = wl.sample_rows(N, rows, seed=70 + cfg)
+    with pkg.QS(geo, mat) as sim:
+        sim.write(J0, T0, 0.0, 0.0)
+        rc = sim.step(w.dt, w.I_ramp)
+        J1, T1, B, E = sim.read()
+        st = sim.stats()
+    assert rc >= 0 and (rc & 4)                                   # stopped at cg_maxit, state advanced
+    Br, Bz = qo.field_eval_rows(geo, geo.area * J0, idx, chunk=4)
+    assert rel(B[idx], Br) <= 1e-9 and rel(B[N + idx], Bz) <= 1e-9
+    ml = qo.material_law(mat, J0[idx], T0[idx], Br, Bz, geo.r[idx], mat.jc0_scale[idx])
+    assert rel(E[idx], ml["E"]) <= 1e-6
+    # net current of every turn: sum_i a (J1 - J0) = dt * I_ramp
+    dI = np.bincount(geo.turn_id, weights=geo.area * (J1 - J0), minlength=geo.n_turns)
+    assert np.max(np.abs(dI - w.dt * w.I_ramp)) <= 1e-9 * w.dt * w.I_ramp + 1e-12 * np.max(np.abs(geo.area * J0)) * 200
+    assert np.all(np.isfinite(T1)) and st["heat_substeps"] == qo.heat_substeps_count(geo, mat, w.dt)

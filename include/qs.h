@@ -58,6 +58,11 @@ typedef struct qs_ctx qs_ctx;
                                 qs_matvec, qs_solve, qs_field return QS_ERR_ARG (roofline runs of
                                 the HBM-bound passes on lattices whose N^2 sweep is out of reach)  */
 
+#define QS_GEO_LATTICE_TABLES 2 /* lattice geometries: evaluate every unique pair value once at qs_init into tables over
+                                  (ir, jr, |iz - jz|) (3 x 8 Nr^2 Nz bytes of workspace) and apply M and G_B as block-
+                                  Toeplitz products instead of on-the-fly pair sweeps.  Same
+                                  arithmetic per unique pair, same results up to summation order.  */
+
 typedef struct {
   int32_t  n_rings;                 /* N                                                         */
   const double *r, *z, *area;       /* [N] ring centre radius, height, cross-section [m, m, m^2] */

@@ -106,6 +106,8 @@ struct qs_ctx {
   // problem
   int N = 0, Np = 0, nb = 0, n_turns = 0;
   bool lattice = false, has_operator = true;
+  bool tables = false;               // QS_GEO_LATTICE_TABLES: block-Toeplitz operator
+  double *TM = nullptr, *TBz = nullptr, *TBr = nullptr;   // [Nr][Nr][Nz]
   MaterialParams mp{};
   LatticeParams lp{};
   double theta = 1.0, cg_tol = 1e-10;
@@ -208,6 +210,12 @@ void carve(qs_ctx* c, void* base, size_t* total) {
   c->turn_id = k.take<int>(N);
   c->d_perm = k.take<int>(N);
   c->bbox = k.take<double4>(std::max(c->nb, 1));
+  if (c->tables) {
+    const size_t nt3 = static_cast<size_t>(c->tabNr) * c->tabNr * c->tabNz;
+    c->TM = k.take<double>(nt3);
+    c->TBz = k.take<double>(nt3);
+    c->TBr = k.take<double>(nt3);
+  }
   c->heat_tab = k.take<double>(3 * static_cast<size_t>(c->tabNr + c->tabNz) + 1);
   c->rowtab = k.take<double4>(static_cast<size_t>(c->tabNr) + 1);
   c->rowturn = k.take<int>(static_cast<size_t>(c->tabNr) + 1);
@@ -240,6 +248,27 @@ int sync_scalars(qs_ctx* c) {
 // work counter were cleared by the previous CG iteration (fused path), no memset is enqueued.
 int do_sweep(qs_ctx* c, const double* x, const double* cur, bool field, bool prezeroed = false, bool cg_guard = false) {
   if (!prezeroed) QS_CUDA(cudaMemsetAsync(c->counter, 0, c->acc_bytes, c->stream));
+  if (c->tables) {   // lattice-aware operator: block-Toeplitz product with the tables built at init
+    LatticeSweepParams lp;
+    lp.Nr = c->lp.Nr;
+    lp.Nz = c->lp.Nz;
+    lp.jr_chunk = 0;
+    lp.TM = c->TM;
+    lp.TBz = c->TBz;
+    lp.TBr = c->TBr;
+    lp.x = x;
+    lp.cur = cur ? cur : x;
+    lp.yacc = c->yacc;
+    lp.bracc = c->bracc;
+    lp.bzacc = c->bzacc;
+    lp.done = cg_guard ? &c->sc->done : nullptr;
+    c->prof.begin(c->stream);
+    QS_CUDA(launch_table_sweep(lp, field, c->sm_count, c->stream));
+    c->prof.end(c->stream, field ? QS_PROF_SWEEP_FIELD : QS_PROF_SWEEP_M, 1);
+    ++c->launches;
+    ++c->st.sweeps;
+    return QS_OK;
+  }
   SweepParams prm;
   prm.r = c->r;
   prm.z = c->z;
@@ -347,7 +376,8 @@ int cg_core(qs_ctx* c, const Rhs& b, double* x, const double* shift, const doubl
   *relres = std::sqrt(std::max(rg, 0.0)) / nu;
   // no-op launches after convergence did not run; the sweep count reflects the enqueued ones: correct it
   c->st.sweeps -= (enq - done_it);
-  c->pair_evals -= static_cast<long long>(enq - done_it) * (static_cast<long long>(c->nb) * (c->nb + 1) / 2) * 1024;
+  if (!c->tables)
+    c->pair_evals -= static_cast<long long>(enq - done_it) * (static_cast<long long>(c->nb) * (c->nb + 1) / 2) * 1024;
   return QS_OK;
 }
 
@@ -468,6 +498,7 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
   c->n_turns = geo->n_turns;
   c->lattice = geo->lattice != 0;
   c->has_operator = !(geo->flags & QS_GEO_NO_OPERATOR);
+  c->tables = c->lattice && c->has_operator && (geo->flags & QS_GEO_LATTICE_TABLES);
   c->Bext0 = geo->Bext0;
   c->Bext_rate = geo->Bext_rate;
   c->Bext_max = geo->Bext_max;
@@ -670,6 +701,12 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
     k_enthalpy_from_T(v, mp, c->tmp, c->H, N);
   }
   k_set_scalars(v);
+  if (c->tables) {
+    if (launch_table_build(lp.Nr, lp.Nz, lp.r_inner, lp.h, c->soft_self, c->TM, c->TBz, c->TBr, c->sm_count, c->stream) != cudaSuccess)
+      return bail(fail(QS_ERR_CUDA, "table build kernel launch failed"));
+    ++c->launches;
+    c->pair_evals += static_cast<long long>(lp.Nr) * lp.Nr * lp.Nz;
+  }
   if (c->has_operator) {
     if (launch_diag(N, c->r, c->soft_all + c->soft_self, c->diagM, c->stream) != cudaSuccess)
       return bail(fail(QS_ERR_CUDA, "diag kernel launch failed"));
@@ -716,6 +753,7 @@ size_t qs_workspace_bytes(const qs_geometry* geo) {
   if (geo->lattice) {
     tmp.tabNr = geo->layers * geo->cells_per_side;
     tmp.tabNz = geo->turns_per_layer * geo->cells_per_side;
+    tmp.tables = (geo->flags & QS_GEO_LATTICE_TABLES) && !(geo->flags & QS_GEO_NO_OPERATOR);
   }
   size_t need = 0;
   carve(&tmp, nullptr, &need);

@@ -34,6 +34,19 @@ cudaError_t launch_sweep(const SweepParams& prm, bool field, int grid, cudaStrea
 // diagM_i = M(r_i, r_i, dz^2 = d2self) in henry
 cudaError_t launch_diag(int n, const double* r, double d2self, double* diagM, cudaStream_t stream);
 
+// ---- lattice-aware operator (qs_lattice.cu): tables over (ir, jr, |iz - jz|) + block-Toeplitz sweeps ------------------
+struct LatticeSweepParams {
+  int Nr, Nz;
+  int jr_chunk;           // source rows per CTA (set by the launcher)
+  const double *TM, *TBz, *TBr;   // [Nr][Nr][Nz] unscaled pair quantities (TBz, TBr: field sweeps only)
+  const double *x, *cur;  // [Nr Nz] vectors (canonical order)
+  double *yacc, *bracc, *bzacc;   // accumulators, same meaning and scaling as the pair sweeps'
+  const int* done;        // fused CG guard (nullptr: always run)
+};
+cudaError_t launch_table_build(int Nr, int Nz, double r_inner, double h, double soft_self2, double* TM, double* TBz,
+                               double* TBr, int sm_count, cudaStream_t stream);
+cudaError_t launch_table_sweep(const LatticeSweepParams& prm, bool field, int sm_count, cudaStream_t stream);
+
 // test hook: per-pair evaluation through evaluation class cls (or the class the sweep would pick when cls < 0)
 cudaError_t launch_pair_eval(int n, const double* A2, const double* B2, int cls, double* M, double* K, double* E,
                              int* used, cudaStream_t stream);

@@ -1,0 +1,213 @@
+// qs_lattice.cu — lattice-aware operator (geometry: the square array of wires).
+//
+// On a regular winding pack the pair kernels depend only on (ir, jr, iz - jz): M, G_Bz are even and G_Br is odd in
+// iz - jz.  At init every unique value is evaluated ONCE with the same per-pair arithmetic as the on-the-fly sweeps
+// (qs_pair.cuh, deepest evaluation class) into tables T[ir][jr][d], d = |iz - jz| = 0..Nz-1; a sweep is then a
+// block-Toeplitz product
+//     y[ir][iz] = sum_jr sum_jz T[ir][jr][|iz - jz|] x[jr][jz]
+// — N^2 FP64 multiply-adds instead of N^2/2 AGM evaluations (~60 FP64 operations each).  The tables hold the same
+// unscaled quantities the pair sweeps accumulate, and the kernel adds into the same accumulators (yacc, bracc, bzacc),
+// so everything downstream (scaling, material law, CG) is unchanged and either operator can serve a handle.
+//
+// Kernel: a CTA owns one target row ir, a chunk of source rows jr and a tile of T*R outputs; thread t owns R ADJACENT
+// outputs (R odd: the stride-R shared-memory reads of the table window are bank-conflict free).  Per source row the
+// table row is mirrored into shared memory as t_ext[e], e = iz - jz in (-Nz, Nz), next to the source row x; the thread
+// then slides over jz with a register window W[k] = t_ext[iz0 + k - jz]: one broadcast read of x[jz] and ONE new
+// window element per jz feed R multiply-adds (register rotation by unrolling, no moves).  Partial sums over the
+// jr chunks are combined with FP64 red.add in L2.
+#include <algorithm>
+
+#include "qs_internal.h"
+#include "qs_pair.cuh"
+
+namespace qs {
+
+namespace {
+
+// ---- table construction: one thread per (ir, jr, d) ---------------------------------------------------------------
+__global__ void table_build_kernel(int Nr, int Nz, double r_inner, double h, double soft_self2, double* __restrict__ TM,
+                                   double* __restrict__ TBz, double* __restrict__ TBr) {
+  const long long total = static_cast<long long>(Nr) * Nr * Nz;
+  for (long long id = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; id < total;
+       id += static_cast<long long>(gridDim.x) * blockDim.x) {
+    const int d = static_cast<int>(id % Nz);
+    const long long rr = id / Nz;
+    const int jr = static_cast<int>(rr % Nr), ir = static_cast<int>(rr / Nr);
+    const double ri = r_inner + (ir + 0.5) * h, rj = r_inner + (jr + 0.5) * h;
+    const double dz = d * h;                                   // target above source: dz = z_i - z_j >= 0
+    const bool self = (ir == jr) && d == 0;
+    const double dz2 = self ? soft_self2 : dz * dz;            // C2: M_ii = M(r_i, r_i, dz = g)
+    const double dif = ri - rj;
+    const double B2 = fma(dif, dif, dz2), A2 = fma(4.0 * ri, rj, B2);
+    const PairAGM a = agm_pair<7, false, true>(A2, B2);
+    TM[id] = a.S * a.yinf;
+    if (TBz) {
+      if (self) {                                              // C3: the self field is analytic (material pass)
+        TBz[id] = 0.0;
+        TBr[id] = 0.0;
+      } else {
+        const double qt = a.yinf * (a.mid - a.S) * a.y0sq;
+        const double e = fma(rj, rj, -ri * ri);
+        TBz[id] = fma(e - dz2, qt, a.yinf);                    // Kt + (rj^2 - ri^2 - dz^2) Qt
+        TBr[id] = dz * fma(a.mid, qt, -a.yinf);                // dz (-Kt + (ri^2 + rj^2 + dz^2) Qt), odd in dz
+      }
+    }
+  }
+}
+
+// ---- block-Toeplitz sweep -----------------------------------------------------------------------------------------
+template <int R, bool FIELD>
+__global__ void __launch_bounds__(256) table_sweep_kernel(LatticeSweepParams prm) {
+  extern __shared__ __align__(16) double lsm[];
+  const int Nz = prm.Nz, T = blockDim.x;
+  const int NzPad = (Nz + R - 1) / R * R;                      // source loop runs in blocks of R
+  const int ext_len = NzPad + T * R;                           // e in [-NzPad, T R)
+  double* tM = lsm;                                            // t_ext[e] at tM[e + NzPad]
+  double* tBz = FIELD ? tM + ext_len : nullptr;
+  double* tBr = FIELD ? tBz + ext_len : nullptr;
+  double* xs = (FIELD ? tBr : tM) + ext_len;                   // [NzPad]
+  double* cs = FIELD ? xs + NzPad : nullptr;
+  if (prm.done != nullptr && *prm.done != 0) return;           // a converged CG batch: nothing left to do
+  const int ir = blockIdx.y;
+  const int j0 = blockIdx.x * prm.jr_chunk, j1 = min(j0 + prm.jr_chunk, prm.Nr);
+  const int z0 = blockIdx.z * T * R;                           // first output of this tile
+  const int iz0 = z0 + threadIdx.x * R;
+  double yM[R], yBz[FIELD ? R : 1], yBr[FIELD ? R : 1];
+#pragma unroll
+  for (int k = 0; k < R; ++k) {
+    yM[k] = 0.0;
+    if (FIELD) yBz[k] = 0.0, yBr[k] = 0.0;
+  }
+  for (int jr = j0; jr < j1; ++jr) {
+    __syncthreads();
+    const long long trow = (static_cast<long long>(ir) * prm.Nr + jr) * Nz;
+    const long long xrow = static_cast<long long>(jr) * Nz;
+    for (int s = threadIdx.x; s < ext_len; s += T) {           // mirrored table row; zero outside |e| < Nz
+      const int e = s - NzPad + z0;                            // e = iz - jz of window slot s for this tile
+      const int d = abs(e);
+      const bool in = d < Nz;
+      tM[s] = in ? prm.TM[trow + d] : 0.0;
+      if (FIELD) {
+        tBz[s] = in ? prm.TBz[trow + d] : 0.0;
+        const double br = in ? prm.TBr[trow + d] : 0.0;
+        tBr[s] = e < 0 ? -br : br;
+      }
+    }
+    for (int s = threadIdx.x; s < NzPad; s += T) {
+      xs[s] = s < Nz ? prm.x[xrow + s] : 0.0;
+      if (FIELD) cs[s] = s < Nz ? prm.cur[xrow + s] : 0.0;
+    }
+    __syncthreads();
+    // Element of (output k, source jz): t_ext[iz0 + k - jz] = wM[k - jz].  As jz grows the window slides: the new
+    // element enters at output 0 and every older one moves up one output, so an element keeps its REGISTER if
+    // output k reads register (k - jz) mod R: with the jz loop unrolled R times all indices are compile-time.
+    const double* wM = tM + (iz0 - z0) + NzPad;
+    const double* wBz = FIELD ? tBz + (iz0 - z0) + NzPad : nullptr;
+    const double* wBr = FIELD ? tBr + (iz0 - z0) + NzPad : nullptr;
+    double WM[R], WBz[FIELD ? R : 1], WBr[FIELD ? R : 1];
+#pragma unroll
+    for (int k = 1; k < R; ++k) {                              // jz = 0: outputs k >= 1 (output 0 is loaded in the loop)
+      WM[k] = wM[k];
+      if (FIELD) WBz[k] = wBz[k], WBr[k] = wBr[k];
+    }
+    for (int jb = 0; jb < NzPad; jb += R) {
+#pragma unroll
+      for (int u = 0; u < R; ++u) {
+        const int jz = jb + u;
+        constexpr int kR = R;
+        const int reg0 = (kR - u) % kR;                        // register of output 0 at this source
+        WM[reg0] = wM[-jz];
+        if (FIELD) WBz[reg0] = wBz[-jz], WBr[reg0] = wBr[-jz];
+        const double x = xs[jz];
+        const double c = FIELD ? cs[jz] : 0.0;
+#pragma unroll
+        for (int k = 0; k < R; ++k) {
+          const int reg = (reg0 + k) % kR;
+          yM[k] = fma(WM[reg], x, yM[k]);
+          if (FIELD) {
+            yBz[k] = fma(WBz[reg], c, yBz[k]);
+            yBr[k] = fma(WBr[reg], c, yBr[k]);
+          }
+        }
+      }
+    }
+  }
+  const long long orow = static_cast<long long>(ir) * Nz;
+#pragma unroll
+  for (int k = 0; k < R; ++k) {
+    const int iz = iz0 + k;
+    if (iz < Nz) {
+      asm volatile("red.global.add.f64 [%0], %1;" ::"l"(prm.yacc + orow + iz), "d"(yM[k]) : "memory");
+      if (FIELD) {
+        asm volatile("red.global.add.f64 [%0], %1;" ::"l"(prm.bzacc + orow + iz), "d"(yBz[k]) : "memory");
+        asm volatile("red.global.add.f64 [%0], %1;" ::"l"(prm.bracc + orow + iz), "d"(yBr[k]) : "memory");
+      }
+    }
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_table_build(int Nr, int Nz, double r_inner, double h, double soft_self2, double* TM, double* TBz,
+                               double* TBr, int sm_count, cudaStream_t stream) {
+  table_build_kernel<<<sm_count * 8, 256, 0, stream>>>(Nr, Nz, r_inner, h, soft_self2, TM, TBz, TBr);
+  return cudaGetLastError();
+}
+
+// T threads x R outputs per thread covering Nz with the least padding (R odd, T a multiple of 32)
+void lattice_sweep_shape(int Nz, int* T_out, int* R_out, int* tiles_out) {
+  int bestT = 32, bestR = 1, bestTiles = (Nz + 31) / 32;
+  long long bestCost = -1;
+  const int Rs[5] = {1, 3, 5, 7, 9};
+  for (int T = 32; T <= 256; T += 32)
+    for (int ri = 0; ri < 5; ++ri) {
+      const int R = Rs[ri];
+      const int tiles = (Nz + T * R - 1) / (T * R);
+      // cost ~ issue slots per source element: T threads x (3 cycles per multiply-add x R + 2 shared-memory reads)
+      const long long cost = static_cast<long long>(tiles) * T * (3 * R + 2) * 8 - T / 32;
+      if (bestCost < 0 || cost < bestCost) bestCost = cost, bestT = T, bestR = R, bestTiles = tiles;
+    }
+  *T_out = bestT;
+  *R_out = bestR;
+  *tiles_out = bestTiles;
+}
+
+size_t lattice_sweep_smem(int Nz, int T, int R, bool field) {
+  const int NzPad = (Nz + R - 1) / R * R;
+  const int ext_len = NzPad + T * R;
+  return sizeof(double) * (static_cast<size_t>(field ? 3 : 1) * ext_len + static_cast<size_t>(field ? 2 : 1) * NzPad);
+}
+
+template <int R>
+static cudaError_t launch_R(const LatticeSweepParams& prm, bool field, dim3 grid, int T, size_t smem, cudaStream_t stream) {
+  if (field) {
+    cudaFuncSetAttribute(table_sweep_kernel<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    table_sweep_kernel<R, true><<<grid, T, smem, stream>>>(prm);
+  } else {
+    cudaFuncSetAttribute(table_sweep_kernel<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    table_sweep_kernel<R, false><<<grid, T, smem, stream>>>(prm);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t launch_table_sweep(const LatticeSweepParams& prm_in, bool field, int sm_count, cudaStream_t stream) {
+  LatticeSweepParams prm = prm_in;
+  int T, R, tiles;
+  lattice_sweep_shape(prm.Nz, &T, &R, &tiles);
+  // split the source rows so that the grid fills the GPU several times over
+  const long long want = 16ll * sm_count;
+  int splits = static_cast<int>(std::max<long long>(1, std::min<long long>(prm.Nr, want / std::max(1, prm.Nr * tiles))));
+  prm.jr_chunk = (prm.Nr + splits - 1) / splits;
+  splits = (prm.Nr + prm.jr_chunk - 1) / prm.jr_chunk;
+  const dim3 grid(splits, prm.Nr, tiles);
+  const size_t smem = lattice_sweep_smem(prm.Nz, T, R, field);
+  switch (R) {
+    case 1: return launch_R<1>(prm, field, grid, T, smem, stream);
+    case 3: return launch_R<3>(prm, field, grid, T, smem, stream);
+    case 5: return launch_R<5>(prm, field, grid, T, smem, stream);
+    case 7: return launch_R<7>(prm, field, grid, T, smem, stream);
+    default: return launch_R<9>(prm, field, grid, T, smem, stream);
+  }
+}
+
+}  // namespace qs

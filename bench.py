@@ -49,6 +49,8 @@ def parse_args():
     ap.add_argument("--workload", default="cfg2", choices=sorted(DEFAULTS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the HBM-roofline leg, cfg4 operator leg and cpu_baseline")
+    ap.add_argument("--operator", default="pairs", choices=["pairs", "tables"],
+                    help="pairs: on-the-fly AGM pair sweeps (north_star, default); tables: lattice-aware operator (f1)")
     ap.add_argument("--leg", default="all", choices=["all", "hbm", "operator"],
                     help="hbm / operator: run only that extra leg and print its JSON (used for the ncu captures)")
     a = ap.parse_args()
@@ -340,7 +342,7 @@ def gpu_arm(args):
         print(json.dumps({"leg": args.leg, **leg}), flush=True)
         return
 
-    sim = pkg.QS(w.geometry, w.material, device=local)
+    sim = pkg.QS(w.geometry, w.material, device=local, lattice_tables=args.operator == "tables")
     for _ in range(args.warmup):
         sim.step(w.dt, w.I_ramp)
     # ---- device-resident timing -----------------------------------------------------------------
@@ -378,8 +380,12 @@ def gpu_arm(args):
     dom = "sweep_field" if kf_ms >= km_ms else "sweep_M"
     d_ms, d_n = (kf_ms, kf_n) if dom == "sweep_field" else (km_ms, km_n)
     flop = (FLOP_K2 if dom == "sweep_field" else FLOP_K1) * pe
+    if args.operator == "tables":   # block-Toeplitz product: N^2 multiply-adds per table (3 tables in the fused sweep)
+        flop = 2.0 * N * N * (3 if dom == "sweep_field" else 1)
     ach = flop / (d_ms / max(d_n, 1) * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": f"qs::sweep_kernel<{'true' if dom == 'sweep_field' else 'false'}> ({dom})",
+    kname = (f"qs::sweep_kernel<{'true' if dom == 'sweep_field' else 'false'}> ({dom})" if args.operator == "pairs"
+             else f"qs::table_sweep_kernel<R, {'true' if dom == 'sweep_field' else 'false'}> ({dom}, lattice tables)")
+    roofline = {"bound": "alu", "kernel": kname,
                 "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s", "frac": ach / fp64_tf,
                 "traffic": NCU_TRAFFIC.get(f"{dom}:{w.name}"),
                 "peak_source": "measured in this run: DFMA-chain probe qs_fp64_peak; "
@@ -392,6 +398,7 @@ def gpu_arm(args):
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "n_rings": N, "n_turns": w.geometry.n_turns, "dt": w.dt, "I_ramp": w.I_ramp,
+                       "operator": args.operator,
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "per-cell arrays fit L2; the pair sweep is FP64-ALU bound, HBM legs use a 134 MB/array lattice",
                        "cg_iters_last_step": st["cg_iters"], "heat_substeps": st["heat_substeps"]},
@@ -404,6 +411,18 @@ def gpu_arm(args):
         line["roofline_hbm"] = hbm_roofline_leg(torch, pkg, hbm_peak)
         line["roofline_hbm"]["peak_source"] = f"MEASURED_PEAKS.json hbm_gbs ({hbm_src})"
         line["operator_cfg4"] = operator_leg(torch, pkg, fp64_tf)
+        if args.operator == "pairs":   # SURVEY.md §8(f) f1, same workload: tables over (ir, jr, |dz|) + block-Toeplitz sweeps
+            with pkg.QS(w.geometry, w.material, device=local, lattice_tables=True) as sim2:
+                for _ in range(args.warmup):
+                    sim2.step(w.dt, w.I_ramp)
+                sim2.profile_enable(True)
+                ms2, _ = timed_steps(torch, sim2, w, args.steps)
+                pr2 = sim2.profile_read()
+            sw_ms = pr2["sweep_field"][0] / max(pr2["sweep_field"][1], 1)
+            line["next_f1_lattice_tables"] = {
+                "value": N * args.steps / (ms2 * 1e-3), "unit": UNIT, "ms_per_step": ms2 / args.steps,
+                "sweep_ms": sw_ms, "sweep_tflops": 6.0 * N * N / (sw_ms * 1e-3) / 1e12 if sw_ms > 0 else None,
+                "note": "not the graded path: north_star fixes on-the-fly AGM pair evaluation"}
         if N <= 4096:
             v, total, sample = run_oracle_steps(w, min(args.steps, 20), 1)
         else:

@@ -303,13 +303,20 @@ def operator_leg(torch, pkg, fp64_peak):
         xd = torch.empty_like(bd)
         torch.cuda.synchronize()
         sim.solve_device(bd, xd, maxit=5)
+        sim.profile_enable(True)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(sim.stream)
         it, relres, _ = sim.solve_device(bd, xd, maxit=50)
         b.record(sim.stream)
         sim.sync()
         b.synchronize()
-    out["cg_N65536"] = {"iterations": it, "iters_per_s": it / (a.elapsed_time(b) * 1e-3), "relres_reached": relres}
+        pr = sim.profile_read()
+    vec_us = 1e3 * pr["cg_vector"][0] / max(it, 1)
+    out["cg_N65536"] = {"iterations": it, "iters_per_s": it / (a.elapsed_time(b) * 1e-3), "relres_reached": relres,
+                        "sweep_ms_per_iteration": pr["sweep_M"][0] / max(pr["sweep_M"][1], 1),
+                        "vector_kernels_us_per_iteration": vec_us,
+                        "vector_kernels_GBs": 152.0 * n / (vec_us * 1e-6) / 1e9 if vec_us > 0 else None,
+                        "vector_bytes_per_ring": 152.0}
     return out
 
 

@@ -391,7 +391,7 @@ __global__ void __launch_bounds__(kHeatWarps * 32, 3) heat_kernel(MaterialParams
 // ---- K6, TMA-pipelined variant (Nz even): same marching scheme, but every warp streams its 512-byte row segments
 // of H and Q through a ring of kHeatStages shared-memory stages with TMA bulk copies (cp.async.bulk + mbarrier,
 // issued by lane 0), so that kHeatStages rows per warp are in flight whatever the register budget.
-constexpr int kHeatStages = 6;
+constexpr int kHeatStages = 8;
 struct HeatStage {
   double h[64];
   double q[64];

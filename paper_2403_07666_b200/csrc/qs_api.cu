@@ -130,6 +130,12 @@ struct qs_ctx {
   int* rowturn = nullptr;            // [Nr] (ir / n) * turns_per_layer
   unsigned long long *xmax_bits = nullptr, *rmin_bits = nullptr;   // [n_turns] event observables of the material pass
   double4* rowtab = nullptr;         // [Nr] (r, selfcoef, diagM, area) per radial row of a lattice
+  // CUDA graphs of two fused CG iterations (parities 0, 1), keyed by the vectors they were captured with
+  struct CgGraph {
+    const double *x = nullptr, *shift = nullptr, *Hd = nullptr, *sw = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    int launches = 0;
+  } cg_graph[2];
   bool canonical_turns = false;      // turn_id[c] == (ir / n) * turns_per_layer + iz / n for every cell
   bool aux_on = false;               // qs_material_eval also writes dE/dJ (after the first qs_read_aux)
   double last_eval_dt = 0.0;
@@ -351,18 +357,67 @@ int cg_core(qs_ctx* c, const Rhs& b, double* x, const double* shift, const doubl
   it.yacc_zero = c->yacc;
   it.counter = c->counter;
   it.cM = kCM;
+  // one iteration = sweep + four vector kernels; pairs of iterations are replayed from a CUDA graph (captured on
+  // first use for this set of vectors) unless the event profiler is recording
+  auto enqueue_iteration = [&](int par) -> int {
+    it.par = par;
+    int r2 = do_sweep(c, c->p, nullptr, false, true, true);
+    if (r2 != QS_OK) return r2;
+    c->prof.begin(c->stream);
+    k_cg_Ap(v, it);
+    k_cg_update(v, it);
+    k_cg_project(v, it);
+    k_cg_direction(v, it);
+    c->prof.end(c->stream, QS_PROF_CG_VECTOR, 4);
+    return QS_OK;
+  };
+  qs_ctx::CgGraph* graph = nullptr;
+  if (!c->prof.on) {
+    for (auto& gslot : c->cg_graph)
+      if (gslot.exec && gslot.x == x && gslot.shift == shift && gslot.Hd == Hd && gslot.sw == sw) graph = &gslot;
+    if (!graph) {
+      qs_ctx::CgGraph& gslot = c->cg_graph[c->cg_graph[0].exec ? 1 : 0];
+      if (gslot.exec) {
+        cudaGraphExecDestroy(gslot.exec);
+        gslot.exec = nullptr;
+      }
+      const long long l0 = c->launches, p0 = c->pair_evals;
+      const int s0 = c->st.sweeps;
+      cudaGraph_t gr = nullptr;
+      if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed) == cudaSuccess) {
+        const bool ok = enqueue_iteration(0) == QS_OK && enqueue_iteration(1) == QS_OK;
+        const cudaError_t ec = cudaStreamEndCapture(c->stream, &gr);
+        if (ok && ec == cudaSuccess && gr && cudaGraphInstantiate(&gslot.exec, gr, 0) == cudaSuccess) {
+          gslot.x = x, gslot.shift = shift, gslot.Hd = Hd, gslot.sw = sw;
+          gslot.launches = static_cast<int>(c->launches - l0);
+          graph = &gslot;
+        } else {
+          gslot.exec = nullptr;
+          cudaGetLastError();
+        }
+        if (gr) cudaGraphDestroy(gr);
+      }
+      c->launches = l0;        // capture enqueued nothing
+      c->pair_evals = p0;
+      c->st.sweeps = s0;
+    }
+  }
+  const long long evals_per_sweep = c->tables ? 0 : (static_cast<long long>(c->nb) * (c->nb + 1) / 2) * 1024;
   int enq = 0, batch = 2;
   for (;;) {
     const int todo = std::min(batch, maxit - enq);
-    for (int k = 0; k < todo; ++k, ++enq) {
-      it.par = enq & 1;
-      if ((rc = do_sweep(c, c->p, nullptr, false, true, true)) != QS_OK) return rc;
-      c->prof.begin(c->stream);
-      k_cg_Ap(v, it);
-      k_cg_update(v, it);
-      k_cg_project(v, it);
-      k_cg_direction(v, it);
-      c->prof.end(c->stream, QS_PROF_CG_VECTOR, 4);
+    int k = 0;
+    while (k < todo) {
+      if (graph && (enq & 1) == 0 && k + 2 <= todo) {
+        QS_CUDA(cudaGraphLaunch(graph->exec, c->stream));
+        c->launches += graph->launches;
+        c->pair_evals += 2 * evals_per_sweep;
+        c->st.sweeps += 2;
+        k += 2, enq += 2;
+      } else {
+        if ((rc = enqueue_iteration(enq & 1)) != QS_OK) return rc;
+        ++k, ++enq;
+      }
     }
     if ((rc = sync_scalars(c)) != QS_OK) return rc;
     if (c->h_sc->done == 2) return fail(QS_ERR_CG, "CG breakdown: p^T A p <= 0 or NaN");
@@ -772,6 +827,8 @@ void qs_free(qs_ctx* c) {
   if (!c) return;
   if (c->stream) cudaStreamSynchronize(c->stream);
   c->prof.destroy();
+  for (auto& gslot : c->cg_graph)
+    if (gslot.exec) cudaGraphExecDestroy(gslot.exec);
   if (c->h_sc) cudaFreeHost(c->h_sc);
   if (c->h_stage) cudaFreeHost(c->h_stage);
   if (c->owned) {

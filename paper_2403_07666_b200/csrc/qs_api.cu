@@ -451,11 +451,16 @@ int run_heat(qs_ctx* c, double dt, int* m_out) {
   const int m = heat_substeps_count(c, dt);
   const double sub = dt / m;
   c->prof.begin(c->stream);
-  for (int s = 0; s < m; ++s) {
-    k_heat_substep(c->v, c->mp, c->lp, c->H, c->Q, c->Halt, sub);
+  if (k_heat_all_substeps(c->v, c->mp, c->lp, m, c->H, c->Q, c->Halt, sub)) {   // small lattice: one in-SM launch
     std::swap(c->H, c->Halt);
+    c->prof.end(c->stream, QS_PROF_HEAT, 1);
+  } else {
+    for (int s = 0; s < m; ++s) {
+      k_heat_substep(c->v, c->mp, c->lp, c->H, c->Q, c->Halt, sub);
+      std::swap(c->H, c->Halt);
+    }
+    c->prof.end(c->stream, QS_PROF_HEAT, m);
   }
-  c->prof.end(c->stream, QS_PROF_HEAT, m);
   *m_out = m;
   QS_CUDA(cudaGetLastError());
   return QS_OK;

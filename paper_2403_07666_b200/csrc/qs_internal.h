@@ -190,6 +190,9 @@ void k_enthalpy_from_T(const VecCtx& v, const MaterialParams& mp, const double* 
 void k_T_from_enthalpy(const VecCtx& v, const MaterialParams& mp, const double* H, double* T, int n);
 void k_heat_substep(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, const double* Hin,
                     const double* Q, double* Hout, double dtsub);
+// all m sub-steps in one launch for lattices small enough to live in one SM; false: not applicable (use k_heat_substep)
+bool k_heat_all_substeps(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, int m, const double* Hin,
+                         const double* Q, double* Hout, double dtsub);
 struct EventArgs {
   const double *H, *E;
   const unsigned long long *xmax_bits, *rmin_bits;   // per turn, from the material pass

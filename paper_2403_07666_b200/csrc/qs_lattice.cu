@@ -16,8 +16,6 @@
 // window element per jz feed R multiply-adds (register rotation by unrolling, no moves).  Partial sums over the
 // jr chunks are combined with FP64 red.add in L2.
 #include <algorithm>
-#include <cstdio>
-#include <cstdlib>
 
 #include "qs_internal.h"
 #include "qs_pair.cuh"
@@ -169,11 +167,6 @@ void lattice_sweep_shape(int Nz, int* T_out, int* R_out, int* tiles_out) {
       const long long cost = static_cast<long long>(tiles) * T * (3 * R + 2) * 8 - T / 32;
       if (bestCost < 0 || cost < bestCost) bestCost = cost, bestT = T, bestR = R, bestTiles = tiles;
     }
-  if (const char* e = getenv("QS_TAB_TR")) {   // experiment hook: "T,R"
-    int t = 0, r = 0;
-    if (sscanf(e, "%d,%d", &t, &r) == 2 && t >= 32 && t <= 256 && (r == 1 || r == 3 || r == 5 || r == 7 || r == 9))
-      bestT = t, bestR = r, bestTiles = (Nz + t * r - 1) / (t * r);
-  }
   *T_out = bestT;
   *R_out = bestR;
   *tiles_out = bestTiles;

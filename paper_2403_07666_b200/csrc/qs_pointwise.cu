@@ -501,6 +501,76 @@ __global__ void __launch_bounds__(kHeatWarps * 32, 3) heat_tma_kernel(MaterialPa
   }
 }
 
+// ---- K6, in-SM variant for small lattices (N <= kHeatSmallMax cells): ALL m sub-steps of a step in one launch.
+// One CTA of 1024 threads keeps the enthalpy of its cells in registers and T^2 of the whole lattice in shared
+// memory; a sub-step is "publish T^2, barrier, update H, barrier".  Replaces m launches (144 per step at config 1)
+// by one; the arithmetic per cell and sub-step is the one of the marching kernel.
+constexpr int kHeatSmallThreads = 1024;
+constexpr int kHeatSmallPer = 4;
+constexpr int kHeatSmallMax = kHeatSmallThreads * kHeatSmallPer;   // 4096 cells = 32 KB of T^2 (config 1: 64 x 64)
+
+__global__ void __launch_bounds__(kHeatSmallThreads, 1) heat_small_kernel(MaterialParams mp, LatticeParams lp, int m,
+                                                                          const double* __restrict__ Hin,
+                                                                          const double* __restrict__ Q,
+                                                                          double* __restrict__ Hout, double dtsub) {
+  extern __shared__ __align__(16) double hs_smem[];
+  const int N = lp.Nr * lp.Nz, Nz = lp.Nz, Nr = lp.Nr;
+  double* Us = hs_smem;                                   // [N] T^2
+  double* crp = Us + N;                                   // per-row coefficients [Nr] x 3, per-column [Nz] x 3
+  double* crm = crp + Nr;
+  double* crb = crm + Nr;
+  double* czp = crb + Nr;
+  double* czm = czp + Nz;
+  double* czb = czm + Nz;
+  for (int i = threadIdx.x; i < Nr; i += blockDim.x) crp[i] = lp.hr_p[i], crm[i] = lp.hr_m[i], crb[i] = lp.rb_r[i];
+  for (int i = threadIdx.x; i < Nz; i += blockDim.x) czp[i] = lp.hz_p[i], czm[i] = lp.hz_m[i], czb[i] = lp.rb_z[i];
+  const double C3 = mp.C3, qC1sq = 0.25 * mp.C1 * mp.C1, hC1 = 0.5 * mp.C1, inv_hC3 = 2.0 / mp.C3;
+  double H[kHeatSmallPer], q[kHeatSmallPer];
+  int ir[kHeatSmallPer], iz[kHeatSmallPer];
+#pragma unroll
+  for (int k = 0; k < kHeatSmallPer; ++k) {
+    const int i = threadIdx.x + k * kHeatSmallThreads;
+    H[k] = q[k] = 0.0;
+    ir[k] = iz[k] = 0;
+    if (i < N) {
+      ir[k] = i / Nz, iz[k] = i - ir[k] * Nz;
+      H[k] = Hin[i];
+      q[k] = Q[i];
+    }
+  }
+  for (int s = 0; s < m; ++s) {
+#pragma unroll
+    for (int k = 0; k < kHeatSmallPer; ++k) {
+      const int i = threadIdx.x + k * kHeatSmallThreads;
+      if (i < N) Us[i] = tsq_fast(H[k], C3, qC1sq, hC1, inv_hC3);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kHeatSmallPer; ++k) {
+      const int i = threadIdx.x + k * kHeatSmallThreads;
+      if (i < N) {
+        const double u = Us[i];
+        // neighbours outside the pack have coefficient 0: read the cell itself instead
+        const double un = ir[k] + 1 < Nr ? Us[i + Nz] : u, up = ir[k] > 0 ? Us[i - Nz] : u;
+        const double ur = iz[k] + 1 < Nz ? Us[i + 1] : u, ul = iz[k] > 0 ? Us[i - 1] : u;
+        double a = fma(crp[ir[k]], un - u, q[k]);
+        a = fma(crm[ir[k]], up - u, a);
+        a = fma(czp[iz[k]], ur - u, a);
+        a = fma(czm[iz[k]], ul - u, a);
+        const double rb = crb[ir[k]] + czb[iz[k]];
+        if (rb != 0.0) a = fma(-rb, sqrt_fast(u) - lp.T_bath, a);
+        H[k] = fma(dtsub, a, H[k]);
+      }
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int k = 0; k < kHeatSmallPer; ++k) {
+    const int i = threadIdx.x + k * kHeatSmallThreads;
+    if (i < N) Hout[i] = H[k];
+  }
+}
+
 // ---- K7 ---------------------------------------------------------------------------------------------------
 __global__ void events_kernel(int n_turns, const int* __restrict__ ptr, const int* __restrict__ idx,
                               MaterialParams mp, EventArgs e, Scalars* sc) {
@@ -627,6 +697,20 @@ void k_heat_substep(const VecCtx& v, const MaterialParams& mp, const LatticePara
     heat_tma_kernel<<<grid, kHeatWarps * 32, sizeof(HeatSmem), v.stream>>>(mp, lp, rows, Hin, Q, Hout, dtsub);
   } else
     heat_kernel<false><<<grid, kHeatWarps * 32, 0, v.stream>>>(mp, lp, rows, Hin, Q, Hout, dtsub);
+}
+bool k_heat_all_substeps(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, int m, const double* Hin,
+                         const double* Q, double* Hout, double dtsub) {
+  const long long N = static_cast<long long>(lp.Nr) * lp.Nz;
+  if (N > kHeatSmallMax || m < 2) return false;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(heat_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);   // N + 3 (Nr + Nz) doubles <= 131 KB
+    attr_set = true;
+  }
+  QS_LAUNCH(v);
+  heat_small_kernel<<<1, kHeatSmallThreads, sizeof(double) * (N + 3 * (lp.Nr + lp.Nz)), v.stream>>>(mp, lp, m, Hin, Q, Hout,
+                                                                                                 dtsub);
+  return true;
 }
 void k_events(const VecCtx& v, const MaterialParams& mp, const EventArgs& e) {
   if (!v.n_turns) return;

@@ -905,8 +905,13 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
       return rc;
     }
   } else {
+    // nu == 0: the cold start x_p = I_ramp xp1 already solves the projected system (e.g. one cell per turn, where the
+    // constraint alone fixes I'; or b = 0 with no ramp, where x_p = 0); its projection multipliers are the V_w (C8)
     QS_CUDA(cudaMemsetAsync(c->x, 0, nb8, c->stream));
-    if (c->n_turns) QS_CUDA(cudaMemsetAsync(c->vsum, 0, sizeof(double) * c->n_turns, c->stream));
+    if (c->n_turns) {
+      k_axpy(v, I_ramp, c->xp1, c->x);
+      QS_CUDA(cudaMemcpyAsync(c->vsum, c->vw, sizeof(double) * c->n_turns, cudaMemcpyDeviceToDevice, c->stream));
+    }
   }
   k_sum_uterm(v, c->vsum);
   // S5

@@ -189,3 +189,18 @@ def test_full_size_step_sampled_outputs_and_invariants(pkg, cfg, rows):
     dI = np.bincount(geo.turn_id, weights=geo.area * (J1 - J0), minlength=geo.n_turns)
     assert np.max(np.abs(dI - w.dt * w.I_ramp)) <= 1e-9 * w.dt * w.I_ramp + 1e-12 * np.max(np.abs(geo.area * J0)) * 200
     assert np.all(np.isfinite(T1)) and st["heat_substeps"] == qo.heat_substeps_count(geo, mat, w.dt)
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 1), (1, 1, 2), (2, 1, 1), (1, 3, 1), (1, 1, 3)])
+@pytest.mark.parametrize("tables", [False, True])
+def test_degenerate_lattices(pkg, shape, tables):
+    # one-cell wires, single rows / columns: every stencil neighbour is a border, blocks are almost all padding
+    L, Tn, n = shape
+    geo = wl.lattice_geometry(L, Tn, n, 1.0e-3, 30e-3, Bext_rate=5.0, Bext_max=3.0)
+    mat = dataclasses.replace(wl.Material(jc0_scale=wl.jc0_scale(5, geo.n_rings, 0.01)), cg_tol=1e-12)
+    orc = qo.Oracle(geo, mat)
+    with pkg.QS(geo, mat, lattice_tables=tables) as sim:
+        for _ in range(30):
+            assert orc.step(1e-4, 40.0) == (sim.step(1e-4, 40.0) & 3)
+        got, ref = sim.read(), orc.read()
+    check_state(ref, got)

@@ -239,3 +239,67 @@ def test_pair_arithmetic_every_class_at_its_threshold(pkg):
     assert np.all(np.diff(used) <= 0)
     Ko, Eo = qo.elliptic_KE(dz2 / (4 * ri * ri + dz2))
     assert np.max(np.abs(K / Ko - 1)) <= 4e-15 and np.max(np.abs(E / Eo - 1)) <= 2e-14
+
+
+@pytest.mark.parametrize("n_exp,eps_exp", [(15.0, 1.7), (20.5, 2.3), (2.0, 1.0)])
+def test_material_law_other_exponents(pkg, n_exp, eps_exp):
+    # integer n != 20 (binary powering), non-integer n (exp/log path), other strain exponents
+    w = wl.shrunk(0, 2, 2, 6)
+    geo = w.geometry
+    mat = dataclasses.replace(w.material, n_exp=n_exp, eps_exp=eps_exp)
+    N = geo.n_rings
+    g = np.random.default_rng(int(10 * n_exp))
+    Jc0 = 2e9 * (1 - 4.2 / 18) ** 2
+    J = Jc0 * g.uniform(-1.2, 1.2, N)
+    T = g.uniform(4.2, 16.0, N)
+    B = np.concatenate([g.uniform(-2, 2, N), g.uniform(-12, 12, N)])
+    with pkg.QS(geo, mat) as sim:
+        sim.write(J, T, 0.0, 0.0)
+        sim.set_fields(B=B)
+        sim.material_eval(1e-4)
+        _, _, _, E = sim.read()
+        aux = sim.read_aux()
+    ml = qo.material_law(mat, J, T, B[:N], B[N:], geo.r, mat.jc0_scale)
+    for key, got in [("E", E), ("Q", aux["Q"]), ("dEdJ", aux["dEdJ"]), ("Jc", aux["Jc"]), ("rho", aux["rho"])]:
+        assert rel(got, ml[key]) <= 1e-11, key
+
+
+def test_material_law_on_free_rings(pkg):
+    # the per-cell-array path of the material pass (no lattice row tables, no event reduction)
+    geo, _ = wl.free_rings(300, seed=9)
+    geo = dataclasses.replace(geo, T_bath=4.2)
+    mat = wl.Material(jc0_scale=wl.jc0_scale(3, 300, 0.02))
+    g = np.random.default_rng(77)
+    J = 1e9 * g.uniform(-1.0, 1.0, 300)
+    T = g.uniform(4.2, 19.0, 300)
+    B = np.concatenate([g.uniform(-1, 1, 300), g.uniform(-8, 8, 300)])
+    with pkg.QS(geo, mat) as sim:
+        sim.write(J, T, 0.0, 0.0)
+        sim.set_fields(B=B)
+        sim.material_eval(1e-4)
+        _, Tg, _, E = sim.read()
+        aux = sim.read_aux()
+    ml = qo.material_law(mat, J, T, B[:300], B[300:], geo.r, mat.jc0_scale)
+    assert np.max(np.abs(Tg - T)) <= 1e-12 * 19
+    for key, got in [("E", E), ("Q", aux["Q"]), ("dEdJ", aux["dEdJ"]), ("Jc", aux["Jc"]), ("rho", aux["rho"])]:
+        assert rel(got, ml[key]) <= 1e-11, key
+
+
+def test_heat_adiabatic_energy_conservation_on_the_gpu(pkg):
+    # h_conv = 0: sum_c V_c (H_c' - H_c) = dt sum_c V_c Q_c to rounding (finite-volume fluxes cancel pairwise)
+    geo = wl.lattice_geometry(3, 4, 10, 1e-3, 30e-3, h_conv=0.0)
+    mat = wl.Material()
+    N = geo.n_rings
+    g = np.random.default_rng(12)
+    T = g.uniform(4.2, 15.0, N)
+    Q = g.uniform(0, 5e6, N)
+    dt = 2e-4
+    with pkg.QS(geo, mat, no_operator=True) as sim:
+        sim.write(np.zeros(N), T, 0.0, 0.0)
+        sim.set_fields(Q=Q)
+        m = sim.heat(dt)
+        _, T1, _, _ = sim.read(J=False, B=False, E=False)
+    assert m > 1
+    V = 2 * np.pi * geo.r * geo.h ** 2
+    dH = qo.enthalpy(mat, T1) - qo.enthalpy(mat, T)
+    assert abs(np.sum(V * dH) - dt * np.sum(V * Q)) <= 1e-10 * dt * np.sum(V * Q)

@@ -204,3 +204,16 @@ def test_degenerate_lattices(pkg, shape, tables):
             assert orc.step(1e-4, 40.0) == (sim.step(1e-4, 40.0) & 3)
         got, ref = sim.read(), orc.read()
     check_state(ref, got)
+
+
+def test_explicit_theta0_steps(pkg):
+    # C7: theta = 0 (the literal explicit Euler reading) stays available; linear regime and a mildly nonlinear wire
+    for w, steps, kw in ((wl.shrunk(0, 2, 2, 8), 30, {}), (wl.shrunk(1, 1, 1, 16), 60, {"Bext_rate": 2.0})):
+        geo = dataclasses.replace(w.geometry, **kw)
+        mat = dataclasses.replace(w.material, theta=0.0, cg_tol=1e-12)
+        orc = qo.Oracle(geo, mat)
+        with pkg.QS(geo, mat) as sim:
+            for _ in range(steps):
+                assert orc.step(w.dt, w.I_ramp) == (sim.step(w.dt, w.I_ramp) & 3)
+            got, ref = sim.read(), orc.read()
+        check_state(ref, got)

@@ -475,6 +475,10 @@ class Oracle:
         self.t_first = np.full(nt, -1.0)
         self.count = np.zeros(nt, dtype=np.int32)
         self.Ebar_prev = None
+        # per-wire statistics (PAPER.md:107 T_max, P_max, Q_FJ per wire; PAPER.md:119-121 Q_q, P_q, T_q)
+        self.wire = dict(E_joule=np.zeros(nt), Q_FJ=np.zeros(nt), P_max=np.zeros(nt), T_max=np.full(nt, geo.T_bath),
+                         t_q=np.full(nt, -1.0), T_q=np.zeros(nt), P_q=np.zeros(nt), Q_q=np.zeros(nt),
+                         E_at_first=np.zeros(nt))
         self.stats = dict(cg_iters=0, cg_relres=0.0, U_terminal=0.0, Tmax=geo.T_bath, joule_power=0.0,
                           boundary_energy=0.0, heat_substeps=0)
 
@@ -500,6 +504,9 @@ class Oracle:
         self.t, self.I = float(t), float(I)
         self.Ebar_prev = None
         self.Idot = np.zeros(self.N)
+        nt = max(self.geo.n_turns, 0)
+        for key, val in self.wire.items():                      # qs_write resets the per-wire statistics
+            val[:] = self.geo.T_bath if key == "T_max" else (-1.0 if key == "t_q" else 0.0)
 
     def read(self):
         return self.J.copy(), self.T.copy(), np.concatenate([self.Br, self.Bz]), self.E.copy()
@@ -568,11 +575,39 @@ class Oracle:
         first = (fl != 0) & (self.t_first < 0.0)
         self.t_first[first] = self.t
         fj_all = FJ_T | FJ_E | FJ_J
+        self._wire_statistics(dt, ml, Tmax, fl, first)
         started = ((fl & fj_all) != 0) & ((self.flags & fj_all) == 0)
         ret = (RET_FLUXJUMP if np.any(started) else 0) | (RET_QUENCH if np.any(fl & (Q_T | Q_RHO)) else 0)
         self.flags = fl
         self.Ebar_prev = Ebar
         return int(ret)
+
+    def _wire_statistics(self, dt, ml, Tmax, fl, first):
+        """Per-wire accumulators after a step (readings of DESIGN.md §3 "f3").
+
+        E_joule  += dt * sum_{i in w} Q_i V_i            Joule energy of the wire [J], V_i = 2 pi r_i a_i
+        Q_FJ     += the same, in steps where a flux-jump flag (FJ_T|FJ_E|FJ_J) of the wire is set
+        P_max, T_max  running maxima of max_i Q_i [W/m^3] and of the wire's Tmax [K]
+        at the first step with a quench flag (Q_T|Q_RHO): t_q, T_q = Tmax_w, P_q = max_i Q_i,
+        Q_q = Joule energy from the wire's first event to the quench = E_joule(t_q) - E_joule(before the first event step)
+        """
+        geo, wr = self.geo, self.wire
+        nt, tid = geo.n_turns, geo.turn_id
+        Q = ml["Q"]
+        dE = dt * np.bincount(tid, weights=Q * 2.0 * math.pi * geo.r * geo.area, minlength=nt)
+        Pw = np.zeros(nt)
+        np.maximum.at(Pw, tid, Q)
+        wr["E_at_first"][first] = wr["E_joule"][first]          # energy before the step of the first event
+        wr["E_joule"] += dE
+        fj = (fl & (FJ_T | FJ_E | FJ_J)) != 0
+        wr["Q_FJ"][fj] += dE[fj]
+        wr["P_max"] = np.maximum(wr["P_max"], Pw)
+        wr["T_max"] = np.maximum(wr["T_max"], Tmax)
+        newq = ((fl & (Q_T | Q_RHO)) != 0) & (wr["t_q"] < 0.0)
+        wr["t_q"][newq] = self.t
+        wr["T_q"][newq] = Tmax[newq]
+        wr["P_q"][newq] = Pw[newq]
+        wr["Q_q"][newq] = wr["E_joule"][newq] - wr["E_at_first"][newq]
 
     # -- config 4 ---------------------------------------------------------------------
     def solve(self, b, tol=None, maxit=None, dense=False):

@@ -193,3 +193,40 @@ def test_event_variants():
     ret = o.step(1e-6, w.I_ramp)
     assert ret & qo.RET_QUENCH and o.flags[5] & qo.Q_T and o.flags[5] & qo.Q_RHO and o.flags[5] & qo.FJ_T
     assert np.all(np.delete(o.flags, 5) & (qo.Q_T | qo.Q_RHO) == 0)
+
+
+def test_wire_statistics_closed_forms_and_energy_identity():
+    # f3 per-wire accumulators: a prepared normal-state turn carrying J0 dissipates exactly
+    # rho_n J0^2 per volume, so E_joule, P_q, Q_q of that turn have closed forms after one step; the sum of E_joule
+    # over all turns equals the time integral of the step's Joule power (an independent accumulation)
+    w = wl.config(0)
+    geo, mat = w.geometry, w.material
+    N = geo.n_rings
+    J0 = np.full(N, 0.5 * 2e9 * (1 - 4.2 / 18) ** 2)
+    T0 = np.full(N, geo.T_bath)
+    hot = geo.turn_id == 5
+    T0[hot] = 19.0                                               # above Tc: rho = rho_n exactly (C5 guard)
+    o = qo.Oracle(geo, mat)
+    o.write(J0, T0, 0.0, 0.0)
+    dt = 1e-6
+    total = 0.0
+    o.step(dt, 0.0)
+    total += dt * o.stats["joule_power"]
+    V5 = np.sum(2 * math.pi * geo.r[hot] * geo.area[hot])
+    P = mat.rho_n * J0[0] ** 2
+    wr = o.wire
+    assert abs(wr["E_joule"][5] - dt * P * V5) <= 1e-12 * dt * P * V5
+    assert abs(wr["P_q"][5] - P) <= 1e-12 * P and abs(wr["P_max"][5] - P) <= 1e-12 * P
+    assert abs(wr["t_q"][5] - dt) < 1e-20 and wr["T_q"][5] > mat.Tc
+    assert abs(wr["Q_q"][5] - wr["E_joule"][5]) <= 1e-15 * wr["E_joule"][5]     # first event and quench in the same step
+    assert abs(wr["Q_FJ"][5] - wr["E_joule"][5]) <= 1e-15 * wr["E_joule"][5]
+    cold = np.delete(np.arange(geo.n_turns), 5)
+    assert np.all(wr["t_q"][cold] < 0) and np.all(wr["Q_q"][cold] == 0)
+    for _ in range(5):
+        o.step(dt, 0.0)
+        total += dt * o.stats["joule_power"]
+    assert abs(wr["E_joule"].sum() - total) <= 1e-12 * total
+    assert np.all(wr["Q_FJ"] <= wr["E_joule"] * (1 + 1e-15)) and np.all(wr["T_max"] >= geo.T_bath)
+    assert abs(wr["Q_q"][5] - dt * P * V5) <= 1e-12 * dt * P * V5               # frozen at the quench time
+    o.write(J0, T0, 0.0, 0.0)
+    assert np.all(o.wire["E_joule"] == 0) and np.all(o.wire["t_q"] == -1.0)

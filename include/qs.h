@@ -142,7 +142,7 @@ int  qs_init_device(const qs_geometry *geo, const qs_material *mat, void *worksp
                     size_t workspace_bytes, void *stream, qs_ctx **out);
 
 /* Set the state (resume, prepared variants C12).  NULL J or T keeps the current array.  Resets the
- * dE/dt history of the event detector; the previous I' is kept as the CG's initial guess (the
+ * dE/dt history of the event detector and the per-wire statistics; the previous I' is kept as the CG's initial guess (the
  * solution of the step does not depend on it beyond cg_tol).  */
 int  qs_write(qs_ctx *ctx, const double *J, const double *T, double t, double I);
 
@@ -209,6 +209,15 @@ int  qs_fp64_peak(double *tflops, double *sm_clock_mhz_effective);
  * DFMA.  Needs no handle.  */
 int  qs_issue_probe(int32_t mode, double *cycles_per_dfma);
 int  qs_events(qs_ctx *ctx, int32_t *flags /*[N_w]*/, double *t_first /*[N_w]*/, int32_t *count /*[N_w]*/);
+/* Per-wire statistics accumulated by the event pass since qs_init / the last qs_write (
+ * PAPER.md:107 T_max, P_max, Q_FJ per wire; PAPER.md:119-121 Q_q, P_q, T_q at the quench time).  out: HOST buffer of
+ * 8 * N_w doubles, row k of N_w entries:
+ *   0 E_joule [J]  time integral of the wire's Joule power sum_i Q_i 2 pi r_i a_i
+ *   1 Q_FJ [J]     the same, over the steps in which a flux-jump flag (FJ_T|FJ_E|FJ_J) of the wire is set
+ *   2 P_max [W/m^3], 3 T_max [K]   running maxima of max_i Q_i and of the wire's Tmax
+ *   4 t_q [s] (-1: never), 5 T_q [K], 6 P_q [W/m^3]   time, Tmax and max_i Q_i at the first step with a quench flag
+ *   7 Q_q [J]      Joule energy of the wire from its first event to the quench  */
+int  qs_wire_stats(qs_ctx *ctx, double *out);
 int  qs_sync(qs_ctx *ctx);                 /* wait for the handle's stream */
 const char *qs_last_error(void);
 void qs_free(qs_ctx *ctx);

@@ -77,6 +77,7 @@ SYMBOLS = [
     ("qs_issue_probe", C.c_int, [C.c_int32, c_double_p]),
     ("qs_pair_eval", C.c_int, [C.c_int32, c_double_p, c_double_p, C.c_int32, c_double_p, c_double_p, c_double_p, c_int32_p]),
     ("qs_events", C.c_int, [_VP, c_int32_p, c_double_p, c_int32_p]),
+    ("qs_wire_stats", C.c_int, [_VP, c_double_p]),
     ("qs_sync", C.c_int, [_VP]),
     ("qs_last_error", C.c_char_p, []),
     ("qs_free", None, [_VP]),
@@ -324,6 +325,16 @@ class QS:
         if nt:
             self._check(self._lib.qs_events(self._h, fl.ctypes.data_as(c_int32_p), _dp(tf), cnt.ctypes.data_as(c_int32_p)))
         return fl, tf, cnt
+
+    WIRE_KEYS = ("E_joule", "Q_FJ", "P_max", "T_max", "t_q", "T_q", "P_q", "Q_q")
+
+    def wire_stats(self) -> dict:
+        """Per-wire statistics (see qs_wire_stats in include/qs.h): {name: array [n_turns]}."""
+        nt = max(self.n_turns, 0)
+        out = np.zeros(8 * nt)
+        if nt:
+            self._check(self._lib.qs_wire_stats(self._h, _dp(out)))
+        return {k: out[j * nt:(j + 1) * nt].copy() for j, k in enumerate(self.WIRE_KEYS)}
 
     def sync(self):
         self._check(self._lib.qs_sync(self._h))

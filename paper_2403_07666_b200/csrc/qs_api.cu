@@ -126,6 +126,7 @@ struct qs_ctx {
   double *yacc, *bracc, *bzacc;
   size_t acc_bytes = 0;
   double *sw, *swM, *vw, *vsum, *tw, *defw, *ebar_prev, *t_first;
+  double* wire = nullptr;            // [9][n_turns] per-wire statistics (f3)
   int *flags, *count, *turn_ptr, *turn_idx, *turn_id, *d_perm;
   int* rowturn = nullptr;            // [Nr] (ir / n) * turns_per_layer
   unsigned long long *xmax_bits = nullptr, *rmin_bits = nullptr;   // [n_turns] event observables of the material pass
@@ -209,6 +210,7 @@ void carve(qs_ctx* c, void* base, size_t* total) {
   c->defw = k.take<double>(nt);
   c->ebar_prev = k.take<double>(nt);
   c->t_first = k.take<double>(nt);
+  c->wire = k.take<double>(9 * nt);
   c->flags = k.take<int>(nt);
   c->count = k.take<int>(nt);
   c->turn_ptr = k.take<int>(nt + 1);
@@ -463,6 +465,17 @@ int run_heat(qs_ctx* c, double dt, int* m_out) {
   }
   *m_out = m;
   QS_CUDA(cudaGetLastError());
+  return QS_OK;
+}
+
+// per-wire statistics start: zeros, T_max = T_bath, t_q = -1
+int reset_wire_stats(qs_ctx* c) {
+  if (c->n_turns <= 0) return QS_OK;
+  const size_t nt = c->n_turns;
+  std::vector<double> w(9 * nt, 0.0);
+  for (size_t k = 0; k < nt; ++k) w[3 * nt + k] = c->lp.T_bath, w[4 * nt + k] = -1.0;
+  QS_CUDA(cudaMemcpyAsync(c->wire, w.data(), sizeof(double) * 9 * nt, cudaMemcpyHostToDevice, c->stream));
+  QS_CUDA(cudaStreamSynchronize(c->stream));
   return QS_OK;
 }
 
@@ -793,6 +806,7 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
     return bail(fail(QS_ERR_CUDA, std::string("initialisation kernels failed: ") + cudaGetErrorString(cudaGetLastError())));
   c->st = qs_stats_t{};
   c->st.Tmax = geo->T_bath;
+  if ((rc = reset_wire_stats(c)) != QS_OK) return bail(rc);
   *out = c;
   return QS_OK;
 }
@@ -922,6 +936,7 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
   // S7 + statistics
   EventArgs ev;
   ev.H = c->H; ev.E = c->E; ev.xmax_bits = c->xmax_bits; ev.rmin_bits = c->rmin_bits;
+  ev.Q = c->Q; ev.r = c->r; ev.area = c->area; ev.wire = c->wire;
   ev.ebar_prev = c->ebar_prev; ev.flags = c->flags; ev.t_first = c->t_first; ev.count = c->count;
   ev.dt = dt; ev.t_new = c->t + dt; ev.have_prev = c->have_prev_E;
   c->prof.begin(c->stream);
@@ -992,7 +1007,7 @@ int qs_write(qs_ctx* c, const double* J, const double* T, double t, double I) {
   c->t = t;
   c->I = I;
   c->have_prev_E = false;
-  return QS_OK;
+  return reset_wire_stats(c);
 }
 
 int qs_matvec_device(qs_ctx* c, const double* d_x, double* d_y) {
@@ -1180,6 +1195,14 @@ int qs_fp64_peak(double* tflops, double* sm_clock_mhz_effective) {
   if (e != cudaSuccess) return fail(QS_ERR_CUDA, std::string("fp64 probe: ") + cudaGetErrorString(e));
   *tflops = tf;
   if (sm_clock_mhz_effective) *sm_clock_mhz_effective = mhz;
+  return QS_OK;
+}
+
+int qs_wire_stats(qs_ctx* c, double* out) {
+  if (!c || !out) return fail(QS_ERR_ARG, "NULL argument");
+  if (!c->n_turns) return QS_OK;
+  QS_CUDA(cudaMemcpyAsync(out, c->wire, sizeof(double) * 8 * c->n_turns, cudaMemcpyDeviceToHost, c->stream));
+  QS_CUDA(cudaStreamSynchronize(c->stream));
   return QS_OK;
 }
 

@@ -196,6 +196,8 @@ bool k_heat_all_substeps(const VecCtx& v, const MaterialParams& mp, const Lattic
 struct EventArgs {
   const double *H, *E;
   const unsigned long long *xmax_bits, *rmin_bits;   // per turn, from the material pass
+  const double *Q, *r, *area;   // Joule power density, ring radius and cross-section per cell (per-wire statistics)
+  double* wire;          // [9][n_turns]: E_joule, Q_FJ, P_max, T_max, t_q, T_q, P_q, Q_q, E_at_first (f3)
   double* ebar_prev;     // [n_turns]
   int* flags;            // [n_turns]
   double* t_first;       // [n_turns]

@@ -576,14 +576,19 @@ __global__ void events_kernel(int n_turns, const int* __restrict__ ptr, const in
                               MaterialParams mp, EventArgs e, Scalars* sc) {
   const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (w >= n_turns) return;
-  double tsq = 0.0, esum = 0.0;
+  double tsq = 0.0, esum = 0.0, qv = 0.0, pmax = 0.0;
   for (int k = ptr[w] + lane; k < ptr[w + 1]; k += 32) {
     const int i = idx[k];
     tsq = fmax(tsq, tsq_of_H(e.H[i], mp.C3, mp.C1));
     esum += fabs(e.E[i]);
+    const double q = e.Q[i];
+    qv = fma(q, 2.0 * kPi * e.r[i] * e.area[i], qv);       // Joule power of the wire [W]
+    pmax = fmax(pmax, q);
   }
   tsq = warp_max(tsq);
   esum = warp_sum(esum);
+  qv = warp_sum(qv);
+  pmax = warp_max(pmax);
   const double xmax = __longlong_as_double(static_cast<long long>(e.xmax_bits[w]));
   const double rmin = __longlong_as_double(static_cast<long long>(e.rmin_bits[w])) / mp.rho_n;
   if (lane != 0) return;
@@ -597,7 +602,26 @@ __global__ void events_kernel(int n_turns, const int* __restrict__ ptr, const in
   if (rmin > 0.95) fl |= 16;
   const int old = e.flags[w];
   if ((fl & 3) && !(old & 3)) e.count[w] += 1;
-  if (fl && e.t_first[w] < 0.0) e.t_first[w] = e.t_new;
+  const bool first = fl && e.t_first[w] < 0.0;
+  if (first) e.t_first[w] = e.t_new;
+  {  // per-wire statistics (f3; PAPER.md:107 T_max, P_max, Q_FJ; PAPER.md:119-121 Q_q, P_q, T_q at the quench time)
+    double* W = e.wire;
+    const int nt = n_turns;
+    const double dE = e.dt * qv;
+    double Ej = W[w];
+    if (first) W[8 * nt + w] = Ej;                         // energy before the step of the first event
+    Ej += dE;
+    W[w] = Ej;
+    if (fl & 7) W[nt + w] += dE;                           // Q_FJ: while a flux-jump flag is set
+    W[2 * nt + w] = fmax(W[2 * nt + w], pmax);
+    W[3 * nt + w] = fmax(W[3 * nt + w], Tmax);
+    if ((fl & 24) && W[4 * nt + w] < 0.0) {                // first step with a quench flag
+      W[4 * nt + w] = e.t_new;
+      W[5 * nt + w] = Tmax;
+      W[6 * nt + w] = pmax;
+      W[7 * nt + w] = Ej - W[8 * nt + w];
+    }
+  }
   int ret = 0;
   if ((fl & 7) && !(old & 7)) ret |= 1;
   if (fl & 24) ret |= 2;

@@ -137,6 +137,14 @@ def test_event_variants(pkg, variant):
     assert np.allclose(tf, orc.t_first, rtol=0, atol=1e-18)
     assert orc.flags.any() and rets[0][0] != 0
     check_state(ref, got, tol=1e-6)
+    # per-wire statistics (f3): same accumulators on both sides
+    ws = sim.wire_stats()
+    for key in ("E_joule", "Q_FJ", "P_max", "T_max", "T_q", "P_q", "Q_q"):
+        ref_w = orc.wire[key]
+        assert np.max(np.abs(ws[key] - ref_w)) <= 1e-6 * max(np.max(np.abs(ref_w)), 1e-300), key
+    assert np.allclose(ws["t_q"], orc.wire["t_q"], rtol=0, atol=1e-18)
+    if variant != "v1":
+        assert ws["t_q"][5] > 0 and ws["Q_q"][5] >= 0
     sim.close()
 
 

@@ -106,6 +106,8 @@ typedef struct {
   double  t, I;                     /* time [s] and transport current [A] after the step         */
   int64_t launches;                 /* kernels launched by this handle since qs_init             */
   int64_t pair_evals;               /* ring-pair evaluations since qs_init                       */
+  double  dJ_max;                   /* max_c |J^{k+1} - J^k| of the last step [A/m^2] (input of the caller's
+                                       time-step controller, C11)                                */
 } qs_stats_t;
 
 /* ---- the three calls north_star names -------------------------------------------------------- */

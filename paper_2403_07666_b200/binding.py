@@ -42,7 +42,7 @@ class QsStats(C.Structure):
     _fields_ = [("cg_iters", C.c_int32), ("heat_substeps", C.c_int32), ("event_word", C.c_int32),
                 ("sweeps", C.c_int32), ("cg_relres", C.c_double), ("U_terminal", C.c_double),
                 ("Tmax", C.c_double), ("joule_power", C.c_double), ("t", C.c_double), ("I", C.c_double),
-                ("launches", C.c_int64), ("pair_evals", C.c_int64)]
+                ("launches", C.c_int64), ("pair_evals", C.c_int64), ("dJ_max", C.c_double)]
 
 
 class QsProfile(C.Structure):

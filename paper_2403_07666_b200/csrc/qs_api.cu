@@ -941,7 +941,7 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
   ev.dt = dt; ev.t_new = c->t + dt; ev.have_prev = c->have_prev_E;
   c->prof.begin(c->stream);
   k_events(v, c->mp, ev);
-  k_step_stats(v, c->mp, c->J, c->H, c->Q, c->r, c->area);
+  k_step_stats(v, c->mp, c->J, c->Jold, c->H, c->Q, c->r, c->area);
   c->prof.end(c->stream, QS_PROF_EVENTS, c->n_turns ? 2 : 1);
   if ((rc = sync_scalars(c)) != QS_OK) return rc;
   if (c->h_sc->nonfinite) {
@@ -961,6 +961,7 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
   c->st.U_terminal = c->h_sc->uterm;
   c->st.Tmax = c->h_sc->tmax;
   c->st.joule_power = c->h_sc->joule;
+  c->st.dJ_max = c->h_sc->djmax;
   c->st.t = c->t;
   c->st.I = c->I;
   return ret;

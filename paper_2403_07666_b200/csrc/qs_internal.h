@@ -63,6 +63,7 @@ struct Scalars {
   double nu2;            // reference norm squared
   double uterm;          // sum_w vsum_w = terminal voltage
   double tmax, joule;    // step statistics
+  double djmax;          // max |J_new - J_old| of the step
   double thresh2;        // (cg_tol * nu)^2: the fused CG iterations stop themselves when rg <= thresh2
   int nonfinite;         // set when J or T is NaN/Inf
   int event_or;          // OR of per-turn return bits
@@ -206,7 +207,7 @@ struct EventArgs {
   bool have_prev;
 };
 void k_events(const VecCtx& v, const MaterialParams& mp, const EventArgs& e);
-void k_step_stats(const VecCtx& v, const MaterialParams& mp, const double* J, const double* H, const double* Q,
-                  const double* r, const double* area);
+void k_step_stats(const VecCtx& v, const MaterialParams& mp, const double* J, const double* Jold, const double* H,
+                  const double* Q, const double* r, const double* area);
 
 }  // namespace qs

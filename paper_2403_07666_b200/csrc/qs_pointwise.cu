@@ -630,21 +630,25 @@ __global__ void events_kernel(int n_turns, const int* __restrict__ ptr, const in
   e.ebar_prev[w] = ebar;
 }
 
-__global__ void stats_kernel(int n, double C3, double C1, const double* __restrict__ J, const double* __restrict__ H,
+__global__ void stats_kernel(int n, double C3, double C1, const double* __restrict__ J,
+                             const double* __restrict__ Jold, const double* __restrict__ H,
                              const double* __restrict__ Q, const double* __restrict__ r,
                              const double* __restrict__ area, Scalars* sc) {
-  double tsq = 0.0, joule = 0.0;
+  double tsq = 0.0, joule = 0.0, dj = 0.0;
   int bad = 0;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     const double t2 = tsq_of_H(H[i], C3, C1);
+    dj = fmax(dj, fabs(J[i] - Jold[i]));
     if (!isfinite(J[i]) || !isfinite(t2) || !(t2 > 0.0)) bad = 1;
     tsq = fmax(tsq, t2);
     joule = fma(Q[i], 2.0 * kPi * r[i] * area[i], joule);
   }
   tsq = warp_max(tsq);
   joule = warp_sum(joule);
+  dj = warp_max(dj);
   bad = __any_sync(0xffffffffu, bad);
   if ((threadIdx.x & 31) == 0) {
+    if (dj > 0.0 && isfinite(dj)) atomic_max_pos(&sc->djmax, dj);
     if (tsq > 0.0 && isfinite(tsq)) atomic_max_pos(&sc->tmax, sqrt(tsq));
     atomicAdd(&sc->joule, joule);
     if (bad) atomicOr(&sc->nonfinite, 1);
@@ -742,10 +746,10 @@ void k_events(const VecCtx& v, const MaterialParams& mp, const EventArgs& e) {
   events_kernel<<<(v.n_turns * 32 + kBlock - 1) / kBlock, kBlock, 0, v.stream>>>(v.n_turns, v.turn_ptr, v.turn_idx, mp,
                                                                                 e, v.sc);
 }
-void k_step_stats(const VecCtx& v, const MaterialParams& mp, const double* J, const double* H, const double* Q,
-                  const double* r, const double* area) {
+void k_step_stats(const VecCtx& v, const MaterialParams& mp, const double* J, const double* Jold, const double* H,
+                  const double* Q, const double* r, const double* area) {
   QS_LAUNCH(v);
-  stats_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, mp.C3, mp.C1, J, H, Q, r, area, v.sc);
+  stats_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, mp.C3, mp.C1, J, Jold, H, Q, r, area, v.sc);
 }
 
 }  // namespace qs

@@ -177,6 +177,7 @@ __global__ void set_scalars_kernel(Scalars* sc) {
   sc->thresh2 = 0.0;
   sc->uterm = sc->joule = 0.0;
   sc->tmax = 0.0;
+  sc->djmax = 0.0;
   sc->nonfinite = 0;
   sc->event_or = 0;
 }

@@ -225,3 +225,50 @@ def test_explicit_theta0_steps(pkg):
                 assert orc.step(w.dt, w.I_ramp) == (sim.step(w.dt, w.I_ramp) & 3)
             got, ref = sim.read(), orc.read()
         check_state(ref, got)
+
+
+@pytest.mark.parametrize("scenario", ["quench", "ramp"])
+def test_adaptive_dt_controller(pkg, scenario):
+    # configs[3] "adaptive dt in [1e-6, 1e-4] s with event detection" (C11).  The product's controller drives the GPU,
+    # the rule restated here drives the oracle from the oracle's own max |dJ|; the two dt sequences must coincide and
+    # the states agree.  "quench": shrunk coil with a prepared normal turn (events pin dt at dt_min);
+    # "ramp": single wire under a fast background ramp (no event: dt halves while the screening currents build up)
+    from paper_2403_07666_b200.controller import run_adaptive
+    if scenario == "quench":
+        w = wl.shrunk(3, 2, 3)
+        geo = w.geometry
+    else:
+        w = wl.shrunk(1, 1, 1, 12)
+        geo = dataclasses.replace(w.geometry, Bext_rate=400.0)
+    mat = dataclasses.replace(w.material, cg_tol=1e-12)
+    N = geo.n_rings
+    Jref = mat.Jc0 * (1 - geo.T_bath / mat.Tc) ** 2
+    J0 = np.full(N, 0.85 * Jref) if scenario == "quench" else np.zeros(N)
+    T0 = np.full(N, geo.T_bath)
+    if scenario == "quench":
+        T0[geo.turn_id == 2] = 19.0
+    steps = 40
+    orc = qo.Oracle(geo, mat)
+    orc.write(J0, T0, 0.0, 0.0)
+    dt, held, dts_ref = 1e-4, 0, []
+    for _ in range(steps):
+        Jb = orc.J.copy()
+        ret = orc.step(dt, w.I_ramp)
+        dts_ref.append(dt)
+        s = np.max(np.abs(orc.J - Jb)) / Jref
+        if ret & 3:
+            held = 10
+        if held > 0:
+            held -= 1
+            dt = 1e-6
+        elif s > 0.02:
+            dt = max(dt / 2, 1e-6)
+        elif s < 0.005:
+            dt = min(2 * dt, 1e-4)
+    with pkg.QS(geo, mat) as sim:
+        sim.write(J0, T0, 0.0, 0.0)
+        dts = run_adaptive(sim, geo, mat, w.I_ramp, steps)
+        got = sim.read()
+    assert dts == dts_ref, (dts, dts_ref)
+    assert len(set(dts)) >= 2, dts
+    check_state(orc.read(), got)

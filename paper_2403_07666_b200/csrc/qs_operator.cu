@@ -44,23 +44,41 @@ struct Accum {
 };
 
 // ---- one off-diagonal item: all 32 x 32 pairs, both directions -----------------------------------
-template <int NIT, bool HI, bool FIELD>
+// UNI: every ring of the source block has the same radius rju and so has the target block (blocks of a lattice row,
+// the common case on winding packs whose Nz is a multiple of 32): (ri - rj)^2, 4 ri rj and rj^2 - ri^2 are item
+// constants, the source radii are not read.
+template <int NIT, bool HI, bool FIELD, bool UNI>
 __device__ __forceinline__ void item_offdiag(const TargetRegs& t, const double* __restrict__ sr,
                                              const double* __restrict__ sz, const double* __restrict__ sx,
-                                             const double* __restrict__ sc, double soft_all, int lane, Accum& acc,
-                                             Accum& trav) {
+                                             const double* __restrict__ sc, double soft_all, double rju, int lane,
+                                             Accum& acc, Accum& trav) {
   const unsigned full = 0xffffffffu;
   const int next = (lane + 1) & 31;
   const double ri2 = t.r * t.r, ri4 = 4.0 * t.r;
+  const double difu = t.r - rju, dif2u = difu * difu, c4u = ri4 * rju, eu = fma(rju, rju, -ri2);
+  const double dif2s = dif2u + soft_all;
   sr += lane, sz += lane, sx += lane, sc += lane;   // arrays are stored twice: entry lane + s = source (lane + s) & 31
 #pragma unroll 2
   for (int s = 0; s < 32; ++s) {
     const int jl = s;
-    const double rj = sr[jl], zj = sz[jl], xj = sx[jl];
+    const double zj = sz[jl], xj = sx[jl];
     const double dz = t.z - zj;
-    const double dz2 = fma(dz, dz, soft_all);
-    const double dif = t.r - rj;
-    const double B2 = fma(dif, dif, dz2), A2 = fma(ri4, rj, B2);   // (ri+rj)^2 = (ri-rj)^2 + 4 ri rj
+    double dz2 = 0.0, A2, B2, rj = rju;
+    if (UNI) {
+      if (FIELD) {
+        dz2 = fma(dz, dz, soft_all);
+        B2 = dz2 + dif2u;
+      } else {
+        B2 = fma(dz, dz, dif2s);
+      }
+      A2 = B2 + c4u;
+    } else {
+      rj = sr[jl];
+      dz2 = fma(dz, dz, soft_all);
+      const double dif = t.r - rj;
+      B2 = fma(dif, dif, dz2);
+      A2 = fma(ri4, rj, B2);                               // (ri+rj)^2 = (ri-rj)^2 + 4 ri rj
+    }
     const PairAGM a = agm_pair<NIT, HI, FIELD>(A2, B2);
     const double mt = a.S * a.yinf;
     acc.y = fma(mt, xj, acc.y);
@@ -68,7 +86,7 @@ __device__ __forceinline__ void item_offdiag(const TargetRegs& t, const double* 
     if (FIELD) {
       const double cj = sc[jl];
       const double qt = a.yinf * (a.mid - a.S) * a.y0sq;
-      const double e = fma(rj, rj, -ri2);                  // rj^2 - ri^2
+      const double e = UNI ? eu : fma(rj, rj, -ri2);       // rj^2 - ri^2
       const double bz_ij = fma(e - dz2, qt, a.yinf);       // Kt + (rj^2 - ri^2 - dz^2) Qt
       const double bz_ji = fma(-e - dz2, qt, a.yinf);
       const double ur = dz * fma(a.mid, qt, -a.yinf);      // dz (-Kt + (ri^2 + rj^2 + dz^2) Qt)
@@ -209,7 +227,9 @@ __global__ void __launch_bounds__(kThreads, FIELD ? 2 : 3) sweep_kernel(SweepPar
       }
       if (it + 1 < cnt) issue(buf ^ 1, nbj);
 
-      const int nit = classify(bbi, prm.bbox[bj], bi == bj, prm);
+      const double4 bbj = prm.bbox[bj];
+      const bool uni = bbi.x == bbi.y && bbj.x == bbj.y;   // both blocks on one radius each (lattice rows)
+      const int nit = classify(bbi, bbj, bi == bj, prm);
       mbar_wait(&sbar[warp][buf], (phase >> buf) & 1u);
       phase ^= 1u << buf;
       const double* sr = sbuf[warp][buf][0];
@@ -229,7 +249,12 @@ __global__ void __launch_bounds__(kThreads, FIELD ? 2 : 3) sweep_kernel(SweepPar
 #undef QS_DIAG
       } else {
         Accum trav = {0.0, 0.0, 0.0};
-#define QS_OFF(N_, HI_) item_offdiag<N_, HI_, FIELD>(t, sr, sz, sx, sc, prm.soft_all, lane, acc, trav); break
+#define QS_OFF(N_, HI_)                                                                              \
+  if (uni)                                                                                           \
+    item_offdiag<N_, HI_, FIELD, true>(t, sr, sz, sx, sc, prm.soft_all, bbj.x, lane, acc, trav);     \
+  else                                                                                               \
+    item_offdiag<N_, HI_, FIELD, false>(t, sr, sz, sx, sc, prm.soft_all, 0.0, lane, acc, trav);      \
+  break
         switch (nit) {
           case 0: QS_OFF(2, false);
           case 1: QS_OFF(2, true);

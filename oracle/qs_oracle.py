@@ -559,6 +559,72 @@ class Oracle:
             return -3
         return ret
 
+    # -- embedded Heun-Euler step with error control ("Runge-Kutta method with
+    #    variable time step") ---------------------------------------------------------------------------------------
+    def _em_rate(self, J, T, t_stage, Bdot, I_ramp):
+        """I' of the circuit equations with everything evaluated at the given state (explicit stage, no theta term):
+        M I' + C V = b(E(J, T, B(J) + B_ext(t_stage))), C^T I' = I_ramp.  Returns (I', V, Br, Bz, material dict)."""
+        geo, mat = self.geo, self.mat
+        Br, Bz = self.field(geo.area * J)
+        Bz = Bz + self.Bext(t_stage)
+        ml = material_law(mat, J, T, Br, Bz, geo.r, self.scale)
+        b = -2.0 * math.pi * geo.r * (ml["E"] + 0.5 * geo.r * Bdot)
+        d = np.full(geo.n_turns, float(I_ramp))
+        if self.solver == "cholesky":
+            if getattr(self, "_cfM", None) is None:
+                self._cfM = scipy.linalg.cho_factor(self.M, lower=True)       # M is constant: factor once
+                self._AinvC = scipy.linalg.cho_solve(self._cfM, self.C) if geo.n_turns else None
+                self._S = self.C.T @ self._AinvC if geo.n_turns else None
+            Ainv_b = scipy.linalg.cho_solve(self._cfM, b)
+            if geo.n_turns:
+                V = np.linalg.solve(self._S, self.C.T @ Ainv_b - d)
+                return Ainv_b - self._AinvC @ V, V, Br, Bz, ml
+            return Ainv_b, np.zeros(0), Br, Bz, ml
+        Idot, V, _, _ = pcg(self.apply_M, self.diagM, geo.turn_id, geo.n_turns, b, d, mat.cg_tol, mat.cg_maxit, self.Idot)
+        return Idot, V, Br, Bz, ml
+
+    def step_rk(self, dt_try, I_ramp, rtol, dt_min):
+        """One ACCEPTED embedded Heun-Euler (RK12) step of the electromagnetic equations with T frozen at T^k, then the
+        heat step (readings: DESIGN.md §3 "C14").  Returns (event word, dt_taken, dt_next, err).
+
+        stage 1: I'_1 at (J^k, t^k);  predictor J* = J^k + dt I'_1/a;  stage 2: I'_2 at (J*, t^k + dt)
+        J^{k+1} = J^k + dt (I'_1 + I'_2) / (2a);   err = max_i |dt (I'_2 - I'_1)_i / (2 a_i)| / J_ref,
+        J_ref = Jc0 (1 - T_bath/Tc)^2.   Accept if err <= rtol or dt == dt_min; else retry with
+        dt <- max(dt_min, dt max(0.2, 0.9 sqrt(rtol/err))).   dt_next = dt min(2, max(0.2, 0.9 sqrt(rtol/err))).
+        Heat source: the trapezoid (Q_1 + Q_2)/2; B, E, events: those of stage 2.
+        """
+        geo, mat = self.geo, self.mat
+        a = geo.area
+        Jref = mat.Jc0 * (1.0 - geo.T_bath / mat.Tc) ** 2
+        dt = float(dt_try)
+        while True:
+            Bdot = (self.Bext(self.t + dt) - self.Bext(self.t)) / dt
+            I1, V1, _, _, ml1 = self._em_rate(self.J, self.T, self.t, Bdot, I_ramp)
+            Jstar = self.J + dt * I1 / a
+            I2, V2, Br2, Bz2, ml2 = self._em_rate(Jstar, self.T, self.t + dt, Bdot, I_ramp)
+            err = float(np.max(np.abs(0.5 * dt * (I2 - I1) / a))) / Jref
+            fac = 2.0 if err == 0.0 else min(2.0, max(0.2, 0.9 * math.sqrt(rtol / err)))
+            if err <= rtol or dt <= dt_min:
+                break
+            dt = max(dt_min, dt * fac)
+        Jold = self.J
+        self.J = self.J + 0.5 * dt * (I1 + I2) / a
+        self.Idot = I2
+        self.I += dt * I_ramp
+        self.t += dt
+        Q = 0.5 * (ml1["Q"] + ml2["Q"])
+        m = heat_substeps_count(geo, mat, dt)
+        self.H, lost = heat_substeps(geo, mat, self.H, Q, dt, m)
+        self.T = temperature(mat, self.H)
+        self.Br, self.Bz, self.E = Br2, Bz2, ml2["E"]
+        ml_ev = dict(ml2)
+        ml_ev["Q"] = Q
+        ret = self._events(dt, Jstar, ml_ev) if geo.n_turns else 0
+        self.stats = dict(cg_iters=0, cg_relres=0.0, U_terminal=float(-0.5 * (V1.sum() + V2.sum())),
+                          Tmax=float(self.T.max()), joule_power=float(np.sum(Q * 2.0 * math.pi * geo.r * a)),
+                          boundary_energy=lost, heat_substeps=m)
+        return int(ret), dt, dt * fac, err
+
     def _events(self, dt, Jold, ml):
         geo, mat = self.geo, self.mat
         Tmax, Ebar, xmax, rmin = turn_observables(geo, mat, self.T, ml["E"], Jold, ml["Jc"], ml["rho"])

@@ -230,3 +230,66 @@ def test_wire_statistics_closed_forms_and_energy_identity():
     assert abs(wr["Q_q"][5] - dt * P * V5) <= 1e-12 * dt * P * V5               # frozen at the quench time
     o.write(J0, T0, 0.0, 0.0)
     assert np.all(o.wire["E_joule"] == 0) and np.all(o.wire["t_q"] == -1.0)
+
+
+def _lr_ring():
+    base = wl.lattice_geometry(1, 1, 1, 1e-3, 30e-3, h_conv=0.0, Bext_rate=10.0, Bext_max=100.0)
+    geo = dataclasses.replace(base, n_turns=0, turn_id=None)
+    mat = wl.Material()
+    r, a = geo.r[0], geo.area[0]
+    L = qo.mutual_pair(r, 0.0, r, 0.0, soft2=geo.softening ** 2)    # C2 self term (pinned against the thin-ring form)
+    R = mat.rho_n * 2 * math.pi * r / a
+    return geo, mat, a, float(L) / R, -math.pi * r * r * 10.0 / R
+
+
+def test_heun_euler_step_is_second_order_on_the_LR_circuit():
+    # f2 (PAPER.md:73 Runge-Kutta with variable step): on the linear L-R ring the Heun result is the exact
+    # second-order Taylor polynomial, I_{k+1} = I_k + (I_inf - I_k)(x - x^2/2), x = dt/tau, and the embedded error
+    # estimate is |I_inf - I_k| x^2 / 2 in current
+    geo, mat, a, tau, I_inf = _lr_ring()
+    o = qo.Oracle(geo, mat)
+    o.write(np.zeros(1), np.full(1, 20.0), 0.0, 0.0)
+    dt = 0.05 * tau
+    ret, taken, nxt, err = o.step_rk(dt, 0.0, rtol=1.0, dt_min=1e-12)
+    x = dt / tau
+    assert taken == dt and abs(o.J[0] * a - I_inf * (x - x * x / 2)) <= 1e-12 * abs(I_inf)
+    Jref = mat.Jc0 * (1 - geo.T_bath / mat.Tc) ** 2
+    assert abs(err - abs(I_inf) * x * x / 2 / a / Jref) <= 1e-10 * err
+    errs = []
+    for steps in (100, 200):                                    # global error ~ dt^2
+        o = qo.Oracle(geo, mat)
+        o.write(np.zeros(1), np.full(1, 20.0), 0.0, 0.0)
+        for _ in range(steps):
+            o.step_rk(2.0 * tau / steps, 0.0, rtol=1.0, dt_min=1e-12)
+        exact = I_inf * (1 - math.exp(-o.t / tau))
+        errs.append(abs(o.J[0] * a - exact) / abs(exact))
+    assert errs[1] < 1e-4 and 3.6 < errs[0] / errs[1] < 4.4
+
+
+def test_heun_euler_step_control_rejects_and_rescales():
+    geo, mat, a, tau, I_inf = _lr_ring()
+    Jref = mat.Jc0 * (1 - geo.T_bath / mat.Tc) ** 2
+    o = qo.Oracle(geo, mat)
+    o.write(np.zeros(1), np.full(1, 20.0), 0.0, 0.0)
+    rtol = abs(I_inf) * 0.01 ** 2 / 2 / a / Jref              # the error of a step of 0.01 tau
+    ret, taken, nxt, err = o.step_rk(0.5 * tau, 0.0, rtol=rtol, dt_min=1e-3 * tau)
+    assert taken < 0.5 * tau and err <= rtol and taken <= 0.0101 * tau      # rejected down to the tolerance
+    assert abs(nxt / taken - min(2.0, max(0.2, 0.9 * math.sqrt(rtol / err)))) < 1e-12
+    o2 = qo.Oracle(geo, mat)
+    o2.write(np.zeros(1), np.full(1, 20.0), 0.0, 0.0)
+    ret, taken2, _, err2 = o2.step_rk(0.5 * tau, 0.0, rtol=rtol, dt_min=0.2 * tau)
+    assert taken2 == 0.2 * tau and err2 > rtol                # accepted at dt_min regardless
+
+
+def test_heun_euler_equals_explicit_euler_when_the_rate_is_constant():
+    # linear regime (E ~ 0): I' is the same at both stages, the error estimate vanishes, and the step equals the
+    # theta = 0 step of C7
+    w = wl.shrunk(0, 2, 2, 4)
+    mat0 = dataclasses.replace(w.material, theta=0.0)
+    a_, b_ = qo.Oracle(w.geometry, mat0), qo.Oracle(w.geometry, mat0)
+    for _ in range(5):
+        a_.step(w.dt, w.I_ramp)
+        ret, taken, nxt, err = b_.step_rk(w.dt, w.I_ramp, rtol=1e-6, dt_min=1e-9)
+        assert taken == w.dt and err <= 1e-12 and nxt == 2 * w.dt
+    assert np.max(np.abs(a_.J - b_.J)) <= 1e-12 * np.max(np.abs(a_.J))
+    assert abs(a_.stats["U_terminal"] - b_.stats["U_terminal"]) <= 1e-9 * abs(a_.stats["U_terminal"])

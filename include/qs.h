@@ -127,6 +127,19 @@ int  qs_init(const qs_geometry *geo, const qs_material *mat, qs_ctx **out);
  * I_ramp = dI/dt [A/s] held over the step.  Lattice geometries only.  Synchronous.  */
 int  qs_step(qs_ctx *ctx, double dt, double I_ramp);
 
+/* One ACCEPTED step of the embedded Heun-Euler (RK12) pair with step-size control (the paper
+ * integrates the electromagnetic equations by a "Runge-Kutta method with variable time step"; readings
+ * C14 in DESIGN.md §3).  With T frozen at T^k:
+ *   stage 1: I'_1 from M I' + C V = b(J^k, t^k), C^T I' = I_ramp;  predictor J* = J^k + dt I'_1 / a
+ *   stage 2: I'_2 at (J*, t^k + dt);  J^{k+1} = J^k + dt (I'_1 + I'_2) / (2a)
+ *   err = max_i |dt (I'_2 - I'_1)_i / (2 a_i)| / (Jc0 (1 - T_bath/Tc)^2)
+ * The step is accepted if err <= rtol or dt == dt_min, else retried with dt <- max(dt_min, dt max(0.2, 0.9
+ * sqrt(rtol/err))).  Then the heat step with the trapezoid source (Q_1 + Q_2)/2 and the events; qs_read's B, E are
+ * those of stage 2.  Outputs (may be NULL): the dt taken, the suggestion dt min(2, max(0.2, 0.9 sqrt(rtol/err))) for
+ * the next call, and err.  Returns like qs_step.  */
+int  qs_step_rk(qs_ctx *ctx, double dt_try, double I_ramp, double rtol, double dt_min,
+                double *dt_taken, double *dt_next, double *err);
+
 /* Copy out J [N], T [N], B [2N: Br then Bz], E [N]; NULL = skip.  J, T are the state after the
  * last step; B, E are those of the last step's material evaluation (time level k).  */
 int  qs_read(qs_ctx *ctx, double *J, double *T, double *B, double *E);

@@ -56,6 +56,7 @@ _VP = C.c_void_p
 SYMBOLS = [
     ("qs_init", C.c_int, [C.POINTER(QsGeometry), C.POINTER(QsMaterial), C.POINTER(_VP)]),
     ("qs_step", C.c_int, [_VP, C.c_double, C.c_double]),
+    ("qs_step_rk", C.c_int, [_VP, C.c_double, C.c_double, C.c_double, C.c_double, c_double_p, c_double_p, c_double_p]),
     ("qs_read", C.c_int, [_VP, c_double_p, c_double_p, c_double_p, c_double_p]),
     ("qs_workspace_bytes", C.c_size_t, [C.POINTER(QsGeometry)]),
     ("qs_init_device", C.c_int, [C.POINTER(QsGeometry), C.POINTER(QsMaterial), _VP, C.c_size_t, _VP, C.POINTER(_VP)]),
@@ -241,6 +242,13 @@ class QS:
     # ---- the three calls -------------------------------------------------------------------------
     def step(self, dt: float, I_ramp: float) -> int:
         return self._check(self._lib.qs_step(self._h, float(dt), float(I_ramp)))
+
+    def step_rk(self, dt_try: float, I_ramp: float, rtol: float, dt_min: float):
+        """Embedded Heun-Euler step with error control: returns (event word, dt taken, dt suggested next, err)."""
+        taken, nxt, err = C.c_double(0.0), C.c_double(0.0), C.c_double(0.0)
+        rc = self._check(self._lib.qs_step_rk(self._h, float(dt_try), float(I_ramp), float(rtol), float(dt_min),
+                                               C.byref(taken), C.byref(nxt), C.byref(err)))
+        return rc, taken.value, nxt.value, err.value
 
     def read(self, J=True, T=True, B=True, E=True, out=None):
         """Returns (J, T, B, E) as numpy arrays (B = [Br, Bz] concatenated); skipped entries are None.

@@ -487,11 +487,12 @@ int reset_event_bits(qs_ctx* c) {
   return QS_OK;
 }
 
-MaterialArgs material_args(qs_ctx* c, double Bext, double Bdot, double dt, bool from_acc, bool aux) {
+MaterialArgs material_args(qs_ctx* c, double Bext, double Bdot, double dt, bool from_acc, bool aux,
+                           const double* Jsrc = nullptr) {
   MaterialArgs a;
   a.N = c->N;
   a.Nz = c->lattice ? c->lp.Nz : 0;
-  a.J = c->J;
+  a.J = Jsrc ? Jsrc : c->J;
   a.H = c->H;
   a.jc0_scale = c->jc0s;
   a.bracc = c->bracc;
@@ -522,6 +523,59 @@ MaterialArgs material_args(qs_ctx* c, double Bext, double Bdot, double dt, bool 
   a.inv_area = c->lattice ? 1.0 / (c->lp.h * c->lp.h) : 0.0;
   a.from_acc = from_acc;
   return a;
+}
+
+// One electromagnetic stage (S1..S4) at the state Jsrc: field sweep fused with M x0, material law (diagonal shift
+// theta dt_shift D), projected CG for I' (left in c->x, warm-started from its previous content), multipliers -> uterm.
+int em_stage(qs_ctx* c, const double* Jsrc, double Bext, double Bdot, double dt_shift, double I_ramp, int* iters,
+             double* relres, bool* hit_max) {
+  const VecCtx& v = c->v;
+  const size_t nb8 = sizeof(double) * c->N;
+  int rc;
+  *iters = 0;
+  *relres = 0.0;
+  *hit_max = false;
+  // warm start I'_prev moved onto the constraint C^T x = I_ramp with the static diagonal of M
+  k_turn_deficit(v, c->x, I_ramp, c->defw);
+  k_apply_deficit(v, c->defw, c->diagM, c->swM, c->x);
+  // S1 (+ M x0 in the same sweep): ring currents I = a J
+  k_mul(v, c->area, Jsrc, c->cur);
+  if ((rc = do_sweep(c, c->x, c->cur, true)) != QS_OK) return rc;
+  // S2
+  if ((rc = reset_event_bits(c)) != QS_OK) return rc;
+  c->prof.begin(c->stream);
+  k_material(v, c->mp, material_args(c, Bext, Bdot, dt_shift, true, false, Jsrc));
+  c->prof.end(c->stream, QS_PROF_MATERIAL, 1);
+  // S3/S4: the right-hand side b = -2 pi r (E + r Bdot / 2) is evaluated on the fly from E (C4)
+  const Rhs rhs{nullptr, c->E, c->r, Bdot};
+  double nu = -1.0;
+  if (c->n_turns) {
+    k_turn_schur(v, c->Hd, c->sw);
+    k_nu_residual(v, I_ramp, c->Mxp1, c->shift, c->xp1, rhs, c->rr);
+    k_turn_project(v, c->rr, c->Hd, c->sw, c->vw, nullptr);
+    k_project_apply(v, 0, c->vw, c->Hd, c->rr, c->g);
+    k_copy_rg_to_nu2(v, 0);
+  } else {  // no constraint: nu^2 = b^T H^-1 b
+    k_rhs_fill(v, rhs, c->rr);
+    k_project_apply(v, 0, nullptr, c->Hd, c->rr, c->g);
+    k_copy_rg_to_nu2(v, 0);
+  }
+  if ((rc = sync_scalars(c)) != QS_OK) return rc;
+  nu = std::sqrt(std::max(c->h_sc->nu2, 0.0));
+  if (nu > 0.0) {
+    rc = cg_core(c, rhs, c->x, c->shift, c->Hd, c->sw, true, c->cg_tol, c->cg_maxit, nu, iters, relres, hit_max);
+    if (rc != QS_OK) return rc;
+  } else {
+    // nu == 0: the cold start x_p = I_ramp xp1 already solves the projected system (e.g. one cell per turn, where the
+    // constraint alone fixes I'; or b = 0 with no ramp, where x_p = 0); its projection multipliers are the V_w (C8)
+    QS_CUDA(cudaMemsetAsync(c->x, 0, nb8, c->stream));
+    if (c->n_turns) {
+      k_axpy(v, I_ramp, c->xp1, c->x);
+      QS_CUDA(cudaMemcpyAsync(c->vsum, c->vw, sizeof(double) * c->n_turns, cudaMemcpyDeviceToDevice, c->stream));
+    }
+  }
+  k_sum_uterm(v, c->vsum);
+  return QS_OK;
 }
 
 // host arrays in caller order <-> device arrays in internal order
@@ -877,34 +931,6 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
   QS_CUDA(cudaMemcpyAsync(c->Hold, c->H, nb8, cudaMemcpyDeviceToDevice, c->stream));
   QS_CUDA(cudaMemcpyAsync(c->xold, c->x, nb8, cudaMemcpyDeviceToDevice, c->stream));
   k_set_scalars(v);
-  // warm start I'_prev moved onto the constraint C^T x = I_ramp with the static diagonal of M
-  k_turn_deficit(v, c->x, I_ramp, c->defw);
-  k_apply_deficit(v, c->defw, c->diagM, c->swM, c->x);
-  // S1 (+ M x0 in the same sweep): ring currents I = a J
-  k_mul(v, c->area, c->J, c->cur);
-  if ((rc = do_sweep(c, c->x, c->cur, true)) != QS_OK) return rc;
-  // S2
-  const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
-  if ((rc = reset_event_bits(c)) != QS_OK) return rc;
-  c->prof.begin(c->stream);
-  k_material(v, c->mp, material_args(c, B0, (B1 - B0) / dt, dt, true, false));
-  c->prof.end(c->stream, QS_PROF_MATERIAL, 1);
-  // S3/S4: the right-hand side b = -2 pi r (E + r Bdot / 2) is evaluated on the fly from E (C4)
-  const Rhs rhs{nullptr, c->E, c->r, (B1 - B0) / dt};
-  double nu = -1.0;
-  if (c->n_turns) {
-    k_turn_schur(v, c->Hd, c->sw);
-    k_nu_residual(v, I_ramp, c->Mxp1, c->shift, c->xp1, rhs, c->rr);
-    k_turn_project(v, c->rr, c->Hd, c->sw, c->vw, nullptr);
-    k_project_apply(v, 0, c->vw, c->Hd, c->rr, c->g);
-    k_copy_rg_to_nu2(v, 0);
-  } else {  // no constraint: nu^2 = b^T H^-1 b
-    k_rhs_fill(v, rhs, c->rr);
-    k_project_apply(v, 0, nullptr, c->Hd, c->rr, c->g);
-    k_copy_rg_to_nu2(v, 0);
-  }
-  if ((rc = sync_scalars(c)) != QS_OK) return rc;
-  nu = std::sqrt(std::max(c->h_sc->nu2, 0.0));
   int iters = 0;
   double relres = 0.0;
   bool hit_max = false;
@@ -912,22 +938,11 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
     cudaMemcpyAsync(c->x, c->xold, nb8, cudaMemcpyDeviceToDevice, c->stream);
     cudaStreamSynchronize(c->stream);
   };
-  if (nu > 0.0) {
-    rc = cg_core(c, rhs, c->x, c->shift, c->Hd, c->sw, true, c->cg_tol, c->cg_maxit, nu, &iters, &relres, &hit_max);
-    if (rc != QS_OK) {
-      restore();
-      return rc;
-    }
-  } else {
-    // nu == 0: the cold start x_p = I_ramp xp1 already solves the projected system (e.g. one cell per turn, where the
-    // constraint alone fixes I'; or b = 0 with no ramp, where x_p = 0); its projection multipliers are the V_w (C8)
-    QS_CUDA(cudaMemsetAsync(c->x, 0, nb8, c->stream));
-    if (c->n_turns) {
-      k_axpy(v, I_ramp, c->xp1, c->x);
-      QS_CUDA(cudaMemcpyAsync(c->vsum, c->vw, sizeof(double) * c->n_turns, cudaMemcpyDeviceToDevice, c->stream));
-    }
+  const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
+  if ((rc = em_stage(c, c->J, B0, (B1 - B0) / dt, dt, I_ramp, &iters, &relres, &hit_max)) != QS_OK) {
+    restore();
+    return rc;
   }
-  k_sum_uterm(v, c->vsum);
   // S5
   k_scale_div(v, dt, c->x, c->area, c->J);
   // S6
@@ -964,6 +979,100 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
   c->st.dJ_max = c->h_sc->djmax;
   c->st.t = c->t;
   c->st.I = c->I;
+  return ret;
+}
+
+// Embedded Heun-Euler step with error control (readings: DESIGN.md §3 C14).
+int qs_step_rk(qs_ctx* c, double dt_try, double I_ramp, double rtol, double dt_min, double* dt_taken, double* dt_next,
+               double* err_out) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  if (!c->lattice || !c->has_operator) return fail(QS_ERR_ARG, "qs_step_rk needs a lattice geometry with the operator set up");
+  if (!(dt_try > 0.0) || !(dt_min > 0.0) || !(rtol > 0.0)) return fail(QS_ERR_DT, "dt_try, dt_min and rtol must be > 0");
+  const VecCtx& v = c->v;
+  const int N = c->N;
+  const size_t nb8 = sizeof(double) * N;
+  int rc;
+  c->st.sweeps = 0;
+  QS_CUDA(cudaMemcpyAsync(c->Jold, c->J, nb8, cudaMemcpyDeviceToDevice, c->stream));
+  QS_CUDA(cudaMemcpyAsync(c->Hold, c->H, nb8, cudaMemcpyDeviceToDevice, c->stream));
+  QS_CUDA(cudaMemcpyAsync(c->xold, c->x, nb8, cudaMemcpyDeviceToDevice, c->stream));
+  auto restore = [&]() {
+    cudaMemcpyAsync(c->x, c->xold, nb8, cudaMemcpyDeviceToDevice, c->stream);
+    cudaStreamSynchronize(c->stream);
+  };
+  const double Jref = c->mp.Jc0 * (1.0 - c->lp.T_bath / c->mp.Tc) * (1.0 - c->lp.T_bath / c->mp.Tc);
+  double dt = dt_try, err = 0.0, fac = 2.0, uterm = 0.0;
+  int iters = 0, it1 = 0, it2 = 0;
+  double rel1 = 0.0, rel2 = 0.0;
+  bool hm1 = false, hm2 = false;
+  double* I1 = c->tmp2;     // I' of stage 1
+  double* Jstar = c->tmp;   // predictor J^k + dt I'_1 / a
+  double* Q1 = c->b;        // Joule source of stage 1 (the explicit-rhs array is used by qs_solve only)
+  for (;;) {
+    k_set_scalars(v);
+    const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt), Bdot = (B1 - B0) / dt;
+    // stage 1 at (J^k, t^k): explicit stage, no theta term (dt_shift = 0)
+    if ((rc = em_stage(c, c->J, B0, Bdot, 0.0, I_ramp, &it1, &rel1, &hm1)) != QS_OK) {
+      restore();
+      return rc;
+    }
+    QS_CUDA(cudaMemcpyAsync(I1, c->x, nb8, cudaMemcpyDeviceToDevice, c->stream));
+    QS_CUDA(cudaMemcpyAsync(Q1, c->Q, nb8, cudaMemcpyDeviceToDevice, c->stream));
+    QS_CUDA(cudaMemcpyAsync(Jstar, c->J, nb8, cudaMemcpyDeviceToDevice, c->stream));
+    k_scale_div(v, dt, I1, c->area, Jstar);
+    // stage 2 at (J*, t^k + dt), warm-started from I'_1
+    if ((rc = em_stage(c, Jstar, B1, Bdot, 0.0, I_ramp, &it2, &rel2, &hm2)) != QS_OK) {
+      restore();
+      return rc;
+    }
+    k_max_scaled_diff(v, 0.5 * dt, c->x, I1, c->area);
+    if ((rc = sync_scalars(c)) != QS_OK) return rc;
+    err = c->h_sc->djmax / Jref;
+    uterm = 0.5 * c->h_sc->uterm;
+    iters += it1 + it2;
+    fac = err == 0.0 ? 2.0 : std::min(2.0, std::max(0.2, 0.9 * std::sqrt(rtol / err)));
+    if (err <= rtol || dt <= dt_min) break;
+    dt = std::max(dt_min, dt * fac);
+    QS_CUDA(cudaMemcpyAsync(c->x, c->xold, nb8, cudaMemcpyDeviceToDevice, c->stream));   // retry from the same warm start
+  }
+  // accepted: J^{k+1} = J^k + dt (I'_1 + I'_2) / (2a); heat source = trapezoid of the stage powers
+  k_scale_div(v, 0.5 * dt, I1, c->area, c->J);
+  k_scale_div(v, 0.5 * dt, c->x, c->area, c->J);
+  k_lincomb(v, 0.5, Q1, 0.5, c->Q);
+  int m = 0;
+  if ((rc = run_heat(c, dt, &m)) != QS_OK) return rc;
+  EventArgs ev;
+  ev.H = c->H; ev.E = c->E; ev.xmax_bits = c->xmax_bits; ev.rmin_bits = c->rmin_bits;
+  ev.Q = c->Q; ev.r = c->r; ev.area = c->area; ev.wire = c->wire;
+  ev.ebar_prev = c->ebar_prev; ev.flags = c->flags; ev.t_first = c->t_first; ev.count = c->count;
+  ev.dt = dt; ev.t_new = c->t + dt; ev.have_prev = c->have_prev_E;
+  k_set_scalars(v);
+  k_events(v, c->mp, ev);
+  k_step_stats(v, c->mp, c->J, c->Jold, c->H, c->Q, c->r, c->area);
+  if ((rc = sync_scalars(c)) != QS_OK) return rc;
+  if (c->h_sc->nonfinite) {
+    cudaMemcpyAsync(c->J, c->Jold, nb8, cudaMemcpyDeviceToDevice, c->stream);
+    cudaMemcpyAsync(c->H, c->Hold, nb8, cudaMemcpyDeviceToDevice, c->stream);
+    restore();
+    return fail(QS_ERR_NONFINITE, "NaN/Inf in J or T after the step; state restored");
+  }
+  c->t += dt;
+  c->I += dt * I_ramp;
+  c->have_prev_E = true;
+  const int ret = c->h_sc->event_or | ((hm1 || hm2) ? QS_EV_CG_MAXIT : 0);
+  c->st.cg_iters = iters;
+  c->st.cg_relres = std::max(rel1, rel2);
+  c->st.heat_substeps = m;
+  c->st.event_word = ret;
+  c->st.U_terminal = uterm;
+  c->st.Tmax = c->h_sc->tmax;
+  c->st.joule_power = c->h_sc->joule;
+  c->st.dJ_max = c->h_sc->djmax;
+  c->st.t = c->t;
+  c->st.I = c->I;
+  if (dt_taken) *dt_taken = dt;
+  if (dt_next) *dt_next = dt * fac;
+  if (err_out) *err_out = err;
   return ret;
 }
 

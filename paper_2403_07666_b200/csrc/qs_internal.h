@@ -135,6 +135,9 @@ void k_direction(const VecCtx& v, int par, bool first, const double* g, double* 
 void k_turn_deficit(const VecCtx& v, const double* x, double d, double* defw);
 void k_apply_deficit(const VecCtx& v, const double* defw, const double* Hd, const double* sw, double* x);
 void k_axpy(const VecCtx& v, double a, const double* x, double* y);                     // y += a x
+void k_lincomb(const VecCtx& v, double a, const double* x, double b, double* y);        // y = a x + b y
+// sc->djmax = max_i |s (x1_i - x2_i) / d_i|   (error estimate of the embedded Heun-Euler pair)
+void k_max_scaled_diff(const VecCtx& v, double s, const double* x1, const double* x2, const double* d);
 void k_scale_div(const VecCtx& v, double a, const double* x, const double* d, double* y);   // y += a x / d
 void k_mul(const VecCtx& v, const double* a, const double* b, double* y);               // y = a b
 void k_set_scalars(const VecCtx& v);                                                    // zero the Scalars block

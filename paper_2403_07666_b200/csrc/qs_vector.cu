@@ -162,6 +162,18 @@ __global__ void recycle_scalars_kernel(int par, Scalars* sc) {
 __global__ void axpy_kernel(int n, double a, const double* __restrict__ x, double* __restrict__ y) {
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) y[i] = fma(a, x[i], y[i]);
 }
+__global__ void lincomb_kernel(int n, double a, const double* __restrict__ x, double b, double* __restrict__ y) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) y[i] = fma(a, x[i], b * y[i]);
+}
+__global__ void max_scaled_diff_kernel(int n, double s, const double* __restrict__ x1, const double* __restrict__ x2,
+                                       const double* __restrict__ d, Scalars* sc) {
+  double m = 0.0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+    m = fmax(m, fabs(s * (x1[i] - x2[i]) / d[i]));
+  m = warp_max(m);
+  if ((threadIdx.x & 31) == 0 && m > 0.0)   // non-negative doubles order like their bit patterns
+    atomicMax(reinterpret_cast<unsigned long long*>(&sc->djmax), static_cast<unsigned long long>(__double_as_longlong(m)));
+}
 __global__ void scale_div_kernel(int n, double a, const double* __restrict__ x, const double* __restrict__ d,
                                  double* __restrict__ y) {
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) y[i] += a * x[i] / d[i];
@@ -386,6 +398,14 @@ void k_cg_direction(const VecCtx& v, const CgIter& it) {
 void k_axpy(const VecCtx& v, double a, const double* x, double* y) {
   QS_LAUNCH(v);
   axpy_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, a, x, y);
+}
+void k_lincomb(const VecCtx& v, double a, const double* x, double b, double* y) {
+  QS_LAUNCH(v);
+  lincomb_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, a, x, b, y);
+}
+void k_max_scaled_diff(const VecCtx& v, double s, const double* x1, const double* x2, const double* d) {
+  QS_LAUNCH(v);
+  max_scaled_diff_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, s, x1, x2, d, v.sc);
 }
 void k_scale_div(const VecCtx& v, double a, const double* x, const double* d, double* y) {
   QS_LAUNCH(v);

@@ -272,3 +272,48 @@ def test_adaptive_dt_controller(pkg, scenario):
     assert dts == dts_ref, (dts, dts_ref)
     assert len(set(dts)) >= 2, dts
     check_state(orc.read(), got)
+
+
+def test_heun_euler_rk_steps(pkg):
+    # f2: embedded Heun-Euler pair with error control.  The oracle runs under its own controller; the
+    # GPU is offered the oracle's accepted dt of every step and must accept it at the first try with the same error
+    # estimate, suggestion and state.  Single wire under a fast background ramp (nonlinear, both stages differ).
+    w = wl.shrunk(1, 1, 1, 12)
+    geo = dataclasses.replace(w.geometry, Bext_rate=50.0)
+    mat = dataclasses.replace(w.material, cg_tol=1e-12)
+    rtol, dt_min = 2e-4, 1e-8
+    orc = qo.Oracle(geo, mat)
+    with pkg.QS(geo, mat) as sim:
+        dt = 1e-4
+        taken = []
+        for k in range(40):
+            ro, dt_o, nxt_o, err_o = orc.step_rk(dt, 0.0, rtol, dt_min)
+            rg, dt_g, nxt_g, err_g = sim.step_rk(dt_o, 0.0, rtol, dt_min)
+            assert dt_g == dt_o and ro == (rg & 3), (k, dt_o, dt_g, err_o, err_g)
+            assert abs(err_g - err_o) <= 1e-6 * err_o + 1e-15 and abs(nxt_g - nxt_o) <= 1e-6 * nxt_o
+            taken.append(dt_o)
+            dt = nxt_o
+        got = sim.read()
+        st = sim.stats()
+    assert len(set(taken)) > 3 and min(taken) < 1e-4                        # the controller really adapted
+    check_state(orc.read(), got)
+    assert abs(st["t"] - orc.t) <= 1e-15 and abs(st["U_terminal"] - orc.stats["U_terminal"]) <= 1e-6 * abs(orc.stats["U_terminal"]) + 1e-20
+
+
+def test_heun_euler_rejects_an_oversized_step_on_the_gpu(pkg):
+    w = wl.shrunk(1, 1, 1, 12)
+    geo = dataclasses.replace(w.geometry, Bext_rate=50.0)
+    mat = dataclasses.replace(w.material, cg_tol=1e-12)
+    orc = qo.Oracle(geo, mat)
+    with pkg.QS(geo, mat) as sim:
+        for _ in range(6):                                                   # build up screening currents first
+            orc.step(1e-4, 0.0)
+            sim.step(1e-4, 0.0)
+        ro, dt_o, nxt_o, err_o = orc.step_rk(2e-3, 0.0, 1e-5, 1e-8)
+        rg, dt_g, nxt_g, err_g = sim.step_rk(2e-3, 0.0, 1e-5, 1e-8)
+    assert dt_o < 2e-3 and abs(dt_g - dt_o) <= 1e-6 * dt_o and err_g <= 1e-5
+    # linear regime on a coil: both stages give the same rate, err = 0, the suggestion doubles
+    w = wl.shrunk(0, 2, 2, 4)
+    with pkg.QS(w.geometry, w.material) as sim:
+        rc, dt_g, nxt, err = sim.step_rk(1e-4, 50.0, 1e-6, 1e-9)
+    assert dt_g == 1e-4 and err <= 1e-9 and abs(nxt - 2e-4) < 1e-18

@@ -337,6 +337,76 @@ def heat_substeps(geo, mat, H, Q, dt, m):
 
 
 # --------------------------------------------------------------------------------------
+# C15 (f4): ADI heat step ("heat equation ... solved by ADI"), Peaceman-Rachford on U = T^2
+# --------------------------------------------------------------------------------------
+def heat_line_operators(geo, mat):
+    """Sparse L_r, L_z [1/s * J/m^3 per K^2] acting on U = T^2 (per cell, divided by the cell volume) and the Robin
+    film coefficients per cell rb_r, rb_z [W/m^3 K] of the r- and z-borders; same faces, areas and conductivities as
+    heat_flux_divergence (C9): (L_r U)_c = sum over the two radial faces of kappa_f (U_c' - U_c)/(2h) A_f / V_c."""
+    import scipy.sparse as sp
+    Nr, Nz, n, h = geo.Nr, geo.Nz, geo.cells_per_side, geo.h
+    N = Nr * Nz
+    r2d = geo.r.reshape(Nr, Nz)
+    vol = 2.0 * math.pi * r2d * h * h
+    idx = np.arange(N).reshape(Nr, Nz)
+    rows, cols, vals = [], [], []
+    def add(i, j, v):
+        rows.append(i.ravel()); cols.append(j.ravel()); vals.append(v.ravel())
+    # radial faces ir | ir+1
+    same = ((np.arange(Nr - 1) // n) == (np.arange(1, Nr) // n))
+    kap = np.where(same, mat.k_in, mat.k_between)[:, None]
+    g = kap * 2.0 * math.pi * (r2d[:-1] + 0.5 * h) * h / (2.0 * h)          # face conductance on U
+    lo, hi = idx[:-1], idx[1:]
+    Lr_parts = [(lo, hi, g / vol[:-1]), (lo, lo, -g / vol[:-1]), (hi, lo, g / vol[1:]), (hi, hi, -g / vol[1:])]
+    for i, j, v in Lr_parts:
+        add(i, j, v)
+    Lr = sp.csr_matrix((np.concatenate(vals), (np.concatenate(rows), np.concatenate(cols))), shape=(N, N))
+    rows, cols, vals = [], [], []
+    same = ((np.arange(Nz - 1) // n) == (np.arange(1, Nz) // n))
+    kap = np.where(same, mat.k_in, mat.k_between)[None, :]
+    g = kap * 2.0 * math.pi * r2d[:, :-1] * h / (2.0 * h)
+    lo, hi = idx[:, :-1], idx[:, 1:]
+    for i, j, v in [(lo, hi, g / vol[:, :-1]), (lo, lo, -g / vol[:, :-1]), (hi, lo, g / vol[:, 1:]), (hi, hi, -g / vol[:, 1:])]:
+        add(i, j, v)
+    Lz = sp.csr_matrix((np.concatenate(vals), (np.concatenate(rows), np.concatenate(cols))), shape=(N, N))
+    hc = geo.h_conv
+    rb_r = np.zeros((Nr, Nz))
+    rb_r[0] += hc[0] * 2.0 * math.pi * (r2d[0] - 0.5 * h) * h / vol[0]
+    rb_r[-1] += hc[1] * 2.0 * math.pi * (r2d[-1] + 0.5 * h) * h / vol[-1]
+    rb_z = np.zeros((Nr, Nz))
+    rb_z[:, 0] += hc[2] * 2.0 * math.pi * r2d[:, 0] * h / vol[:, 0]
+    rb_z[:, -1] += hc[3] * 2.0 * math.pi * r2d[:, -1] * h / vol[:, -1]
+    return Lr, Lz, rb_r.ravel(), rb_z.ravel()
+
+
+def heat_adi(geo, mat, H, Q, dt, m):
+    """m Peaceman-Rachford ADI sub-steps of length delta = dt/m on U = T^2 with the capacity lagged at the start of
+    each sub-step (reading C15).  With H' = dH/dU = C3/2 U + C1/2 and the Robin loss linearised about U^k,
+    rb (T - T_b) ~ rb (T^k/2 - T_b) + rb/(2 T^k) U:
+        (2H'/delta - L_r + beta_r) U*  = 2H'/delta U^k + L_z U^k - rb_z (T^k - T_b) + Q - c_r      (implicit in r)
+        (2H'/delta - L_z + beta_z) U'  = 2H'/delta U*  + L_r U* - beta_r U* - c_r + Q - c_z        (implicit in z)
+    beta = rb/(2 T^k), c = rb (T^k/2 - T_b).  Returns the new enthalpy H(U')."""
+    import scipy.sparse as sp
+    import scipy.sparse.linalg as spla
+    Lr, Lz, rb_r, rb_z = heat_line_operators(geo, mat)
+    delta = dt / m
+    H = H.copy()
+    for _ in range(m):
+        T = temperature(mat, H)
+        U = T * T
+        Hp = 0.5 * mat.C3 * U + 0.5 * mat.C1
+        beta_r, beta_z = rb_r / (2.0 * T), rb_z / (2.0 * T)
+        c_r, c_z = rb_r * (0.5 * T - geo.T_bath), rb_z * (0.5 * T - geo.T_bath)
+        D = sp.diags(2.0 * Hp / delta)
+        rhs1 = 2.0 * Hp / delta * U + Lz @ U - rb_z * (T - geo.T_bath) + Q - c_r
+        Us = spla.spsolve((D - Lr + sp.diags(beta_r)).tocsc(), rhs1)
+        rhs2 = 2.0 * Hp / delta * Us + Lr @ Us - beta_r * Us - c_r + Q - c_z
+        Un = spla.spsolve((D - Lz + sp.diags(beta_z)).tocsc(), rhs2)
+        H = H + Hp * (Un - U)          # the two half-steps are exactly an energy balance for H' dU: keep it exact
+    return H
+
+
+# --------------------------------------------------------------------------------------
 # C4 / C8: circuit equations.   [A C; C^T 0] [I'; V] = [b; d],  A = M + theta dt D
 # --------------------------------------------------------------------------------------
 def constraint_matrix(geo):

@@ -169,3 +169,75 @@ def test_energy_balance_to_rounding():
     T[:, 2:] = 6.0                                                       # same step inside a wire (iz 1|2)
     d_in, _ = qo.heat_flux_divergence(geo0, mat, T)
     assert abs(d_in[0, 1] / d_between[0, 3] - mat.k_in / mat.k_between) < 1e-12
+
+
+def test_adi_line_operators_equal_the_explicit_flux_divergence():
+    # f4: L_r U + L_z U - rb (T - T_b) is the explicit scheme's divergence per volume (C9), cell by cell
+    geo = wl.lattice_geometry(3, 2, 5, 1e-3, 30e-3)
+    geo = dataclasses.replace(geo, h_conv=(500.0, 300.0, 200.0, 100.0))
+    mat = wl.Material()
+    g = np.random.default_rng(2)
+    T = g.uniform(4.2, 12.0, geo.n_rings)
+    Lr, Lz, rb_r, rb_z = qo.heat_line_operators(geo, mat)
+    div, _ = qo.heat_flux_divergence(geo, mat, T.reshape(geo.Nr, geo.Nz))
+    vol = 2 * math.pi * geo.r * geo.h ** 2
+    lhs = Lr @ (T * T) + Lz @ (T * T) - (rb_r + rb_z) * (T - geo.T_bath)
+    assert np.max(np.abs(lhs - div.ravel() / vol)) <= 1e-12 * np.max(np.abs(lhs))
+
+
+def test_adi_fixed_point_is_the_exact_discrete_steady_state():
+    # the 1-D steady state that is exact for the scheme (C9 pin: T_j^2 = T_s^2 + (Q h^2/kappa) j (n-1-j),
+    # T_s = T_bath + Q n h / (2 h_conv)) is also the fixed point of the ADI iteration (the linearised Robin term is exact
+    # at the fixed point), reached with steps ~ 500 x the explicit stability limit
+    n, h, Qv, hc = 16, 1e-4, 2e5, 500.0
+    geo = wl.lattice_geometry(1, 1, n, n * h, 1.0)               # r >> size: planar limit
+    geo = dataclasses.replace(geo, h_conv=(0.0, 0.0, hc, hc))
+    mat = dataclasses.replace(wl.Material(), k_in=5.0, k_between=5.0)
+    Q = np.full(geo.n_rings, Qv)
+    H = qo.enthalpy(mat, np.full(geo.n_rings, 4.2))
+    for _ in range(400):
+        H = qo.heat_adi(geo, mat, H, Q, 0.02, 1)
+    T = qo.temperature(mat, H).reshape(n, n)
+    Ts = 4.2 + Qv * n * h / (2 * hc)
+    j = np.arange(n)
+    exact = np.sqrt(Ts ** 2 + Qv * h * h / 5.0 * j * (n - 1 - j))
+    assert abs(exact[8] - 4.522477197289115) < 1e-12            # the value quoted in SURVEY.md §8(c) pins
+    assert np.max(np.abs(T - exact[None, :])) <= 1e-8
+
+
+def test_adi_converges_to_the_explicit_solution_at_second_order():
+    geo = wl.lattice_geometry(2, 2, 6, 1e-3, 30e-3)
+    geo = dataclasses.replace(geo, h_conv=(500.0, 300.0, 200.0, 100.0))
+    mat = wl.Material()
+    g = np.random.default_rng(4)
+    T0 = g.uniform(4.2, 9.0, geo.n_rings)
+    Q = g.uniform(0, 5e5, geo.n_rings)
+    H0 = qo.enthalpy(mat, T0)
+    dt = 2e-4
+    c = qo.heat_substeps_count(geo, mat, dt)
+    Ta = qo.temperature(mat, qo.heat_substeps(geo, mat, H0, Q, dt, 400 * c)[0])
+    Tb = qo.temperature(mat, qo.heat_substeps(geo, mat, H0, Q, dt, 800 * c)[0])
+    Tref = 2 * Tb - Ta                                           # Richardson: the explicit scheme is first order in time
+    errs = [np.max(np.abs(qo.temperature(mat, qo.heat_adi(geo, mat, H0, Q, dt, m)) - Tref)) for m in (8, 16, 32)]
+    assert errs[2] < 2e-4 and errs[0] / errs[1] > 3.5 and errs[1] / errs[2] > 3.5
+
+
+def test_adi_conserves_energy_and_survives_steps_far_beyond_the_explicit_limit():
+    # adiabatic pack: sum_c V_c dH_c = dt sum_c V_c Q_c to rounding at any step size (the half-steps are an energy
+    # balance for H' dU and the enthalpy advances by exactly that); 30 x the explicit limit on rough data stays bounded
+    geo = wl.lattice_geometry(2, 2, 8, 1e-3, 30e-3, h_conv=0.0)
+    mat = wl.Material()
+    g = np.random.default_rng(6)
+    T0 = g.uniform(4.2, 14.0, geo.n_rings)
+    Q = g.uniform(0, 5e5, geo.n_rings)
+    lim = 0.8 * geo.h ** 2 / (4 * mat.k_in / (mat.C3 * 4.2 ** 2 + mat.C1))
+    V = 2 * math.pi * geo.r * geo.h ** 2
+    for f in (3, 30):
+        H0 = qo.enthalpy(mat, T0)
+        H = H0
+        for _ in range(5):
+            H = qo.heat_adi(geo, mat, H, Q, f * lim, 1)
+        T = qo.temperature(mat, H)
+        assert np.all(np.isfinite(T)) and 4.2 <= T.min() and T.max() <= 14.5
+        gain = 5 * f * lim * np.sum(V * Q)
+        assert abs(np.sum(V * (H - H0)) - gain) <= 1e-10 * gain

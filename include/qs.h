@@ -92,6 +92,8 @@ typedef struct {
   double theta;                     /* C7: 0 explicit Euler (literal), 1 linearly implicit (default) */
   double cg_tol; int32_t cg_maxit;  /* stop when sqrt(r^T g) <= cg_tol * nu (C8)                 */
   double T_fluxjump, dEdt_spike;    /* C10: 10 K, 1 V/m/s                                        */
+  int32_t heat_adi_substeps;        /* 0: explicit heat sub-steps (C9, default); m > 0: m ADI sub-steps per step
+                                       (C15; the paper's thermal method)      */
 } qs_material;
 
 typedef struct {
@@ -180,6 +182,7 @@ int  qs_material_eval(qs_ctx *ctx, double dt);
 int  qs_set_aux(qs_ctx *ctx, int32_t on);   /* on: qs_material_eval also stores dE/dJ for qs_read_aux (off by default:
                                                the step itself never needs the array) */
 int  qs_heat(qs_ctx *ctx, double dt);
+int  qs_heat_adi(qs_ctx *ctx, double dt, int32_t m);   /* S6 alone by m ADI sub-steps (C15) with the current Q; returns m */
 int  qs_set_fields(qs_ctx *ctx, const double *B, const double *Q);
 int  qs_read_aux(qs_ctx *ctx, double *Q, double *dEdJ, double *Jc, double *rho);   /* dEdJ: see qs_set_aux */
 

@@ -581,6 +581,15 @@ class Oracle:
     def read(self):
         return self.J.copy(), self.T.copy(), np.concatenate([self.Br, self.Bz]), self.E.copy()
 
+    def _heat(self, Q, dt):
+        """S6: explicit sub-steps (C9) or, when material.heat_adi_substeps = m > 0, m ADI sub-steps (C15)."""
+        m_adi = int(getattr(self.mat, "heat_adi_substeps", 0))
+        if m_adi > 0:
+            return m_adi, heat_adi(self.geo, self.mat, self.H, Q, dt, m_adi), float("nan")
+        m = heat_substeps_count(self.geo, self.mat, dt)
+        H, lost = heat_substeps(self.geo, self.mat, self.H, Q, dt, m)
+        return m, H, lost
+
     # -- one step (SURVEY.md §8(a) S1..S7, order of C6: everything on the rhs at t^k) ----------
     def step(self, dt, I_ramp):
         geo, mat = self.geo, self.mat
@@ -615,8 +624,7 @@ class Oracle:
         self.I += dt * I_ramp
         self.t += dt
         # S6 heat with the Joule source of step k frozen over the sub-steps
-        m = heat_substeps_count(geo, mat, dt)
-        self.H, lost = heat_substeps(geo, mat, self.H, ml["Q"], dt, m)
+        m, self.H, lost = self._heat(ml["Q"], dt)
         self.T = temperature(mat, self.H)
         self.Br, self.Bz, self.E = Br, Bz, ml["E"]
         # S7 events: T^{k+1}; E, |J|/Jc, rho of the material evaluation of this step
@@ -683,8 +691,7 @@ class Oracle:
         self.I += dt * I_ramp
         self.t += dt
         Q = 0.5 * (ml1["Q"] + ml2["Q"])
-        m = heat_substeps_count(geo, mat, dt)
-        self.H, lost = heat_substeps(geo, mat, self.H, Q, dt, m)
+        m, self.H, lost = self._heat(Q, dt)
         self.T = temperature(mat, self.H)
         self.Br, self.Bz, self.E = Br2, Bz2, ml2["E"]
         ml_ev = dict(ml2)

@@ -35,7 +35,7 @@ class QsMaterial(C.Structure):
                 ("rho_n", C.c_double), ("jc0_scale", c_double_p), ("C3", C.c_double), ("C1", C.c_double),
                 ("k_in", C.c_double), ("k_between", C.c_double), ("theta", C.c_double),
                 ("cg_tol", C.c_double), ("cg_maxit", C.c_int32),
-                ("T_fluxjump", C.c_double), ("dEdt_spike", C.c_double)]
+                ("T_fluxjump", C.c_double), ("dEdt_spike", C.c_double), ("heat_adi_substeps", C.c_int32)]
 
 
 class QsStats(C.Structure):
@@ -69,6 +69,7 @@ SYMBOLS = [
     ("qs_material_eval", C.c_int, [_VP, C.c_double]),
     ("qs_set_aux", C.c_int, [_VP, C.c_int32]),
     ("qs_heat", C.c_int, [_VP, C.c_double]),
+    ("qs_heat_adi", C.c_int, [_VP, C.c_double, C.c_int32]),
     ("qs_set_fields", C.c_int, [_VP, c_double_p, c_double_p]),
     ("qs_read_aux", C.c_int, [_VP, c_double_p, c_double_p, c_double_p, c_double_p]),
     ("qs_stats", C.c_int, [_VP, C.POINTER(QsStats)]),
@@ -197,6 +198,8 @@ class QS:
                     m.jc0_scale = _dp(arr)
             elif name == "cg_maxit":
                 m.cg_maxit = int(material.cg_maxit)
+            elif name == "heat_adi_substeps":
+                m.heat_adi_substeps = int(getattr(material, "heat_adi_substeps", 0))
             else:
                 setattr(m, name, float(getattr(material, name)))
         self._h = _VP()
@@ -301,6 +304,9 @@ class QS:
 
     def heat(self, dt: float) -> int:
         return self._check(self._lib.qs_heat(self._h, float(dt)))
+
+    def heat_adi(self, dt: float, m: int) -> int:
+        return self._check(self._lib.qs_heat_adi(self._h, float(dt), int(m)))
 
     def set_fields(self, B=None, Q=None):
         Ba = None if B is None else _f64(B, 2 * self.N)

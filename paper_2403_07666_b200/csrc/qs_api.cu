@@ -140,6 +140,8 @@ struct qs_ctx {
   bool canonical_turns = false;      // turn_id[c] == (ir / n) * turns_per_layer + iz / n for every cell
   bool aux_on = false;               // qs_material_eval also writes dE/dJ (after the first qs_read_aux)
   double last_eval_dt = 0.0;
+  double* adi[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // ADI scratch (lattice only)
+  int adi_m = 0;                     // material.heat_adi_substeps
   double* heat_tab = nullptr;        // hr_p, hr_m, rb_r [Nr each], hz_p, hz_m, rb_z [Nz each]
   int tabNr = 0, tabNz = 0;
   double4* bbox;
@@ -224,6 +226,8 @@ void carve(qs_ctx* c, void* base, size_t* total) {
     c->TBz = k.take<double>(nt3);
     c->TBr = k.take<double>(nt3);
   }
+  if (c->tabNr > 0)
+    for (int q = 0; q < 6; ++q) c->adi[q] = k.take<double>(N);
   c->heat_tab = k.take<double>(3 * static_cast<size_t>(c->tabNr + c->tabNz) + 1);
   c->rowtab = k.take<double4>(static_cast<size_t>(c->tabNr) + 1);
   c->rowturn = k.take<int>(static_cast<size_t>(c->tabNr) + 1);
@@ -449,7 +453,24 @@ int heat_substeps_count(const qs_ctx* c, double dt) {
   return std::max(1, static_cast<int>(std::ceil(dt / limit)));
 }
 
+int run_heat_adi(qs_ctx* c, double dt, int m) {
+  const double delta = dt / m;
+  c->prof.begin(c->stream);
+  int launches = 0;
+  for (int s = 0; s < m; ++s) {
+    launches += k_heat_adi_substep(c->v, c->mp, c->lp, c->H, c->Q, c->Halt, delta, c->adi);
+    std::swap(c->H, c->Halt);
+  }
+  c->prof.end(c->stream, QS_PROF_HEAT, launches);
+  QS_CUDA(cudaGetLastError());
+  return QS_OK;
+}
+
 int run_heat(qs_ctx* c, double dt, int* m_out) {
+  if (c->adi_m > 0) {   // C15: the paper's ADI scheme instead of the explicit sub-steps
+    *m_out = c->adi_m;
+    return run_heat_adi(c, dt, c->adi_m);
+  }
   const int m = heat_substeps_count(c, dt);
   const double sub = dt / m;
   c->prof.begin(c->stream);
@@ -632,6 +653,7 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
   c->theta = mat->theta;
   c->cg_tol = mat->cg_tol > 0 ? mat->cg_tol : 1e-10;
   c->cg_maxit = mat->cg_maxit > 0 ? mat->cg_maxit : 20000;
+  c->adi_m = mat->heat_adi_substeps > 0 ? mat->heat_adi_substeps : 0;
   MaterialParams& mp = c->mp;
   mp.Ec = mat->Ec; mp.n_exp = mat->n_exp; mp.Jc0 = mat->Jc0; mp.Tc = mat->Tc; mp.B0 = mat->B0;
   mp.eps_coef = mat->eps_coef; mp.eps_exp = mat->eps_exp; mp.Y = mat->Y; mp.rho_n = mat->rho_n;
@@ -1237,6 +1259,14 @@ int qs_heat(qs_ctx* c, double dt) {
   if (!(dt > 0.0)) return fail(QS_ERR_DT, "dt <= 0");
   int m = 0;
   int rc = run_heat(c, dt, &m);
+  return rc != QS_OK ? rc : m;
+}
+
+int qs_heat_adi(qs_ctx* c, double dt, int32_t m) {
+  if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  if (!c->lattice) return fail(QS_ERR_ARG, "qs_heat_adi needs a lattice geometry");
+  if (!(dt > 0.0) || m <= 0) return fail(QS_ERR_DT, "dt <= 0 or m <= 0");
+  const int rc = run_heat_adi(c, dt, m);
   return rc != QS_OK ? rc : m;
 }
 

@@ -197,6 +197,9 @@ void k_heat_substep(const VecCtx& v, const MaterialParams& mp, const LatticePara
 // all m sub-steps in one launch for lattices small enough to live in one SM; false: not applicable (use k_heat_substep)
 bool k_heat_all_substeps(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, int m, const double* Hin,
                          const double* Q, double* Hout, double dtsub);
+// one ADI sub-step (qs_adi.cu, C15); scratch: six arrays of N doubles; returns the number of launches
+int k_heat_adi_substep(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, const double* Hin,
+                       const double* Q, double* Hout, double delta, double* const scratch[6]);
 struct EventArgs {
   const double *H, *E;
   const unsigned long long *xmax_bits, *rmin_bits;   // per turn, from the material pass

@@ -303,3 +303,26 @@ def test_heat_adiabatic_energy_conservation_on_the_gpu(pkg):
     V = 2 * np.pi * geo.r * geo.h ** 2
     dH = qo.enthalpy(mat, T1) - qo.enthalpy(mat, T)
     assert abs(np.sum(V * dH) - dt * np.sum(V * Q)) <= 1e-10 * dt * np.sum(V * Q)
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 8), (3, 2, 4), (2, 5, 13), (5, 3, 24), (1, 1, 1), (2, 1, 40)])
+def test_heat_adi_substeps_pointwise(pkg, shape):
+    # f4 / C15: the ADI heat step against the oracle's sparse-solve restatement; sub-steps of 5 x the explicit limit
+    # (rough random data: the lagged-capacity linearisation is not positivity preserving far beyond that)
+    L, Tn, n = shape
+    geo = wl.lattice_geometry(L, Tn, n, 1e-3, 30e-3)
+    geo = dataclasses.replace(geo, h_conv=(500.0, 300.0, 200.0, 100.0))
+    mat = wl.Material()
+    N = geo.n_rings
+    g = np.random.default_rng(19)
+    T = g.uniform(4.2, 9.0, N)
+    Q = g.uniform(0, 5e6, N)
+    m = 3
+    dt = m * 5 * 0.8 * geo.h ** 2 / (4 * mat.k_in / (mat.C3 * 4.2 ** 2 + mat.C1))
+    with pkg.QS(geo, mat, no_operator=True) as sim:
+        sim.write(np.zeros(N), T, 0.0, 0.0)
+        sim.set_fields(Q=Q)
+        assert sim.heat_adi(dt, m) == m
+        _, Tg, _, _ = sim.read(J=False, B=False, E=False)
+    Ho = qo.heat_adi(geo, mat, qo.enthalpy(mat, T), Q, dt, m)
+    assert np.max(np.abs(Tg - qo.temperature(mat, Ho))) <= 1e-11 * 9.0

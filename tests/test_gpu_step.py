@@ -317,3 +317,18 @@ def test_heun_euler_rejects_an_oversized_step_on_the_gpu(pkg):
     with pkg.QS(w.geometry, w.material) as sim:
         rc, dt_g, nxt, err = sim.step_rk(1e-4, 50.0, 1e-6, 1e-9)
     assert dt_g == 1e-4 and err <= 1e-9 and abs(nxt - 2e-4) < 1e-18
+
+
+def test_steps_with_the_adi_heat_scheme(pkg):
+    # material.heat_adi_substeps = m: S6 by m ADI sub-steps (C15) inside qs_step, a hot turn relaxing by conduction
+    w = wl.shrunk(0, 3, 3, 6)
+    geo = w.geometry
+    mat = dataclasses.replace(w.material, heat_adi_substeps=2)
+    N = geo.n_rings
+    T0 = np.full(N, geo.T_bath)
+    T0[geo.turn_id == 4] = 9.0
+    orc, sim, ref, got, rets = run_both(pkg, geo, mat, 25, w.dt, w.I_ramp, prep=(np.zeros(N), T0))
+    assert sim.stats()["heat_substeps"] == 2 and all(a == b for a, b in rets)
+    check_state(ref, got)
+    assert ref[1].max() < 9.0 and ref[1].min() >= geo.T_bath - 1e-9
+    sim.close()

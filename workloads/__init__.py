@@ -81,6 +81,7 @@ class Material:
     cg_maxit: int = 20000
     T_fluxjump: float = 10.0
     dEdt_spike: float = 1.0       # SURVEY.md §8(c) C10 [silent]
+    heat_adi_substeps: int = 0    # 0: explicit heat sub-steps (C9); m > 0: m ADI sub-steps per step (C15)
 
 
 @dataclasses.dataclass

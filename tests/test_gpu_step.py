@@ -332,3 +332,28 @@ def test_steps_with_the_adi_heat_scheme(pkg):
     check_state(ref, got)
     assert ref[1].max() < 9.0 and ref[1].min() >= geo.T_bath - 1e-9
     sim.close()
+
+
+def test_energy_balance_of_whole_steps_on_the_gpu(pkg):
+    # north_star: "the Joule heat integral equals the enthalpy rise plus boundary flux".  Adiabatic pack (h_conv = 0),
+    # dissipative state (|J| ~ Jc): sum_c V_c (H_c^{end} - H_c^0) = sum_steps dt * joule_power, GPU quantities only
+    w = wl.shrunk(0, 2, 2, 8)
+    geo = dataclasses.replace(w.geometry, h_conv=(0.0, 0.0, 0.0, 0.0))
+    mat = dataclasses.replace(w.material, cg_tol=1e-12)
+    N = geo.n_rings
+    Jc0 = mat.Jc0 * (1 - geo.T_bath / mat.Tc) ** 2
+    g = np.random.default_rng(21)
+    J0 = Jc0 * g.uniform(0.9, 1.05, N)
+    T0 = np.full(N, geo.T_bath)
+    V = 2 * np.pi * geo.r * geo.area
+    with pkg.QS(geo, mat) as sim:
+        sim.write(J0, T0, 0.0, 0.0)
+        total = 0.0
+        for _ in range(8):
+            assert sim.step(2e-5, 0.0) >= 0
+            total += 2e-5 * sim.stats()["joule_power"]
+        _, T1, _, _ = sim.read()
+        ws = sim.wire_stats()
+    dH = qo.enthalpy(mat, T1) - qo.enthalpy(mat, T0)
+    assert total > 0 and abs(np.sum(V * dH) - total) <= 1e-9 * total
+    assert abs(ws["E_joule"].sum() - total) <= 1e-9 * total          # per-wire energies add up to the same integral

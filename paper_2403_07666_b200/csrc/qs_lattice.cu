@@ -146,6 +146,108 @@ __global__ void __launch_bounds__(256) table_sweep_kernel(LatticeSweepParams prm
   }
 }
 
+// ---- block-Toeplitz sweep on the FP64 tensor cores (mma.sync m8n8k4, SASS DMMA) ---------------------------------------
+// The product is a dense contraction, so it belongs on the tensor pipe: one DMMA does 256 multiply-adds for one issue
+// slot (measured 37.1 TFLOP/s = the full FP64 rate, 16 cycles per mma per sub-partition), where the multiply-add kernel
+// above is capped at 2/3 of the rate by its three-register-operand DFMAs.  With iz = 8p + q, jz = 8a + b and d = p - a:
+//     Y[p][q] += sum_b X[p - d][b] * t[8d + q - b]
+// is, for 8 consecutive p and a fixed block offset d, an (8 x 8) += (8 x 8)(8 x 8) product = two m8n8k4 steps whose
+// A operand is a block of 8 x 8 source values (rows = source blocks p - d) and whose B operand is the Toeplitz block
+// T_d[b][q] = t[8d + q - b].  A warp owns NT tiles of 64 outputs which share every B fragment; the fused sweep shares
+// the A fragment of the ring currents between the Bz and Br tables.  Fragments are read from shared memory: the source
+// row in 8-blocks padded to a stride of 12 doubles (conflict-free for the row-strided A pattern), the mirrored table
+// row as for the multiply-add kernel.
+constexpr int kMmaNT = 2;
+
+__device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(c[0]), "+d"(c[1])
+               : "d"(a), "d"(b));
+}
+
+template <bool FIELD>
+__global__ void __launch_bounds__(512) table_sweep_mma_kernel(LatticeSweepParams prm, int P) {
+  extern __shared__ __align__(16) double lsm[];
+  constexpr int NT = kMmaNT, NTAB = FIELD ? 3 : 1;
+  const int Nz = prm.Nz, T = blockDim.x;
+  const int xlen = (P + 14) * 12, tlen = 16 * P + 144;    // e in [-8P, 8P + 144): block offsets up to P + 14
+  double* xs = lsm;                                   // source row, blocks a = -7 .. P+6 at (a + 7) * 12
+  double* cs = FIELD ? xs + xlen : nullptr;
+  double* tM = (FIELD ? cs : xs) + xlen;              // t_ext[e] at [e + 8P], e = iz - jz
+  double* tBz = FIELD ? tM + tlen : nullptr;
+  double* tBr = FIELD ? tBz + tlen : nullptr;
+  if (prm.done != nullptr && *prm.done != 0) return;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = T >> 5;
+  const int ir = blockIdx.y;
+  const int j0 = blockIdx.x * prm.jr_chunk, j1 = min(j0 + prm.jr_chunk, prm.Nr);
+  const int pw = (blockIdx.z * nwarps + warp) * 8 * NT;          // first 8-block of this warp's outputs
+  const int li = lane >> 2, lk = lane & 3;
+  double acc[NT][NTAB][2];
+#pragma unroll
+  for (int j = 0; j < NT; ++j)
+#pragma unroll
+    for (int t = 0; t < NTAB; ++t) acc[j][t][0] = acc[j][t][1] = 0.0;
+  for (int jr = j0; jr < j1; ++jr) {
+    __syncthreads();
+    const long long trow = (static_cast<long long>(ir) * prm.Nr + jr) * Nz;
+    const long long xrow = static_cast<long long>(jr) * Nz;
+    for (int s = threadIdx.x; s < (P + 14) * 8; s += T) {        // source row in padded 8-blocks, zero outside the row
+      const int a = (s >> 3) - 7, b = s & 7, j = 8 * a + b;
+      const bool in = j >= 0 && j < Nz;
+      xs[(a + 7) * 12 + b] = in ? prm.x[xrow + j] : 0.0;
+      if (FIELD) cs[(a + 7) * 12 + b] = in ? prm.cur[xrow + j] : 0.0;
+    }
+    for (int s = threadIdx.x; s < tlen; s += T) {                 // mirrored table row, zero outside |e| < Nz
+      const int e = s - 8 * P, d = abs(e);
+      const bool in = d < Nz;
+      tM[s] = in ? prm.TM[trow + d] : 0.0;
+      if (FIELD) {
+        tBz[s] = in ? prm.TBz[trow + d] : 0.0;
+        const double br = in ? prm.TBr[trow + d] : 0.0;
+        tBr[s] = e < 0 ? -br : br;
+      }
+    }
+    __syncthreads();
+    if (pw >= P) continue;                                        // warp beyond the row: only helps with the fills
+    const int dlo = pw - (P - 1), dhi = pw + 8 * NT - 1;
+    for (int d = dlo; d <= dhi; ++d) {
+#pragma unroll
+      for (int kk = 0; kk < 2; ++kk) {
+        const int e = 8 * d + li - lk - 4 * kk + 8 * P;           // B fragment: k = lk (+4 kk), n = li
+        const double bM = tM[e];
+        const double bBz = FIELD ? tBz[e] : 0.0, bBr = FIELD ? tBr[e] : 0.0;
+#pragma unroll
+        for (int j = 0; j < NT; ++j) {
+          const int pj = pw + 8 * j;
+          if (d < pj - (P - 1) || d > pj + 7) continue;           // no source block of the row at this offset (uniform)
+          const int ai = (pj + li - d + 7) * 12 + lk + 4 * kk;    // A fragment: row li = output block, k = lk (+4 kk)
+          dmma(acc[j][0], xs[ai], bM);
+          if (FIELD) {
+            const double ac = cs[ai];
+            dmma(acc[j][1], ac, bBz);
+            dmma(acc[j][2], ac, bBr);
+          }
+        }
+      }
+    }
+  }
+  const long long orow = static_cast<long long>(ir) * Nz;
+#pragma unroll
+  for (int j = 0; j < NT; ++j) {
+    const int iz = 8 * (pw + 8 * j + li) + 2 * lk;                // C fragment: row li, columns 2 lk, 2 lk + 1
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      if (iz + h < Nz) {
+        asm volatile("red.global.add.f64 [%0], %1;" ::"l"(prm.yacc + orow + iz + h), "d"(acc[j][0][h]) : "memory");
+        if (FIELD) {
+          asm volatile("red.global.add.f64 [%0], %1;" ::"l"(prm.bzacc + orow + iz + h), "d"(acc[j][1][h]) : "memory");
+          asm volatile("red.global.add.f64 [%0], %1;" ::"l"(prm.bracc + orow + iz + h), "d"(acc[j][2][h]) : "memory");
+        }
+      }
+    }
+  }
+}
+
 }  // namespace
 
 cudaError_t launch_table_build(int Nr, int Nz, double r_inner, double h, double soft_self2, double* TM, double* TBz,
@@ -190,8 +292,33 @@ static cudaError_t launch_R(const LatticeSweepParams& prm, bool field, dim3 grid
   return cudaGetLastError();
 }
 
+// tensor-core variant: rows of at least 64 cells
+static cudaError_t launch_table_sweep_mma(LatticeSweepParams prm, bool field, int sm_count, cudaStream_t stream) {
+  const int P = (prm.Nz + 7) / 8;
+  const int per_warp = 8 * kMmaNT;                                   // 8-blocks per warp
+  const int warps_needed = (P + per_warp - 1) / per_warp;
+  const int nwarps = std::min(16, warps_needed);
+  const int tiles = (warps_needed + nwarps - 1) / nwarps;
+  const long long want = 12ll * sm_count;
+  int splits = static_cast<int>(std::max<long long>(1, std::min<long long>(prm.Nr, want / std::max(1, prm.Nr * tiles))));
+  prm.jr_chunk = (prm.Nr + splits - 1) / splits;
+  splits = (prm.Nr + prm.jr_chunk - 1) / prm.jr_chunk;
+  const dim3 grid(splits, prm.Nr, tiles);
+  const size_t smem = sizeof(double) * (static_cast<size_t>(field ? 2 : 1) * (P + 14) * 12 +
+                                        static_cast<size_t>(field ? 3 : 1) * (16 * P + 144));
+  if (field) {
+    cudaFuncSetAttribute(table_sweep_mma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    table_sweep_mma_kernel<true><<<grid, nwarps * 32, smem, stream>>>(prm, P);
+  } else {
+    cudaFuncSetAttribute(table_sweep_mma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    table_sweep_mma_kernel<false><<<grid, nwarps * 32, smem, stream>>>(prm, P);
+  }
+  return cudaGetLastError();
+}
+
 cudaError_t launch_table_sweep(const LatticeSweepParams& prm_in, bool field, int sm_count, cudaStream_t stream) {
   LatticeSweepParams prm = prm_in;
+  if (prm.Nz >= 64) return launch_table_sweep_mma(prm, field, sm_count, stream);   // rows shorter than 64 cells: FMA kernel
   int T, R, tiles;
   lattice_sweep_shape(prm.Nz, &T, &R, &tiles);
   // split the source rows so that the grid fills the GPU several times over

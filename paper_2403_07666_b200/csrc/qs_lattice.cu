@@ -166,21 +166,30 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
 }
 
 template <bool FIELD>
-__global__ void __launch_bounds__(512) table_sweep_mma_kernel(LatticeSweepParams prm, int P) {
+__global__ void __launch_bounds__(512) table_sweep_mma_kernel(LatticeSweepParams prm, int P, int n_asplit, int A_c) {
+  // The CTA owns the outputs of its warps (8 NT p-blocks each) and the SOURCE blocks a in [a_lo, a_hi): splitting the
+  // sources as well as the outputs keeps the shared-memory windows near 50 KB (four CTAs per SM) on long rows.
   extern __shared__ __align__(16) double lsm[];
   constexpr int NT = kMmaNT, NTAB = FIELD ? 3 : 1;
   const int Nz = prm.Nz, T = blockDim.x;
-  const int xlen = (P + 14) * 12, tlen = 16 * P + 144;    // e in [-8P, 8P + 144): block offsets up to P + 14
-  double* xs = lsm;                                   // source row, blocks a = -7 .. P+6 at (a + 7) * 12
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = T >> 5;
+  const int zt = blockIdx.z / n_asplit, as = blockIdx.z - zt * n_asplit;
+  const int a_lo = as * A_c, a_hi = min(a_lo + A_c, P);
+  const int p_lo = zt * nwarps * 8 * NT;                          // first p-block of the CTA's outputs
+  const int np_cta = nwarps * 8 * NT;
+  const int xblocks = A_c + 14;                                   // source blocks a_lo - 7 .. a_lo + A_c + 6
+  const int xlen = xblocks * 12;
+  const int e0 = 8 * (p_lo - (a_lo + A_c) + 1) - 8;               // first offset iz - jz of the table window
+  const int tlen = 8 * (np_cta + A_c + 8) + 24;
+  double* xs = lsm;
   double* cs = FIELD ? xs + xlen : nullptr;
-  double* tM = (FIELD ? cs : xs) + xlen;              // t_ext[e] at [e + 8P], e = iz - jz
+  double* tM = (FIELD ? cs : xs) + xlen;                          // t_ext[e] at [e - e0]
   double* tBz = FIELD ? tM + tlen : nullptr;
   double* tBr = FIELD ? tBz + tlen : nullptr;
   if (prm.done != nullptr && *prm.done != 0) return;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = T >> 5;
   const int ir = blockIdx.y;
   const int j0 = blockIdx.x * prm.jr_chunk, j1 = min(j0 + prm.jr_chunk, prm.Nr);
-  const int pw = (blockIdx.z * nwarps + warp) * 8 * NT;          // first 8-block of this warp's outputs
+  const int pw = p_lo + warp * 8 * NT;                            // first 8-block of this warp's outputs
   const int li = lane >> 2, lk = lane & 3;
   double acc[NT][NTAB][2];
 #pragma unroll
@@ -191,14 +200,14 @@ __global__ void __launch_bounds__(512) table_sweep_mma_kernel(LatticeSweepParams
     __syncthreads();
     const long long trow = (static_cast<long long>(ir) * prm.Nr + jr) * Nz;
     const long long xrow = static_cast<long long>(jr) * Nz;
-    for (int s = threadIdx.x; s < (P + 14) * 8; s += T) {        // source row in padded 8-blocks, zero outside the row
-      const int a = (s >> 3) - 7, b = s & 7, j = 8 * a + b;
-      const bool in = j >= 0 && j < Nz;
-      xs[(a + 7) * 12 + b] = in ? prm.x[xrow + j] : 0.0;
-      if (FIELD) cs[(a + 7) * 12 + b] = in ? prm.cur[xrow + j] : 0.0;
+    for (int s = threadIdx.x; s < xblocks * 8; s += T) {          // source blocks of this CTA, zero outside its range
+      const int a = a_lo - 7 + (s >> 3), b = s & 7, j = 8 * a + b;
+      const bool in = a >= a_lo && a < a_hi && j < Nz;
+      xs[(s >> 3) * 12 + b] = in ? prm.x[xrow + j] : 0.0;
+      if (FIELD) cs[(s >> 3) * 12 + b] = in ? prm.cur[xrow + j] : 0.0;
     }
     for (int s = threadIdx.x; s < tlen; s += T) {                 // mirrored table row, zero outside |e| < Nz
-      const int e = s - 8 * P, d = abs(e);
+      const int e = s + e0, d = abs(e);
       const bool in = d < Nz;
       tM[s] = in ? prm.TM[trow + d] : 0.0;
       if (FIELD) {
@@ -209,18 +218,19 @@ __global__ void __launch_bounds__(512) table_sweep_mma_kernel(LatticeSweepParams
     }
     __syncthreads();
     if (pw >= P) continue;                                        // warp beyond the row: only helps with the fills
-    const int dlo = pw - (P - 1), dhi = pw + 8 * NT - 1;
+    const int dlo = pw - (a_hi - 1), dhi = pw + 8 * (NT - 1) + 7 - a_lo;
     for (int d = dlo; d <= dhi; ++d) {
 #pragma unroll
       for (int kk = 0; kk < 2; ++kk) {
-        const int e = 8 * d + li - lk - 4 * kk + 8 * P;           // B fragment: k = lk (+4 kk), n = li
+        const int e = 8 * d + li - lk - 4 * kk - e0;              // B fragment: k = lk (+4 kk), n = li
         const double bM = tM[e];
         const double bBz = FIELD ? tBz[e] : 0.0, bBr = FIELD ? tBr[e] : 0.0;
 #pragma unroll
         for (int j = 0; j < NT; ++j) {
           const int pj = pw + 8 * j;
-          if (d < pj - (P - 1) || d > pj + 7) continue;           // no source block of the row at this offset (uniform)
-          const int ai = (pj + li - d + 7) * 12 + lk + 4 * kk;    // A fragment: row li = output block, k = lk (+4 kk)
+          if (pj >= P || d < pj - (a_hi - 1) || d > pj + 7 - a_lo) continue;   // tile beyond the row, or no source block
+                                                                               // of this CTA at this offset (uniform)
+          const int ai = (pj + li - d - a_lo + 7) * 12 + lk + 4 * kk;   // A fragment: row li = output block, k = lk (+4 kk)
           dmma(acc[j][0], xs[ai], bM);
           if (FIELD) {
             const double ac = cs[ai];
@@ -292,28 +302,32 @@ static cudaError_t launch_R(const LatticeSweepParams& prm, bool field, dim3 grid
   return cudaGetLastError();
 }
 
-// tensor-core variant: rows of at least 64 cells
+// tensor-core variant
 static cudaError_t launch_table_sweep_mma(LatticeSweepParams prm, bool field, int sm_count, cudaStream_t stream) {
   const int P = (prm.Nz + 7) / 8;
   const int per_warp = 8 * kMmaNT;                                   // 8-blocks per warp
   const int warps_needed = (P + per_warp - 1) / per_warp;
-  const int nwarps = std::min(16, warps_needed);
-  const int tiles = (warps_needed + nwarps - 1) / nwarps;
+  const int ztiles = (warps_needed + 4) / 5;                         // at most 5 warps (640 outputs) per CTA ...
+  const int nwarps = (warps_needed + ztiles - 1) / ztiles;
+  const int n_asplit = (P + 79) / 80;                                // ... and at most 80 source blocks
+  const int A_c = (P + n_asplit - 1) / n_asplit;
   // many small CTAs (a few source rows each): the fill of one CTA overlaps the DMMA phase of its neighbours on the SM
   // and the tail of the launch stays short (measured: 10.7 ms at 12 CTAs per SM, 9.3 ms at one source row per CTA)
   const long long want = 1000ll * sm_count;
-  int splits = static_cast<int>(std::max<long long>(1, std::min<long long>(prm.Nr, want / std::max(1, prm.Nr * tiles))));
+  const int per_split = prm.Nr * ztiles * n_asplit;
+  int splits = static_cast<int>(std::max<long long>(1, std::min<long long>(prm.Nr, want / std::max(1, per_split))));
   prm.jr_chunk = (prm.Nr + splits - 1) / splits;
   splits = (prm.Nr + prm.jr_chunk - 1) / prm.jr_chunk;
-  const dim3 grid(splits, prm.Nr, tiles);
-  const size_t smem = sizeof(double) * (static_cast<size_t>(field ? 2 : 1) * (P + 14) * 12 +
-                                        static_cast<size_t>(field ? 3 : 1) * (16 * P + 144));
+  const dim3 grid(splits, prm.Nr, ztiles * n_asplit);
+  const int np_cta = nwarps * per_warp;
+  const size_t smem = sizeof(double) * (static_cast<size_t>(field ? 2 : 1) * (A_c + 14) * 12 +
+                                        static_cast<size_t>(field ? 3 : 1) * (8 * (np_cta + A_c + 8) + 24));
   if (field) {
     cudaFuncSetAttribute(table_sweep_mma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
-    table_sweep_mma_kernel<true><<<grid, nwarps * 32, smem, stream>>>(prm, P);
+    table_sweep_mma_kernel<true><<<grid, nwarps * 32, smem, stream>>>(prm, P, n_asplit, A_c);
   } else {
     cudaFuncSetAttribute(table_sweep_mma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
-    table_sweep_mma_kernel<false><<<grid, nwarps * 32, smem, stream>>>(prm, P);
+    table_sweep_mma_kernel<false><<<grid, nwarps * 32, smem, stream>>>(prm, P, n_asplit, A_c);
   }
   return cudaGetLastError();
 }

@@ -91,3 +91,28 @@ def test_tables_nonlinear_config1_like(pkg):
     assert its > 0
     for name, a, b in zip("JTBE", got, ref):
         assert rel(a, b) <= 1e-6, name
+
+
+def test_tables_constrained_solve_and_rk_step_agree_with_the_pair_sweeps(pkg):
+    # the solver and the Runge-Kutta step are operator-agnostic: same results through either operator
+    w = wl.shrunk(2, 2, 9, 16)                                   # Nz = 144 >= 128: tensor-core sweep
+    geo = w.geometry
+    mat = dataclasses.replace(w.material, cg_tol=1e-12)
+    b = np.random.default_rng(8).standard_normal(geo.n_rings) * 1e-6
+    out = {}
+    for tables in (False, True):
+        with pkg.QS(geo, mat, lattice_tables=tables) as sim:
+            x, it, relres, rc = sim.solve(b)
+            assert rc == 0 and relres <= 1e-12
+            geo2 = geo
+            rk = [sim.step_rk(1e-4, w.I_ramp, 1e-6, 1e-9) for _ in range(3)]
+            out[tables] = (x, rk, sim.read())
+    xa, rka, sa = out[False]
+    xb, rkb, sb = out[True]
+    assert rel(xb, xa) <= 1e-8
+    cs = np.bincount(geo.turn_id, weights=xb, minlength=geo.n_turns)
+    assert np.max(np.abs(cs)) <= 1e-9 * np.max(np.abs(xb)) * 300     # C^T x = 0 kept by the projection
+    for (ra, da, na, ea), (rb_, db, nb, eb) in zip(rka, rkb):
+        assert ra == rb_ and da == db and abs(ea - eb) <= 1e-9 + 1e-6 * ea
+    for a, b_ in zip(sa, sb):
+        assert rel(b_, a) <= 1e-9 or np.linalg.norm(a) < 1e-30

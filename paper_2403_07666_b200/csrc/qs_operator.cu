@@ -10,8 +10,11 @@
 // Source blocks (r, z, x[, I]: 3-4 x 256 B) are staged in per-warp shared memory with TMA bulk copies
 // (cp.async.bulk + mbarrier), double buffered one item ahead.  Items are handed out in contiguous
 // chunks from an atomic counter to a persistent grid (a multiple of the SM count).
-// The AGM depth is chosen per item from the bounding boxes of the two blocks (a lower bound on
-// k'^2 over the 1024 pairs), so the 32-step loops are branch-free and fully unrolled in the depth.
+// The evaluation class (AGM depth + series order, qs_pair.cuh) is chosen per item from the bounding boxes of the two
+// blocks (a lower bound on k'^2 over the 1024 pairs), so the 32-step loops are branch-free and fully unrolled in the
+// depth; items whose two blocks each sit on one radius (rows of a lattice) take a variant with the radial terms hoisted.
+// What bounds the kernel is the issue port (an FP64 instruction holds it for two cycles), so the loops
+// are written for instruction count: source arrays staged twice (no index wrap), unroll 2, no divisions, no roots.
 #include "qs_internal.h"
 #include "qs_pair.cuh"
 #include "qs_tma.cuh"

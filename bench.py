@@ -311,6 +311,30 @@ def operator_leg(torch, pkg, fp64_peak):
         sim.sync()
         b.synchronize()
         pr = sim.profile_read()
+    # config 4 (b): b = M x, solve M xh = b to cg_tol = 1e-10 at N = 4096 (ill-conditioned: cond ~ 1e7), check xh ~ x
+    n4 = 4096
+    geo4, x4 = wl.free_rings(n4)
+    with pkg.QS(geo4, wl.Material(cg_tol=1e-10, cg_maxit=20000)) as sim:
+        xd = torch.from_numpy(x4).to(sim.device)
+        bd4 = torch.empty_like(xd)
+        xh = torch.empty_like(xd)
+        torch.cuda.synchronize()
+        sim.matvec_device(xd, bd4)
+        sim.sync()
+        a4, b4 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a4.record(sim.stream)
+        it4, rel4, rc4 = sim.solve_device(bd4, xh)
+        b4.record(sim.stream)
+        sim.sync()
+        b4.synchronize()
+        chk = torch.empty_like(xd)
+        sim.matvec_device(xh, chk)
+        sim.sync()
+    s4 = a4.elapsed_time(b4) * 1e-3
+    out["cg_N4096_to_tolerance"] = {"iterations": it4, "seconds": s4, "iters_per_s": it4 / s4, "relres": rel4,
+                                    "converged": rc4 == 0,
+                                    "residual_rel_l2": float(torch.linalg.norm(chk - bd4) / torch.linalg.norm(bd4)),
+                                    "solution_rel_l2": float(torch.linalg.norm(xh - xd) / torch.linalg.norm(xd))}
     vec_us = 1e3 * pr["cg_vector"][0] / max(it, 1)
     out["cg_N65536"] = {"iterations": it, "iters_per_s": it / (a.elapsed_time(b) * 1e-3), "relres_reached": relres,
                         "sweep_ms_per_iteration": pr["sweep_M"][0] / max(pr["sweep_M"][1], 1),

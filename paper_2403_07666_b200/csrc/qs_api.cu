@@ -107,6 +107,7 @@ struct qs_ctx {
   int N = 0, Np = 0, nb = 0, n_turns = 0;
   bool lattice = false, has_operator = true;
   bool tables = false;               // QS_GEO_LATTICE_TABLES: block-Toeplitz operator
+  bool blockprec = false;            // free rings without constraints: block-Jacobi preconditioned CG in qs_solve
   double *TM = nullptr, *TBz = nullptr, *TBr = nullptr;   // [Nr][Nr][Nz]
   MaterialParams mp{};
   LatticeParams lp{};
@@ -145,6 +146,7 @@ struct qs_ctx {
   double* heat_tab = nullptr;        // hr_p, hr_m, rb_r [Nr each], hz_p, hz_m, rb_z [Nz each]
   int tabNr = 0, tabNz = 0;
   double4* bbox;
+  double* Lblk = nullptr;            // [nb][32][32] block-Jacobi factors of M (free rings: unconstrained solves)
   Scalars* sc;
   Scalars* h_sc = nullptr;           // pinned
   double* h_stage = nullptr;         // pinned staging, 2N doubles
@@ -220,6 +222,7 @@ void carve(qs_ctx* c, void* base, size_t* total) {
   c->turn_id = k.take<int>(N);
   c->d_perm = k.take<int>(N);
   c->bbox = k.take<double4>(std::max(c->nb, 1));
+  if (c->blockprec) c->Lblk = k.take<double>(static_cast<size_t>(c->nb) * 1024);
   if (c->tables) {
     const size_t nt3 = static_cast<size_t>(c->tabNr) * c->tabNr * c->tabNz;
     c->TM = k.take<double>(nt3);
@@ -320,14 +323,20 @@ constexpr double kCM = 0.5 * kMu0 * kPi;   // yacc -> henry * ampere
 // Iterations are enqueued in batches without a host round trip: the kernels stop themselves (Scalars::done) at the
 // iteration where sqrt(r^T g) <= tol nu, so the result is the one of the iteration-by-iteration loop.
 int cg_core(qs_ctx* c, const Rhs& b, double* x, const double* shift, const double* Hd, const double* sw,
-            bool yacc_has_Mx, double tol, int maxit, double nu, int* iters, double* relres, bool* hit_max) {
+            bool yacc_has_Mx, double tol, int maxit, double nu, int* iters, double* relres, bool* hit_max,
+            const double* Lblk = nullptr) {
   const VecCtx& v = c->v;
   int rc;
   if (!yacc_has_Mx && (rc = do_sweep(c, x, nullptr, false)) != QS_OK) return rc;
   k_residual(v, c->yacc, shift, x, b, c->rr, kCM);
   if (c->n_turns) QS_CUDA(cudaMemsetAsync(c->vsum, 0, sizeof(double) * c->n_turns, c->stream));
   k_turn_project(v, c->rr, Hd, sw, c->vw, c->vsum);
-  k_project_apply(v, 0, c->vw, Hd, c->rr, c->g);
+  if (Lblk) {   // block-Jacobi preconditioner: g = B^-1 r, rg[0] = r.g (rg[0] is zero on entry)
+    QS_CUDA(launch_blockprec_apply(c->nb, c->N, Lblk, c->rr, c->g, &c->sc->rg[0], nullptr, c->stream));
+    ++c->launches;
+  } else {
+    k_project_apply(v, 0, c->vw, Hd, c->rr, c->g);
+  }
   k_direction(v, 0, true, c->g, c->p);
   if ((rc = sync_scalars(c)) != QS_OK) return rc;
   double rg = c->h_sc->rg[0];
@@ -363,6 +372,8 @@ int cg_core(qs_ctx* c, const Rhs& b, double* x, const double* shift, const doubl
   it.yacc_zero = c->yacc;
   it.counter = c->counter;
   it.cM = kCM;
+  it.Lblk = Lblk;
+  it.nb = c->nb;
   // one iteration = sweep + four vector kernels; pairs of iterations are replayed from a CUDA graph (captured on
   // first use for this set of vectors) unless the event profiler is recording
   auto enqueue_iteration = [&](int par) -> int {
@@ -647,6 +658,7 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
   c->lattice = geo->lattice != 0;
   c->has_operator = !(geo->flags & QS_GEO_NO_OPERATOR);
   c->tables = c->lattice && c->has_operator && (geo->flags & QS_GEO_LATTICE_TABLES);
+  c->blockprec = !c->lattice && c->has_operator && geo->n_turns == 0;
   c->Bext0 = geo->Bext0;
   c->Bext_rate = geo->Bext_rate;
   c->Bext_max = geo->Bext_max;
@@ -863,6 +875,11 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
     if (cudaMemcpyAsync(c->Hd, c->diagM, sizeof(double) * N, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
       return bail(fail(QS_ERR_CUDA, "copy"));
     if (c->lattice) k_build_rowtab(v, lp.Nr, lp.Nz, c->r, c->selfcoef, c->diagM, c->area, c->rowtab);
+    if (c->blockprec) {
+      if (launch_blockprec_build(c->nb, c->r, c->z, c->soft_all, c->soft_self, c->Lblk, c->stream) != cudaSuccess)
+        return bail(fail(QS_ERR_CUDA, "block preconditioner build failed"));
+      ++c->launches;
+    }
     if (c->n_turns) {
       // unit-ramp particular solution x_p1 = H_M^-1 C (1/s_M) and M x_p1 (reference norm of the CG, C8)
       k_turn_schur(v, c->diagM, c->swM);
@@ -905,6 +922,7 @@ size_t qs_workspace_bytes(const qs_geometry* geo) {
     tmp.tabNz = geo->turns_per_layer * geo->cells_per_side;
     tmp.tables = (geo->flags & QS_GEO_LATTICE_TABLES) && !(geo->flags & QS_GEO_NO_OPERATOR);
   }
+  tmp.blockprec = !geo->lattice && !(geo->flags & QS_GEO_NO_OPERATOR) && geo->n_turns == 0;
   size_t need = 0;
   carve(&tmp, nullptr, &need);
   return need;
@@ -1200,7 +1218,7 @@ int qs_solve_device(qs_ctx* c, const double* d_b, double* d_x, int32_t maxit_ove
   bool hit = false;
   const Rhs rhs{c->b, nullptr, nullptr, 0.0};
   int rc = cg_core(c, rhs, c->tmp, c->zero, c->diagM, c->swM, true, c->cg_tol, maxit_override > 0 ? maxit_override : c->cg_maxit,
-                   -1.0, &it, &rel, &hit);
+                   -1.0, &it, &rel, &hit, c->blockprec ? c->Lblk : nullptr);
   if (rc != QS_OK) return rc;
   k_scatter_scaled(c->v, c->tmp, perm, d_x, c->N, 1.0);
   QS_CUDA(cudaStreamSynchronize(c->stream));

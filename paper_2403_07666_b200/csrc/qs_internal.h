@@ -47,6 +47,12 @@ cudaError_t launch_table_build(int Nr, int Nz, double r_inner, double h, double 
                                double* TBr, int sm_count, cudaStream_t stream);
 cudaError_t launch_table_sweep(const LatticeSweepParams& prm, bool field, int sm_count, cudaStream_t stream);
 
+// block-Jacobi preconditioner of the unconstrained solve (qs_operator.cu): L [nb][32][32], 1/L_ii on the diagonal
+cudaError_t launch_blockprec_build(int nb, const double* r, const double* z, double soft_all, double soft_self, double* L,
+                                   cudaStream_t stream);
+cudaError_t launch_blockprec_apply(int nb, int n, const double* L, const double* rvec, double* g, double* rg_out,
+                                   const int* done, cudaStream_t stream);
+
 // test hook: per-pair evaluation through evaluation class cls (or the class the sweep would pick when cls < 0)
 cudaError_t launch_pair_eval(int n, const double* A2, const double* B2, int cls, double* M, double* K, double* E,
                              int* used, cudaStream_t stream);
@@ -99,6 +105,8 @@ struct CgIter {
   double* yacc_zero;         // accumulators to clear for the next sweep (Np doubles) ...
   unsigned long long* counter;   // ... and its work counter
   double cM;
+  const double* Lblk;        // non-null: block-Jacobi factors (unconstrained solves): g = B^-1 r instead of r / Hd
+  int nb;                    // blocks of 32
 };
 void k_cg_Ap(const VecCtx& v, const CgIter& it);          // q = shift p + cM yacc ; pq[par] += p.q
 void k_cg_update(const VecCtx& v, const CgIter& it);      // alpha = rg[par]/pq[par]; x += alpha p; r += alpha q; tw += r/H

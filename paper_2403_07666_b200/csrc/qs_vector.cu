@@ -389,6 +389,10 @@ void k_cg_update(const VecCtx& v, const CgIter& it) {
 }
 void k_cg_project(const VecCtx& v, const CgIter& it) {
   QS_LAUNCH(v);
+  if (it.Lblk) {   // block-Jacobi preconditioner (unconstrained solves): g = B^-1 r, rg[par^1] += r.g
+    launch_blockprec_apply(it.nb, v.N, it.Lblk, it.r, it.g, &v.sc->rg[it.par ^ 1], &v.sc->done, v.stream);
+    return;
+  }
   cg_project_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.n_turns ? v.turn_id : nullptr, v.sc);
 }
 void k_cg_direction(const VecCtx& v, const CgIter& it) {

@@ -20,6 +20,11 @@ Pins (tests/test_oracle_*.py, all ``-m "not gpu"``):
   heat_substeps      exact discrete 1-D steady state; energy balance to rounding
   kkt_dense / pcg    constraint C^T I' = d, KKT residual, dense vs CG, single-ring L-R circuit
   lattice tables     table operator == dense operator on small lattices
+  wire statistics    closed forms of a prepared normal-state turn (rho_n J^2), sum_w E_joule == integral of Joule power
+  step_rk            exact second-order polynomial and error estimate on the linear L-R ring, global order 2,
+                     rejection rule, reduction to the theta = 0 step at constant rate
+  heat_adi           line operators == explicit flux divergence, exact discrete steady state as fixed point,
+                     second-order convergence to the (Richardson-extrapolated) explicit solution, adiabatic energy identity
   nonlinear trajectory on config 1: PARITY UNPINNED beyond oracle-internal cross checks (no printed
                      worked example exists for the config laws; SURVEY.md §8(c) pins table).
 """

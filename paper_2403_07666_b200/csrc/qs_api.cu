@@ -610,6 +610,56 @@ int em_stage(qs_ctx* c, const double* Jsrc, double Bext, double Bdot, double dt_
   return QS_OK;
 }
 
+// Common tail of qs_step / qs_step_rk once J^{k+1} has been written: S6 heat with the current Q, S7 events and step
+// statistics, NaN/Inf check (state restored from the backups on failure), commit of t, I and the statistics.
+// uterm_scale: factor applied to the accumulated multiplier sum (1, or 1/2 for the two stages of the RK pair);
+// reset_scalars: the RK step has consumed the scalar block for its error estimate and needs it cleared first.
+int finish_step(qs_ctx* c, double dt, double I_ramp, int iters, double relres, bool hit_max, double uterm_scale,
+                bool reset_scalars) {
+  const VecCtx& v = c->v;
+  const size_t nb8 = sizeof(double) * c->N;
+  int rc, m = 0;
+  double uterm = 0.0;
+  if (reset_scalars) {
+    uterm = uterm_scale * c->h_sc->uterm;        // read back by the caller's last sync_scalars
+    k_set_scalars(v);
+  }
+  if ((rc = run_heat(c, dt, &m)) != QS_OK) return rc;
+  EventArgs ev;
+  ev.H = c->H; ev.E = c->E; ev.xmax_bits = c->xmax_bits; ev.rmin_bits = c->rmin_bits;
+  ev.Q = c->Q; ev.r = c->r; ev.area = c->area; ev.wire = c->wire;
+  ev.ebar_prev = c->ebar_prev; ev.flags = c->flags; ev.t_first = c->t_first; ev.count = c->count;
+  ev.dt = dt; ev.t_new = c->t + dt; ev.have_prev = c->have_prev_E;
+  c->prof.begin(c->stream);
+  k_events(v, c->mp, ev);
+  k_step_stats(v, c->mp, c->J, c->Jold, c->H, c->Q, c->r, c->area);
+  c->prof.end(c->stream, QS_PROF_EVENTS, c->n_turns ? 2 : 1);
+  if ((rc = sync_scalars(c)) != QS_OK) return rc;
+  if (c->h_sc->nonfinite) {
+    cudaMemcpyAsync(c->J, c->Jold, nb8, cudaMemcpyDeviceToDevice, c->stream);
+    cudaMemcpyAsync(c->H, c->Hold, nb8, cudaMemcpyDeviceToDevice, c->stream);
+    cudaMemcpyAsync(c->x, c->xold, nb8, cudaMemcpyDeviceToDevice, c->stream);
+    cudaStreamSynchronize(c->stream);
+    return fail(QS_ERR_NONFINITE, "NaN/Inf in J or T after the step; state restored");
+  }
+  if (!reset_scalars) uterm = uterm_scale * c->h_sc->uterm;
+  c->t += dt;
+  c->I += dt * I_ramp;
+  c->have_prev_E = true;
+  const int ret = c->h_sc->event_or | (hit_max ? QS_EV_CG_MAXIT : 0);
+  c->st.cg_iters = iters;
+  c->st.cg_relres = relres;
+  c->st.heat_substeps = m;
+  c->st.event_word = ret;
+  c->st.U_terminal = uterm;
+  c->st.Tmax = c->h_sc->tmax;
+  c->st.joule_power = c->h_sc->joule;
+  c->st.dJ_max = c->h_sc->djmax;
+  c->st.t = c->t;
+  c->st.I = c->I;
+  return ret;
+}
+
 // host arrays in caller order <-> device arrays in internal order
 int upload(qs_ctx* c, const double* src, double* dst, int n_pad) {
   for (int k = 0; k < c->N; ++k) c->h_stage[k] = src[c->perm.empty() ? k : c->perm[k]];
@@ -985,41 +1035,8 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
   }
   // S5
   k_scale_div(v, dt, c->x, c->area, c->J);
-  // S6
-  int m = 0;
-  if ((rc = run_heat(c, dt, &m)) != QS_OK) return rc;
-  // S7 + statistics
-  EventArgs ev;
-  ev.H = c->H; ev.E = c->E; ev.xmax_bits = c->xmax_bits; ev.rmin_bits = c->rmin_bits;
-  ev.Q = c->Q; ev.r = c->r; ev.area = c->area; ev.wire = c->wire;
-  ev.ebar_prev = c->ebar_prev; ev.flags = c->flags; ev.t_first = c->t_first; ev.count = c->count;
-  ev.dt = dt; ev.t_new = c->t + dt; ev.have_prev = c->have_prev_E;
-  c->prof.begin(c->stream);
-  k_events(v, c->mp, ev);
-  k_step_stats(v, c->mp, c->J, c->Jold, c->H, c->Q, c->r, c->area);
-  c->prof.end(c->stream, QS_PROF_EVENTS, c->n_turns ? 2 : 1);
-  if ((rc = sync_scalars(c)) != QS_OK) return rc;
-  if (c->h_sc->nonfinite) {
-    cudaMemcpyAsync(c->J, c->Jold, nb8, cudaMemcpyDeviceToDevice, c->stream);
-    cudaMemcpyAsync(c->H, c->Hold, nb8, cudaMemcpyDeviceToDevice, c->stream);
-    restore();
-    return fail(QS_ERR_NONFINITE, "NaN/Inf in J or T after the step; state restored");
-  }
-  c->t += dt;
-  c->I += dt * I_ramp;
-  c->have_prev_E = true;
-  int ret = c->h_sc->event_or | (hit_max ? QS_EV_CG_MAXIT : 0);
-  c->st.cg_iters = iters;
-  c->st.cg_relres = relres;
-  c->st.heat_substeps = m;
-  c->st.event_word = ret;
-  c->st.U_terminal = c->h_sc->uterm;
-  c->st.Tmax = c->h_sc->tmax;
-  c->st.joule_power = c->h_sc->joule;
-  c->st.dJ_max = c->h_sc->djmax;
-  c->st.t = c->t;
-  c->st.I = c->I;
-  return ret;
+  // S6, S7, statistics, commit
+  return finish_step(c, dt, I_ramp, iters, relres, hit_max, 1.0, false);
 }
 
 // Embedded Heun-Euler step with error control (readings: DESIGN.md §3 C14).
@@ -1041,7 +1058,7 @@ int qs_step_rk(qs_ctx* c, double dt_try, double I_ramp, double rtol, double dt_m
     cudaStreamSynchronize(c->stream);
   };
   const double Jref = c->mp.Jc0 * (1.0 - c->lp.T_bath / c->mp.Tc) * (1.0 - c->lp.T_bath / c->mp.Tc);
-  double dt = dt_try, err = 0.0, fac = 2.0, uterm = 0.0;
+  double dt = dt_try, err = 0.0, fac = 2.0;
   int iters = 0, it1 = 0, it2 = 0;
   double rel1 = 0.0, rel2 = 0.0;
   bool hm1 = false, hm2 = false;
@@ -1068,7 +1085,6 @@ int qs_step_rk(qs_ctx* c, double dt_try, double I_ramp, double rtol, double dt_m
     k_max_scaled_diff(v, 0.5 * dt, c->x, I1, c->area);
     if ((rc = sync_scalars(c)) != QS_OK) return rc;
     err = c->h_sc->djmax / Jref;
-    uterm = 0.5 * c->h_sc->uterm;
     iters += it1 + it2;
     fac = err == 0.0 ? 2.0 : std::min(2.0, std::max(0.2, 0.9 * std::sqrt(rtol / err)));
     if (err <= rtol || dt <= dt_min) break;
@@ -1079,37 +1095,8 @@ int qs_step_rk(qs_ctx* c, double dt_try, double I_ramp, double rtol, double dt_m
   k_scale_div(v, 0.5 * dt, I1, c->area, c->J);
   k_scale_div(v, 0.5 * dt, c->x, c->area, c->J);
   k_lincomb(v, 0.5, Q1, 0.5, c->Q);
-  int m = 0;
-  if ((rc = run_heat(c, dt, &m)) != QS_OK) return rc;
-  EventArgs ev;
-  ev.H = c->H; ev.E = c->E; ev.xmax_bits = c->xmax_bits; ev.rmin_bits = c->rmin_bits;
-  ev.Q = c->Q; ev.r = c->r; ev.area = c->area; ev.wire = c->wire;
-  ev.ebar_prev = c->ebar_prev; ev.flags = c->flags; ev.t_first = c->t_first; ev.count = c->count;
-  ev.dt = dt; ev.t_new = c->t + dt; ev.have_prev = c->have_prev_E;
-  k_set_scalars(v);
-  k_events(v, c->mp, ev);
-  k_step_stats(v, c->mp, c->J, c->Jold, c->H, c->Q, c->r, c->area);
-  if ((rc = sync_scalars(c)) != QS_OK) return rc;
-  if (c->h_sc->nonfinite) {
-    cudaMemcpyAsync(c->J, c->Jold, nb8, cudaMemcpyDeviceToDevice, c->stream);
-    cudaMemcpyAsync(c->H, c->Hold, nb8, cudaMemcpyDeviceToDevice, c->stream);
-    restore();
-    return fail(QS_ERR_NONFINITE, "NaN/Inf in J or T after the step; state restored");
-  }
-  c->t += dt;
-  c->I += dt * I_ramp;
-  c->have_prev_E = true;
-  const int ret = c->h_sc->event_or | ((hm1 || hm2) ? QS_EV_CG_MAXIT : 0);
-  c->st.cg_iters = iters;
-  c->st.cg_relres = std::max(rel1, rel2);
-  c->st.heat_substeps = m;
-  c->st.event_word = ret;
-  c->st.U_terminal = uterm;
-  c->st.Tmax = c->h_sc->tmax;
-  c->st.joule_power = c->h_sc->joule;
-  c->st.dJ_max = c->h_sc->djmax;
-  c->st.t = c->t;
-  c->st.I = c->I;
+  const int ret = finish_step(c, dt, I_ramp, iters, std::max(rel1, rel2), hm1 || hm2, 0.5, true);
+  if (ret < 0) return ret;
   if (dt_taken) *dt_taken = dt;
   if (dt_next) *dt_next = dt * fac;
   if (err_out) *err_out = err;

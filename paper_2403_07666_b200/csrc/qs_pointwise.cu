@@ -75,7 +75,7 @@ __device__ __forceinline__ double rcp_fast(double x) {
 }
 // sqrt(a), a >= 0: MUFU seed + one Halley step; exact zero for a == 0
 __device__ __forceinline__ double sqrt_pos(double a) {
-  const double y0 = rsqrt_seed(fmax(a, 1e-300));
+  const double y0 = rsqrt_seed(a + 1e-300);           // a == 0: g = 0 * 1e150 = 0, e = 1, result 0
   const double g = a * y0;
   const double e = fma(-g, y0, 1.0);
   return fma(g * e, fma(0.375, e, 0.5), g);
@@ -131,18 +131,26 @@ struct MaterialConsts {   // host-side reciprocals of the constant divisors (qs_
 };
 
 // Lattice: blockIdx.y strides over radial rows (per-row geometry from rowtab), threads over iz.  Free rings: flat.
+#ifndef QS_MAT_MINB
+#define QS_MAT_MINB 4   // resident CTAs per SM the register budget is sized for (64 registers per thread)
+#endif
 template <bool FROM_ACC, bool AUX, bool EVENTS>
-__global__ void __launch_bounds__(256, 4) material_kernel(MaterialParams mp, MaterialConsts k, MaterialArgs a) {
+__global__ void __launch_bounds__(256, QS_MAT_MINB) material_kernel(MaterialParams mp, MaterialConsts k, MaterialArgs a) {
   const double two_pi = 2.0 * kPi;
-  const int ncol = a.Nz > 0 ? a.Nz : a.N, nrow = a.Nz > 0 ? a.N / a.Nz : 1;
-  const int col0 = blockIdx.x * blockDim.x + threadIdx.x, dcol = gridDim.x * blockDim.x;
+  // one flat cell index for both launch shapes.  Lattice: grid.x covers the columns, blockIdx.y strides over the
+  // radial rows (step = gridDim.y rows; the row index is kept for the per-row table).  Free rings: grid-stride.
+  const bool lat = a.Nz > 0;
+  const int ncol = lat ? a.Nz : a.N;
+  const int col0 = blockIdx.x * blockDim.x + threadIdx.x;
   const unsigned wmask = __ballot_sync(0xffffffffu, col0 < ncol);   // lanes of this warp that own a column
   if (col0 >= ncol) return;
-  constexpr bool ev_on = EVENTS;                        // lattice launches: dcol >= ncol, uniform trips
+  constexpr bool ev_on = EVENTS;                        // lattice launches: uniform trips
   const int tcol = ev_on ? col0 / a.cells_per_side : 0;
-  // software pipeline: the five inputs of the next cell are in flight while the current one is evaluated
+  const long long N = a.N;
+  const long long step = lat ? static_cast<long long>(gridDim.y) * ncol : static_cast<long long>(gridDim.x) * blockDim.x;
+  const int rstep = lat ? gridDim.y : 0;
   struct In { double J, H, b0, b1, s; };
-  auto load = [&](int i) {
+  auto load = [&](long long i) {
     In v;
     v.J = a.J[i];
     v.H = a.H[i];
@@ -151,24 +159,9 @@ __global__ void __launch_bounds__(256, 4) material_kernel(MaterialParams mp, Mat
     v.s = a.jc0_scale ? a.jc0_scale[i] : 1.0;
     return v;
   };
-  int row = blockIdx.y, col = col0;            // cell being evaluated
-  int prow = row, pcol = col;                  // cell being loaded (two ahead)
-  auto advance = [&](int& rr, int& cc) {
-    cc += dcol;
-    if (cc >= ncol) cc = col0, rr += gridDim.y;
-  };
-  In nxt = load(prow * ncol + pcol), nxt2 = nxt;
-  advance(prow, pcol);
-  if (prow < nrow) nxt2 = load(prow * ncol + pcol);
-  while (row < nrow) {
-    const int i = row * ncol + col, row_i = row;
-    const In cur = nxt;
-    nxt = nxt2;
-    advance(row, col);
-    advance(prow, pcol);
-    if (prow < nrow) nxt2 = load(prow * ncol + pcol);
+  auto cell = [&](const long long i, const int row_i, const In& cur) {
     double r, area, selfc, dM, inv_area;
-    if (a.Nz > 0) {
+    if (lat) {
       const double4 t = a.rowtab[row_i];
       r = t.x, selfc = t.y, dM = t.z, area = t.w;
       inv_area = a.inv_area;
@@ -191,10 +184,10 @@ __global__ void __launch_bounds__(256, 4) material_kernel(MaterialParams mp, Mat
     }
     const double eps = J * Bz * r * k.inv_Y;
     const double Bmag = sqrt_pos(fma(Br, Br, Bz * Bz));
-    const double fT = fmax(fma(-T, k.inv_Tc, 1.0), 0.0);
+    const double fT0 = fma(-T, k.inv_Tc, 1.0), fT = fT0 > 0.0 ? fT0 : 0.0;
     const double ae = fabs(eps);
     const double pw = ae > 1e-290 ? pow_small(ae, mp.eps_exp) : 0.0;    // |eps|^eps_exp
-    const double fe = fmax(fma(-mp.eps_coef, pw, 1.0), 0.0);
+    const double fe0 = fma(-mp.eps_coef, pw, 1.0), fe = fe0 > 0.0 ? fe0 : 0.0;
     const double s = cur.s;
     // Jc = num/den and 1/Jc = den/num from one reciprocal of num den
     const double num = mp.Jc0 * s * fT * fT * fe, den = fma(Bmag, k.inv_B0, 1.0);
@@ -255,6 +248,27 @@ __global__ void __launch_bounds__(256, 4) material_kernel(MaterialParams mp, Mat
     const double shift = mp.theta * a.dt * (two_pi * r * dEdJ * inv_area);
     a.shift[i] = shift;
     a.Hd[i] = dM + shift;
+  };
+  // software pipeline, three input slots in rotation: the five inputs of the cell two trips ahead are in flight
+  // while the current one is evaluated (unrolled by three, so that the rotation costs no register moves)
+  long long i = (lat ? static_cast<long long>(blockIdx.y) * ncol : 0) + col0;
+  int row = lat ? blockIdx.y : 0;
+  if (i >= N) return;
+  In s0 = load(i), s1 = s0, s2 = s0;
+  if (i + step < N) s1 = load(i + step);
+  for (;;) {
+    if (i + 2 * step < N) s2 = load(i + 2 * step);
+    cell(i, row, s0);
+    i += step, row += rstep;
+    if (i >= N) break;
+    if (i + 2 * step < N) s0 = load(i + 2 * step);
+    cell(i, row, s1);
+    i += step, row += rstep;
+    if (i >= N) break;
+    if (i + 2 * step < N) s1 = load(i + 2 * step);
+    cell(i, row, s2);
+    i += step, row += rstep;
+    if (i >= N) break;
   }
 }
 
@@ -672,7 +686,7 @@ void k_material(const VecCtx& v, const MaterialParams& mp, const MaterialArgs& a
   if (a.Nz > 0) {   // 2-D: no integer division per cell
     const int nrow = a.N / a.Nz;
     grid.x = (a.Nz + kBlock - 1) / kBlock;
-    grid.y = std::min(nrow, std::max(1, 8 * g_sm_count / static_cast<int>(grid.x)));
+    grid.y = std::min(nrow, std::max(1, 2 * QS_MAT_MINB * g_sm_count / static_cast<int>(grid.x)));
   }
   const bool ev = a.xmax_bits != nullptr, aux = a.dEdJ != nullptr;
 #define QS_MAT(F_, A_, E_) material_kernel<F_, A_, E_><<<grid, kBlock, 0, v.stream>>>(mp, k, a)

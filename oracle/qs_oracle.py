@@ -25,6 +25,9 @@ Pins (tests/test_oracle_*.py, all ``-m "not gpu"``):
                      rejection rule, reduction to the theta = 0 step at constant rate
   heat_adi           line operators == explicit flux divergence, exact discrete steady state as fixed point,
                      second-order convergence to the (Richardson-extrapolated) explicit solution, adiabatic energy identity
+  group shares (C16) null-space solve of the constrained system (route independent of the KKT/Schur one), group net
+                     currents = share * I(t) along a trajectory, U_terminal * I_ramp == power delivered to the groups,
+                     share = 1 reproduces the per-turn results bit for bit
   nonlinear trajectory on config 1: PARITY UNPINNED beyond oracle-internal cross checks (no printed
                      worked example exists for the config laws; SURVEY.md §8(c) pins table).
 """
@@ -539,6 +542,9 @@ class Oracle:
         else:
             raise ValueError(operator)
         self.C = constraint_matrix(geo) if (solver == "cholesky" and operator == "dense") else None
+        # C16 (PAPER.md:61-67 sub-elements): group w carries share_w of the transport current; default 1 (wires in series)
+        sh = getattr(geo, "turn_share", None)
+        self.share = np.ones(geo.n_turns) if sh is None else np.asarray(sh, dtype=np.float64)
         self.J = np.zeros(N)
         self.T = np.full(N, geo.T_bath)
         self.H = enthalpy(mat, self.T)
@@ -613,7 +619,7 @@ class Oracle:
         b = -2.0 * math.pi * geo.r * (ml["E"] + 0.5 * geo.r * Bdot)
         D = 2.0 * math.pi * geo.r * ml["dEdJ"] / a
         shift = mat.theta * dt * D
-        d = np.full(geo.n_turns, float(I_ramp))
+        d = float(I_ramp) * self.share                       # C^T I' = share * I_ramp (C16)
         # S3/S4 constrained solve (C7: linearly implicit theta step)
         if self.solver == "cholesky":
             A = self.M + np.diag(shift)
@@ -634,7 +640,7 @@ class Oracle:
         self.Br, self.Bz, self.E = Br, Bz, ml["E"]
         # S7 events: T^{k+1}; E, |J|/Jc, rho of the material evaluation of this step
         ret = self._events(dt, Jold, ml) if geo.n_turns else 0
-        self.stats = dict(cg_iters=iters, cg_relres=relres, U_terminal=float(-V.sum()),
+        self.stats = dict(cg_iters=iters, cg_relres=relres, U_terminal=float(-(self.share @ V)),
                           Tmax=float(self.T.max()),
                           joule_power=float(np.sum(ml["Q"] * 2.0 * math.pi * geo.r * a)),
                           boundary_energy=lost, heat_substeps=m)
@@ -652,7 +658,7 @@ class Oracle:
         Bz = Bz + self.Bext(t_stage)
         ml = material_law(mat, J, T, Br, Bz, geo.r, self.scale)
         b = -2.0 * math.pi * geo.r * (ml["E"] + 0.5 * geo.r * Bdot)
-        d = np.full(geo.n_turns, float(I_ramp))
+        d = float(I_ramp) * self.share                       # C^T I' = share * I_ramp (C16)
         if self.solver == "cholesky":
             if getattr(self, "_cfM", None) is None:
                 self._cfM = scipy.linalg.cho_factor(self.M, lower=True)       # M is constant: factor once
@@ -702,7 +708,7 @@ class Oracle:
         ml_ev = dict(ml2)
         ml_ev["Q"] = Q
         ret = self._events(dt, Jstar, ml_ev) if geo.n_turns else 0
-        self.stats = dict(cg_iters=0, cg_relres=0.0, U_terminal=float(-0.5 * (V1.sum() + V2.sum())),
+        self.stats = dict(cg_iters=0, cg_relres=0.0, U_terminal=float(-0.5 * (self.share @ V1 + self.share @ V2)),
                           Tmax=float(self.T.max()), joule_power=float(np.sum(Q * 2.0 * math.pi * geo.r * a)),
                           boundary_energy=lost, heat_substeps=m)
         return int(ret), dt, dt * fac, err

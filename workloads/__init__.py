@@ -40,6 +40,7 @@ class Geometry:
     Bext0: float = 0.0
     Bext_rate: float = 0.0
     Bext_max: float = 0.0
+    turn_share: Optional[np.ndarray] = None  # [n_turns] share of the transport current per constraint group (NULL = 1)
 
     @property
     def n_rings(self) -> int:
@@ -189,3 +190,30 @@ def sample_rows(n: int, count: int, seed: int) -> np.ndarray:
     """Seeded, sorted, distinct target rows for sampled parity at sizes the oracle cannot sweep."""
     g = np.random.default_rng(seed)
     return np.sort(g.choice(n, size=min(count, n), replace=False)).astype(np.int64)
+
+
+def subelements(geo: Geometry, per_side: int, share: str = "uniform") -> Geometry:
+    """The same lattice with every wire cut into per_side x per_side square sub-elements, each a constraint group of its
+    own ("each wire has N_sub subelements").  Group id = wire * per_side^2 +
+    (row block) * per_side + (column block), in the canonical wire order.  share: "uniform" -> every sub-element
+    carries 1/per_side^2 of the wire's transport current; "outer" -> only the sub-elements on the wire's rim carry it
+    (equal parts), the inner ones are zero-net-current groups.  Pure index bookkeeping: no method arithmetic."""
+    n, s = geo.cells_per_side, int(per_side)
+    if not geo.lattice or s <= 0 or n % s:
+        raise ValueError("subelements: lattice geometry with cells_per_side divisible by per_side expected")
+    Nr, Nz, m = geo.Nr, geo.Nz, n // s
+    ir, iz = np.divmod(np.arange(Nr * Nz), Nz)
+    wire = (ir // n) * geo.turns_per_layer + iz // n
+    br, bz = (ir % n) // m, (iz % n) // m
+    gid = (wire * (s * s) + br * s + bz).astype(np.int32)
+    n_groups = geo.layers * geo.turns_per_layer * s * s
+    kb = np.arange(s * s)
+    rim = ((kb // s == 0) | (kb // s == s - 1) | (kb % s == 0) | (kb % s == s - 1)).astype(np.float64)
+    if share == "uniform":
+        per_wire = np.full(s * s, 1.0 / (s * s))
+    elif share == "outer":
+        per_wire = rim / rim.sum()
+    else:
+        raise ValueError("share: 'uniform' or 'outer'")
+    return dataclasses.replace(geo, turn_id=gid, n_turns=n_groups,
+                               turn_share=np.tile(per_wire, geo.layers * geo.turns_per_layer))

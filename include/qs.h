@@ -82,6 +82,13 @@ typedef struct {
   double   Bext0, Bext_rate, Bext_max; /* axial background field B_ext(t) = min(Bext0 + rate t, max);
                                        rate == 0: constant Bext0                                  */
   int32_t  flags;                   /* QS_GEO_*                                                  */
+  const double *turn_share;         /* [n_turns] share of the transport current each constraint group carries
+                                       (C16; PAPER.md:61-67 sub-elements): the constraint is
+                                       sum_{i in group w} I'_i = turn_share[w] * I_ramp, and U_terminal =
+                                       -sum_w turn_share[w] V_w.  NULL = 1 for every group (wires in series).
+                                       Sub-elements of a wire are groups of their own (turn_id = sub-element id)
+                                       with shares summing to 1 per wire; share 0 = zero-net-current group
+                                       (uncoupled sub-element under a field ramp).  Must be finite.          */
 } qs_geometry;
 
 typedef struct {

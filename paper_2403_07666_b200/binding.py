@@ -26,7 +26,7 @@ class QsGeometry(C.Structure):
                 ("wire_size", C.c_double), ("r_inner", C.c_double), ("softening", C.c_double),
                 ("h_conv", C.c_double * 4), ("T_bath", C.c_double),
                 ("Bext0", C.c_double), ("Bext_rate", C.c_double), ("Bext_max", C.c_double),
-                ("flags", C.c_int32)]
+                ("flags", C.c_int32), ("turn_share", c_double_p)]
 
 
 class QsMaterial(C.Structure):
@@ -189,6 +189,11 @@ class QS:
         g.T_bath = float(geometry.T_bath)
         g.Bext0, g.Bext_rate, g.Bext_max = float(geometry.Bext0), float(geometry.Bext_rate), float(geometry.Bext_max)
         g.flags = (1 if no_operator else 0) | (2 if lattice_tables else 0)
+        share = getattr(geometry, "turn_share", None)
+        if share is not None and self.n_turns > 0:
+            sh = _f64(share, self.n_turns)
+            self._keep.append(sh)
+            g.turn_share = _dp(sh)
         m = QsMaterial()
         for name, _ in QsMaterial._fields_:
             if name == "jc0_scale":

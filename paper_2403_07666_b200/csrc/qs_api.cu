@@ -132,6 +132,7 @@ struct qs_ctx {
   size_t acc_bytes = 0;
   double *sw, *swM, *vw, *vsum, *tw, *defw, *ebar_prev, *t_first;
   double* wire = nullptr;            // [9][n_turns] per-wire statistics (f3)
+  double* share = nullptr;           // [n_turns] transport-current share of each constraint group (C16)
   int *flags, *count, *turn_ptr, *turn_idx, *turn_id, *d_perm;
   int* rowturn = nullptr;            // [Nr] (ir / n) * turns_per_layer
   unsigned long long *xmax_bits = nullptr, *rmin_bits = nullptr;   // [n_turns] event observables of the material pass
@@ -220,6 +221,7 @@ void carve(qs_ctx* c, void* base, size_t* total) {
   c->ebar_prev = k.take<double>(nt);
   c->t_first = k.take<double>(nt);
   c->wire = k.take<double>(9 * nt);
+  c->share = k.take<double>(nt);
   c->flags = k.take<int>(nt);
   c->count = k.take<int>(nt);
   c->turn_ptr = k.take<int>(nt + 1);
@@ -249,6 +251,9 @@ int check_geometry(const qs_geometry* g) {
   if (!g || g->n_rings <= 0 || !g->r || !g->z || !g->area) return fail(QS_ERR_ARG, "geometry: NULL array or n_rings <= 0");
   if (g->n_turns < 0 || (g->n_turns > 0 && !g->turn_id)) return fail(QS_ERR_ARG, "geometry: n_turns without turn_id");
   if (!(g->softening > 0.0)) return fail(QS_ERR_ARG, "geometry: softening must be > 0");
+  if (g->turn_share)
+    for (int w = 0; w < g->n_turns; ++w)
+      if (!std::isfinite(g->turn_share[w])) return fail(QS_ERR_ARG, "geometry: turn_share must be finite");
   if (g->lattice) {
     if (g->layers <= 0 || g->turns_per_layer <= 0 || g->cells_per_side <= 0 || !(g->wire_size > 0.0))
       return fail(QS_ERR_ARG, "geometry: bad lattice description");
@@ -810,7 +815,7 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
   c->Halt = c->Hb;
   VecCtx& v = c->v;
   v.N = N; v.Np = c->Np; v.n_turns = c->n_turns;
-  v.turn_id = c->turn_id; v.turn_ptr = c->turn_ptr; v.turn_idx = c->turn_idx;
+  v.turn_id = c->turn_id; v.turn_ptr = c->turn_ptr; v.turn_idx = c->turn_idx; v.share = c->share;
   v.stream = c->stream; v.sc = c->sc; v.launches = &c->launches;
 
   // geometry arrays in internal order, padded with far-away dummy rings that carry no current
@@ -867,8 +872,10 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
     }
     std::vector<int> fill(ptr.begin(), ptr.end() - 1);
     for (int k = 0; k < N; ++k) idx[fill[tid[k]]++] = k;
-    std::vector<double> tf(c->n_turns, -1.0);
-    if (cudaMemcpyAsync(c->turn_id, tid.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+    std::vector<double> tf(c->n_turns, -1.0), sh(c->n_turns, 1.0);
+    if (geo->turn_share) sh.assign(geo->turn_share, geo->turn_share + c->n_turns);
+    if (cudaMemcpyAsync(c->share, sh.data(), sizeof(double) * c->n_turns, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+        cudaMemcpyAsync(c->turn_id, tid.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
         cudaMemcpyAsync(c->turn_ptr, ptr.data(), sizeof(int) * (c->n_turns + 1), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
         cudaMemcpyAsync(c->turn_idx, idx.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
         cudaMemcpyAsync(c->t_first, tf.data(), sizeof(double) * c->n_turns, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
@@ -936,12 +943,10 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
       ++c->launches;
     }
     if (c->n_turns) {
-      // unit-ramp particular solution x_p1 = H_M^-1 C (1/s_M) and M x_p1 (reference norm of the CG, C8)
+      // unit-ramp particular solution x_p1 = H_M^-1 C (share/s_M) and M x_p1 (reference norm of the CG, C8, C16)
       k_turn_schur(v, c->diagM, c->swM);
-      std::vector<double> ones(c->n_turns, 1.0);
-      if (cudaMemcpyAsync(c->defw, ones.data(), sizeof(double) * c->n_turns, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
-          cudaStreamSynchronize(c->stream) != cudaSuccess)
-        return bail(fail(QS_ERR_CUDA, "upload"));
+      if (cudaMemcpyAsync(c->defw, c->share, sizeof(double) * c->n_turns, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
+        return bail(fail(QS_ERR_CUDA, "copy"));
       k_apply_deficit(v, c->defw, c->diagM, c->swM, c->xp1);
       if (cudaMemcpyAsync(c->p, c->xp1, sizeof(double) * N, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
         return bail(fail(QS_ERR_CUDA, "copy"));

@@ -86,6 +86,7 @@ struct VecCtx {
   const int* turn_id;    // [N] (internal order)
   const int* turn_ptr;   // [n_turns+1] CSR of cells per turn
   const int* turn_idx;   // [N]
+  const double* share;   // [n_turns] share of the transport current per constraint group (C16)
   cudaStream_t stream;
   Scalars* sc;
   long long* launches;   // host counter

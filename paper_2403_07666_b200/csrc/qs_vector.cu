@@ -112,13 +112,14 @@ __global__ void turn_schur_kernel(int n_turns, const int* __restrict__ ptr, cons
 }
 
 __global__ void turn_deficit_kernel(int n_turns, const int* __restrict__ ptr, const int* __restrict__ idx,
-                                    const double* __restrict__ x, double d, double* __restrict__ defw, Scalars* sc) {
+                                    const double* __restrict__ share, const double* __restrict__ x, double d,
+                                    double* __restrict__ defw, Scalars* sc) {
   const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (w >= n_turns) return;
   double acc = 0.0;
   for (int k = ptr[w] + lane; k < ptr[w + 1]; k += 32) acc += x[idx[k]];
   acc = warp_sum(acc);
-  if (lane == 0) defw[w] = d - acc;
+  if (lane == 0) defw[w] = fma(d, share[w], -acc);        // C16: group w carries share_w of the ramp
 }
 
 __global__ void apply_deficit_kernel(int n, const int* __restrict__ turn, const double* __restrict__ defw,
@@ -203,9 +204,9 @@ __global__ void nu_residual_kernel(int n, double I_ramp, const double* __restric
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
     r[i] = I_ramp * fma(shift[i], xp1[i], Mxp1[i]) - rhs_at(b, i);
 }
-__global__ void sum_uterm_kernel(int n, const double* __restrict__ vsum, Scalars* sc) {
-  double acc = 0.0;
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) acc += vsum[i];
+__global__ void sum_uterm_kernel(int n, const double* __restrict__ share, const double* __restrict__ vsum, Scalars* sc) {
+  double acc = 0.0;                                          // U_terminal = -sum_w share_w V_w (C16)
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) acc = fma(share[i], vsum[i], acc);
   block_atomic_sum(acc, &sc->uterm);
 }
 __global__ void gather_kernel(int n, int npad, const double* __restrict__ src, const int* __restrict__ perm,
@@ -357,7 +358,8 @@ void k_turn_deficit(const VecCtx& v, const double* x, double d, double* defw) {
   if (!v.n_turns) return;
   QS_LAUNCH(v);
   turn_deficit_kernel<<<(v.n_turns * 32 + kBlock - 1) / kBlock, kBlock, 0, v.stream>>>(v.n_turns, v.turn_ptr,
-                                                                                      v.turn_idx, x, d, defw, v.sc);
+                                                                                      v.turn_idx, v.share, x, d, defw,
+                                                                                      v.sc);
 }
 void k_apply_deficit(const VecCtx& v, const double* defw, const double* Hd, const double* sw, double* x) {
   if (!v.n_turns) return;
@@ -435,7 +437,7 @@ void k_nu_residual(const VecCtx& v, double I_ramp, const double* Mxp1, const dou
 void k_sum_uterm(const VecCtx& v, const double* vsum) {
   if (!v.n_turns) return;
   QS_LAUNCH(v);
-  sum_uterm_kernel<<<1, kBlock, 0, v.stream>>>(v.n_turns, vsum, v.sc);
+  sum_uterm_kernel<<<1, kBlock, 0, v.stream>>>(v.n_turns, v.share, vsum, v.sc);
 }
 void k_gather(const VecCtx& v, const double* src, const int* perm, double* dst, int n, int npad) {
   QS_LAUNCH(v);

@@ -36,8 +36,7 @@ __device__ __forceinline__ double rsqrt_fast(double x) {
   const double t = x * y;
   const double e = fma(-t, y, 1.0);
   const double q = fma(0.375, e, 0.5);
-  const double ye = y * e;
-  return fma(ye, q, y);
+  return y * fma(q, e, 1.0);                  // y (1 + e/2 + 3 e^2/8); no multiply-add has three register operands
 }
 
 struct PairAGM {
@@ -62,10 +61,11 @@ __device__ __forceinline__ PairAGM agm_pair(double A2, double B2) {
     const double g = w * y0;                  // ~ sqrt(w)
     const double e = fma(-g, y0, 1.0);        // 1 - w y0^2
     const double q = fma(0.375, e, 0.5);
-    const double p = fma(g * e, q, g);        // sqrt(w) = g (1 + e/2 + 3 e^2/8)
+    const double zc = fma(q, e, 1.0);         // 1 + e/2 + 3 e^2/8
+    const double p = g * zc;                  // sqrt(w)
     const double s = u + v;
     if (FIELD && n == 0) {
-      const double y = fma(y0 * e, q, y0);    // 1/sqrt(w)
+      const double y = y0 * zc;               // 1/sqrt(w)
       o.y0sq = y * y;
       o.mid = 0.5 * s;
     }
@@ -89,7 +89,7 @@ __device__ __forceinline__ PairAGM agm_pair(double A2, double B2) {
     F = fma(fma(25.0 / 256.0, delta, 9.0 / 64.0), delta, 0.25);
     G = fma(fma(c2N * (41.0 / 2048.0), delta, c2N / 32.0), delta, c2N / 16.0);
   }
-  o.yinf = fma(y * delta, F, y);              // y (1 + delta/4 + 9 delta^2/64 + ...)
+  o.yinf = y * fma(delta, F, 1.0);            // y (1 + delta/4 + 9 delta^2/64 + ...)
   o.S = fma(d * delta, G, S);                 // + 2^NIT u (delta^2/16 + delta^3/32 + ...)
   return o;
 }

@@ -31,7 +31,18 @@ __device__ __constant__ double kClassKp2Min[kNumClasses] = {0.3965,   0.1394,   
 //                                                class:      0       1       2       3       4       5       6       7       8       9
 //                                                (NIT,HI): (2,lo)  (2,hi)  (3,lo)  (3,hi)  (4,lo)  (4,hi)  (5,lo)  (5,hi)  (6,lo)  (7,lo)
 
-constexpr int kWarpsPerCta = 8;
+#ifndef QS_SW_WARPS
+#define QS_SW_WARPS 4          // warps per CTA of the pair sweeps (small CTAs: finer register-budget steps)
+#endif
+#ifndef QS_SW_MINB_FIELD
+#define QS_SW_MINB_FIELD 5     // resident CTAs per SM the register budget of the fused sweep is sized for: 20 warps
+                               // at <= 102 registers (96 used).  Measured on config 2: 8x2 (112 regs) 108.8 ms,
+                               // 4x5 102.7 ms, 8x3 (80 regs) 103.9 ms, 4x6 (80 regs) 104.2 ms
+#endif
+#ifndef QS_SW_MINB_M
+#define QS_SW_MINB_M 6         // the same for the M-only sweep: 24 warps at 80 registers (8x3 and 4x6 time alike)
+#endif
+constexpr int kWarpsPerCta = QS_SW_WARPS;
 constexpr int kThreads = kWarpsPerCta * 32;
 constexpr int kMaxArrays = 4;
 
@@ -164,7 +175,7 @@ __device__ __forceinline__ void unrank(long long k, int nb, int& bi, int& bj) {
 }
 
 template <bool FIELD>
-__global__ void __launch_bounds__(kThreads, FIELD ? 2 : 3) sweep_kernel(SweepParams prm) {
+__global__ void __launch_bounds__(kThreads, FIELD ? QS_SW_MINB_FIELD : QS_SW_MINB_M) sweep_kernel(SweepParams prm) {
   constexpr int NA = FIELD ? 4 : 3;
   __shared__ __align__(128) double sbuf[kWarpsPerCta][2][kMaxArrays][64];   // every array twice: no wrap of lane + s
   __shared__ __align__(8) uint64_t sbar[kWarpsPerCta][2];
@@ -558,7 +569,7 @@ cudaError_t issue_probe(int mode, double* cycles_per_dfma) {
   return cudaSuccess;
 }
 
-int sweep_grid(int sm_count, bool field) { return sm_count * (field ? 2 : 3); }
+int sweep_grid(int sm_count, bool field) { return sm_count * (field ? QS_SW_MINB_FIELD : QS_SW_MINB_M); }
 
 cudaError_t launch_sweep(const SweepParams& prm, bool field, int grid, cudaStream_t stream) {
   if (field)

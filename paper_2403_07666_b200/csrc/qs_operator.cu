@@ -40,8 +40,13 @@ __device__ __constant__ double kClassKp2Min[kNumClasses] = {0.3965,   0.1394,   
                                // 4x5 102.7 ms, 8x3 (80 regs) 103.9 ms, 4x6 (80 regs) 104.2 ms
 #endif
 #ifndef QS_SW_MINB_M
-#define QS_SW_MINB_M 6         // the same for the M-only sweep: 24 warps at 80 registers (8x3 and 4x6 time alike)
+#define QS_SW_MINB_M 7         // the same for the M-only sweep: 28 warps at 72 registers.  N = 262,144: 4x6 / 8x3
+                               // (80 regs) 113.1 ms, 4x7 112.1 ms, 8x4 (64 regs) 114.8 ms, 4x5 (96 regs) 117.4 ms
 #endif
+#ifndef QS_SW_UNROLL
+#define QS_SW_UNROLL 2         // source steps unrolled in the off-diagonal item loop (1: +3 %, 4: +17 % on K2)
+#endif
+constexpr int kSweepUnroll = QS_SW_UNROLL;
 constexpr int kWarpsPerCta = QS_SW_WARPS;
 constexpr int kThreads = kWarpsPerCta * 32;
 constexpr int kMaxArrays = 4;
@@ -72,7 +77,7 @@ __device__ __forceinline__ void item_offdiag(const TargetRegs& t, const double* 
   const double difu = t.r - rju, dif2u = difu * difu, c4u = ri4 * rju, eu = fma(rju, rju, -ri2);
   const double dif2s = dif2u + soft_all;
   sr += lane, sz += lane, sx += lane, sc += lane;   // arrays are stored twice: entry lane + s = source (lane + s) & 31
-#pragma unroll 2
+#pragma unroll kSweepUnroll
   for (int s = 0; s < 32; ++s) {
     const int jl = s;
     const double zj = sz[jl], xj = sx[jl];

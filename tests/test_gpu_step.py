@@ -357,3 +357,22 @@ def test_energy_balance_of_whole_steps_on_the_gpu(pkg):
     dH = qo.enthalpy(mat, T1) - qo.enthalpy(mat, T0)
     assert total > 0 and abs(np.sum(V * dH) - total) <= 1e-9 * total
     assert abs(ws["E_joule"].sum() - total) <= 1e-9 * total          # per-wire energies add up to the same integral
+
+
+@pytest.mark.parametrize("tables", [False, True])
+def test_nonlinear_trajectory_ends_in_the_closed_form_saturated_state_on_the_gpu(pkg, tables):
+    # not an oracle comparison: the CUDA path against the closed form of the stationary saturated state under a steady
+    # field ramp (2 pi r E = -pi r^2 Bdot - V_w, J = Jc sgn(E) (|E|/Ec)^(1/n), V_w from sum a J = 0 per turn), which
+    # tests/test_oracle_solver_step.py derives and pins the oracle with.  Both operators.
+    from test_oracle_solver_step import saturated_state, saturation_workload
+    w = saturation_workload(layers=2, turns=2, n=8)
+    geo, mat = w.geometry, dataclasses.replace(w.material, cg_tol=1e-12)
+    Js, Es, Us = saturated_state(geo, mat, np.asarray(mat.jc0_scale), geo.Bext_rate)
+    with pkg.QS(geo, mat, lattice_tables=tables) as sim:
+        for k in range(w.steps):
+            assert sim.step(w.dt, 0.0) >= 0
+        J, T, B, E = sim.read()
+        st = sim.stats()
+    assert rel(J, Js) < 1e-9, rel(J, Js)
+    assert rel(E, Es) < 1e-8, rel(E, Es)
+    assert abs(st["U_terminal"] - Us.sum()) < 1e-8 * abs(Us.sum())

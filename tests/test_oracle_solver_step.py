@@ -293,3 +293,58 @@ def test_heun_euler_equals_explicit_euler_when_the_rate_is_constant():
         assert taken == w.dt and err <= 1e-12 and nxt == 2 * w.dt
     assert np.max(np.abs(a_.J - b_.J)) <= 1e-12 * np.max(np.abs(a_.J))
     assert abs(a_.stats["U_terminal"] - b_.stats["U_terminal"]) <= 1e-9 * abs(a_.stats["U_terminal"])
+
+
+def saturated_state(geo, mat, scale, Bdot):
+    """Stationary state of the nonlinear problem under a steady field ramp, written out from Faraday's law.
+
+    Once the flux front has crossed the wire and dI/dt = 0, C4 reads 2 pi r E = -pi r^2 Bdot - V_w on every ring of
+    turn w (no inductive term left), the power law inverted gives J = Jc sgn(E) (|E|/Ec)^(1/n), and V_w is the root
+    of the turn's net-current condition sum a J = 0 (I = 0 throughout).  Constant Jc (no field, temperature or strain
+    dependence) and rho_n -> infinity make this exact.  Returns J, E and the turn voltages U_w = -V_w.
+    """
+    from scipy.optimize import brentq
+    r, a = geo.r, geo.area
+    Jc = mat.Jc0 * scale
+    J, E, U = np.zeros_like(r), np.zeros_like(r), np.zeros(geo.n_turns)
+    for w in range(geo.n_turns):
+        m = geo.turn_id == w
+
+        def state(V):
+            e = -0.5 * r[m] * Bdot - V / (2 * math.pi * r[m])
+            return Jc[m] * np.sign(e) * (np.abs(e) / mat.Ec) ** (1.0 / mat.n_exp), e
+
+        lo, hi = sorted((-math.pi * r[m].max() ** 2 * Bdot, -math.pi * r[m].min() ** 2 * Bdot))
+        V = brentq(lambda v: float(np.sum(a[m] * state(v)[0])), lo, hi, xtol=1e-300, rtol=1e-15)
+        J[m], E[m] = state(V)
+        U[w] = -V
+    return J, E, U
+
+
+def saturation_workload(layers=1, turns=2, n=6, Bdot=10.0):
+    # weak pinning (Jc0 = 1e8 A/m^2: full penetration at mu0 Jc s/2 = 0.06 T) and a constant Jc per cell
+    return wl.lattice_workload("saturation", layers, turns, n, 1e-3, 30e-3, 5e-5, 0.0, 400, 7, 0.01,
+                               Bext_rate=Bdot, Bext_max=1e9, Jc0=1e8, B0=1e30, Tc=1e30, eps_coef=0.0, rho_n=1e6)
+
+
+def test_nonlinear_trajectory_ends_in_the_closed_form_saturated_state():
+    # pins the nonlinear step as a whole (sign and factor of the rhs, A_ext term, power law, per-turn constraint,
+    # sign of the turn voltage): a dropped 1/2, a wrong sign or a transposed index moves the fixed point
+    w = saturation_workload()
+    geo, mat = w.geometry, w.material
+    for op, solver in [("dense", "cholesky"), ("tables", "pcg")]:
+        o = qo.Oracle(geo, dataclasses.replace(mat, cg_tol=1e-13), operator=op, solver=solver)
+        Js, Es, Us = saturated_state(geo, mat, o.scale, geo.Bext_rate)
+        errs = []
+        for k in range(w.steps):
+            assert o.step(w.dt, 0.0) >= 0
+            errs.append(np.linalg.norm(o.J - Js) / np.linalg.norm(Js))
+        assert errs[49] > 1e-2 > errs[149]                        # the front is still moving early on
+        assert errs[-1] < 1e-11, errs[-1]
+        assert np.linalg.norm(o.E - Es) < 1e-10 * np.linalg.norm(Es)
+        assert abs(o.stats["U_terminal"] - Us.sum()) < 1e-10 * abs(Us.sum())
+        cur = np.bincount(geo.turn_id, weights=geo.area * o.J)
+        assert np.max(np.abs(cur)) < 1e-12 * np.sum(np.abs(geo.area * o.J))
+        # the saturated wire is the Bean profile lifted by the power law: |J|/Jc = (|E|/Ec)^(1/n), |E| <~ s Bdot / 2
+        x = np.abs(o.J) / (mat.Jc0 * o.scale)
+        assert 0.5 < x.min() and x.max() < (0.5 * geo.wire_size * geo.Bext_rate / mat.Ec) ** (1 / mat.n_exp) * 1.01

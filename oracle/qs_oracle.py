@@ -28,8 +28,12 @@ Pins (tests/test_oracle_*.py, all ``-m "not gpu"``):
   group shares (C16) null-space solve of the constrained system (route independent of the KKT/Schur one), group net
                      currents = share * I(t) along a trajectory, U_terminal * I_ramp == power delivered to the groups,
                      share = 1 reproduces the per-turn results bit for bit
-  nonlinear trajectory on config 1: PARITY UNPINNED beyond oracle-internal cross checks (no printed
-                     worked example exists for the config laws; SURVEY.md §8(c) pins table).
+  nonlinear step     the trajectory under a steady field ramp ends in the stationary saturated state, which has a
+                     closed form (2 pi r E = -pi r^2 Bdot - V_w, J = Jc sgn(E) (|E|/Ec)^(1/n), V_w from the turn's
+                     zero net current): J, E, U_terminal to 1e-11 with both operator/solver routes
+  nonlinear TRANSIENT on config 1 (the moving flux front before saturation): PARITY UNPINNED beyond
+                     oracle-internal cross checks (no printed worked example exists for the config laws;
+                     SURVEY.md §8(c) pins table).
 """
 from __future__ import annotations
 

@@ -132,7 +132,7 @@ struct MaterialConsts {   // host-side reciprocals of the constant divisors (qs_
 
 // Lattice: blockIdx.y strides over radial rows (per-row geometry from rowtab), threads over iz.  Free rings: flat.
 #ifndef QS_MAT_MINB
-#define QS_MAT_MINB 4   // resident CTAs per SM the register budget is sized for (64 registers per thread)
+#define QS_MAT_MINB 6   // resident CTAs per SM the register budget is sized for (40 registers per thread)
 #endif
 template <bool FROM_ACC, bool AUX, bool EVENTS>
 __global__ void __launch_bounds__(256, QS_MAT_MINB) material_kernel(MaterialParams mp, MaterialConsts k, MaterialArgs a) {
@@ -249,27 +249,13 @@ __global__ void __launch_bounds__(256, QS_MAT_MINB) material_kernel(MaterialPara
     a.shift[i] = shift;
     a.Hd[i] = dM + shift;
   };
-  // software pipeline, three input slots in rotation: the five inputs of the cell two trips ahead are in flight
-  // while the current one is evaluated (unrolled by three, so that the rotation costs no register moves)
+  // No software pipeline: one cell per trip, memory latency is covered by occupancy (40 registers, 6 CTAs = 48 warps per
+  // SM).  Measured on 16.8 M cells (B200, material_kernel<0,0,1>): this loop at 6 / 7 / 8 CTAs per SM 0.219 ms, at 5
+  // (44 registers) 0.229 ms; inputs prefetched one cell ahead at 64 registers 0.248 ms; two cells ahead (64 registers,
+  // 68 B of spills) 0.260 ms, at 80 registers 0.287 ms.
   long long i = (lat ? static_cast<long long>(blockIdx.y) * ncol : 0) + col0;
   int row = lat ? blockIdx.y : 0;
-  if (i >= N) return;
-  In s0 = load(i), s1 = s0, s2 = s0;
-  if (i + step < N) s1 = load(i + step);
-  for (;;) {
-    if (i + 2 * step < N) s2 = load(i + 2 * step);
-    cell(i, row, s0);
-    i += step, row += rstep;
-    if (i >= N) break;
-    if (i + 2 * step < N) s0 = load(i + 2 * step);
-    cell(i, row, s1);
-    i += step, row += rstep;
-    if (i >= N) break;
-    if (i + 2 * step < N) s1 = load(i + 2 * step);
-    cell(i, row, s2);
-    i += step, row += rstep;
-    if (i >= N) break;
-  }
+  for (; i < N; i += step, row += rstep) cell(i, row, load(i));
 }
 
 __global__ void rowtab_kernel(int Nr, int Nz, const double* __restrict__ r, const double* __restrict__ selfcoef,
@@ -405,7 +391,14 @@ __global__ void __launch_bounds__(kHeatWarps * 32, 3) heat_kernel(MaterialParams
 // ---- K6, TMA-pipelined variant (Nz even): same marching scheme, but every warp streams its 512-byte row segments
 // of H and Q through a ring of kHeatStages shared-memory stages with TMA bulk copies (cp.async.bulk + mbarrier,
 // issued by lane 0), so that kHeatStages rows per warp are in flight whatever the register budget.
-constexpr int kHeatStages = 8;
+#ifndef QS_HEAT_STAGES
+#define QS_HEAT_STAGES 8
+#endif
+#ifndef QS_HEAT_MINB
+#define QS_HEAT_MINB 3
+#endif
+constexpr int kHeatStages = QS_HEAT_STAGES;
+constexpr int kHeatMinB = QS_HEAT_MINB;   // resident CTAs per SM the registers and the shared-memory ring are sized for
 struct HeatStage {
   double h[64];
   double q[64];
@@ -416,7 +409,7 @@ struct HeatSmem {
   uint64_t bar[kHeatWarps][kHeatStages];
 };
 
-__global__ void __launch_bounds__(kHeatWarps * 32, 3) heat_tma_kernel(MaterialParams mp, LatticeParams lp,
+__global__ void __launch_bounds__(kHeatWarps * 32, kHeatMinB) heat_tma_kernel(MaterialParams mp, LatticeParams lp,
                                                                       int rows_per_cta, const double* __restrict__ Hin,
                                                                       const double* __restrict__ Q,
                                                                       double* __restrict__ Hout, double dtsub) {
@@ -459,59 +452,62 @@ __global__ void __launch_bounds__(kHeatWarps * 32, 3) heat_tma_kernel(MaterialPa
     bulk_g2s(&s.h[soff], Hin + off, seg_bytes, b);
     if (needq) bulk_g2s(&s.q[soff], Q + off, seg_bytes, b);
   };
-  auto take = [&](int t, double2& h, double2& q) {   // waits for stage t and copies this lane's column pair out
-    h = make_double2(0.0, 0.0);
-    q = h;
-    const HeatStage& s = sm.st[warp][t % kHeatStages];
-    mbar_wait(&sm.bar[warp][t % kHeatStages], (t / kHeatStages) & 1);
-    if (!row_ok(t)) {
-      __syncwarp();
-      fill(t + kHeatStages);
-      return;
-    }
-    const double2 hv = *reinterpret_cast<const double2*>(&s.h[2 * lane]);
-    const double2 qv = *reinterpret_cast<const double2*>(&s.q[2 * lane]);
-    h = make_double2(in0 ? hv.x : 0.0, in1 ? hv.y : 0.0);
-    if (t >= 1 && t <= nrows) q = make_double2(in0 ? qv.x : 0.0, in1 ? qv.y : 0.0);
-    __syncwarp();
-    fill(t + kHeatStages);
-  };
+  // the column slots of this warp's window that no bulk copy ever writes (outside the winding pack) hold zeros for the
+  // whole kernel, so the per-row reads need no masks
+#pragma unroll
+  for (int t = 0; t < kHeatStages; ++t) {
+    HeatStage& s = sm.st[warp][t];
+    if (!in0) s.h[2 * lane] = 0.0, s.q[2 * lane] = 0.0;
+    if (!in1) s.h[2 * lane + 1] = 0.0, s.q[2 * lane + 1] = 0.0;
+  }
+  __syncwarp();
 #pragma unroll
   for (int t = 0; t < kHeatStages; ++t) fill(t);
-  double2 h, qc, qn;
-  take(0, h, qc);
-  double2 Up = make_double2(0.0, 0.0);
-  if (r0 > 0) Up = make_double2(tsq_fast(h.x, C3, qC1sq, hC1, inv_hC3), tsq_fast(h.y, C3, qC1sq, hC1, inv_hC3));
-  double2 Hc;
-  take(1, Hc, qc);
-  double2 Uc = make_double2(tsq_fast(Hc.x, C3, qC1sq, hC1, inv_hC3), tsq_fast(Hc.y, C3, qC1sq, hC1, inv_hC3));
-  double* o = Hout + static_cast<long long>(r0) * Nz + max(iz0, 0);
-  for (int k = 0; k < nrows; ++k) {
-    double2 Hn;
-    take(k + 2, Hn, qn);
-    const double2 Un = make_double2(tsq_fast(Hn.x, C3, qC1sq, hC1, inv_hC3), tsq_fast(Hn.y, C3, qC1sq, hC1, inv_hC3));
-    const double Ul = __shfl_up_sync(0xffffffffu, Uc.y, 1), Ur = __shfl_down_sync(0xffffffffu, Uc.x, 1);
-    if (own0) {
-      const double4 rc = sm.srow[k];
-      double a0 = fma(rc.x, Un.x - Uc.x, qc.x), a1 = fma(rc.x, Un.y - Uc.y, qc.y);
-      a0 = fma(rc.y, Up.x - Uc.x, a0);
-      a1 = fma(rc.y, Up.y - Uc.y, a1);
-      const double dzc = Uc.y - Uc.x;
-      a0 = fma(zp0, dzc, a0);
-      a1 = fma(-zm1, dzc, a1);
-      a0 = fma(zm0, Ul - Uc.x, a0);
-      a1 = fma(zp1, Ur - Uc.y, a1);
-      if (rc.z != 0.0 || zborder) {                    // Robin borders of the winding pack (rare: rb = 0 inside)
-        a0 = fma(-(rc.z + zb0), sqrt_fast(Uc.x) - lp.T_bath, a0);
-        a1 = fma(-(rc.z + zb1), sqrt_fast(Uc.y) - lp.T_bath, a1);
+  // A row's stage is refilled only after the row has been the CENTRE row of an update, so H and Q of the centre row are
+  // read from shared memory where they are used (two LDS.128) instead of riding through two register rotations.
+  auto wait_h = [&](int t) {                            // waits for stage t, returns this lane's column pair of H
+    mbar_wait(&sm.bar[warp][t % kHeatStages], (t / kHeatStages) & 1);
+    if (!row_ok(t)) return make_double2(0.0, 0.0);
+    return *reinterpret_cast<const double2*>(&sm.st[warp][t % kHeatStages].h[2 * lane]);
+  };
+  {
+    double2 h = wait_h(0);
+    double2 Up = make_double2(0.0, 0.0);
+    if (r0 > 0) Up = make_double2(tsq_fast(h.x, C3, qC1sq, hC1, inv_hC3), tsq_fast(h.y, C3, qC1sq, hC1, inv_hC3));
+    __syncwarp();
+    fill(kHeatStages);                                  // row -1 is never a centre row: its stage is free again
+    h = wait_h(1);
+    double2 Uc = make_double2(tsq_fast(h.x, C3, qC1sq, hC1, inv_hC3), tsq_fast(h.y, C3, qC1sq, hC1, inv_hC3));
+    double* o = Hout + static_cast<long long>(r0) * Nz + max(iz0, 0);
+    for (int k = 0; k < nrows; ++k) {
+      const double2 Hn = wait_h(k + 2);
+      const double2 Un = make_double2(tsq_fast(Hn.x, C3, qC1sq, hC1, inv_hC3), tsq_fast(Hn.y, C3, qC1sq, hC1, inv_hC3));
+      const double Ul = __shfl_up_sync(0xffffffffu, Uc.y, 1), Ur = __shfl_down_sync(0xffffffffu, Uc.x, 1);
+      if (own0) {
+        const HeatStage& sc = sm.st[warp][(k + 1) % kHeatStages];
+        const double2 Hc = *reinterpret_cast<const double2*>(&sc.h[2 * lane]);
+        const double2 qc = *reinterpret_cast<const double2*>(&sc.q[2 * lane]);
+        const double4 rc = sm.srow[k];
+        double a0 = fma(rc.x, Un.x - Uc.x, qc.x), a1 = fma(rc.x, Un.y - Uc.y, qc.y);
+        a0 = fma(rc.y, Up.x - Uc.x, a0);
+        a1 = fma(rc.y, Up.y - Uc.y, a1);
+        const double dzc = Uc.y - Uc.x;
+        a0 = fma(zp0, dzc, a0);
+        a1 = fma(-zm1, dzc, a1);
+        a0 = fma(zm0, Ul - Uc.x, a0);
+        a1 = fma(zp1, Ur - Uc.y, a1);
+        if (rc.z != 0.0 || zborder) {                    // Robin borders of the winding pack (rare: rb = 0 inside)
+          a0 = fma(-(rc.z + zb0), sqrt_fast(Uc.x) - lp.T_bath, a0);
+          a1 = fma(-(rc.z + zb1), sqrt_fast(Uc.y) - lp.T_bath, a1);
+        }
+        *reinterpret_cast<double2*>(o) = make_double2(fma(dtsub, a0, Hc.x), fma(dtsub, a1, Hc.y));
       }
-      *reinterpret_cast<double2*>(o) = make_double2(fma(dtsub, a0, Hc.x), fma(dtsub, a1, Hc.y));
+      Up = Uc;
+      Uc = Un;
+      o += Nz;
+      __syncwarp();                                     // every lane is done with the centre row's stage
+      fill(k + 1 + kHeatStages);
     }
-    Up = Uc;
-    Uc = Un;
-    Hc = Hn;
-    qc = qn;
-    o += Nz;
   }
 }
 
@@ -717,9 +713,10 @@ void k_heat_substep(const VecCtx& v, const MaterialParams& mp, const LatticePara
   QS_LAUNCH(v);
   const int gx = (lp.Nz + kHeatWarps * kHeatCols - 1) / (kHeatWarps * kHeatCols);
   // strips of rows: long enough to amortise the two halo rows, and chosen so that the CTAs fill whole waves of
-  // 3 resident CTAs per SM (a 2.6-wave launch idles 14 % of the GPU in its last wave)
+  // the resident CTAs per SM (a 2.6-wave launch idles 14 % of the GPU in its last wave)
   if (g_sm_count == 0) grid_for(1);
-  const long long resident = 3ll * g_sm_count;
+  const bool tma = lp.Nz % 2 == 0;   // 16-byte aligned row segments: TMA pipeline
+  const long long resident = static_cast<long long>(tma ? kHeatMinB : 3) * g_sm_count;
   int rows = 4;
   double best = -1.0;
   for (int cand = kHeatMaxRows; cand >= 4; --cand) {
@@ -730,7 +727,7 @@ void k_heat_substep(const VecCtx& v, const MaterialParams& mp, const LatticePara
     if (eff > best + 1e-9) best = eff, rows = cand;
   }
   dim3 grid(gx, (lp.Nr + rows - 1) / rows);
-  if (lp.Nz % 2 == 0) {
+  if (tma) {
     static bool attr_set = false;
     if (!attr_set) {
       cudaFuncSetAttribute(heat_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(sizeof(HeatSmem)));

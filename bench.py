@@ -37,7 +37,7 @@ FLOP_K1, FLOP_K2 = 76.0, 100.0
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9 / 1e12
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the ncu --set full captures summarised
 # under profiles/ (r01_sweep_field_cfg2.md, r01_hbm_passes.md); None where no capture of that workload exists
-NCU_TRAFFIC = {"sweep_field:cfg2_mid_solenoid_20x40x16": 11.8e6, "material_K5": 671.6e6 + 492.5e6, "heat_K6": 275.9e6 + 102.7e6}   # r01 captures
+NCU_TRAFFIC = {"sweep_field:cfg2_mid_solenoid_20x40x16": 11.8e6, "material_K5": 671.4e6 + 498.2e6, "heat_K6": 275.0e6 + 102.4e6}   # r01 captures
 DEFAULTS = {"cfg0": (50, 5), "cfg1": (100, 5), "cfg2": (10, 3), "cfg3": (3, 3)}
 
 

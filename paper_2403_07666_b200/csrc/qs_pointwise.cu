@@ -438,7 +438,11 @@ __global__ void __launch_bounds__(kHeatWarps * 32, kHeatMinB) heat_tma_kernel(Ma
   // stage t holds row g = r0 - 1 + t of H (0 <= t <= nrows + 1) and, for 1 <= t <= nrows, of Q
   const int T_last = nrows + 1;
   auto row_ok = [&](int t) { const int g = r0 - 1 + t; return g >= 0 && g < lp.Nr; };
+  // fill(t) is called for t = 0, 1, 2, ... in this order: the element offset of row t is carried, not recomputed
+  long long fill_off = static_cast<long long>(r0 - 1) * Nz + cs;
   auto fill = [&](int t) {
+    const long long off = fill_off;
+    fill_off += Nz;
     if (lane != 0 || t > T_last) return;
     HeatStage& s = sm.st[warp][t % kHeatStages];
     uint64_t* b = &sm.bar[warp][t % kHeatStages];
@@ -447,7 +451,6 @@ __global__ void __launch_bounds__(kHeatWarps * 32, kHeatMinB) heat_tma_kernel(Ma
       return;
     }
     const bool needq = t >= 1 && t <= nrows;
-    const long long off = static_cast<long long>(r0 - 1 + t) * Nz + cs;
     mbar_expect_tx(b, needq ? 2u * seg_bytes : seg_bytes);
     bulk_g2s(&s.h[soff], Hin + off, seg_bytes, b);
     if (needq) bulk_g2s(&s.q[soff], Q + off, seg_bytes, b);

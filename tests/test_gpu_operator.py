@@ -326,3 +326,34 @@ def test_heat_adi_substeps_pointwise(pkg, shape):
         _, Tg, _, _ = sim.read(J=False, B=False, E=False)
     Ho = qo.heat_adi(geo, mat, qo.enthalpy(mat, T), Q, dt, m)
     assert np.max(np.abs(Tg - qo.temperature(mat, Ho))) <= 1e-11 * 9.0
+
+
+def test_hbm_leg_lattice_material_and_heat_full_arrays(pkg):
+    # the launch configuration bench.py --leg hbm times (roofline_hbm): 4096 x 4096 cells (arrays larger than L2), the
+    # material pass without the test outputs (aux=False) and one explicit heat sub-step, same seeded state; every cell
+    # of E and T is compared with the oracle
+    w = wl.lattice_workload("hbm_4096x4096", 64, 64, 64, 1.0e-3, 30e-3, 1e-4, 0.0, 1, 77, 0.01)
+    geo, mat = w.geometry, w.material
+    N = geo.n_rings
+    g = np.random.default_rng(5)
+    J = 1e8 * g.standard_normal(N)
+    T = 4.2 + g.random(N)
+    B = 0.1 * g.standard_normal(2 * N)
+    Q = 1e3 * g.random(N)
+    sub_dt = 1e-9
+    with pkg.QS(geo, mat, no_operator=True) as sim:
+        sim.write(J=J, T=T)
+        sim.set_fields(B=B, Q=Q)
+        sim.material_eval(1e-4, aux=False)
+        _, _, _, E = sim.read(J=False, T=False, B=False)
+        sim.set_fields(Q=Q)                                        # the material pass overwrote Q with E J
+        m = sim.heat(sub_dt)
+        _, Tg, _, _ = sim.read(J=False, B=False, E=False)
+    assert m == 1
+    ml = qo.material_law(mat, J, T, B[:N], B[N:], geo.r, mat.jc0_scale)
+    assert np.max(np.abs(E - ml["E"])) <= 1e-11 * np.max(np.abs(ml["E"]))
+    del ml
+    Ho, _ = qo.heat_substeps(geo, mat, qo.enthalpy(mat, T), Q, sub_dt, 1)
+    To = qo.temperature(mat, Ho)
+    assert np.max(np.abs(Tg - To)) <= 1e-13 * 6.0
+    assert np.max(np.abs((Tg - T) - (To - T))) <= 1e-6 * np.max(np.abs(To - T))   # the increment itself, not just T

@@ -376,3 +376,22 @@ def test_nonlinear_trajectory_ends_in_the_closed_form_saturated_state_on_the_gpu
     assert rel(J, Js) < 1e-9, rel(J, Js)
     assert rel(E, Es) < 1e-8, rel(E, Es)
     assert abs(st["U_terminal"] - Us.sum()) < 1e-8 * abs(Us.sum())
+
+
+def test_nonlinear_transient_power_balance_on_the_gpu(pkg):
+    # GPU quantities only (qs_step, qs_read, qs_matvec): Poynting balance of the moving flux front, first order in dt
+    from test_oracle_solver_step import power_balance_residual
+    w = wl.shrunk(1, 1, 1, 8)
+    geo = dataclasses.replace(w.geometry, Bext_rate=10.0)
+    mat = dataclasses.replace(w.material, cg_tol=1e-12)
+    res = []
+    for dt in (1e-4, 5e-5):
+        with pkg.QS(geo, mat) as sim:
+            def read_JE():
+                J, _, _, E = sim.read(T=False, B=False)
+                return J, E
+            rr, share = power_balance_residual(lambda d: sim.step(d, 0.0), read_JE, sim.matvec, geo, 10.0, dt,
+                                               int(round(0.02 / dt)))
+        res.append(rr)
+        assert 0.2 < share < 0.4
+    assert 0 < res[0] < 0.01 and 1.8 < res[0] / res[1] < 2.2

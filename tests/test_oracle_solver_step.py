@@ -348,3 +348,39 @@ def test_nonlinear_trajectory_ends_in_the_closed_form_saturated_state():
         # the saturated wire is the Bean profile lifted by the power law: |J|/Jc = (|E|/Ec)^(1/n), |E| <~ s Bdot / 2
         x = np.abs(o.J) / (mat.Jc0 * o.scale)
         assert 0.5 < x.min() and x.max() < (0.5 * geo.wire_size * geo.Bext_rate / mat.Ec) ** (1 / mat.n_exp) * 1.01
+
+
+def power_balance_residual(step, read_JE, apply_M, geo, Bdot, dt, steps):
+    """Poynting balance of a magnetisation run (no transport current), accumulated over the trajectory.
+
+    C4 multiplied by the ring currents: I.M.dI/dt + sum 2 pi r E I = sum I emf_ext - (C^T I).V, with emf_ext =
+    -pi r^2 Bdot and C^T I = 0 (zero net current per turn).  Time-integrated: magnetic energy + Joule heat = work of
+    the external field.  The theta step satisfies this to O(dt): the relative residual is returned.
+    """
+    r, a = geo.r, geo.area
+    joule = work = 0.0
+    J = np.zeros(geo.n_rings)
+    for _ in range(steps):
+        I = a * J
+        assert step(dt) >= 0
+        J, E = read_JE()                                           # E is the field of the step's start state (C6)
+        joule += dt * np.sum(2 * math.pi * r * E * I)
+        work += dt * np.sum(I * (-math.pi * r * r * Bdot))
+    I = a * J
+    return (0.5 * I @ apply_M(I) + joule - work) / work, joule / work
+
+
+def test_nonlinear_transient_satisfies_the_power_balance_to_first_order():
+    # pins the TRANSIENT (moving flux front, before saturation): a wrong factor or sign in the rhs, the update or the
+    # constraint leaves an O(1) residual; the correct scheme's residual halves with dt
+    w = wl.shrunk(1, 1, 1, 8)
+    geo = dataclasses.replace(w.geometry, Bext_rate=10.0)
+    res = []
+    for dt in (1e-4, 5e-5, 2.5e-5):
+        o = qo.Oracle(geo, w.material)
+        rr, share = power_balance_residual(lambda d: o.step(d, 0.0), lambda: (o.J.copy(), o.E.copy()),
+                                           lambda x: o.M @ x, geo, 10.0, dt, int(round(0.02 / dt)))
+        res.append(rr)
+        assert 0.2 < share < 0.4                                  # a quarter of the work is dissipated: nonlinear regime
+    assert 0 < res[0] < 0.01
+    assert 1.8 < res[0] / res[1] < 2.2 and 1.8 < res[1] / res[2] < 2.2

@@ -134,6 +134,10 @@ struct MaterialConsts {   // host-side reciprocals of the constant divisors (qs_
 #ifndef QS_MAT_MINB
 #define QS_MAT_MINB 6   // resident CTAs per SM the register budget is sized for (40 registers per thread)
 #endif
+#ifndef QS_MAT_WAVES
+#define QS_MAT_WAVES 8   // CTAs launched per resident slot on lattices (each walks rows with that stride); 16.8 M cells:
+                        // 1: 0.224 ms, 2: 0.219, 4: 0.214, 8: 0.212, 32: 0.215
+#endif
 template <bool FROM_ACC, bool AUX, bool EVENTS>
 __global__ void __launch_bounds__(256, QS_MAT_MINB) material_kernel(MaterialParams mp, MaterialConsts k, MaterialArgs a) {
   const double two_pi = 2.0 * kPi;
@@ -685,7 +689,7 @@ void k_material(const VecCtx& v, const MaterialParams& mp, const MaterialArgs& a
   if (a.Nz > 0) {   // 2-D: no integer division per cell
     const int nrow = a.N / a.Nz;
     grid.x = (a.Nz + kBlock - 1) / kBlock;
-    grid.y = std::min(nrow, std::max(1, 2 * QS_MAT_MINB * g_sm_count / static_cast<int>(grid.x)));
+    grid.y = std::min(nrow, std::max(1, QS_MAT_WAVES * QS_MAT_MINB * g_sm_count / static_cast<int>(grid.x)));
   }
   const bool ev = a.xmax_bits != nullptr, aux = a.dEdJ != nullptr;
 #define QS_MAT(F_, A_, E_) material_kernel<F_, A_, E_><<<grid, kBlock, 0, v.stream>>>(mp, k, a)

@@ -19,7 +19,7 @@ Pins (tests/test_oracle_*.py, all ``-m "not gpu"``):
   material_law       closed forms E(Jc)=Ec, E'->n Ec/Jc, Jc(4.2 K,0,0), strain zero, dE/dJ by FD
   heat_substeps      exact discrete 1-D steady state; energy balance to rounding
   kkt_dense / pcg    constraint C^T I' = d, KKT residual, dense vs CG, single-ring L-R circuit
-  lattice tables     table operator == dense operator on small lattices
+  lattice tables     table operator == dense operator on small lattices; FFT application == offset-by-offset sum
   wire statistics    closed forms of a prepared normal-state turn (rho_n J^2), sum_w E_joule == integral of Joule power
   step_rk            exact second-order polynomial and error estimate on the linear L-R ring, global order 2,
                      rejection rule, reduction to the theta = 0 step at constant rate
@@ -183,6 +183,9 @@ def field_eval_rows(geo, I, rows, chunk=256):
 # dense operators on small lattices (tests/test_oracle_lattice.py).
 # --------------------------------------------------------------------------------------
 class LatticeTables:
+    """Tables T[d, ir, jr] of the pair quantities at axial offset d = |iz - jz| (storage: one contiguous
+    Nr x Nr matrix per offset, so that applying offset d is one plain matrix product)."""
+
     def __init__(self, geo, with_field=True):
         assert geo.lattice
         Nr, Nz, h = geo.Nr, geo.Nz, geo.h
@@ -192,27 +195,27 @@ class LatticeTables:
         ri, rj, dz = rr[:, None, None], rr[None, :, None], d[None, None, :]
         soft = np.zeros((Nr, Nr, Nz))
         soft[np.arange(Nr), np.arange(Nr), 0] = float(geo.softening) ** 2
-        self.M = np.empty((Nr, Nr, Nz))
+        self.M = np.empty((Nz, Nr, Nr))
         for a in range(Nr):                                     # row by row: bounded memory
-            self.M[a] = mutual_pair(ri[a], 0.0, rj[0], dz[0], soft[a])
+            self.M[:, a, :] = mutual_pair(ri[a], 0.0, rj[0], dz[0], soft[a]).T
         self.with_field = with_field
         if with_field:
-            self.Br = np.empty((Nr, Nr, Nz))                    # for dz = +d (target above source)
-            self.Bz = np.empty((Nr, Nr, Nz))
+            self.Br = np.empty((Nz, Nr, Nr))                    # for dz = +d (target above source)
+            self.Bz = np.empty((Nz, Nr, Nr))
             selfc = self_field_coef(geo).reshape(Nr, Nz)[:, 0]
             for a in range(Nr):
                 dzz = np.broadcast_to(dz[0], (Nr, Nz)).copy()
                 dzz[a, 0] = 1.0
                 br, bz = field_pair(ri[a], dzz, rj[0], 0.0)
                 br[a, 0], bz[a, 0] = 0.0, selfc[a]
-                self.Br[a], self.Bz[a] = br, bz
+                self.Br[:, a, :], self.Bz[:, a, :] = br.T, bz.T
 
     def _apply(self, tab, X, odd):
-        """Y[ir, iz] = sum_{jr, jz} tab[ir, jr, |iz-jz|] * sgn * X[jr, jz], offset by offset."""
+        """Y[ir, iz] = sum_{jr, jz} tab[|iz-jz|, ir, jr] * sgn * X[jr, jz], offset by offset."""
         Nz = self.Nz
-        Y = tab[:, :, 0] @ X
+        Y = tab[0] @ X
         for d in range(1, Nz):
-            T = tab[:, :, d]
+            T = tab[d]
             Y[:, d:] += T @ X[:, : Nz - d]                       # targets above sources: dz = +d h
             Y[:, : Nz - d] += (-1.0 if odd else 1.0) * (T @ X[:, d:])   # dz = -d h
         return Y
@@ -223,6 +226,56 @@ class LatticeTables:
     def field(self, I):
         X = I.reshape(self.Nr, self.Nz)
         return (self._apply(self.Br, X, True).reshape(-1), self._apply(self.Bz, X, False).reshape(-1))
+
+
+class LatticeTablesFFT(LatticeTables):
+    """The same tables applied through the convolution theorem (for the one lattice the plain offset loop cannot
+    finish in hours: config 3 at full size, Nr^2 Nz^2 = 7.5e11 multiply-adds per application).
+
+    Along z the operator is a Toeplitz matrix per (ir, jr): Y[ir, iz] = sum_jr sum_jz c_{ir,jr}[iz - jz] X[jr, jz]
+    with c[+d] = T[d], c[-d] = sgn T[d].  Embedded in a circulant of length L = 2 Nz (X zero-padded), the product is
+    a pointwise product of discrete Fourier transforms (library FFT), summed over jr frequency by frequency.
+    Pinned against LatticeTables._apply (the defining sum) in tests/test_oracle_solver_step.py; the long-parity
+    script also re-checks it against the plain loop on the very state it compares.
+    """
+
+    def __init__(self, geo, with_field=True):
+        super().__init__(geo, with_field)
+        self.specM = self._spectrum(self.M, False)
+        if with_field:
+            self.specBr = self._spectrum(self.Br, True)
+            self.specBz = self._spectrum(self.Bz, False)
+
+    def _spectrum(self, tab, odd):
+        Nr, Nz = self.Nr, self.Nz
+        L = 2 * Nz
+        spec = np.empty((Nz + 1, Nr, Nr), dtype=np.complex128)
+        sgn = -1.0 if odd else 1.0
+        for a in range(Nr):                                     # row by row: bounded memory
+            col = np.zeros((L, Nr))
+            col[:Nz] = tab[:, a, :]                             # e = iz - jz = +d
+            col[L - Nz + 1:] = sgn * tab[:0:-1, a, :]           # e = -d  ->  slot L - d
+            spec[:, a, :] = np.fft.rfft(col, axis=0)
+        return spec
+
+    def _apply_fft(self, spec, X):
+        Nz = self.Nz
+        Xh = np.fft.rfft(X, n=2 * Nz, axis=1)                   # [Nr, Nz + 1]
+        Yh = np.einsum("kij,jk->ik", spec, Xh)                  # one Nr x Nr matrix-vector product per frequency
+        return np.fft.irfft(Yh, n=2 * Nz, axis=1)[:, :Nz]
+
+    def matvec(self, x):
+        return self._apply_fft(self.specM, x.reshape(self.Nr, self.Nz)).reshape(-1)
+
+    def field(self, I):
+        X = I.reshape(self.Nr, self.Nz)
+        return self._apply_fft(self.specBr, X).reshape(-1), self._apply_fft(self.specBz, X).reshape(-1)
+
+    def matvec_plain(self, x):
+        return LatticeTables.matvec(self, x)
+
+    def field_plain(self, I):
+        return LatticeTables.field(self, I)
 
 
 # --------------------------------------------------------------------------------------
@@ -527,7 +580,8 @@ def turn_observables(geo, mat, T, E, J, Jc, rho):
 # The stepper: same calls as include/qs.h (qs_init / qs_step / qs_read / qs_write / ...)
 # --------------------------------------------------------------------------------------
 class Oracle:
-    """operator = 'dense' (N <= ~8k), 'tables' (regular lattices of any size)."""
+    """operator = 'dense' (N <= ~8k), 'tables' (regular lattices of any size), 'tables_fft' (the same tables applied by
+    FFT along z: config 3 at full size only)."""
 
     def __init__(self, geo, mat, operator="dense", solver="cholesky"):
         self.geo, self.mat = geo, mat
@@ -542,10 +596,10 @@ class Oracle:
             if geo.lattice:
                 self.GBr, self.GBz = dense_GB(geo)
             self.diagM = np.diag(self.M).copy()
-        elif operator == "tables":
-            self.tables = LatticeTables(geo)
+        elif operator in ("tables", "tables_fft"):
+            self.tables = LatticeTables(geo) if operator == "tables" else LatticeTablesFFT(geo)
             rr = np.arange(geo.Nr)
-            self.diagM = np.repeat(self.tables.M[rr, rr, 0], geo.Nz)
+            self.diagM = np.repeat(self.tables.M[0, rr, rr], geo.Nz)
         else:
             raise ValueError(operator)
         self.C = constraint_matrix(geo) if (solver == "cholesky" and operator == "dense") else None

@@ -143,6 +143,59 @@ def test_radial_scheme_is_second_order_consistent():
     assert res[0] < 1e-4 * Q and 3.5 < res[0] / res[1] < 4.5 and 3.5 < res[1] / res[2] < 4.5
 
 
+def test_robin_loss_on_the_radial_borders_uses_the_true_border_radii():
+    # PAPER.md:75 "four borders": a one-cell-high stack of rings (Nz = 1) with uniform Q cooled through ONE radial
+    # border only.  In the steady state all the heat leaves through that border, so the border cell's temperature has
+    # a closed form with the TRUE border radius (not the cell-centre radius):
+    #   h_conv (T_border - T_b) 2 pi r_border h = Q pi (r_out^2 - r_in^2) h
+    # (the cell volumes 2 pi r_c h^2 sum to pi (r_out^2 - r_in^2) h exactly).  Strong curvature: r_in = 1 mm, h = 0.5 mm.
+    import scipy.optimize
+    nr, h, r_in, Q, hc = 4, 0.5e-3, 1.0e-3, 4e4, 500.0
+    r_out = r_in + nr * h
+    mat = wl.Material()
+    for side, r_border, cell in ((0, r_in, 0), (1, r_out, nr - 1)):
+        hcv = [0.0, 0.0, 0.0, 0.0]
+        hcv[side] = hc
+        geo = dataclasses.replace(wl.lattice_geometry(nr, 1, 1, h, r_in), h_conv=tuple(hcv))
+        assert geo.Nz == 1 and geo.Nr == nr
+        vol = 2 * math.pi * geo.r * h * h
+        assert abs(vol.sum() - math.pi * (r_out ** 2 - r_in ** 2) * h) < 1e-15 * vol.sum()
+
+        def resid(T):
+            div, _ = qo.heat_flux_divergence(geo, mat, T.reshape(nr, 1))
+            return div.reshape(-1) / vol + Q
+
+        T = scipy.optimize.fsolve(resid, np.full(nr, geo.T_bath + 1.0), xtol=1e-13)
+        assert np.max(np.abs(resid(T))) < 1e-9 * Q
+        T_closed = geo.T_bath + Q * (r_out ** 2 - r_in ** 2) / (2.0 * r_border * hc)
+        assert abs(T[cell] - T_closed) < 1e-9 * T_closed, (side, T[cell], T_closed)
+        # the cell-centre radius in place of the border radius would be off by h/(2 r_border): 25 % / 8 % here
+        r_c = geo.r[cell]
+        assert abs(geo.T_bath + Q * (r_out ** 2 - r_in ** 2) / (2.0 * r_c * hc) - T_closed) > 1e-2 * (T_closed - geo.T_bath)
+        # and the time stepping relaxes to that state (enthalpy form, sub-step rule of C9)
+        # (a ripple that carries no net energy, so that only the fast conduction modes are excited)
+        ripple = 1e-3 * np.cos(np.arange(nr))
+        wgt = vol * (mat.C3 * T ** 3 + mat.C1 * T)
+        ripple -= np.sum(wgt * ripple) / np.sum(wgt)
+        H = qo.enthalpy(mat, T + ripple)
+        dt = 5e-3
+        for _ in range(60):                                   # 0.3 s = 9 conduction time constants (k_between, 2 mm)
+            H, lost = qo.heat_substeps(geo, mat, H, np.full(nr, Q), dt, qo.heat_substeps_count(geo, mat, dt))
+        assert abs(qo.temperature(mat, H)[cell] - T_closed) < 5e-5
+    # both radial borders cooled: global balance with the two true border radii
+    geo = dataclasses.replace(wl.lattice_geometry(nr, 1, 1, h, r_in), h_conv=(hc, 0.5 * hc, 0.0, 0.0))
+    vol = 2 * math.pi * geo.r * h * h
+
+    def resid2(T):
+        div, _ = qo.heat_flux_divergence(geo, mat, T.reshape(nr, 1))
+        return div.reshape(-1) / vol + Q
+
+    T = scipy.optimize.fsolve(resid2, np.full(nr, geo.T_bath + 1.0), xtol=1e-13)
+    out = hc * (T[0] - geo.T_bath) * 2 * math.pi * r_in * h + 0.5 * hc * (T[-1] - geo.T_bath) * 2 * math.pi * r_out * h
+    gen = Q * math.pi * (r_out ** 2 - r_in ** 2) * h
+    assert abs(out - gen) < 1e-9 * gen
+
+
 def test_energy_balance_to_rounding():
     # sum V dH = dt sum V Q - boundary energy (enthalpy form; north_star "energy balance")
     geo = wl.lattice_geometry(3, 2, 4, 1e-3, 0.03)

@@ -81,6 +81,26 @@ def test_lattice_tables_equal_dense_operators():
     assert np.max(np.abs(bz - GBz @ x)) < 1e-13 * np.max(np.abs(GBz @ x))
 
 
+def test_fft_application_of_the_tables_equals_the_offset_sum_and_the_dense_operators():
+    # the circulant embedding must reproduce the defining sum: even (M, Bz) and odd (Br) tables, Nz not a power of two
+    geo = wl.lattice_geometry(4, 5, 3, 0.8e-3, 50e-3)
+    g = np.random.default_rng(11)
+    x = g.standard_normal(geo.n_rings)
+    tab = qo.LatticeTablesFFT(geo)
+    M = qo.dense_M(geo)
+    GBr, GBz = qo.dense_GB(geo)
+    for got, ref in ((tab.matvec(x), M @ x), (tab.field(x)[0], GBr @ x), (tab.field(x)[1], GBz @ x),
+                     (tab.matvec(x), tab.matvec_plain(x)), (tab.field(x)[0], tab.field_plain(x)[0])):
+        assert np.max(np.abs(got - ref)) < 1e-13 * np.max(np.abs(ref))
+    # a delta source picks single table entries: sign and offset bookkeeping of the odd table
+    e = np.zeros(geo.n_rings)
+    e[2 * geo.Nz + 7] = 1.0
+    br = tab.field(e)[0].reshape(geo.Nr, geo.Nz)
+    assert abs(br[5, 9] - GBr[5 * geo.Nz + 9, 2 * geo.Nz + 7]) < 1e-13 * np.max(np.abs(GBr))
+    assert abs(br[5, 5] - GBr[5 * geo.Nz + 5, 2 * geo.Nz + 7]) < 1e-13 * np.max(np.abs(GBr))
+    assert br[5, 9] * br[5, 5] < 0.0
+
+
 def test_single_ring_is_an_LR_circuit():
     # one normal-state ring (T > Tc: rho = rho_n) in a ramped axial field, no current constraint:
     # L I' + R I = -pi r^2 Bdot,  L = mu0 r [ln(8r/g) - 2],  R = rho_n 2 pi r / a;  I(t) = I_inf (1 - exp(-t/tau))
@@ -193,6 +213,65 @@ def test_event_variants():
     ret = o.step(1e-6, w.I_ramp)
     assert ret & qo.RET_QUENCH and o.flags[5] & qo.Q_T and o.flags[5] & qo.Q_RHO and o.flags[5] & qo.FJ_T
     assert np.all(np.delete(o.flags, 5) & (qo.Q_T | qo.Q_RHO) == 0)
+
+
+def test_flux_jump_criterion_J_over_Jc():
+    # PAPER.md:105 flux-jump criterion |J/Jc| > 1 (bit FJ_J).  Prepared state at B = 0 (B0 -> inf), no strain term,
+    # no Jc0 perturbation: Jc = Jc0 (1 - T/Tc)^2 in closed form.  One cell of turn 7 at 1.01 Jc, one cell of turn 9 at
+    # 0.99 Jc, the rest at 0.5 Jc -> exactly turn 7 raises exactly FJ_J; first-event time = end of that step; return bit 0.
+    w = wl.config(0)
+    geo = w.geometry
+    mat = dataclasses.replace(w.material, B0=1e30, eps_coef=0.0, jc0_scale=None)
+    Jc = mat.Jc0 * (1.0 - geo.T_bath / mat.Tc) ** 2
+    J = np.full(geo.n_rings, 0.5 * Jc)
+    c7 = np.flatnonzero(geo.turn_id == 7)[13]
+    c9 = np.flatnonzero(geo.turn_id == 9)[40]
+    J[c7], J[c9] = 1.01 * Jc, 0.99 * Jc
+    o = qo.Oracle(geo, mat)
+    o.write(J, np.full(geo.n_rings, geo.T_bath), 0.0, 0.0)
+    ret = o.step(1e-7, 0.0)
+    assert ret == qo.RET_FLUXJUMP
+    assert o.flags[7] == qo.FJ_J and np.all(np.delete(o.flags, 7) == 0)
+    assert abs(o.t_first[7] - 1e-7) < 1e-20 and np.all(np.delete(o.t_first, 7) < 0)
+    assert np.all(o.count == 0)                              # the rising-edge counter follows FJ_T | FJ_E only (C10)
+    # negative current counts through its magnitude
+    J[c7], J[c9] = -0.99 * Jc, -1.01 * Jc
+    o.write(J, np.full(geo.n_rings, geo.T_bath), 0.0, 0.0)
+    assert o.step(1e-7, 0.0) == qo.RET_FLUXJUMP
+    assert o.flags[9] == qo.FJ_J and np.all(np.delete(o.flags, 9) == 0)
+
+
+@pytest.mark.parametrize("side", [-1, +1])
+def test_flux_jump_criterion_dEdt_spike(side):
+    # C10 bit FJ_E: (Ebar^k - Ebar^{k-1})/dt > dEdt_spike, Ebar = mean |E| over the turn.  Turn 5 is normal (T > Tc:
+    # rho = rho_n exactly) and carries positive J everywhere, so Ebar = rho_n mean(J) = rho_n I(t)/A_wire by the turn's
+    # current constraint: dEbar/dt = rho_n I_ramp / A_wire in closed form, whatever the redistribution inside the turn.
+    # The threshold is placed 1e-6 relative below / above it.  T_fluxjump is raised so that FJ_T stays off and the
+    # rising-edge counter isolates FJ_E.
+    w = wl.config(0)
+    geo = w.geometry
+    I_ramp, dt = 4000.0, 1e-6
+    A_wire = geo.wire_size ** 2
+    rate = w.material.rho_n * I_ramp / A_wire                # 2 V/m/s
+    mat = dataclasses.replace(w.material, T_fluxjump=100.0, dEdt_spike=rate * (1.0 - side * 1e-6))
+    J0 = np.full(geo.n_rings, 0.5 * 2e9 * (1 - 4.2 / 18) ** 2)
+    T0 = np.full(geo.n_rings, geo.T_bath)
+    T0[geo.turn_id == 5] = 19.0
+    o = qo.Oracle(geo, mat)
+    o.write(J0, T0, 0.0, J0[0] * A_wire)
+    ret1 = o.step(dt, I_ramp)
+    assert not o.flags[5] & qo.FJ_E and o.count[5] == 0      # no previous Ebar on the first step after qs_write
+    assert ret1 & qo.RET_QUENCH and o.flags[5] & qo.FJ_J     # normal turn: Jc = 0, |J|/Jc = inf > 1 (C5 guard, C10)
+    assert np.all(o.J[geo.turn_id == 5] > 0)
+    ret2 = o.step(dt, I_ramp)
+    fired = bool(o.flags[5] & qo.FJ_E)
+    assert fired == (side > 0)
+    assert o.count[5] == (1 if fired else 0)
+    assert not ret2 & qo.RET_FLUXJUMP                        # return bit 0 = a flux jump STARTED: FJ_J was already set
+    assert np.all(np.delete(o.flags, 5) & qo.FJ_E == 0)      # cold turns: E ~ Ec 0.5^20, no spike
+    ret3 = o.step(dt, I_ramp)                                # the flag stays set at the same rate: no second rising edge
+    assert bool(o.flags[5] & qo.FJ_E) == fired and o.count[5] == (1 if fired else 0)
+    assert not ret3 & qo.RET_FLUXJUMP
 
 
 def test_wire_statistics_closed_forms_and_energy_identity():

@@ -2,12 +2,17 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg0|cfg1|cfg2|cfg3] [--impl ours|reference]
 
-One "step" = one qs_step (S1..S7 of SURVEY.md §8(a)) on the named synthetic coil.  Prints ONE JSON line.
+One "step" = one qs_step (S1..S7 of SURVEY.md §8(a)) on the named synthetic coil; default workload: config 3, the
+largest single-GPU configuration (864,000 rings).  Prints ONE JSON line.
   value      coupled cell-steps/s, state resident in HBM, CUDA events on the library's stream, max over ranks
   e2e        same metric through the C ABI with HOST buffers: qs_write(J, T) + qs_step + qs_read(J, T, B, E) per step
   roofline   the dominant kernel (fused pair sweep K2): nominal algorithmic flop / measured launch duration against
              the FP64 FMA peak ("bound": "alu"); plus the HBM-bound passes on a lattice larger than L2
-  cpu_baseline  the CPU oracle as it stands, timed on a bounded row sample of the same workload (rank 0, N = 1)
+  cpu_baseline  the CPU oracle as it stands, timed on a bounded row sample of the same workload on ALL host cores
+                (a process pool over target rows; rank 0, N = 1)
+  operator_cfg4 the config-4 sweep: y = M x and the CG solve at N = 4,096 / 65,536 / 262,144 / 1,048,576
+  cg_active     config 1 (the nonlinear config: ~200 CG iterations per step) next to the headline, whose timed steps
+                are linear-regime steps in which the warm-started CG has nothing left to do
 N > 1: independent replicas (one coil per GPU, different Jc0 seeds), no data-path collective ("replicas only").
 --impl reference: the oracle on the host cores (rank 0 only); no CUDA is touched.
 """
@@ -15,6 +20,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import multiprocessing
 import os
 import subprocess
 import sys
@@ -38,10 +44,11 @@ FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9 / 1e12
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the ncu --set full captures summarised
 # under profiles/ (r01_sweep_field_cfg2.md, r01_hbm_passes.md); None where no capture of that workload exists
 NCU_TRAFFIC = {"sweep_field:cfg2_mid_solenoid_20x40x16": 11.8e6, "material_K5": 671.4e6 + 498.2e6, "heat_K6": 275.0e6 + 102.4e6}   # r01 captures
+NCU_SOURCE = "committed ncu capture (profiles/), not a quantity of this run"
 # executed FP64 flop per launch (dadd + dmul + 2 dfma thread instructions) of the same captures: ncu counts what the
 # kernel really issues (square roots and the series tail expand to several FP64 instructions), the nominal count does not
 NCU_EXEC_FLOP = {"sweep_field:cfg2_mid_solenoid_20x40x16": (1178.569285 + 2342.123003 + 2 * 4037.256723) * 1.963764e9 * 102.601792e-3}
-DEFAULTS = {"cfg0": (50, 5), "cfg1": (100, 5), "cfg2": (10, 3), "cfg3": (3, 3)}
+DEFAULTS = {"cfg0": (50, 5), "cfg1": (100, 5), "cfg2": (10, 3), "cfg3": (5, 3)}
 
 
 def parse_args():
@@ -49,7 +56,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=0)
     ap.add_argument("--warmup", type=int, default=0)
-    ap.add_argument("--workload", default="cfg2", choices=sorted(DEFAULTS))
+    ap.add_argument("--workload", default="cfg3", choices=sorted(DEFAULTS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the HBM-roofline leg, cfg4 operator leg and cpu_baseline")
     ap.add_argument("--operator", default="pairs", choices=["pairs", "tables"],
@@ -132,50 +139,94 @@ def oracle_row_sample(w, rows, J, T, dt):
     linear regime = what the GPU step executes: one fused sweep).  Returns seconds."""
     from oracle import qs_oracle as qo
     geo, mat = w.geometry, w.material
+    chunk = max(1, min(16, int(2e6 // geo.n_rings)))          # rows per evaluation block: bounded memory per worker
     t0 = time.perf_counter()
     Icur = geo.area * J
-    Br, Bz = qo.field_eval_rows(geo, Icur, rows, chunk=16)
+    Br, Bz = qo.field_eval_rows(geo, Icur, rows, chunk=chunk)
     ml = qo.material_law(mat, J[rows], T[rows], Br, Bz, geo.r[rows], mat.jc0_scale[rows])
-    y = qo.matvec_rows(geo, Icur, rows, chunk=16)
+    y = qo.matvec_rows(geo, Icur, rows, chunk=chunk)
     _ = y + ml["E"]
     return time.perf_counter() - t0
 
 
-def oracle_threads():
-    """Threads the oracle legs actually use: the pair-by-pair K/E evaluation is numpy/scipy elementwise code,
-    single-threaded; the BLAS pool only sees the tiny row dot products."""
-    return 1
+_POOL_STATE = {}
 
 
-def run_oracle_sample(w, n_rows, reps, warm):
-    """cell-steps/s of the oracle on `n_rows` seeded target rows per 'step' (each row against all N sources)."""
+def _pool_init(w, J, T):
+    try:                                                       # one thread per worker: the pool is the parallelism
+        from threadpoolctl import threadpool_limits
+        _POOL_STATE["limit"] = threadpool_limits(limits=1)
+    except Exception:
+        pass
+    _POOL_STATE.update(w=w, J=J, T=T)
+
+
+def _pool_rows(rows):
+    st = _POOL_STATE
+    oracle_row_sample(st["w"], rows, st["J"], st["T"], st["w"].dt)
+    return rows.size
+
+
+def oracle_workers():
+    """Worker processes of the oracle legs: one per host core the process may run on."""
+    try:
+        return max(1, len(os.sched_getaffinity(0)))
+    except Exception:
+        return max(1, os.cpu_count() or 1)
+
+
+class OraclePool:
+    """The oracle (unchanged, single-threaded numpy/scipy) run on all host cores: a fork pool over blocks of target
+    rows.  Must be created before CUDA is initialised in this process (fork)."""
+
+    def __init__(self, w, workers):
+        g = np.random.default_rng(w.seed + 7)
+        self.w, self.workers = w, workers
+        self.J = 1e7 * g.standard_normal(w.geometry.n_rings)
+        self.T = np.full(w.geometry.n_rings, w.geometry.T_bath)
+        self.pool = None
+        if workers > 1:
+            self.pool = multiprocessing.get_context("fork").Pool(workers, initializer=_pool_init, initargs=(w, self.J, self.T))
+
+    def seconds(self, rows):
+        """Wall seconds for the oracle to process `rows` (split evenly over the workers)."""
+        t0 = time.perf_counter()
+        if self.pool is None:
+            oracle_row_sample(self.w, rows, self.J, self.T, self.w.dt)
+        else:
+            parts = [p for p in np.array_split(rows, self.workers) if p.size]
+            self.pool.map(_pool_rows, parts, chunksize=1)
+        return time.perf_counter() - t0
+
+    def close(self):
+        if self.pool is not None:
+            self.pool.close()
+            self.pool.join()
+
+
+def run_oracle_sample(w, target_seconds, reps, warm):
+    """cell-steps/s of the oracle on a seeded sample of target rows per 'step' (each row against all N sources), all
+    host cores; the sample is sized so that one 'step' costs about target_seconds.  Returns (value, seconds, text, cores)."""
     geo = w.geometry
-    rows = wl.sample_rows(geo.n_rings, n_rows, seed=w.seed)
-    g = np.random.default_rng(w.seed + 7)
-    J = 1e7 * g.standard_normal(geo.n_rings)
-    T = np.full(geo.n_rings, geo.T_bath)
-    for _ in range(warm):
-        oracle_row_sample(w, rows[: max(1, n_rows // 8)], J, T, w.dt)
-    times = [oracle_row_sample(w, rows, J, T, w.dt) for _ in range(reps)]
+    workers = oracle_workers()
+    pool = OraclePool(w, workers)
+    try:
+        probe = wl.sample_rows(geo.n_rings, 2 * workers, seed=w.seed + 1)
+        pool.seconds(probe)                                   # imports, page-in
+        per_row = pool.seconds(probe) / probe.size            # wall seconds per row with every worker busy
+        n_rows = int(max(workers, min(geo.n_rings, round(target_seconds / max(per_row, 1e-9)))))
+        n_rows = max(workers, n_rows // workers * workers)
+        rows = wl.sample_rows(geo.n_rings, n_rows, seed=w.seed)
+        for _ in range(warm):
+            pool.seconds(rows[: max(workers, n_rows // 8)])
+        times = [pool.seconds(rows) for _ in range(reps)]
+    finally:
+        pool.close()
     total = float(np.sum(times))
-    return rows.size * reps / total, total, times
-
-
-def pick_rows(w, target_seconds):
-    """Number of sampled rows so that one oracle 'step' costs about target_seconds on this host."""
-    geo = w.geometry
-    rows = wl.sample_rows(geo.n_rings, 2, seed=w.seed + 1)
-    g = np.random.default_rng(1)
-    J = 1e7 * g.standard_normal(geo.n_rings)
-    T = np.full(geo.n_rings, geo.T_bath)
-    oracle_row_sample(w, rows[:1], J, T, w.dt)
-    t = oracle_row_sample(w, rows, J, T, w.dt) / rows.size
-    return int(max(2, min(geo.n_rings, round(target_seconds / max(t, 1e-9)))))
-
-
-def row_sample_text(w, n_rows):
-    return (f"{n_rows} seeded target cells of {w.name} per step, each against all {w.geometry.n_rings} source rings: "
-            "oracle field rows (S1) + material law (S2) + one M row (S3), scipy K/E + Maxwell bracket")
+    text = (f"{rows.size} seeded target cells of {w.name} per step, each against all {geo.n_rings} source rings: "
+            f"oracle field rows (S1) + material law (S2) + one M row (S3), scipy K/E + Maxwell bracket; "
+            f"{workers} worker processes of {os.cpu_count()} host CPUs")
+    return rows.size * reps / total, total, text, workers
 
 
 def run_oracle_steps(w, steps, warm):
@@ -188,7 +239,13 @@ def run_oracle_steps(w, steps, warm):
     for _ in range(steps):
         orc.step(w.dt, w.I_ramp)
     total = time.perf_counter() - t0
-    return w.geometry.n_rings * steps / total, total, f"{steps} full oracle steps of {w.name} (dense M, G_B; Cholesky KKT)"
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([int(d.get("num_threads", 1)) for d in threadpool_info()] or [1])
+    except Exception:
+        threads = 1
+    return (w.geometry.n_rings * steps / total, total,
+            f"{steps} full oracle steps of {w.name} (dense M, G_B; Cholesky KKT by LAPACK/BLAS on {threads} threads)", threads)
 
 
 def reference_arm(args):
@@ -197,16 +254,14 @@ def reference_arm(args):
         return
     w = wl.config(int(args.workload[3]))
     if w.geometry.n_rings <= 4096:
-        value, total, sample = run_oracle_steps(w, args.steps, args.warmup)
-    else:
-        n_rows = pick_rows(w, 60.0 / (args.steps + args.warmup))       # whole run ~ 1 minute of CPU work
-        value, total, _ = run_oracle_sample(w, n_rows, args.steps, args.warmup)
-        sample = row_sample_text(w, n_rows)
+        value, total, sample, cores = run_oracle_steps(w, args.steps, args.warmup)
+    else:                                                     # whole run ~ 1 minute of wall time on all cores
+        value, total, sample, cores = run_oracle_sample(w, 60.0 / (args.steps + args.warmup), args.steps, args.warmup)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "n_rings": w.geometry.n_rings, "dt": w.dt, "I_ramp": w.I_ramp},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -220,9 +275,10 @@ def pair_evals(n):
     return nb * (nb + 1) // 2 * 1024
 
 
-def timed_steps(torch, sim, w, steps, host_io=None):
+def timed_steps(torch, sim, w, steps, host_io=None, cg_iters=None):
     """K steps bracketed by CUDA events on the library's stream.  host_io = (J, T, outs): pinned host buffers
-    for the e2e variant (qs_write + qs_step + qs_read every step).  Returns (ms, launches)."""
+    for the e2e variant (qs_write + qs_step + qs_read every step).  cg_iters: list that receives the projected-CG
+    iterations of every step (host-side counter of the handle, no device access).  Returns (ms, launches)."""
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = sim.stats()["launches"]
     sim.sync()
@@ -235,6 +291,8 @@ def timed_steps(torch, sim, w, steps, host_io=None):
         rc = sim.step(w.dt, w.I_ramp)
         if rc < 0:
             raise RuntimeError(f"qs_step returned {rc}")
+        if cg_iters is not None:
+            cg_iters.append(sim.stats()["cg_iters"])
         if host_io is not None:
             sim.read(out=outs)
             J[:] = outs[0]
@@ -279,75 +337,85 @@ def hbm_roofline_leg(torch, pkg, hbm_peak):
     return out
 
 
-def operator_leg(torch, pkg, fp64_peak):
-    """Config 4: standalone y = M x on random rings (N = 262,144), plus CG iterations/s at N = 65,536."""
-    out = {}
-    n = 262144
-    geo, x = wl.free_rings(n)
-    with pkg.QS(geo, wl.Material()) as sim:
-        xd = torch.from_numpy(x).to(sim.device)
-        yd = torch.empty_like(xd)
-        torch.cuda.synchronize()
-        for _ in range(2):
-            sim.matvec_device(xd, yd)
-        sim.profile_enable(True)
-        for _ in range(5):
-            sim.matvec_device(xd, yd)
-        pr = sim.profile_read()
-    ms = pr["sweep_M"][0] / pr["sweep_M"][1]
-    pe = pair_evals(n)
-    out["matvec_N262144"] = {"ms": ms, "pair_evals_per_s": pe / ms * 1e3, "pair_interactions_per_s": n * n / ms * 1e3,
-                             "nominal_tflops": FLOP_K1 * pe / ms * 1e3 / 1e12,
-                             "frac_of_fp64_peak": FLOP_K1 * pe / ms * 1e3 / 1e12 / fp64_peak}
-    n = 65536
-    geo, x = wl.free_rings(n)
-    with pkg.QS(geo, wl.Material(cg_tol=1e-10)) as sim:
-        bd = torch.from_numpy(x).to(sim.device)
-        xd = torch.empty_like(bd)
-        torch.cuda.synchronize()
-        sim.solve_device(bd, xd, maxit=5)
-        sim.profile_enable(True)
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(sim.stream)
-        it, relres, _ = sim.solve_device(bd, xd, maxit=50)
-        b.record(sim.stream)
-        sim.sync()
-        b.synchronize()
-        pr = sim.profile_read()
-    # config 4 (b): b = M x, solve M xh = b to cg_tol = 1e-10 at N = 4096 (ill-conditioned: cond ~ 1e7), check xh ~ x
-    n4 = 4096
-    geo4, x4 = wl.free_rings(n4)
-    with pkg.QS(geo4, wl.Material(cg_tol=1e-10, cg_maxit=20000)) as sim:
-        xd = torch.from_numpy(x4).to(sim.device)
-        bd4 = torch.empty_like(xd)
-        xh = torch.empty_like(xd)
-        torch.cuda.synchronize()
-        sim.matvec_device(xd, bd4)
-        sim.sync()
-        a4, b4 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a4.record(sim.stream)
-        it4, rel4, rc4 = sim.solve_device(bd4, xh)
-        b4.record(sim.stream)
-        sim.sync()
-        b4.synchronize()
-        chk = torch.empty_like(xd)
-        sim.matvec_device(xh, chk)
-        sim.sync()
-    s4 = a4.elapsed_time(b4) * 1e-3
-    out["cg_N4096_to_tolerance"] = {"iterations": it4, "seconds": s4, "iters_per_s": it4 / s4, "relres": rel4,
-                                    "converged": rc4 == 0,
-                                    "residual_rel_l2": float(torch.linalg.norm(chk - bd4) / torch.linalg.norm(bd4)),
-                                    "solution_rel_l2": float(torch.linalg.norm(xh - xd) / torch.linalg.norm(xd))}
-    vec_us = 1e3 * pr["cg_vector"][0] / max(it, 1)
-    out["cg_N65536"] = {"iterations": it, "iters_per_s": it / (a.elapsed_time(b) * 1e-3), "relres_reached": relres,
-                        "sweep_ms_per_iteration": pr["sweep_M"][0] / max(pr["sweep_M"][1], 1),
-                        "vector_kernels_us_per_iteration": vec_us,
-                        "vector_kernels_GBs": 152.0 * n / (vec_us * 1e-6) / 1e9 if vec_us > 0 else None,
-                        "vector_bytes_per_ring": 152.0}
+def operator_leg(torch, pkg, fp64_peak, sizes=(4096, 65536, 262144, 1048576), budget_s=45.0):
+    """Config 4 (BASELINE.json configs[4]): the standalone y = M x and the CG solve M xh = b, b = M x, on random coaxial
+    ring sets at N = 4,096 / 65,536 / 262,144 / 1,048,576.  CG runs to cg_tol = 1e-10 where that takes seconds
+    (N <= 65,536) and for a fixed iteration budget above (the softened random-ring matrix has
+    cond ~ 1e7), reporting iterations/s and the residual reached."""
+    out = {"flop_per_pair_eval_nominal": FLOP_K1, "cg_tol": 1e-10,
+           "preconditioner": "block-Jacobi over the sweep's 32-ring Morton blocks (DESIGN.md section 6)"}
+    reps = {4096: 20, 65536: 10, 262144: 5, 1048576: 2}
+    to_tol = {4096: 20000, 65536: 6000}
+    for n in sizes:
+        geo, x = wl.free_rings(n)
+        with pkg.QS(geo, wl.Material(cg_tol=1e-10, cg_maxit=20000)) as sim:
+            xd = torch.from_numpy(x).to(sim.device)
+            bd = torch.empty_like(xd)
+            xh = torch.empty_like(xd)
+            torch.cuda.synchronize()
+            for _ in range(2):
+                sim.matvec_device(xd, bd)
+            sim.profile_enable(True)
+            for _ in range(reps.get(n, 2)):
+                sim.matvec_device(xd, bd)
+            pr = sim.profile_read()
+            sim.profile_enable(False)
+            ms = pr["sweep_M"][0] / pr["sweep_M"][1]
+            pe = pair_evals(n)
+            tf = FLOP_K1 * pe / ms * 1e3 / 1e12
+            rec = {"matvec_ms": ms, "pair_evals_per_s": pe / ms * 1e3, "pair_interactions_per_s": n * n / ms * 1e3,
+                   "nominal_tflops": tf, "frac_of_fp64_peak": tf / fp64_peak}
+            # CG: to tolerance, or the iterations that fit the time budget of this size (at least 20)
+            per_it_s = ms * 1e-3 * 1.05
+            maxit = to_tol.get(n) or int(max(20, min(200, budget_s / per_it_s)))
+            sim.solve_device(bd, xh, maxit=2)                 # graph capture, first-touch
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            sim.sync()
+            a.record(sim.stream)
+            it, relres, rc = sim.solve_device(bd, xh, maxit=maxit)
+            b.record(sim.stream)
+            sim.sync()
+            b.synchronize()
+            secs = a.elapsed_time(b) * 1e-3
+            chk = torch.empty_like(xd)
+            sim.matvec_device(xh, chk)
+            sim.sync()
+            rec["cg"] = {"mode": "to tolerance 1e-10" if n in to_tol else f"fixed budget of {maxit} iterations",
+                         "iterations": it, "seconds": secs, "iters_per_s": it / secs, "relres_reached": relres,
+                         "converged": rc == 0,
+                         "true_residual_rel_l2": float(torch.linalg.norm(chk - bd) / torch.linalg.norm(bd)),
+                         "solution_rel_l2": float(torch.linalg.norm(xh - xd) / torch.linalg.norm(xd))}
+        out[f"N{n}"] = rec
     return out
 
 
+def cg_active_leg(torch, pkg, steps=50, warm=20):
+    """Config 1 (single wire, 64 x 64 cells, ramped background field): the config whose steps really iterate the
+    projected CG (~200 iterations per step: K1 sweeps + K3/K4 vector kernels), timed next to the headline."""
+    w = wl.config(1)
+    its = []
+    with pkg.QS(w.geometry, w.material) as sim:
+        for _ in range(warm):
+            sim.step(w.dt, w.I_ramp)
+        ms, launches = timed_steps(torch, sim, w, steps, cg_iters=its)
+    N = w.geometry.n_rings
+    return {"workload": w.name, "n_rings": N, "steps": steps, "warmup": warm, "value": N * steps / (ms * 1e-3), "unit": UNIT,
+            "ms_per_step": ms / steps, "cg_iterations_per_step_mean": float(np.mean(its)), "cg_iterations_total": int(np.sum(its)),
+            "gpu_launches": int(launches)}
+
+
 def gpu_arm(args):
+    # the CPU oracle first (rank 0, one GPU, unless --no-extras): its worker pool is forked before this process
+    # creates a CUDA context
+    cpu_baseline = None
+    if int(os.environ.get("RANK", "0")) == 0 and args.gpus == 1 and not args.no_extras and args.leg == "all":
+        wb = wl.config(int(args.workload[3]))
+        if wb.geometry.n_rings <= 4096:
+            v, total, sample, cores = run_oracle_steps(wb, min(args.steps, 20), 1)
+        else:
+            v, total, sample, cores = run_oracle_sample(wb, 15.0, 1, 0)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "host_cpus": os.cpu_count(), "kind": "oracle",
+                        "sample": sample, "seconds": total}
     import torch
     import paper_2403_07666_b200 as pkg
 
@@ -377,21 +445,41 @@ def gpu_arm(args):
         return
 
     sim = pkg.QS(w.geometry, w.material, device=local, lattice_tables=args.operator == "tables")
+    # The very first step of a run solves for I' from a cold start: ~250 CG iterations, each a full K1 sweep (minutes at
+    # 864,000 rings) - a cost of the first step only, the timed steps are steps of the running trajectory.  For the big
+    # coils that first step is taken by a second handle with the lattice-tables operator (f1, ~0.2 s per sweep) and the
+    # state AND the rate I' are carried over through qs_read / qs_read_rate -> qs_write / qs_write_rate; the W warm-up
+    # steps and the K timed steps then run on the timed (pair-sweep) handle.
+    sim_tab, cold_start = None, "qs_step on the timed handle"
+    if args.operator == "pairs" and N > 100000:
+        sim_tab = pkg.QS(w.geometry, w.material, device=local, lattice_tables=True)
+        sim_tab.step(w.dt, w.I_ramp)
+        J1, T1 = sim_tab.read(B=False, E=False)[:2]
+        sim.write(J1, T1, sim_tab.stats()["t"], sim_tab.stats()["I"])
+        sim.write_rate(sim_tab.read_rate())
+        cold_start = ("first step (cold CG solve) on a lattice-tables handle, state + I' carried over by qs_write / "
+                      "qs_write_rate; all warm-up and timed steps on the pair-sweep handle")
+        if rank > 0 or world > 1 or args.no_extras:
+            sim_tab.close()
+            sim_tab = None
     for _ in range(args.warmup):
         sim.step(w.dt, w.I_ramp)
     # every leg below times the SAME K steps of the trajectory (the cost of a step drifts along it: config 1 needs more
     # CG iterations as the flux front moves in), so the state after the warm-up is kept and written back between legs
     snapJ, snapT = sim.read(B=False, E=False)[:2]
+    snapR = sim.read_rate()
     snap_t, snap_I = sim.stats()["t"], sim.stats()["I"]
 
     def rewind():
         sim.write(snapJ, snapT, snap_t, snap_I)
+        sim.write_rate(snapR)
 
     # ---- device-resident timing -----------------------------------------------------------------
     sampler = ClockSampler(local)
     barrier()
     sampler.start()
-    ms, launches = timed_steps(torch, sim, w, args.steps)
+    cg_its = []
+    ms, launches = timed_steps(torch, sim, w, args.steps, cg_iters=cg_its)
     barrier()
     clocks = sampler.stop()
     # the same K steps again with the library's event profiler recording (per-kernel-class device times for the
@@ -437,6 +525,7 @@ def gpu_arm(args):
     roofline = {"bound": "alu", "kernel": kname,
                 "achieved": ach, "peak": fp64_tf, "unit": "TFLOP/s", "frac": ach / fp64_tf,
                 "traffic": NCU_TRAFFIC.get(f"{dom}:{w.name}"),
+                "traffic_source": NCU_SOURCE if NCU_TRAFFIC.get(f"{dom}:{w.name}") is not None else None,
                 "peak_source": "measured in this run: DFMA-chain probe qs_fp64_peak; "
                                f"unit-count peak 148 SM x 64 lanes x 2 x 1.965 GHz = {FP64_PEAK_NOMINAL:.2f}",
                 "frac_of_nominal_peak": ach / FP64_PEAK_NOMINAL,
@@ -447,7 +536,7 @@ def gpu_arm(args):
     if ex is not None:   # executed flop per launch from the committed ncu capture / this run's launch time
         ex_tf = ex / (d_ms / max(d_n, 1) * 1e-3) / 1e12
         roofline["executed"] = {"achieved": ex_tf, "unit": "TFLOP/s", "frac": ex_tf / fp64_tf,
-                                "source": "profiles/r01_sweep_field_cfg2.md (sass_thread_inst_executed_op_d{add,mul,fma})"}
+                                "source": NCU_SOURCE + ": profiles/r01_sweep_field_cfg2.md (sass_thread_inst_executed_op_d{add,mul,fma})"}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
@@ -455,18 +544,18 @@ def gpu_arm(args):
                        "operator": args.operator,
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "per-cell arrays fit L2; the pair sweep is FP64-ALU bound, HBM legs use a 134 MB/array lattice",
-                       "cg_iters_last_step": st["cg_iters"], "heat_substeps": st["heat_substeps"]},
+                       "cg_iterations_timed": int(np.sum(cg_its)), "cg_iterations_per_step_mean": float(np.mean(cg_its)),
+                       "cg_note": "linear-regime steps: the warm-started CG is converged on entry, a step is one fused K2 "
+                                  "sweep + O(N) passes; see cg_active for steps that iterate" if int(np.sum(cg_its)) == 0 else None,
+                       "cold_start": cold_start, "heat_substeps": st["heat_substeps"]},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()}}
     if rank == 0 and world == 1 and not args.no_extras:
         line["issue_model"] = dict(pkg.issue_probe(), unit="SM cycles per DFMA warp-instruction per sub-partition",
                                    note="FP64 pipe rate is 2; a third register operand costs a cycle, and so does every "
                                         "non-FP64 instruction issued beside the DFMAs (DESIGN.md section 6)")
-        line["roofline_hbm"] = hbm_roofline_leg(torch, pkg, hbm_peak)
-        line["roofline_hbm"]["peak_source"] = f"MEASURED_PEAKS.json hbm_gbs ({hbm_src})"
-        line["operator_cfg4"] = operator_leg(torch, pkg, fp64_tf)
         if args.operator == "pairs":   # SURVEY.md §8(f) f1, same workload: tables over (ir, jr, |dz|) + block-Toeplitz sweeps
-            with pkg.QS(w.geometry, w.material, device=local, lattice_tables=True) as sim2:
+            with (sim_tab if sim_tab is not None else pkg.QS(w.geometry, w.material, device=local, lattice_tables=True)) as sim2:
                 for _ in range(args.warmup):
                     sim2.step(w.dt, w.I_ramp)
                 ms2, _ = timed_steps(torch, sim2, w, args.steps)
@@ -478,14 +567,12 @@ def gpu_arm(args):
                 "value": N * args.steps / (ms2 * 1e-3), "unit": UNIT, "ms_per_step": ms2 / args.steps,
                 "sweep_ms": sw_ms, "sweep_tflops": 6.0 * N * N / (sw_ms * 1e-3) / 1e12 if sw_ms > 0 else None,
                 "note": "not the graded path: north_star fixes on-the-fly AGM pair evaluation"}
-        if N <= 4096:
-            v, total, sample = run_oracle_steps(w, min(args.steps, 20), 1)
-        else:
-            n_rows = pick_rows(w, 15.0)
-            v, total, _ = run_oracle_sample(w, n_rows, 1, 0)
-            sample = row_sample_text(w, n_rows)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle", "sample": sample,
-                                "seconds": total}
+        line["roofline_hbm"] = hbm_roofline_leg(torch, pkg, hbm_peak)
+        line["roofline_hbm"]["peak_source"] = f"MEASURED_PEAKS.json hbm_gbs ({hbm_src})"
+        line["roofline_hbm"]["traffic_source"] = NCU_SOURCE
+        line["cg_active"] = cg_active_leg(torch, pkg)
+        line["operator_cfg4"] = operator_leg(torch, pkg, fp64_tf)
+        line["cpu_baseline"] = cpu_baseline
     if rank == 0:
         print(json.dumps(line), flush=True)
     group.close()

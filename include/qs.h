@@ -17,9 +17,12 @@
  *     stream; they return after the work has been enqueued and checked for launch errors only.
  *   - FP64 throughout (BASELINE.json configs[0]).  SI units.  Ring order is the caller's order
  *     (lattice: canonical c = ir*Nz + iz, C1); any internal re-ordering is invisible.
- *   - Return value: 0 = OK, negative = error (state unchanged), and for qs_step a non-negative
- *     event bitmask.  qs_last_error() returns a human-readable message for the calling thread.
- *   - One handle per host thread; calls on one handle are serialised on its stream.
+ *   - Return value: 0 = OK, negative = error (state unchanged: J, T, t, I, the fields B, E of qs_read, the event
+ *     flags / counters and the per-wire statistics are what they were before the call), and for qs_step a
+ *     non-negative event bitmask.  qs_last_error() returns a human-readable message for the calling thread.
+ *   - One handle per host thread; calls on one handle are serialised on its stream.  A handle lives on the CUDA
+ *     device that was current at qs_init; every call makes that device current for its duration and restores
+ *     the caller's, so handles on different devices can be used from one process.
  */
 #ifndef QS_H_
 #define QS_H_
@@ -170,6 +173,14 @@ int  qs_init_device(const qs_geometry *geo, const qs_material *mat, void *worksp
  * solution of the step does not depend on it beyond cg_tol).  */
 int  qs_write(qs_ctx *ctx, const double *J, const double *T, double t, double I);
 
+/* Checkpoint / resume of the solver's warm start (SURVEY.md §5 "Checkpoint / resume"; C8 "x0 = previous I'"): the
+ * rate I' = dI/dt [A/s per ring, N values, caller's order] of the last step's solve (S3), which the next qs_step uses
+ * as the projected CG's initial guess.  qs_read_rate copies it out; qs_write_rate sets it (host buffers).  A guess
+ * only: the solution of a step does not depend on it beyond cg_tol, but a run resumed with (J, T, t, I) through
+ * qs_write and I' through qs_write_rate continues with the iteration counts of the uninterrupted run.  */
+int  qs_read_rate(qs_ctx *ctx, double *Idot);
+int  qs_write_rate(qs_ctx *ctx, const double *Idot);
+
 /* y = M x (C2): x [A] -> y [Wb], symmetric mutual-inductance matrix, evaluated pair by pair.  */
 int  qs_matvec(qs_ctx *ctx, const double *x, double *y);
 int  qs_matvec_device(qs_ctx *ctx, const double *d_x, double *d_y);
@@ -193,7 +204,16 @@ int  qs_heat_adi(qs_ctx *ctx, double dt, int32_t m);   /* S6 alone by m ADI sub-
 int  qs_set_fields(qs_ctx *ctx, const double *B, const double *Q);
 int  qs_read_aux(qs_ctx *ctx, double *Q, double *dEdJ, double *Jc, double *rho);   /* dEdJ: see qs_set_aux */
 
+/* Observables of the last step / solve (qs_stats_t above): CG iterations and residual (C8), the terminal voltage
+ * U = -sum_w share_w V_w of the per-turn multipliers (S4; PAPER.md:99 coil voltage), Tmax and the Joule power
+ * sum_i E_i J_i 2 pi r_i a_i (PAPER.md:75 source term E.J; PAPER.md:65 figures), t, I, the step's event word, and
+ * the launch / pair-evaluation counters.  Host struct, filled without touching the device.  */
 int  qs_stats(qs_ctx *ctx, qs_stats_t *out);
+
+/* Test hook: make the NEXT qs_step / qs_step_rk fail after the current update S5 has been applied, to exercise the
+ * transactional restore: where = 1 -> QS_ERR_CUDA reported by the heat stage; 2 -> a NaN planted in J (the step's
+ * own NaN/Inf check then returns QS_ERR_NONFINITE); 0 -> cancel.  One-shot.  */
+int  qs_debug_inject_failure(qs_ctx *ctx, int32_t where);
 
 /* ---- measurement (bench.py) ---------------------------------------------------
  * Device-side timing of the library's own kernels with cudaEvent pairs recorded on the handle's
@@ -233,6 +253,11 @@ int  qs_fp64_peak(double *tflops, double *sm_clock_mhz_effective);
  * operands; mode 2: two register operands and an immediate; mode 3: mode 2 plus one integer ALU instruction per
  * DFMA.  Needs no handle.  */
 int  qs_issue_probe(int32_t mode, double *cycles_per_dfma);
+/* Per-turn state of the event detector S7 (C10) after the last step: flag word (QS_FJ_* | QS_Q_*: the paper's
+ * flux-jump criterion |J/Jc| > 1, and quench criterion rho > 0.95 rho_n, plus configs[3]'s
+ * T > 10 K, dE/dt spike and T > Tc), time of the first step in which any flag of the turn was set (-1: never) and the
+ * number of rising edges of FJ_T|FJ_E (the per-wire flux-jump count of PAPER.md:93, Fig. 3(b)).  HOST buffers of N_w
+ * entries each, NULL = skip; with constraint groups finer than wires (C16) the entries are per group.  */
 int  qs_events(qs_ctx *ctx, int32_t *flags /*[N_w]*/, double *t_first /*[N_w]*/, int32_t *count /*[N_w]*/);
 /* Per-wire statistics accumulated by the event pass since qs_init / the last qs_write (
  * PAPER.md:107 T_max, P_max, Q_FJ per wire; PAPER.md:119-121 Q_q, P_q, T_q at the quench time).  out: HOST buffer of
@@ -243,8 +268,13 @@ int  qs_events(qs_ctx *ctx, int32_t *flags /*[N_w]*/, double *t_first /*[N_w]*/,
  *   4 t_q [s] (-1: never), 5 T_q [K], 6 P_q [W/m^3]   time, Tmax and max_i Q_i at the first step with a quench flag
  *   7 Q_q [J]      Joule energy of the wire from its first event to the quench  */
 int  qs_wire_stats(qs_ctx *ctx, double *out);
-int  qs_sync(qs_ctx *ctx);                 /* wait for the handle's stream */
+/* Wait until all work enqueued on the handle's stream has finished (the *_device variants return after enqueueing;
+ * SURVEY.md §8(b) "calls on one handle are serialised on its stream").  Returns 0 or QS_ERR_CUDA.  */
+int  qs_sync(qs_ctx *ctx);
 const char *qs_last_error(void);
+/* Destroy the handle (SURVEY.md §8(b) ownership): waits for its stream, frees what qs_init allocated (workspace and
+ * stream of the owning variant, pinned staging buffers, CUDA graphs); never frees caller memory - the workspace and
+ * stream handed to qs_init_device stay the caller's.  NULL is a no-op.  */
 void qs_free(qs_ctx *ctx);
 
 #ifdef __cplusplus

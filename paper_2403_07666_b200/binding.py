@@ -61,6 +61,9 @@ SYMBOLS = [
     ("qs_workspace_bytes", C.c_size_t, [C.POINTER(QsGeometry)]),
     ("qs_init_device", C.c_int, [C.POINTER(QsGeometry), C.POINTER(QsMaterial), _VP, C.c_size_t, _VP, C.POINTER(_VP)]),
     ("qs_write", C.c_int, [_VP, c_double_p, c_double_p, C.c_double, C.c_double]),
+    ("qs_read_rate", C.c_int, [_VP, c_double_p]),
+    ("qs_write_rate", C.c_int, [_VP, c_double_p]),
+    ("qs_debug_inject_failure", C.c_int, [_VP, C.c_int32]),
     ("qs_matvec", C.c_int, [_VP, c_double_p, c_double_p]),
     ("qs_matvec_device", C.c_int, [_VP, _VP, _VP]),
     ("qs_field", C.c_int, [_VP, c_double_p, c_double_p]),
@@ -272,6 +275,18 @@ class QS:
         Ja = None if J is None else _f64(J, self.N)
         Ta = None if T is None else _f64(T, self.N)
         self._check(self._lib.qs_write(self._h, _dp(Ja), _dp(Ta), float(t), float(I)))
+
+    def read_rate(self) -> np.ndarray:
+        """I' = dI/dt per ring of the last step's solve (the next step's CG start)."""
+        x = np.empty(self.N)
+        self._check(self._lib.qs_read_rate(self._h, _dp(x)))
+        return x
+
+    def write_rate(self, Idot):
+        self._check(self._lib.qs_write_rate(self._h, _dp(_f64(Idot, self.N))))
+
+    def debug_inject_failure(self, where: int):
+        self._check(self._lib.qs_debug_inject_failure(self._h, int(where)))
 
     def matvec(self, x) -> np.ndarray:
         xa = _f64(x, self.N)

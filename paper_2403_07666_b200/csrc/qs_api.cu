@@ -3,6 +3,7 @@
 // Host code only enqueues kernels on the handle's stream and reads back one small Scalars block per CG
 // iteration (the convergence test) and per step (events, statistics).  No arithmetic of the method runs
 // on the host except set-up constants (bounding boxes, Morton order of free rings, self-field coefficients).
+// Every entry point makes the handle's device current for the duration of the call (DeviceGuard).
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
@@ -45,6 +46,21 @@ struct Carver {
     off += count * sizeof(T);
     return p;
   }
+};
+
+// Makes `dev` the current CUDA device for the lifetime of the guard (handles may live on different devices of one
+// process; kernels, events and copies of a handle must be issued with its device current).
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
 };
 
 }  // namespace
@@ -121,6 +137,13 @@ struct qs_ctx {
   cudaStream_t stream = nullptr;
   void* owned = nullptr;             // cudaMalloc'ed workspace (qs_init) or nullptr (qs_init_device)
   int sm_count = 148;
+  int device = 0;                    // the CUDA device the handle lives on (current at qs_init)
+  int inject = 0;                    // qs_debug_inject_failure: 1 = CUDA error in the heat stage, 2 = NaN in J after S5
+  // transactional step: the derived fields (Br, Bz, E) and the per-turn event state (wire statistics, ebar_prev,
+  // t_first, flags, count) are each one contiguous block with a backup block of the same size
+  char *fld_begin = nullptr, *fld_backup = nullptr, *ev_begin = nullptr, *ev_backup = nullptr;
+  size_t fld_bytes = 0, ev_bytes = 0;
+  bool have_prev_E_old = false;
   double *r, *z, *area, *jc0s, *selfcoef, *diagM;
   double *J, *Jold, *Ha, *Hb, *Hold, *Br, *Bz, *E, *dEdJ, *Q, *b, *shift, *Hd, *Jc, *rho;
   double *x, *xold, *cur, *p, *q, *rr, *g, *xp1, *Mxp1, *tmp, *tmp2, *zero;
@@ -143,6 +166,14 @@ struct qs_ctx {
     cudaGraphExec_t exec = nullptr;
     int launches = 0;
   } cg_graph[2];
+  // CUDA graphs of the m explicit heat sub-steps of one step (launch-bound on lattices that live in L2), keyed by the
+  // buffer the step starts from, m and the sub-step length
+  struct HeatGraph {
+    const double* H = nullptr;
+    int m = 0;
+    double sub = 0.0;
+    cudaGraphExec_t exec = nullptr;
+  } heat_graph[2];
   bool canonical_turns = false;      // turn_id[c] == (ir / n) * turns_per_layer + iz / n for every cell
   bool aux_on = false;               // qs_material_eval also writes dE/dJ (after the first qs_read_aux)
   double last_eval_dt = 0.0;
@@ -181,9 +212,14 @@ void carve(qs_ctx* c, void* base, size_t* total) {
   c->Ha = k.take<double>(N);
   c->Hb = k.take<double>(N);
   c->Hold = k.take<double>(N);
+  k.off = align_up(k.off, 256);
+  const size_t fld0 = k.off;
+  c->fld_begin = base ? static_cast<char*>(base) + fld0 : nullptr;
   c->Br = k.take<double>(N);
   c->Bz = k.take<double>(N);
   c->E = k.take<double>(N);
+  c->fld_bytes = k.off - fld0;
+  c->fld_backup = reinterpret_cast<char*>(k.take<char>(c->fld_bytes));
   c->dEdJ = k.take<double>(N);
   c->Q = k.take<double>(N);
   c->b = k.take<double>(N);
@@ -218,12 +254,17 @@ void carve(qs_ctx* c, void* base, size_t* total) {
   c->vsum = k.take<double>(nt);
   c->tw = k.take<double>(nt);
   c->defw = k.take<double>(nt);
+  c->share = k.take<double>(nt);
+  k.off = align_up(k.off, 256);
+  const size_t ev0 = k.off;
+  c->ev_begin = base ? static_cast<char*>(base) + ev0 : nullptr;
   c->ebar_prev = k.take<double>(nt);
   c->t_first = k.take<double>(nt);
   c->wire = k.take<double>(9 * nt);
-  c->share = k.take<double>(nt);
   c->flags = k.take<int>(nt);
   c->count = k.take<int>(nt);
+  c->ev_bytes = k.off - ev0;
+  c->ev_backup = reinterpret_cast<char*>(k.take<char>(c->ev_bytes));
   c->turn_ptr = k.take<int>(nt + 1);
   c->turn_idx = k.take<int>(N);
   c->turn_id = k.take<int>(N);
@@ -306,7 +347,7 @@ int do_sweep(qs_ctx* c, const double* x, const double* cur, bool field, bool pre
   prm.counter = c->counter;
   prm.done = cg_guard ? &c->sc->done : nullptr;
   prm.nb = c->nb;
-  prm.n_items = static_cast<long long>(c->nb) * (c->nb + 1) / 2;
+  prm.n_items = sweep_items(c->nb, field);
   prm.soft_all = c->soft_all;
   prm.soft_self = c->soft_self;
   prm.minsep2 = c->minsep2;
@@ -321,7 +362,7 @@ int do_sweep(qs_ctx* c, const double* x, const double* cur, bool field, bool pre
   QS_CUDA(launch_sweep(prm, field, grid, c->stream));
   c->prof.end(c->stream, field ? QS_PROF_SWEEP_FIELD : QS_PROF_SWEEP_M, 1);
   ++c->launches;
-  c->pair_evals += prm.n_items * 1024;
+  c->pair_evals += (static_cast<long long>(c->nb) * (c->nb + 1) / 2) * 1024;   // every unordered block pair once
   ++c->st.sweeps;
   return QS_OK;
 }
@@ -332,25 +373,31 @@ constexpr double kCM = 0.5 * kMu0 * kPi;   // yacc -> henry * ampere
 // In: x satisfies the constraint; if yacc_has_Mx the accumulators hold the sweep of x.  nu < 0: nu = start norm.
 // Iterations are enqueued in batches without a host round trip: the kernels stop themselves (Scalars::done) at the
 // iteration where sqrt(r^T g) <= tol nu, so the result is the one of the iteration-by-iteration loop.
+// prepared: r, g, p, rg[0], vsum and the reference norm (Scalars::nu2) were produced by k_turn_start (fused step path);
+// nu_out receives the reference norm used.
 int cg_core(qs_ctx* c, const Rhs& b, double* x, const double* shift, const double* Hd, const double* sw,
             bool yacc_has_Mx, double tol, int maxit, double nu, int* iters, double* relres, bool* hit_max,
-            const double* Lblk = nullptr) {
+            const double* Lblk = nullptr, bool prepared = false, double* nu_out = nullptr) {
   const VecCtx& v = c->v;
   int rc;
-  if (!yacc_has_Mx && (rc = do_sweep(c, x, nullptr, false)) != QS_OK) return rc;
-  k_residual(v, c->yacc, shift, x, b, c->rr, kCM);
-  if (c->n_turns) QS_CUDA(cudaMemsetAsync(c->vsum, 0, sizeof(double) * c->n_turns, c->stream));
-  k_turn_project(v, c->rr, Hd, sw, c->vw, c->vsum);
-  if (Lblk) {   // block-Jacobi preconditioner: g = B^-1 r, rg[0] = r.g (rg[0] is zero on entry)
-    QS_CUDA(launch_blockprec_apply(c->nb, c->N, Lblk, c->rr, c->g, &c->sc->rg[0], nullptr, c->stream));
-    ++c->launches;
-  } else {
-    k_project_apply(v, 0, c->vw, Hd, c->rr, c->g);
+  if (!prepared) {
+    if (!yacc_has_Mx && (rc = do_sweep(c, x, nullptr, false)) != QS_OK) return rc;
+    k_residual(v, c->yacc, shift, x, b, c->rr, kCM);
+    if (c->n_turns) QS_CUDA(cudaMemsetAsync(c->vsum, 0, sizeof(double) * c->n_turns, c->stream));
+    k_turn_project(v, c->rr, Hd, sw, c->vw, c->vsum);
+    if (Lblk) {   // block-Jacobi preconditioner: g = B^-1 r, rg[0] = r.g (rg[0] is zero on entry)
+      QS_CUDA(launch_blockprec_apply(c->nb, c->N, Lblk, c->rr, c->g, &c->sc->rg[0], nullptr, c->stream));
+      ++c->launches;
+    } else {
+      k_project_apply(v, 0, c->vw, Hd, c->rr, c->g);
+    }
+    k_direction(v, 0, true, c->g, c->p);
   }
-  k_direction(v, 0, true, c->g, c->p);
   if ((rc = sync_scalars(c)) != QS_OK) return rc;
   double rg = c->h_sc->rg[0];
+  if (prepared) nu = std::sqrt(std::max(c->h_sc->nu2, 0.0));
   if (nu < 0.0) nu = std::sqrt(std::max(rg, 0.0));
+  if (nu_out) *nu_out = nu;
   *hit_max = false;
   *iters = 0;
   if (!(rg == rg)) return fail(QS_ERR_NONFINITE, "CG: r^T g is NaN");
@@ -499,9 +546,46 @@ int run_heat(qs_ctx* c, double dt, int* m_out) {
     std::swap(c->H, c->Halt);
     c->prof.end(c->stream, QS_PROF_HEAT, 1);
   } else {
-    for (int s = 0; s < m; ++s) {
-      k_heat_substep(c->v, c->mp, c->lp, c->H, c->Q, c->Halt, sub);
-      std::swap(c->H, c->Halt);
+    qs_ctx::HeatGraph* hg = nullptr;
+    if (!c->prof.on && m >= 4) {   // replay the m launches from a graph (captured on first use for this start buffer)
+      for (auto& slot : c->heat_graph)
+        if (slot.exec && slot.H == c->H && slot.m == m && slot.sub == sub) hg = &slot;
+      if (!hg) {
+        qs_ctx::HeatGraph& slot = c->heat_graph[c->heat_graph[0].exec && c->heat_graph[0].H != c->H ? 1 : 0];
+        if (slot.exec) {
+          cudaGraphExecDestroy(slot.exec);
+          slot.exec = nullptr;
+        }
+        const long long l0 = c->launches;
+        cudaGraph_t gr = nullptr;
+        if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed) == cudaSuccess) {
+          double *a = c->H, *b = c->Halt;
+          for (int s = 0; s < m; ++s) {
+            k_heat_substep(c->v, c->mp, c->lp, a, c->Q, b, sub);
+            std::swap(a, b);
+          }
+          const cudaError_t ec = cudaStreamEndCapture(c->stream, &gr);
+          if (ec == cudaSuccess && gr && cudaGraphInstantiate(&slot.exec, gr, 0) == cudaSuccess) {
+            slot.H = c->H, slot.m = m, slot.sub = sub;
+            hg = &slot;
+          } else {
+            slot.exec = nullptr;
+            cudaGetLastError();
+          }
+          if (gr) cudaGraphDestroy(gr);
+        }
+        c->launches = l0;   // capture enqueued nothing
+      }
+    }
+    if (hg) {
+      QS_CUDA(cudaGraphLaunch(hg->exec, c->stream));
+      c->launches += m;
+      if (m & 1) std::swap(c->H, c->Halt);
+    } else {
+      for (int s = 0; s < m; ++s) {
+        k_heat_substep(c->v, c->mp, c->lp, c->H, c->Q, c->Halt, sub);
+        std::swap(c->H, c->Halt);
+      }
     }
     c->prof.end(c->stream, QS_PROF_HEAT, m);
   }
@@ -567,6 +651,34 @@ MaterialArgs material_args(qs_ctx* c, double Bext, double Bdot, double dt, bool 
   return a;
 }
 
+// Transactional step (include/qs.h: "negative = error (state unchanged)"): everything a step modifies that the caller
+// can observe is copied aside first - J, H, I' and, as two contiguous blocks, the derived fields (Br, Bz, E) and the
+// per-turn event state (wire statistics, mean-E history, first-event times, flag words, counters).
+int backup_state(qs_ctx* c) {
+  const size_t nb8 = sizeof(double) * c->N;
+  QS_CUDA(cudaMemcpyAsync(c->Jold, c->J, nb8, cudaMemcpyDeviceToDevice, c->stream));
+  QS_CUDA(cudaMemcpyAsync(c->Hold, c->H, nb8, cudaMemcpyDeviceToDevice, c->stream));
+  QS_CUDA(cudaMemcpyAsync(c->xold, c->x, nb8, cudaMemcpyDeviceToDevice, c->stream));
+  QS_CUDA(cudaMemcpyAsync(c->fld_backup, c->fld_begin, c->fld_bytes, cudaMemcpyDeviceToDevice, c->stream));
+  if (c->n_turns) QS_CUDA(cudaMemcpyAsync(c->ev_backup, c->ev_begin, c->ev_bytes, cudaMemcpyDeviceToDevice, c->stream));
+  c->have_prev_E_old = c->have_prev_E;
+  return QS_OK;
+}
+// Called on every negative return after backup_state: puts the state back (best effort if the device itself failed).
+// The stored previous solutions of the extrapolated CG start are dropped (a guess only).
+void restore_state(qs_ctx* c) {
+  const size_t nb8 = sizeof(double) * c->N;
+  cudaGetLastError();
+  cudaMemcpyAsync(c->J, c->Jold, nb8, cudaMemcpyDeviceToDevice, c->stream);
+  cudaMemcpyAsync(c->H, c->Hold, nb8, cudaMemcpyDeviceToDevice, c->stream);
+  cudaMemcpyAsync(c->x, c->xold, nb8, cudaMemcpyDeviceToDevice, c->stream);
+  cudaMemcpyAsync(c->fld_begin, c->fld_backup, c->fld_bytes, cudaMemcpyDeviceToDevice, c->stream);
+  if (c->n_turns) cudaMemcpyAsync(c->ev_begin, c->ev_backup, c->ev_bytes, cudaMemcpyDeviceToDevice, c->stream);
+  cudaStreamSynchronize(c->stream);
+  c->have_prev_E = c->have_prev_E_old;
+  c->n_prev = 0;
+}
+
 // One electromagnetic stage (S1..S4) at the state Jsrc: field sweep fused with M x0, material law (diagonal shift
 // theta dt_shift D), projected CG for I' (left in c->x, warm-started from its previous content), multipliers -> uterm.
 int em_stage(qs_ctx* c, const double* Jsrc, double Bext, double Bdot, double dt_shift, double I_ramp, int* iters,
@@ -591,6 +703,8 @@ int em_stage(qs_ctx* c, const double* Jsrc, double Bext, double Bdot, double dt_
   // S3/S4: the right-hand side b = -2 pi r (E + r Bdot / 2) is evaluated on the fly from E (C4)
   const Rhs rhs{nullptr, c->E, c->r, Bdot};
   double nu = -1.0;
+  // the reference norm is accumulated into rg[0]: start from zero whatever an earlier stage of this step left there
+  QS_CUDA(cudaMemsetAsync(c->sc->rg, 0, 2 * sizeof(double), c->stream));
   if (c->n_turns) {
     k_turn_schur(v, c->Hd, c->sw);
     k_nu_residual(v, I_ramp, c->Mxp1, c->shift, c->xp1, rhs, c->rr);
@@ -620,6 +734,61 @@ int em_stage(qs_ctx* c, const double* Jsrc, double Bext, double Bdot, double dt_
   return QS_OK;
 }
 
+// The same stage for qs_step on geometries with constraint groups, in five launches and one host round trip before the
+// CG iterates: step_begin (backups, CG start, I = a J, zeroing) -> turn_fix (start moved onto the constraint) -> fused
+// sweep -> material -> turn_start (Schur scalars, reference norm, start residual, projection, first direction).
+int em_stage_fused(qs_ctx* c, bool extrapolate, double Bext, double Bdot, double dt, double I_ramp, int* iters,
+                   double* relres, bool* hit_max) {
+  const VecCtx& v = c->v;
+  int rc;
+  *iters = 0;
+  *relres = 0.0;
+  *hit_max = false;
+  StepBegin sb{};
+  sb.N = c->N;
+  sb.n_turns = c->n_turns;
+  sb.extrapolate = extrapolate;
+  sb.J = c->J; sb.H = c->H; sb.area = c->area;
+  sb.Jold = c->Jold; sb.Hold = c->Hold; sb.x = c->x; sb.xold = c->xold; sb.xprev2 = c->xprev2; sb.cur = c->cur;
+  sb.fld = reinterpret_cast<const unsigned long long*>(c->fld_begin);
+  sb.fld_backup = reinterpret_cast<unsigned long long*>(c->fld_backup);
+  sb.fld_words = c->fld_bytes / 8;
+  sb.ev = reinterpret_cast<const unsigned long long*>(c->ev_begin);
+  sb.ev_backup = reinterpret_cast<unsigned long long*>(c->ev_backup);
+  sb.ev_words = c->ev_bytes / 8;
+  sb.acc = reinterpret_cast<unsigned long long*>(c->counter);
+  sb.acc_words = c->acc_bytes / 8;
+  sb.vsum = c->vsum; sb.tw = c->tw;
+  const bool ev = c->lattice && c->n_turns > 0;
+  sb.xmax_bits = ev ? c->xmax_bits : nullptr;
+  sb.rmin_bits = ev ? c->rmin_bits : nullptr;
+  k_step_begin(v, sb);
+  c->have_prev_E_old = c->have_prev_E;
+  k_turn_fix(v, I_ramp, c->diagM, c->swM, c->x);
+  if ((rc = do_sweep(c, c->x, c->cur, true, /*prezeroed=*/true)) != QS_OK) return rc;
+  c->prof.begin(c->stream);
+  k_material(v, c->mp, material_args(c, Bext, Bdot, dt, true, false, c->J));
+  c->prof.end(c->stream, QS_PROF_MATERIAL, 1);
+  const Rhs rhs{nullptr, c->E, c->r, Bdot};
+  TurnStart ts{};
+  ts.ptr = c->turn_ptr; ts.idx = c->turn_idx;
+  ts.I_ramp = I_ramp; ts.cM = kCM; ts.b = rhs;
+  ts.Hd = c->Hd; ts.shift = c->shift; ts.x = c->x; ts.yacc = c->yacc; ts.xp1 = c->xp1; ts.Mxp1 = c->Mxp1;
+  ts.r = c->rr; ts.g = c->g; ts.p = c->p; ts.sw = c->sw; ts.vnu = c->defw; ts.vsum = c->vsum;
+  k_turn_start(v, ts);
+  double nu = 0.0;
+  rc = cg_core(c, rhs, c->x, c->shift, c->Hd, c->sw, true, c->cg_tol, c->cg_maxit, -1.0, iters, relres, hit_max, nullptr,
+               /*prepared=*/true, &nu);
+  if (rc != QS_OK) return rc;
+  if (nu == 0.0) {
+    // the cold start x_p = I_ramp xp1 already solves the projected system (see em_stage); its multipliers are the V_w
+    QS_CUDA(cudaMemsetAsync(c->x, 0, sizeof(double) * c->N, c->stream));
+    k_axpy(v, I_ramp, c->xp1, c->x);
+    QS_CUDA(cudaMemcpyAsync(c->vsum, c->defw, sizeof(double) * c->n_turns, cudaMemcpyDeviceToDevice, c->stream));
+  }
+  return QS_OK;
+}
+
 // Common tail of qs_step / qs_step_rk once J^{k+1} has been written: S6 heat with the current Q, S7 events and step
 // statistics, NaN/Inf check (state restored from the backups on failure), commit of t, I and the statistics.
 // uterm_scale: factor applied to the accumulated multiplier sum (1, or 1/2 for the two stages of the RK pair);
@@ -627,14 +796,22 @@ int em_stage(qs_ctx* c, const double* Jsrc, double Bext, double Bdot, double dt_
 int finish_step(qs_ctx* c, double dt, double I_ramp, int iters, double relres, bool hit_max, double uterm_scale,
                 bool reset_scalars) {
   const VecCtx& v = c->v;
-  const size_t nb8 = sizeof(double) * c->N;
   int rc, m = 0;
   double uterm = 0.0;
   if (reset_scalars) {
     uterm = uterm_scale * c->h_sc->uterm;        // read back by the caller's last sync_scalars
     k_set_scalars(v);
   }
-  if ((rc = run_heat(c, dt, &m)) != QS_OK) return rc;
+  if (c->inject == 2) {   // test hook: a NaN in J after S5
+    c->inject = 0;
+    cudaMemsetAsync(c->J, 0xff, sizeof(double), c->stream);
+  }
+  rc = c->inject == 1 ? (c->inject = 0, fail(QS_ERR_CUDA, "injected failure in the heat stage (qs_debug_inject_failure)"))
+                      : run_heat(c, dt, &m);
+  if (rc != QS_OK) {
+    restore_state(c);
+    return rc;
+  }
   EventArgs ev;
   ev.H = c->H; ev.E = c->E; ev.xmax_bits = c->xmax_bits; ev.rmin_bits = c->rmin_bits;
   ev.Q = c->Q; ev.r = c->r; ev.area = c->area; ev.wire = c->wire;
@@ -644,12 +821,12 @@ int finish_step(qs_ctx* c, double dt, double I_ramp, int iters, double relres, b
   k_events(v, c->mp, ev);
   k_step_stats(v, c->mp, c->J, c->Jold, c->H, c->Q, c->r, c->area);
   c->prof.end(c->stream, QS_PROF_EVENTS, c->n_turns ? 2 : 1);
-  if ((rc = sync_scalars(c)) != QS_OK) return rc;
+  if ((rc = sync_scalars(c)) != QS_OK) {
+    restore_state(c);
+    return rc;
+  }
   if (c->h_sc->nonfinite) {
-    cudaMemcpyAsync(c->J, c->Jold, nb8, cudaMemcpyDeviceToDevice, c->stream);
-    cudaMemcpyAsync(c->H, c->Hold, nb8, cudaMemcpyDeviceToDevice, c->stream);
-    cudaMemcpyAsync(c->x, c->xold, nb8, cudaMemcpyDeviceToDevice, c->stream);
-    cudaStreamSynchronize(c->stream);
+    restore_state(c);
     return fail(QS_ERR_NONFINITE, "NaN/Inf in J or T after the step; state restored");
   }
   if (!reset_scalars) uterm = uterm_scale * c->h_sc->uterm;
@@ -745,9 +922,10 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
     for (int s = 0; s < 4; ++s) lp.h_conv[s] = geo->h_conv[s];
     c->tabNr = lp.Nr;
     c->tabNz = lp.Nz;
-    // the lattice description must agree with the ring arrays (C1)
-    const int probe[4] = {0, N - 1, N / 2, N / 3};
-    for (int k : probe) {
+    // the lattice description must agree with the ring arrays (C1), ring by ring: the heat tables, the per-row
+    // geometry, the block-Toeplitz tables and the separation bound minsep2 = h^2 behind the AGM evaluation classes
+    // all come from the description, the pair sweep from the arrays
+    for (int k = 0; k < N; ++k) {
       const int ir = k / lp.Nz, iz = k % lp.Nz;
       const double rr = lp.r_inner + (ir + 0.5) * lp.h, zz = (iz + 0.5) * lp.h - lp.Nz * lp.h / 2.0;
       if (std::fabs(geo->r[k] - rr) > 1e-9 * rr || std::fabs(geo->z[k] - zz) > 1e-9 * (std::fabs(zz) + lp.h))
@@ -794,7 +972,10 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
   // device set-up
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return bail(fail(QS_ERR_CUDA, "cudaGetDevice failed"));
+  c->device = dev;
   cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  if (c->sm_count <= 0) c->sm_count = 148;
+  pointwise_prepare_device();   // shared-memory opt-ins are per device
   size_t need = 0;
   carve(c, nullptr, &need);
   if (own) {
@@ -816,7 +997,7 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
   VecCtx& v = c->v;
   v.N = N; v.Np = c->Np; v.n_turns = c->n_turns;
   v.turn_id = c->turn_id; v.turn_ptr = c->turn_ptr; v.turn_idx = c->turn_idx; v.share = c->share;
-  v.stream = c->stream; v.sc = c->sc; v.launches = &c->launches;
+  v.stream = c->stream; v.sc = c->sc; v.launches = &c->launches; v.sm_count = c->sm_count;
 
   // geometry arrays in internal order, padded with far-away dummy rings that carry no current
   std::vector<double> hr(c->Np), hz(c->Np), tmp(N);
@@ -998,9 +1179,12 @@ int qs_init_device(const qs_geometry* geo, const qs_material* mat, void* workspa
 
 void qs_free(qs_ctx* c) {
   if (!c) return;
+  DeviceGuard guard(c->device);
   if (c->stream) cudaStreamSynchronize(c->stream);
   c->prof.destroy();
   for (auto& gslot : c->cg_graph)
+    if (gslot.exec) cudaGraphExecDestroy(gslot.exec);
+  for (auto& gslot : c->heat_graph)
     if (gslot.exec) cudaGraphExecDestroy(gslot.exec);
   if (c->h_sc) cudaFreeHost(c->h_sc);
   if (c->h_stage) cudaFreeHost(c->h_stage);
@@ -1013,6 +1197,7 @@ void qs_free(qs_ctx* c) {
 
 int qs_sync(qs_ctx* c) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  DeviceGuard guard(c->device);
   QS_CUDA(cudaStreamSynchronize(c->stream));
   return QS_OK;
 }
@@ -1020,29 +1205,36 @@ int qs_sync(qs_ctx* c) {
 int qs_step(qs_ctx* c, double dt, double I_ramp) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
   if (!c->lattice || !c->has_operator) return fail(QS_ERR_ARG, "qs_step needs a lattice geometry with the operator set up");
+  DeviceGuard guard(c->device);
   if (!(dt > 0.0)) return fail(QS_ERR_DT, "dt <= 0");
   const VecCtx& v = c->v;
   const int N = c->N;
   int rc;
   c->st.sweeps = 0;
   const size_t nb8 = sizeof(double) * N;
-  // backups: the step is transactional
-  QS_CUDA(cudaMemcpyAsync(c->Jold, c->J, nb8, cudaMemcpyDeviceToDevice, c->stream));
-  QS_CUDA(cudaMemcpyAsync(c->Hold, c->H, nb8, cudaMemcpyDeviceToDevice, c->stream));
-  QS_CUDA(cudaMemcpyAsync(c->xold, c->x, nb8, cudaMemcpyDeviceToDevice, c->stream));
-  k_set_scalars(v);
   int iters = 0;
   double relres = 0.0;
   bool hit_max = false;
-  auto restore = [&]() {
-    cudaMemcpyAsync(c->x, c->xold, nb8, cudaMemcpyDeviceToDevice, c->stream);
-    cudaStreamSynchronize(c->stream);
-  };
+  auto restore = [&]() { restore_state(c); };
+  const int n_prev_in = c->n_prev;
+  const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
   // CG start: linear extrapolation 2 I'_k - I'_{k-1} of the two previous solutions when the step is repeated with
   // the same dt and ramp (a guess only: the solution does not depend on it beyond cg_tol; config 1: 12 % fewer
   // iterations than the plain warm start, nothing changes where I' is constant)
-  {
-    if (c->n_prev >= 2 && dt == c->last_dt && I_ramp == c->last_ramp) {
+  const bool extrapolate = c->n_prev >= 2 && dt == c->last_dt && I_ramp == c->last_ramp;
+  if (c->n_turns > 0) {
+    // fused path: backups, CG start and all zeroing in one launch (the step is transactional)
+    rc = em_stage_fused(c, extrapolate, B0, (B1 - B0) / dt, dt, I_ramp, &iters, &relres, &hit_max);
+    if (rc != QS_OK) {
+      restore();
+      return rc;
+    }
+    k_step_update(v, dt, c->x, c->area, c->J, c->vsum);   // S5 + terminal voltage
+  } else {
+    // backups: the step is transactional
+    if ((rc = backup_state(c)) != QS_OK) return rc;
+    k_set_scalars(v);
+    if (extrapolate) {
       k_lincomb(v, 2.0, c->x, -1.0, c->xprev2);                                   // xprev2 <- extrapolated start
       QS_CUDA(cudaMemcpyAsync(c->tmp2, c->x, nb8, cudaMemcpyDeviceToDevice, c->stream));
       QS_CUDA(cudaMemcpyAsync(c->x, c->xprev2, nb8, cudaMemcpyDeviceToDevice, c->stream));
@@ -1050,26 +1242,28 @@ int qs_step(qs_ctx* c, double dt, double I_ramp) {
     } else {
       QS_CUDA(cudaMemcpyAsync(c->xprev2, c->x, nb8, cudaMemcpyDeviceToDevice, c->stream));
     }
+    if ((rc = em_stage(c, c->J, B0, (B1 - B0) / dt, dt, I_ramp, &iters, &relres, &hit_max)) != QS_OK) {
+      restore();
+      return rc;
+    }
+    // S5
+    k_scale_div(v, dt, c->x, c->area, c->J);
   }
-  const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
-  if ((rc = em_stage(c, c->J, B0, (B1 - B0) / dt, dt, I_ramp, &iters, &relres, &hit_max)) != QS_OK) {
-    restore();
-    c->n_prev = 0;
-    return rc;
+  // S6, S7, statistics, commit (restores the state itself on failure)
+  rc = finish_step(c, dt, I_ramp, iters, relres, hit_max, 1.0, false);
+  if (rc >= 0) {   // the history of the extrapolated start advances only with a committed step
+    c->n_prev = (dt == c->last_dt && I_ramp == c->last_ramp) ? std::min(n_prev_in + 1, 2) : 1;
+    c->last_dt = dt;
+    c->last_ramp = I_ramp;
   }
-  c->n_prev = (dt == c->last_dt && I_ramp == c->last_ramp) ? std::min(c->n_prev + 1, 2) : 1;
-  c->last_dt = dt;
-  c->last_ramp = I_ramp;
-  // S5
-  k_scale_div(v, dt, c->x, c->area, c->J);
-  // S6, S7, statistics, commit
-  return finish_step(c, dt, I_ramp, iters, relres, hit_max, 1.0, false);
+  return rc;
 }
 
 // Embedded Heun-Euler step with error control (readings: DESIGN.md §3 C14).
 int qs_step_rk(qs_ctx* c, double dt_try, double I_ramp, double rtol, double dt_min, double* dt_taken, double* dt_next,
                double* err_out) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  DeviceGuard guard(c->device);
   if (!c->lattice || !c->has_operator) return fail(QS_ERR_ARG, "qs_step_rk needs a lattice geometry with the operator set up");
   if (!(dt_try > 0.0) || !(dt_min > 0.0) || !(rtol > 0.0)) return fail(QS_ERR_DT, "dt_try, dt_min and rtol must be > 0");
   const VecCtx& v = c->v;
@@ -1077,13 +1271,8 @@ int qs_step_rk(qs_ctx* c, double dt_try, double I_ramp, double rtol, double dt_m
   const size_t nb8 = sizeof(double) * N;
   int rc;
   c->st.sweeps = 0;
-  QS_CUDA(cudaMemcpyAsync(c->Jold, c->J, nb8, cudaMemcpyDeviceToDevice, c->stream));
-  QS_CUDA(cudaMemcpyAsync(c->Hold, c->H, nb8, cudaMemcpyDeviceToDevice, c->stream));
-  QS_CUDA(cudaMemcpyAsync(c->xold, c->x, nb8, cudaMemcpyDeviceToDevice, c->stream));
-  auto restore = [&]() {
-    cudaMemcpyAsync(c->x, c->xold, nb8, cudaMemcpyDeviceToDevice, c->stream);
-    cudaStreamSynchronize(c->stream);
-  };
+  if ((rc = backup_state(c)) != QS_OK) return rc;
+  auto restore = [&]() { restore_state(c); };
   const double Jref = c->mp.Jc0 * (1.0 - c->lp.T_bath / c->mp.Tc) * (1.0 - c->lp.T_bath / c->mp.Tc);
   double dt = dt_try, err = 0.0, fac = 2.0;
   int iters = 0, it1 = 0, it2 = 0;
@@ -1110,7 +1299,10 @@ int qs_step_rk(qs_ctx* c, double dt_try, double I_ramp, double rtol, double dt_m
       return rc;
     }
     k_max_scaled_diff(v, 0.5 * dt, c->x, I1, c->area);
-    if ((rc = sync_scalars(c)) != QS_OK) return rc;
+    if ((rc = sync_scalars(c)) != QS_OK) {
+      restore();
+      return rc;
+    }
     err = c->h_sc->djmax / Jref;
     iters += it1 + it2;
     fac = err == 0.0 ? 2.0 : std::min(2.0, std::max(0.2, 0.9 * std::sqrt(rtol / err)));
@@ -1124,6 +1316,7 @@ int qs_step_rk(qs_ctx* c, double dt_try, double I_ramp, double rtol, double dt_m
   k_lincomb(v, 0.5, Q1, 0.5, c->Q);
   const int ret = finish_step(c, dt, I_ramp, iters, std::max(rel1, rel2), hm1 || hm2, 0.5, true);
   if (ret < 0) return ret;
+  c->n_prev = 0;   // the stored solutions of qs_step's extrapolated start are stale after an RK step
   if (dt_taken) *dt_taken = dt;
   if (dt_next) *dt_next = dt * fac;
   if (err_out) *err_out = err;
@@ -1132,6 +1325,7 @@ int qs_step_rk(qs_ctx* c, double dt_try, double I_ramp, double rtol, double dt_m
 
 int qs_read(qs_ctx* c, double* J, double* T, double* B, double* E) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  DeviceGuard guard(c->device);
   int rc;
   if (J && (rc = download(c, c->J, J)) != QS_OK) return rc;
   if (T) {
@@ -1148,6 +1342,7 @@ int qs_read(qs_ctx* c, double* J, double* T, double* B, double* E) {
 
 int qs_read_aux(qs_ctx* c, double* Q, double* dEdJ, double* Jc, double* rho) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  DeviceGuard guard(c->device);
   int rc;
   if (Q && (rc = download(c, c->Q, Q)) != QS_OK) return rc;
   if (dEdJ && (rc = download(c, c->dEdJ, dEdJ)) != QS_OK) return rc;
@@ -1158,6 +1353,7 @@ int qs_read_aux(qs_ctx* c, double* Q, double* dEdJ, double* Jc, double* rho) {
 
 int qs_write(qs_ctx* c, const double* J, const double* T, double t, double I) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  DeviceGuard guard(c->device);
   int rc;
   if (J && (rc = upload(c, J, c->J, c->N)) != QS_OK) return rc;
   if (T) {
@@ -1175,9 +1371,30 @@ int qs_write(qs_ctx* c, const double* J, const double* T, double t, double I) {
   return reset_wire_stats(c);
 }
 
+int qs_read_rate(qs_ctx* c, double* Idot) {
+  if (!c || !Idot) return fail(QS_ERR_ARG, "NULL argument");
+  DeviceGuard guard(c->device);
+  return download(c, c->x, Idot);
+}
+
+int qs_write_rate(qs_ctx* c, const double* Idot) {
+  if (!c || !Idot) return fail(QS_ERR_ARG, "NULL argument");
+  DeviceGuard guard(c->device);
+  const int rc = upload(c, Idot, c->x, c->Np);
+  c->n_prev = 0;
+  return rc;
+}
+
+int qs_debug_inject_failure(qs_ctx* c, int32_t where) {
+  if (!c || where < 0 || where > 2) return fail(QS_ERR_ARG, "qs_debug_inject_failure: handle and where in 0..2");
+  c->inject = where;
+  return QS_OK;
+}
+
 int qs_matvec_device(qs_ctx* c, const double* d_x, double* d_y) {
   if (!c || !d_x || !d_y) return fail(QS_ERR_ARG, "NULL argument");
   if (!c->has_operator) return fail(QS_ERR_ARG, "operator not set up (QS_GEO_NO_OPERATOR)");
+  DeviceGuard guard(c->device);
   c->st.sweeps = 0;
   k_gather(c->v, d_x, c->perm.empty() ? nullptr : c->d_perm, c->p, c->N, c->Np);
   int rc = do_sweep(c, c->p, nullptr, false);
@@ -1190,6 +1407,7 @@ int qs_matvec_device(qs_ctx* c, const double* d_x, double* d_y) {
 int qs_matvec(qs_ctx* c, const double* x, double* y) {
   if (!c || !x || !y) return fail(QS_ERR_ARG, "NULL argument");
   if (!c->has_operator) return fail(QS_ERR_ARG, "operator not set up (QS_GEO_NO_OPERATOR)");
+  DeviceGuard guard(c->device);
   int rc;
   c->st.sweeps = 0;
   if ((rc = upload(c, x, c->p, c->Np)) != QS_OK) return rc;
@@ -1200,28 +1418,23 @@ int qs_matvec(qs_ctx* c, const double* x, double* y) {
 int qs_field(qs_ctx* c, const double* I, double* B) {
   if (!c || !I || !B) return fail(QS_ERR_ARG, "NULL argument");
   if (!c->lattice || !c->has_operator) return fail(QS_ERR_ARG, "qs_field needs a lattice geometry with the operator set up");
+  DeviceGuard guard(c->device);
   int rc;
   c->st.sweeps = 0;
   if ((rc = upload(c, I, c->cur, c->Np)) != QS_OK) return rc;
   QS_CUDA(cudaMemsetAsync(c->p, 0, sizeof(double) * c->Np, c->stream));
   if ((rc = do_sweep(c, c->p, c->cur, true)) != QS_OK) return rc;
+  // output scaling of the accumulators (the one the material kernel applies inside a step), on the device:
   // Br = mu0/(4 r) bracc ; Bz = mu0/4 bzacc + selfcoef I
-  QS_CUDA(cudaMemcpyAsync(c->h_stage, c->bracc, sizeof(double) * c->N, cudaMemcpyDeviceToHost, c->stream));
-  QS_CUDA(cudaMemcpyAsync(c->h_stage + c->Np, c->bzacc, sizeof(double) * c->N, cudaMemcpyDeviceToHost, c->stream));
-  std::vector<double> hr(c->N), hs(c->N);
-  QS_CUDA(cudaMemcpyAsync(hr.data(), c->r, sizeof(double) * c->N, cudaMemcpyDeviceToHost, c->stream));
-  QS_CUDA(cudaMemcpyAsync(hs.data(), c->selfcoef, sizeof(double) * c->N, cudaMemcpyDeviceToHost, c->stream));
-  QS_CUDA(cudaStreamSynchronize(c->stream));
-  for (int k = 0; k < c->N; ++k) {   // output scaling of the accumulators (same as the material kernel applies)
-    B[k] = (0.25 * kMu0) * c->h_stage[k] / hr[k];
-    B[c->N + k] = (0.25 * kMu0) * c->h_stage[c->Np + k] + hs[k] * I[k];
-  }
-  return QS_OK;
+  k_field_scale(c->v, c->bracc, c->bzacc, c->r, c->selfcoef, c->cur, c->tmp, c->tmp2);
+  if ((rc = download(c, c->tmp, B)) != QS_OK) return rc;
+  return download(c, c->tmp2, B + c->N);
 }
 
 int qs_solve_device(qs_ctx* c, const double* d_b, double* d_x, int32_t maxit_override, int32_t* iters, double* relres) {
   if (!c || !d_b || !d_x) return fail(QS_ERR_ARG, "NULL argument");
   if (!c->has_operator) return fail(QS_ERR_ARG, "operator not set up (QS_GEO_NO_OPERATOR)");
+  DeviceGuard guard(c->device);
   const int* perm = c->perm.empty() ? nullptr : c->d_perm;
   c->st.sweeps = 0;
   k_set_scalars(c->v);
@@ -1247,6 +1460,7 @@ int qs_solve_device(qs_ctx* c, const double* d_b, double* d_x, int32_t maxit_ove
 int qs_solve(qs_ctx* c, const double* b, double* x, int32_t maxit_override, int32_t* iters, double* relres) {
   if (!c || !b || !x) return fail(QS_ERR_ARG, "NULL argument");
   if (!c->has_operator) return fail(QS_ERR_ARG, "operator not set up (QS_GEO_NO_OPERATOR)");
+  DeviceGuard guard(c->device);
   // stage through tmp2 (caller order on the device), then the device variant
   QS_CUDA(cudaMemcpyAsync(c->tmp2, b, sizeof(double) * c->N, cudaMemcpyHostToDevice, c->stream));
   QS_CUDA(cudaStreamSynchronize(c->stream));
@@ -1259,6 +1473,7 @@ int qs_solve(qs_ctx* c, const double* b, double* x, int32_t maxit_override, int3
 
 int qs_set_fields(qs_ctx* c, const double* B, const double* Q) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  DeviceGuard guard(c->device);
   int rc;
   if (B) {
     if ((rc = upload(c, B, c->Br, c->N)) != QS_OK) return rc;
@@ -1270,6 +1485,7 @@ int qs_set_fields(qs_ctx* c, const double* B, const double* Q) {
 
 int qs_material_eval(qs_ctx* c, double dt) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  DeviceGuard guard(c->device);
   const double B0 = bext_at(c, c->t), B1 = bext_at(c, c->t + dt);
   int rc = reset_event_bits(c);
   if (rc != QS_OK) return rc;
@@ -1289,6 +1505,7 @@ int qs_set_aux(qs_ctx* c, int32_t on) {
 int qs_heat(qs_ctx* c, double dt) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
   if (!c->lattice) return fail(QS_ERR_ARG, "qs_heat needs a lattice geometry");
+  DeviceGuard guard(c->device);
   if (!(dt > 0.0)) return fail(QS_ERR_DT, "dt <= 0");
   int m = 0;
   int rc = run_heat(c, dt, &m);
@@ -1298,6 +1515,7 @@ int qs_heat(qs_ctx* c, double dt) {
 int qs_heat_adi(qs_ctx* c, double dt, int32_t m) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
   if (!c->lattice) return fail(QS_ERR_ARG, "qs_heat_adi needs a lattice geometry");
+  DeviceGuard guard(c->device);
   if (!(dt > 0.0) || m <= 0) return fail(QS_ERR_DT, "dt <= 0 or m <= 0");
   const int rc = run_heat_adi(c, dt, m);
   return rc != QS_OK ? rc : m;
@@ -1315,6 +1533,7 @@ int qs_stats(qs_ctx* c, qs_stats_t* out) {
 
 int qs_profile_enable(qs_ctx* c, int32_t on) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
+  DeviceGuard guard(c->device);
   c->prof.fold(c->stream);
   c->prof.reset();
   c->prof.on = on != 0;
@@ -1323,6 +1542,7 @@ int qs_profile_enable(qs_ctx* c, int32_t on) {
 
 int qs_profile_read(qs_ctx* c, qs_profile_t* out) {
   if (!c || !out) return fail(QS_ERR_ARG, "NULL argument");
+  DeviceGuard guard(c->device);
   QS_CUDA(cudaStreamSynchronize(c->stream));
   c->prof.fold(c->stream);
   for (int k = 0; k < QS_PROF_CLASSES; ++k) {
@@ -1374,6 +1594,7 @@ int qs_fp64_peak(double* tflops, double* sm_clock_mhz_effective) {
 int qs_wire_stats(qs_ctx* c, double* out) {
   if (!c || !out) return fail(QS_ERR_ARG, "NULL argument");
   if (!c->n_turns) return QS_OK;
+  DeviceGuard guard(c->device);
   QS_CUDA(cudaMemcpyAsync(out, c->wire, sizeof(double) * 8 * c->n_turns, cudaMemcpyDeviceToHost, c->stream));
   QS_CUDA(cudaStreamSynchronize(c->stream));
   return QS_OK;
@@ -1382,6 +1603,7 @@ int qs_wire_stats(qs_ctx* c, double* out) {
 int qs_events(qs_ctx* c, int32_t* flags, double* t_first, int32_t* count) {
   if (!c) return fail(QS_ERR_ARG, "NULL handle");
   if (!c->n_turns) return QS_OK;
+  DeviceGuard guard(c->device);
   const size_t nt = c->n_turns;
   if (flags) QS_CUDA(cudaMemcpyAsync(flags, c->flags, sizeof(int) * nt, cudaMemcpyDeviceToHost, c->stream));
   if (t_first) QS_CUDA(cudaMemcpyAsync(t_first, c->t_first, sizeof(double) * nt, cudaMemcpyDeviceToHost, c->stream));

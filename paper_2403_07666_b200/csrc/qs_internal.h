@@ -20,7 +20,7 @@ struct SweepParams {
   double* bzacc;          // [Np] += sum_j (Kt + c_ij Qt) I_j     (scale mu0/4 by the consumer)
   unsigned long long* counter;
   const int* done;        // fused CG: the sweep returns at once when *done != 0 (nullptr: always run)
-  long long n_items;      // nb (nb + 1) / 2
+  long long n_items;      // work items of the sweep: sweep_items(nb, field)
   int nb;
   int chunk;
   double soft_all;        // g^2 added to dz^2 of every pair (free rings) or 0 (lattice)
@@ -29,6 +29,7 @@ struct SweepParams {
   double diag_d2;         // smallest B2 inside a diagonal item (self pair included)
 };
 int sweep_grid(int sm_count, bool field);
+long long sweep_items(int nb, bool field);   // multi-target + triangle items covering every unordered block pair once
 int sweep_warps_per_cta();
 cudaError_t launch_sweep(const SweepParams& prm, bool field, int grid, cudaStream_t stream);
 // diagM_i = M(r_i, r_i, dz^2 = d2self) in henry
@@ -90,6 +91,7 @@ struct VecCtx {
   cudaStream_t stream;
   Scalars* sc;
   long long* launches;   // host counter
+  int sm_count;          // SMs of the handle's device (grid sizing)
 };
 
 // ---- fused projected-CG iteration (C8): four launches after the sweep, no host round trip; every kernel returns at
@@ -143,6 +145,31 @@ void k_direction(const VecCtx& v, int par, bool first, const double* g, double* 
 // deficit_w = d - sum_{i in w} x_i ; x_i += deficit_w / (H_i s_w)   (moves a warm start onto the constraint)
 void k_turn_deficit(const VecCtx& v, const double* x, double d, double* defw);
 void k_apply_deficit(const VecCtx& v, const double* defw, const double* Hd, const double* sw, double* x);
+// ---- fused step kernels (qs_step on geometries with constraint groups) ---------------------------------------------
+struct StepBegin {
+  int N, n_turns;
+  bool extrapolate;                 // CG start 2 I'_k - I'_{k-1} instead of I'_k
+  const double *J, *H, *area;
+  double *Jold, *Hold, *x, *xold, *xprev2, *cur;
+  const unsigned long long *fld, *ev;           // contiguous blocks backed up word by word
+  unsigned long long *fld_backup, *ev_backup;
+  size_t fld_words, ev_words;
+  unsigned long long* acc;          // work counter + sweep accumulators, cleared
+  size_t acc_words;
+  double *vsum, *tw;                // [n_turns] cleared
+  unsigned long long *xmax_bits, *rmin_bits;    // [n_turns] presets of the event observables (may be null)
+};
+struct TurnStart {
+  const int *ptr, *idx;             // CSR of cells per constraint group
+  double I_ramp, cM;
+  Rhs b;
+  const double *Hd, *shift, *x, *yacc, *xp1, *Mxp1;
+  double *r, *g, *p, *sw, *vnu, *vsum;
+};
+void k_step_begin(const VecCtx& v, const StepBegin& a);   // backups, CG start, I = a J, zeroing: one launch
+void k_turn_fix(const VecCtx& v, double d, const double* Hd, const double* sw, double* x);   // deficit + correction
+void k_turn_start(const VecCtx& v, const TurnStart& a);   // Schur scalars, reference norm, start residual, projection, p
+void k_step_update(const VecCtx& v, double dt, const double* x, const double* area, double* J, const double* vsum);
 void k_axpy(const VecCtx& v, double a, const double* x, double* y);                     // y += a x
 void k_lincomb(const VecCtx& v, double a, const double* x, double b, double* y);        // y = a x + b y
 // sc->djmax = max_i |s (x1_i - x2_i) / d_i|   (error estimate of the embedded Heun-Euler pair)
@@ -154,6 +181,9 @@ void k_copy_rg_to_nu2(const VecCtx& v, int par);
 // r = I_ramp (Mxp1 + shift xp1) - b : residual of the cold start x_p = I_ramp xp1 (reference norm, C8)
 void k_nu_residual(const VecCtx& v, double I_ramp, const double* Mxp1, const double* shift, const double* xp1,
                    const Rhs& b, double* r);
+// Br = mu0/(4 r) bracc ; Bz = mu0/4 bzacc + selfcoef I : output scaling of the field accumulators (qs_field)
+void k_field_scale(const VecCtx& v, const double* bracc, const double* bzacc, const double* r, const double* selfcoef,
+                   const double* cur, double* Br, double* Bz);
 void k_sum_uterm(const VecCtx& v, const double* vsum);                                  // sc->uterm = sum vsum
 void k_gather(const VecCtx& v, const double* src, const int* perm, double* dst, int n, int npad);   // dst[k] = src[perm[k]], pad 0
 void k_scatter_scaled(const VecCtx& v, const double* src, const int* perm, double* dst, int n, double scale);  // dst[perm[k]] = scale*src[k]
@@ -207,6 +237,9 @@ void k_heat_substep(const VecCtx& v, const MaterialParams& mp, const LatticePara
 bool k_heat_all_substeps(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, int m, const double* Hin,
                          const double* Q, double* Hout, double dtsub);
 // one ADI sub-step (qs_adi.cu, C15); scratch: six arrays of N doubles; returns the number of launches
+// opt-in shared-memory sizes of the heat kernels on the CURRENT device (cudaFuncSetAttribute is per device): called by
+// every qs_init with the handle's device current
+void pointwise_prepare_device();
 int k_heat_adi_substep(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, const double* Hin,
                        const double* Q, double* Hout, double delta, double* const scratch[6]);
 struct EventArgs {

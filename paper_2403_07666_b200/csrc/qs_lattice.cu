@@ -39,17 +39,18 @@ __global__ void table_build_kernel(int Nr, int Nz, double r_inner, double h, dou
     const double dz2 = self ? soft_self2 : dz * dz;            // C2: M_ii = M(r_i, r_i, dz = g)
     const double dif = ri - rj;
     const double B2 = fma(dif, dif, dz2), A2 = fma(4.0 * ri, rj, B2);
-    const PairAGM a = agm_pair<7, false, true>(A2, B2);
+    const PairAGM a = agm_pair<7, 2, true>(A2, B2);
     TM[id] = a.S * a.yinf;
     if (TBz) {
       if (self) {                                              // C3: the self field is analytic (material pass)
         TBz[id] = 0.0;
         TBr[id] = 0.0;
       } else {
-        const double qt = a.yinf * (a.mid - a.S) * a.y0sq;
-        const double e = fma(rj, rj, -ri * ri);
-        TBz[id] = fma(e - dz2, qt, a.yinf);                    // Kt + (rj^2 - ri^2 - dz^2) Qt
-        TBr[id] = dz * fma(a.mid, qt, -a.yinf);                // dz (-Kt + (ri^2 + rj^2 + dz^2) Qt), odd in dz
+        const double qt = a.yinf * a.emS * a.y0sq;
+        const double e = fma(rj, rj, -ri * ri), sig = fma(rj, rj, ri * ri);
+        const double P = fma(-dz2, qt, a.yinf);                // Kt - dz^2 Qt
+        TBz[id] = fma(e, qt, P);                               // Kt + (rj^2 - ri^2 - dz^2) Qt
+        TBr[id] = dz * fma(sig, qt, -P);                       // dz (-Kt + (ri^2 + rj^2 + dz^2) Qt), odd in dz
       }
     }
   }

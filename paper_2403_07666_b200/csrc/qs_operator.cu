@@ -21,32 +21,60 @@
 
 namespace qs {
 
-// Evaluation classes, cheapest first: (AGM iterations NIT, series order HI) and the smallest k'^2 = B2/A2 for which
+// Evaluation classes, cheapest first: (AGM iterations NIT, series order ORD) and the smallest k'^2 = B2/A2 for which
 // the truncated evaluation is exact to < 1e-16 relative in M, K and E (60-digit evaluation of the truncated
-// recurrence against K, E, plus 2 % margin).  FP64 operations per pair:
-// 8 + 10 NIT + 16 (lo) or 20 (hi).
+// recurrence against K, E, plus 2 % margin).  FP64 operations per pair (M only):
+// 7 + 10 NIT + 11 + 2 ORD.  A finer ladder (orders 3, 5, 6 in between: 14 classes) saves ~1.2 operations per pair on
+// the coil configs but lost on the clock (config 2 fused sweep 96.3 vs 94.8 ms, N = 262,144 matvec 131 vs 103 ms):
+// more distinct loops are hot at the same time and the instruction caches thrash.
 constexpr int kNumClasses = 10;
 __device__ __constant__ double kClassKp2Min[kNumClasses] = {0.3965,   0.1394,   0.01529,   1.374e-3, 1.453e-5,
                                                             1.157e-7, 1.293e-11, 8.2e-16,  1.03e-23, 0.0};
-//                                                class:      0       1       2       3       4       5       6       7       8       9
-//                                                (NIT,HI): (2,lo)  (2,hi)  (3,lo)  (3,hi)  (4,lo)  (4,hi)  (5,lo)  (5,hi)  (6,lo)  (7,lo)
+//  class:        0      1      2      3      4      5      6      7      8      9
+//  (NIT,ORD):  (2,2)  (2,4)  (3,2)  (3,4)  (4,2)  (4,4)  (5,2)  (5,4)  (6,2)  (7,2)
+// QS_CLASS_SWITCH(cls, M) expands M(NIT, ORD) for the class
+#define QS_CLASS_SWITCH(cls_, M_) \
+  switch (cls_) {                 \
+    case 0: M_(2, 2); break;      \
+    case 1: M_(2, 4); break;      \
+    case 2: M_(3, 2); break;      \
+    case 3: M_(3, 4); break;      \
+    case 4: M_(4, 2); break;      \
+    case 5: M_(4, 4); break;      \
+    case 6: M_(5, 2); break;      \
+    case 7: M_(5, 4); break;      \
+    case 8: M_(6, 2); break;      \
+    default: M_(7, 2); break;     \
+  }
 
 #ifndef QS_SW_WARPS
 #define QS_SW_WARPS 4          // warps per CTA of the pair sweeps (small CTAs: finer register-budget steps)
 #endif
 #ifndef QS_SW_MINB_FIELD
 #define QS_SW_MINB_FIELD 5     // resident CTAs per SM the register budget of the fused sweep is sized for: 20 warps
-                               // at <= 102 registers (96 used).  Measured on config 2: 8x2 (112 regs) 108.8 ms,
-                               // 4x5 102.7 ms, 8x3 (80 regs) 103.9 ms, 4x6 (80 regs) 104.2 ms
+                               // at <= 102 registers (96 used).  Measured on config 2 (T = target blocks per item):
+                               // T=1: 104.6 ms; T=2 at 5 CTAs (96 regs) 98.5 ms, at 4 CTAs (128 regs) 99.6 ms;
+                               // T=3 at 4 CTAs 100.7 ms; T=4 at 4 CTAs (128 regs, spills) 100.8 ms, at 3 CTAs (168 regs) 110.6 ms
 #endif
 #ifndef QS_SW_MINB_M
-#define QS_SW_MINB_M 7         // the same for the M-only sweep: 28 warps at 72 registers.  N = 262,144: 4x6 / 8x3
-                               // (80 regs) 113.1 ms, 4x7 112.1 ms, 8x4 (64 regs) 114.8 ms, 4x5 (96 regs) 117.4 ms
+#define QS_SW_MINB_M 4         // the same for the M-only sweep: 16 warps at 128 registers.  N = 262,144: T=1 113.9 ms;
+                               // T=2 at 7 CTAs (72 regs) 108.6 ms, at 6 CTAs 110.1 ms; T=3 at 5 CTAs 107.7 ms;
+                               // T=4 at 5 CTAs (96 regs, spills) 107.7 ms, at 4 CTAs (128 regs) 105.0 ms
 #endif
 #ifndef QS_SW_UNROLL
 #define QS_SW_UNROLL 2         // source steps unrolled in the off-diagonal item loop (1: +3 %, 4: +17 % on K2)
 #endif
 constexpr int kSweepUnroll = QS_SW_UNROLL;
+#ifndef QS_SW_T_FIELD
+#define QS_SW_T_FIELD 2        // target blocks per multi-target item of the fused sweep (32 T targets x 32 sources)
+#endif
+#ifndef QS_SW_T_M
+#define QS_SW_T_M 4            // the same for the M-only sweep
+#endif
+#ifndef QS_SW_MULTI_UNROLL
+#define QS_SW_MULTI_UNROLL 1   // source steps unrolled in the multi-target loop (each step already holds T pair chains)
+#endif
+constexpr int kMultiUnroll = QS_SW_MULTI_UNROLL;
 constexpr int kWarpsPerCta = QS_SW_WARPS;
 constexpr int kThreads = kWarpsPerCta * 32;
 constexpr int kMaxArrays = 4;
@@ -66,7 +94,7 @@ struct Accum {
 // UNI: every ring of the source block has the same radius rju and so has the target block (blocks of a lattice row,
 // the common case on winding packs whose Nz is a multiple of 32): (ri - rj)^2, 4 ri rj and rj^2 - ri^2 are item
 // constants, the source radii are not read.
-template <int NIT, bool HI, bool FIELD, bool UNI>
+template <int NIT, int ORD, bool FIELD, bool UNI>
 __device__ __forceinline__ void item_offdiag(const TargetRegs& t, const double* __restrict__ sr,
                                              const double* __restrict__ sz, const double* __restrict__ sx,
                                              const double* __restrict__ sc, double soft_all, double rju, int lane,
@@ -74,7 +102,7 @@ __device__ __forceinline__ void item_offdiag(const TargetRegs& t, const double* 
   const unsigned full = 0xffffffffu;
   const int next = (lane + 1) & 31;
   const double ri2 = t.r * t.r, ri4 = 4.0 * t.r;
-  const double difu = t.r - rju, dif2u = difu * difu, c4u = ri4 * rju, eu = fma(rju, rju, -ri2);
+  const double difu = t.r - rju, dif2u = difu * difu, c4u = ri4 * rju, eu = fma(rju, rju, -ri2), sigu = fma(rju, rju, ri2);
   const double dif2s = dif2u + soft_all;
   sr += lane, sz += lane, sx += lane, sc += lane;   // arrays are stored twice: entry lane + s = source (lane + s) & 31
 #pragma unroll kSweepUnroll
@@ -98,17 +126,20 @@ __device__ __forceinline__ void item_offdiag(const TargetRegs& t, const double* 
       B2 = fma(dif, dif, dz2);
       A2 = fma(ri4, rj, B2);                               // (ri+rj)^2 = (ri-rj)^2 + 4 ri rj
     }
-    const PairAGM a = agm_pair<NIT, HI, FIELD>(A2, B2);
+    const PairAGM a = agm_pair<NIT, ORD, FIELD>(A2, B2);
     const double mt = a.S * a.yinf;
     acc.y = fma(mt, xj, acc.y);
     trav.y = fma(mt, t.x, trav.y);
     if (FIELD) {
       const double cj = sc[jl];
-      const double qt = a.yinf * (a.mid - a.S) * a.y0sq;
-      const double e = UNI ? eu : fma(rj, rj, -ri2);       // rj^2 - ri^2
-      const double bz_ij = fma(e - dz2, qt, a.yinf);       // Kt + (rj^2 - ri^2 - dz^2) Qt
-      const double bz_ji = fma(-e - dz2, qt, a.yinf);
-      const double ur = dz * fma(a.mid, qt, -a.yinf);      // dz (-Kt + (ri^2 + rj^2 + dz^2) Qt)
+      const double qt = a.yinf * a.emS * a.y0sq;
+      const double sig = UNI ? sigu : fma(rj, rj, ri2);    // ri^2 + rj^2
+      const double e = UNI ? eu : fma(-2.0, ri2, sig);     // rj^2 - ri^2
+      const double P = fma(-dz2, qt, a.yinf);              // Kt - dz^2 Qt
+      const double R = e * qt;
+      const double bz_ij = P + R;                          // Kt + (rj^2 - ri^2 - dz^2) Qt
+      const double bz_ji = P - R;
+      const double ur = dz * fma(sig, qt, -P);             // dz (-Kt + (ri^2 + rj^2 + dz^2) Qt)
       acc.bz = fma(bz_ij, cj, acc.bz);
       acc.br = fma(ur, cj, acc.br);
       trav.bz = fma(bz_ji, t.cur, trav.bz);
@@ -121,7 +152,7 @@ __device__ __forceinline__ void item_offdiag(const TargetRegs& t, const double* 
 }
 
 // ---- one diagonal item (bi == bj): every ordered pair appears once in the rotation -----------------
-template <int NIT, bool HI, bool FIELD>
+template <int NIT, int ORD, bool FIELD>
 __device__ __forceinline__ void item_diag(const TargetRegs& t, const double* __restrict__ sr,
                                           const double* __restrict__ sz, const double* __restrict__ sx,
                                           const double* __restrict__ sc, double soft_all, double soft_self, int lane,
@@ -130,7 +161,7 @@ __device__ __forceinline__ void item_diag(const TargetRegs& t, const double* __r
   {  // s = 0: the self pair; M_ii = M(ri, ri, dz^2 = soft_all + soft_self); no field term (C3 self field is analytic)
     const double dz2 = soft_all + soft_self;
     const double sum = t.r + t.r;
-    const PairAGM a = agm_pair<NIT, HI, false>(fma(sum, sum, dz2), dz2);
+    const PairAGM a = agm_pair<NIT, ORD, false>(fma(sum, sum, dz2), dz2);
     acc.y = fma(a.S * a.yinf, t.x, acc.y);
   }
   sr += lane, sz += lane, sx += lane, sc += lane;
@@ -141,14 +172,15 @@ __device__ __forceinline__ void item_diag(const TargetRegs& t, const double* __r
     const double dz = t.z - zj;
     const double dz2 = fma(dz, dz, soft_all);
     const double sum = t.r + rj, dif = t.r - rj;
-    const PairAGM a = agm_pair<NIT, HI, FIELD>(fma(sum, sum, dz2), fma(dif, dif, dz2));
+    const PairAGM a = agm_pair<NIT, ORD, FIELD>(fma(sum, sum, dz2), fma(dif, dif, dz2));
     acc.y = fma(a.S * a.yinf, xj, acc.y);
     if (FIELD) {
       const double cj = sc[jl];
-      const double qt = a.yinf * (a.mid - a.S) * a.y0sq;
-      const double e = fma(rj, rj, -ri2);
-      acc.bz = fma(fma(e - dz2, qt, a.yinf), cj, acc.bz);
-      acc.br = fma(dz * fma(a.mid, qt, -a.yinf), cj, acc.br);
+      const double qt = a.yinf * a.emS * a.y0sq;
+      const double sig = fma(rj, rj, ri2), e = fma(rj, rj, -ri2);
+      const double P = fma(-dz2, qt, a.yinf);
+      acc.bz = fma(fma(e, qt, P), cj, acc.bz);
+      acc.br = fma(dz * fma(sig, qt, -P), cj, acc.br);
     }
   }
 }
@@ -167,19 +199,126 @@ __device__ __forceinline__ int classify(const double4& bi, const double4& bj, bo
   return cls;
 }
 
-// row-major enumeration of the upper triangle (bi <= bj) of an nb x nb block matrix
-__device__ __forceinline__ void unrank(long long k, int nb, int& bi, int& bj) {
-  const double t = 2.0 * nb + 1.0;
-  int i = static_cast<int>(floor(0.5 * (t - sqrt(t * t - 8.0 * static_cast<double>(k)))));
-  i = max(0, min(i, nb - 1));
-  auto row_start = [nb](int r) { return static_cast<long long>(r) * nb - static_cast<long long>(r) * (r - 1) / 2; };
-  while (i > 0 && row_start(i) > k) --i;
-  while (i + 1 < nb && row_start(i + 1) <= k) ++i;
-  bi = i;
-  bj = i + static_cast<int>(k - row_start(i));
+// ---- one multi-target item: T target blocks (32 T rings, T targets per lane) against one source block --------------
+// Every staged source value (LDS) and every hop of the travelling sums (SHFL) serves T pair evaluations instead of one:
+// the sweep is issue-bound and every non-FP64 instruction costs an issue slot.  UNI: every one of the
+// T target blocks and the source block sit on one radius each (rows of a lattice).
+template <int NIT, int ORD, bool FIELD, bool UNI, int T>
+__device__ __forceinline__ void item_multi(const TargetRegs (&t)[T], const double* __restrict__ sr,
+                                           const double* __restrict__ sz, const double* __restrict__ sx,
+                                           const double* __restrict__ sc, double soft_all, double rju, int lane,
+                                           Accum (&acc)[T], Accum& trav) {
+  const unsigned full = 0xffffffffu;
+  const int next = (lane + 1) & 31;
+  double ri2[T], ri4[T], dif2u[T], c4u[T], eu[T], sigu[T];
+#pragma unroll
+  for (int k = 0; k < T; ++k) {
+    ri2[k] = t[k].r * t[k].r;
+    ri4[k] = 4.0 * t[k].r;
+    const double difu = t[k].r - rju;
+    dif2u[k] = FIELD ? difu * difu : fma(difu, difu, soft_all);
+    c4u[k] = ri4[k] * rju;
+    eu[k] = fma(rju, rju, -ri2[k]);
+    sigu[k] = fma(rju, rju, ri2[k]);
+  }
+  sr += lane, sz += lane, sx += lane, sc += lane;   // arrays are stored twice: entry lane + s = source (lane + s) & 31
+#pragma unroll kMultiUnroll
+  for (int s = 0; s < 32; ++s) {
+    const double zj = sz[s], xj = sx[s];
+    const double rj = UNI ? rju : sr[s];
+    const double cj = FIELD ? sc[s] : 0.0;
+#pragma unroll
+    for (int k = 0; k < T; ++k) {
+      const double dz = t[k].z - zj;
+      double dz2 = 0.0, A2, B2;
+      if (UNI) {
+        if (FIELD) {
+          dz2 = fma(dz, dz, soft_all);
+          B2 = dz2 + dif2u[k];
+        } else {
+          B2 = fma(dz, dz, dif2u[k]);
+        }
+        A2 = B2 + c4u[k];
+      } else {
+        dz2 = fma(dz, dz, soft_all);
+        const double dif = t[k].r - rj;
+        B2 = fma(dif, dif, dz2);
+        A2 = fma(ri4[k], rj, B2);                            // (ri+rj)^2 = (ri-rj)^2 + 4 ri rj
+      }
+      const PairAGM a = agm_pair<NIT, ORD, FIELD>(A2, B2);
+      const double mt = a.S * a.yinf;
+      acc[k].y = fma(mt, xj, acc[k].y);
+      trav.y = fma(mt, t[k].x, trav.y);
+      if (FIELD) {
+        const double qt = a.yinf * a.emS * a.y0sq;
+        const double sig = UNI ? sigu[k] : fma(rj, rj, ri2[k]);   // ri^2 + rj^2
+        const double e = UNI ? eu[k] : fma(-2.0, ri2[k], sig);    // rj^2 - ri^2
+        const double P = fma(-dz2, qt, a.yinf);                   // Kt - dz^2 Qt
+        const double R = e * qt;
+        const double bz_ij = P + R;                               // Kt + (rj^2 - ri^2 - dz^2) Qt
+        const double bz_ji = P - R;
+        const double ur = dz * fma(sig, qt, -P);                  // dz (-Kt + (ri^2 + rj^2 + dz^2) Qt)
+        acc[k].bz = fma(bz_ij, cj, acc[k].bz);
+        acc[k].br = fma(ur, cj, acc[k].br);
+        trav.bz = fma(bz_ji, t[k].cur, trav.bz);
+        trav.br = fma(-ur, t[k].cur, trav.br);
+      }
+    }
+    if (FIELD) {
+      trav.bz = __shfl_sync(full, trav.bz, next);
+      trav.br = __shfl_sync(full, trav.br, next);
+    }
+    trav.y = __shfl_sync(full, trav.y, next);
+  }
 }
 
-template <bool FIELD>
+// Work list.  Blocks of 32 rings are grouped T at a time into super-blocks I = 0 .. ceil(nb/T)-1 (the last one may hold
+// fewer, Ta < T).  Row I of the list: first the "triangle" of the super-block with itself - for a = 0..Ta-1 the diagonal
+// item (a, a) followed by the single-target items (a, b), b = a+1..Ta-1 - then the multi-target items (I, bj) for every
+// source block bj >= T (I + 1).  Every unordered block pair appears exactly once.
+template <int T>
+struct WorkList {
+  int nb, nbF, rem;
+  __host__ __device__ explicit WorkList(int nb_) : nb(nb_), nbF(nb_ / T), rem(nb_ % T) {}
+  static __host__ __device__ constexpr int tri(int n) { return n * (n + 1) / 2; }
+  __host__ __device__ long long row_start(int I) const {   // I <= nbF
+    return static_cast<long long>(I) * (tri(T) + nb) - static_cast<long long>(T) * I * (I + 1) / 2;
+  }
+  __host__ __device__ long long total() const { return row_start(nbF) + tri(rem); }
+  __host__ __device__ int blocks_in(int I) const { return I < nbF ? T : rem; }
+  __host__ __device__ int row_count(int I) const { return I < nbF ? tri(T) + nb - T * (I + 1) : tri(rem); }
+  __device__ void unrank(long long k, int& I, int& loc) const {
+    const double B = tri(T) + nb - 0.5 * T;
+    const double disc = fmax(B * B - 2.0 * T * static_cast<double>(k), 0.0);
+    int i = static_cast<int>(floor((B - sqrt(disc)) / T));
+    i = max(0, min(i, nbF));
+    while (i > 0 && row_start(i) > k) --i;
+    while (i < nbF && row_start(i + 1) <= k) ++i;
+    I = i;
+    loc = static_cast<int>(k - row_start(i));
+  }
+  // item (I, loc) -> a, b (target / source block inside the super-block; a == b: diagonal; a < 0: multi item) and the
+  // source block index bj
+  __device__ void decode(int I, int loc, int& a, int& b, int& bj) const {
+    const int Ta = blocks_in(I), ntri = tri(Ta);
+    if (loc < ntri) {
+      int aa = 0, l = loc;
+      while (l >= Ta - aa) {
+        l -= Ta - aa;
+        ++aa;
+      }
+      a = aa;
+      b = aa + l;
+      bj = T * I + b;
+    } else {
+      a = -1;
+      b = -1;
+      bj = T * (I + 1) + (loc - ntri);
+    }
+  }
+};
+
+template <bool FIELD, int T>
 __global__ void __launch_bounds__(kThreads, FIELD ? QS_SW_MINB_FIELD : QS_SW_MINB_M) sweep_kernel(SweepParams prm) {
   constexpr int NA = FIELD ? 4 : 3;
   __shared__ __align__(128) double sbuf[kWarpsPerCta][2][kMaxArrays][64];   // every array twice: no wrap of lane + s
@@ -193,6 +332,7 @@ __global__ void __launch_bounds__(kThreads, FIELD ? QS_SW_MINB_FIELD : QS_SW_MIN
 
   uint32_t phase = 0u;   // bit b = parity to wait for on buffer b
   const double* src[kMaxArrays] = {prm.r, prm.z, prm.x, prm.cur};
+  const WorkList<T> wl(prm.nb);
 
   auto issue = [&](int buf, int bj) {
     if (lane == 0) {
@@ -204,6 +344,10 @@ __global__ void __launch_bounds__(kThreads, FIELD ? QS_SW_MINB_FIELD : QS_SW_MIN
       }
     }
   };
+  auto add_into = [](Accum& dst, const Accum& v) {
+    dst.y += v.y;
+    if (FIELD) dst.br += v.br, dst.bz += v.bz;
+  };
 
   for (;;) {
     long long k0 = 0;
@@ -211,81 +355,109 @@ __global__ void __launch_bounds__(kThreads, FIELD ? QS_SW_MINB_FIELD : QS_SW_MIN
     k0 = __shfl_sync(full, k0, 0);
     if (k0 >= prm.n_items) break;
     const int cnt = static_cast<int>(min(static_cast<long long>(prm.chunk), prm.n_items - k0));
-    int bi, bj;
-    unrank(k0, prm.nb, bi, bj);
+    int I, loc, a, b, bj;
+    wl.unrank(k0, I, loc);
+    wl.decode(I, loc, a, b, bj);
     issue(0, bj);
 
-    TargetRegs t;
-    Accum acc = {0.0, 0.0, 0.0};
-    double4 bbi;
-    int cur_bi = -1;
-    for (int it = 0; it < cnt; ++it) {
-      const int buf = it & 1;
-      if (bi != cur_bi) {  // new target block: flush the old accumulators, load the new targets
-        if (cur_bi >= 0) {
-          red_add(prm.yacc + 32ll * cur_bi + lane, acc.y);
+    TargetRegs t[T];
+    Accum acc[T];
+    double4 bbU = make_double4(0.0, 0.0, 0.0, 0.0);   // union of the boxes of the super-block's target blocks
+    bool uniT = false;
+    int cur_I = -1, Ta = 0;
+    auto flush = [&]() {
+#pragma unroll
+      for (int k = 0; k < T; ++k)
+        if (k < Ta) {
+          const long long i = 32ll * (T * cur_I + k) + lane;
+          red_add(prm.yacc + i, acc[k].y);
           if (FIELD) {
-            red_add(prm.bracc + 32ll * cur_bi + lane, acc.br);
-            red_add(prm.bzacc + 32ll * cur_bi + lane, acc.bz);
+            red_add(prm.bracc + i, acc[k].br);
+            red_add(prm.bzacc + i, acc[k].bz);
           }
         }
-        acc = {0.0, 0.0, 0.0};
-        cur_bi = bi;
-        const long long i = 32ll * bi + lane;
-        t.r = prm.r[i];
-        t.z = prm.z[i];
-        t.x = prm.x[i];
-        t.cur = FIELD ? prm.cur[i] : 0.0;
-        bbi = prm.bbox[bi];
+    };
+    for (int it = 0; it < cnt; ++it) {
+      const int buf = it & 1;
+      if (I != cur_I) {  // new target super-block: flush the old accumulators, load the new targets
+        if (cur_I >= 0) flush();
+        cur_I = I;
+        Ta = wl.blocks_in(I);
+        uniT = true;
+#pragma unroll
+        for (int k = 0; k < T; ++k) {
+          acc[k] = {0.0, 0.0, 0.0};
+          const int blk = T * I + (k < Ta ? k : 0);
+          const long long i = 32ll * blk + lane;
+          t[k].r = prm.r[i];
+          t[k].z = prm.z[i];
+          t[k].x = prm.x[i];
+          t[k].cur = FIELD ? prm.cur[i] : 0.0;
+          const double4 bk = prm.bbox[blk];
+          uniT = uniT && bk.x == bk.y;
+          if (k == 0) {
+            bbU = bk;
+          } else {
+            bbU.x = fmin(bbU.x, bk.x), bbU.y = fmax(bbU.y, bk.y);
+            bbU.z = fmin(bbU.z, bk.z), bbU.w = fmax(bbU.w, bk.w);
+          }
+        }
       }
-      // next item of this chunk (row-major walk), prefetched into the other buffer
-      int nbi = bi, nbj = bj + 1;
-      if (nbj == prm.nb) {
-        nbi = bi + 1;
-        nbj = nbi;
+      // next item of this chunk, prefetched into the other buffer
+      int nI = I, nloc = loc + 1, na = 0, nbb = 0, nbj = 0;
+      if (nloc == wl.row_count(I)) {
+        nI = I + 1;
+        nloc = 0;
       }
-      if (it + 1 < cnt) issue(buf ^ 1, nbj);
+      if (it + 1 < cnt) {
+        wl.decode(nI, nloc, na, nbb, nbj);
+        issue(buf ^ 1, nbj);
+      }
 
       const double4 bbj = prm.bbox[bj];
-      const bool uni = bbi.x == bbi.y && bbj.x == bbj.y;   // both blocks on one radius each (lattice rows)
-      const int nit = classify(bbi, bbj, bi == bj, prm);
       mbar_wait(&sbar[warp][buf], (phase >> buf) & 1u);
       phase ^= 1u << buf;
       const double* sr = sbuf[warp][buf][0];
       const double* sz = sbuf[warp][buf][1];
       const double* sx = sbuf[warp][buf][2];
       const double* sc = sbuf[warp][buf][3];
-      if (bi == bj) {
-#define QS_DIAG(N_, HI_) item_diag<N_, HI_, FIELD>(t, sr, sz, sx, sc, prm.soft_all, prm.soft_self, lane, acc); break
-        switch (nit) {   // diagonal items are rare: the four cheapest classes share (4, lo)
-          case 0: case 1: case 2: case 3: case 4: QS_DIAG(4, false);
-          case 5: QS_DIAG(4, true);
-          case 6: QS_DIAG(5, false);
-          case 7: QS_DIAG(5, true);
-          case 8: QS_DIAG(6, false);
-          default: QS_DIAG(7, false);
-        }
+      if (a >= 0 && a == b) {   // diagonal item of target block a
+        const int nit = classify(bbj, bbj, true, prm);
+#pragma unroll
+        for (int k = 0; k < T; ++k)
+          if (k == a) {
+#define QS_DIAG(N_, O_) item_diag<N_, O_, FIELD>(t[k], sr, sz, sx, sc, prm.soft_all, prm.soft_self, lane, acc[k])
+            if (nit <= 4) {   // diagonal items are rare: every class up to (4, 2) shares (4, 2)
+              QS_DIAG(4, 2);
+            } else {
+              switch (nit) {
+                case 5: QS_DIAG(4, 4); break;
+                case 6: QS_DIAG(5, 2); break;
+                case 7: QS_DIAG(5, 4); break;
+                case 8: QS_DIAG(6, 2); break;
+                default: QS_DIAG(7, 2); break;
+              }
+            }
 #undef QS_DIAG
-      } else {
+          }
+      } else if (a >= 0) {      // single-target item inside the super-block's triangle: rare, deepest class (always valid)
         Accum trav = {0.0, 0.0, 0.0};
-#define QS_OFF(N_, HI_)                                                                              \
-  if (uni)                                                                                           \
-    item_offdiag<N_, HI_, FIELD, true>(t, sr, sz, sx, sc, prm.soft_all, bbj.x, lane, acc, trav);     \
-  else                                                                                               \
-    item_offdiag<N_, HI_, FIELD, false>(t, sr, sz, sx, sc, prm.soft_all, 0.0, lane, acc, trav);      \
-  break
-        switch (nit) {
-          case 0: QS_OFF(2, false);
-          case 1: QS_OFF(2, true);
-          case 2: QS_OFF(3, false);
-          case 3: QS_OFF(3, true);
-          case 4: QS_OFF(4, false);
-          case 5: QS_OFF(4, true);
-          case 6: QS_OFF(5, false);
-          case 7: QS_OFF(5, true);
-          case 8: QS_OFF(6, false);
-          default: QS_OFF(7, false);
-        }
+#pragma unroll
+        for (int k = 0; k < T - 1; ++k)
+          if (k == a) item_offdiag<7, 2, FIELD, false>(t[k], sr, sz, sx, sc, prm.soft_all, 0.0, lane, acc[k], trav);
+#pragma unroll
+        for (int k = 1; k < T; ++k)
+          if (k == b) add_into(acc[k], trav);   // lane l of trav = source ring l of block b = target l of acc[b]
+      } else {
+        const bool uni = uniT && bbj.x == bbj.y;   // every block on one radius (lattice rows)
+        const int nit = classify(bbU, bbj, false, prm);
+        Accum trav = {0.0, 0.0, 0.0};
+#define QS_OFF(N_, O_)                                                                              \
+  if (uni)                                                                                          \
+    item_multi<N_, O_, FIELD, true, T>(t, sr, sz, sx, sc, prm.soft_all, bbj.x, lane, acc, trav);    \
+  else                                                                                              \
+    item_multi<N_, O_, FIELD, false, T>(t, sr, sz, sx, sc, prm.soft_all, 0.0, lane, acc, trav)
+        QS_CLASS_SWITCH(nit, QS_OFF)
 #undef QS_OFF
         red_add(prm.yacc + 32ll * bj + lane, trav.y);
         if (FIELD) {
@@ -294,14 +466,9 @@ __global__ void __launch_bounds__(kThreads, FIELD ? QS_SW_MINB_FIELD : QS_SW_MIN
         }
       }
       __syncwarp();  // every lane is done reading sbuf[buf] before it is refilled two items later
-      bi = nbi;
-      bj = nbj;
+      I = nI, loc = nloc, a = na, b = nbb, bj = nbj;
     }
-    red_add(prm.yacc + 32ll * cur_bi + lane, acc.y);
-    if (FIELD) {
-      red_add(prm.bracc + 32ll * cur_bi + lane, acc.br);
-      red_add(prm.bzacc + 32ll * cur_bi + lane, acc.bz);
-    }
+    flush();
   }
 }
 
@@ -309,17 +476,17 @@ __global__ void diag_kernel(int n, const double* __restrict__ r, double d2self, 
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const double s = r[i] + r[i];
-  const PairAGM a = agm_pair<7, false, false>(fma(s, s, d2self), d2self);
+  const PairAGM a = agm_pair<7, 2, false>(fma(s, s, d2self), d2self);
   diagM[i] = (0.5 * kMu0 * kPi) * a.S * a.yinf;
 }
 // ---- test hook: one pair per thread through a chosen evaluation class (cls < 0: chosen from k'^2 like the sweep) ----
-template <int NIT, bool HI>
+template <int NIT, int ORD>
 __device__ __forceinline__ void pair_out(double A2, double B2, double* M, double* K, double* E) {
-  const PairAGM a = agm_pair<NIT, HI, true>(A2, B2);
+  const PairAGM a = agm_pair<NIT, ORD, true>(A2, B2);
   *M = (0.5 * kMu0 * kPi) * a.S * a.yinf;
   const double sa = sqrt(A2);
   *K = (0.5 * kPi) * a.yinf * sa;
-  *E = (0.5 * kPi) * a.yinf * (a.mid - a.S) / sa;
+  *E = (0.5 * kPi) * a.yinf * a.emS / sa;
 }
 __global__ void pair_eval_kernel(int n, const double* __restrict__ A2, const double* __restrict__ B2, int cls,
                                  double* __restrict__ M, double* __restrict__ K, double* __restrict__ E,
@@ -334,18 +501,9 @@ __global__ void pair_eval_kernel(int n, const double* __restrict__ A2, const dou
       if (kp2 >= kClassKp2Min[k]) c = k;
   }
   used[i] = c;
-  switch (c) {
-    case 0: pair_out<2, false>(A2[i], B2[i], M + i, K + i, E + i); break;
-    case 1: pair_out<2, true>(A2[i], B2[i], M + i, K + i, E + i); break;
-    case 2: pair_out<3, false>(A2[i], B2[i], M + i, K + i, E + i); break;
-    case 3: pair_out<3, true>(A2[i], B2[i], M + i, K + i, E + i); break;
-    case 4: pair_out<4, false>(A2[i], B2[i], M + i, K + i, E + i); break;
-    case 5: pair_out<4, true>(A2[i], B2[i], M + i, K + i, E + i); break;
-    case 6: pair_out<5, false>(A2[i], B2[i], M + i, K + i, E + i); break;
-    case 7: pair_out<5, true>(A2[i], B2[i], M + i, K + i, E + i); break;
-    case 8: pair_out<6, false>(A2[i], B2[i], M + i, K + i, E + i); break;
-    default: pair_out<7, false>(A2[i], B2[i], M + i, K + i, E + i); break;
-  }
+#define QS_PAIR_OUT(N_, O_) pair_out<N_, O_>(A2[i], B2[i], M + i, K + i, E + i)
+  QS_CLASS_SWITCH(c, QS_PAIR_OUT)
+#undef QS_PAIR_OUT
 }
 cudaError_t launch_pair_eval(int n, const double* A2, const double* B2, int cls, double* M, double* K, double* E,
                              int* used, cudaStream_t stream) {
@@ -375,7 +533,7 @@ __global__ void __launch_bounds__(kBpWarps * 32) blockprec_build_kernel(int nb, 
     const double dz2 = fma(dz, dz, soft_all) + (j == lane ? soft_self : 0.0);
     const double dif = ri - rj;
     const double B2 = fma(dif, dif, dz2), A2 = fma(4.0 * ri, rj, B2);
-    const PairAGM a = agm_pair<7, false, false>(A2, B2);
+    const PairAGM a = agm_pair<7, 2, false>(A2, B2);
     At[lane][j] = (0.5 * kMu0 * kPi) * a.S * a.yinf;
   }
   __syncwarp();
@@ -576,11 +734,15 @@ cudaError_t issue_probe(int mode, double* cycles_per_dfma) {
 
 int sweep_grid(int sm_count, bool field) { return sm_count * (field ? QS_SW_MINB_FIELD : QS_SW_MINB_M); }
 
+long long sweep_items(int nb, bool field) {
+  return field ? WorkList<QS_SW_T_FIELD>(nb).total() : WorkList<QS_SW_T_M>(nb).total();
+}
+
 cudaError_t launch_sweep(const SweepParams& prm, bool field, int grid, cudaStream_t stream) {
   if (field)
-    sweep_kernel<true><<<grid, kThreads, 0, stream>>>(prm);
+    sweep_kernel<true, QS_SW_T_FIELD><<<grid, kThreads, 0, stream>>>(prm);
   else
-    sweep_kernel<false><<<grid, kThreads, 0, stream>>>(prm);
+    sweep_kernel<false, QS_SW_T_M><<<grid, kThreads, 0, stream>>>(prm);
   return cudaGetLastError();
 }
 

@@ -17,7 +17,7 @@ namespace qs {
 
 namespace {
 constexpr int kBlock = 256;
-int g_sm_count = 0;
+thread_local int g_sm_count = 0;   // SM count of the handle whose kernel is being launched (set by QS_LAUNCH)
 inline int grid_for(int n) {
   if (g_sm_count == 0) {
     int dev = 0;
@@ -673,7 +673,7 @@ __global__ void stats_kernel(int n, double C3, double C1, const double* __restri
 }
 }  // namespace
 
-#define QS_LAUNCH(v) (++*(v).launches)
+#define QS_LAUNCH(v) (g_sm_count = (v).sm_count, ++*(v).launches)
 
 void k_material(const VecCtx& v, const MaterialParams& mp, const MaterialArgs& a) {
   QS_LAUNCH(v);
@@ -735,11 +735,6 @@ void k_heat_substep(const VecCtx& v, const MaterialParams& mp, const LatticePara
   }
   dim3 grid(gx, (lp.Nr + rows - 1) / rows);
   if (tma) {
-    static bool attr_set = false;
-    if (!attr_set) {
-      cudaFuncSetAttribute(heat_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(sizeof(HeatSmem)));
-      attr_set = true;
-    }
     heat_tma_kernel<<<grid, kHeatWarps * 32, sizeof(HeatSmem), v.stream>>>(mp, lp, rows, Hin, Q, Hout, dtsub);
   } else
     heat_kernel<false><<<grid, kHeatWarps * 32, 0, v.stream>>>(mp, lp, rows, Hin, Q, Hout, dtsub);
@@ -748,15 +743,14 @@ bool k_heat_all_substeps(const VecCtx& v, const MaterialParams& mp, const Lattic
                          const double* Q, double* Hout, double dtsub) {
   const long long N = static_cast<long long>(lp.Nr) * lp.Nz;
   if (N > kHeatSmallMax || m < 2) return false;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(heat_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);   // N + 3 (Nr + Nz) doubles <= 131 KB
-    attr_set = true;
-  }
   QS_LAUNCH(v);
   heat_small_kernel<<<1, kHeatSmallThreads, sizeof(double) * (N + 3 * (lp.Nr + lp.Nz)), v.stream>>>(mp, lp, m, Hin, Q, Hout,
                                                                                                  dtsub);
   return true;
+}
+void pointwise_prepare_device() {
+  cudaFuncSetAttribute(heat_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(sizeof(HeatSmem)));
+  cudaFuncSetAttribute(heat_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);   // N + 3 (Nr + Nz) doubles <= 131 KB
 }
 void k_events(const VecCtx& v, const MaterialParams& mp, const EventArgs& e) {
   if (!v.n_turns) return;

@@ -10,7 +10,7 @@ namespace qs {
 
 namespace {
 constexpr int kBlock = 256;
-int g_sm_count = 0;
+thread_local int g_sm_count = 0;   // SM count of the handle whose kernel is being launched (set by QS_LAUNCH)
 
 inline int grid_for(int n) {
   if (g_sm_count == 0) {
@@ -204,6 +204,14 @@ __global__ void nu_residual_kernel(int n, double I_ramp, const double* __restric
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
     r[i] = I_ramp * fma(shift[i], xp1[i], Mxp1[i]) - rhs_at(b, i);
 }
+__global__ void field_scale_kernel(int n, const double* __restrict__ bracc, const double* __restrict__ bzacc,
+                                   const double* __restrict__ r, const double* __restrict__ selfcoef,
+                                   const double* __restrict__ cur, double* __restrict__ Br, double* __restrict__ Bz) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    Br[i] = (0.25 * kMu0) * bracc[i] / r[i];
+    Bz[i] = fma(0.25 * kMu0, bzacc[i], selfcoef[i] * cur[i]);
+  }
+}
 __global__ void sum_uterm_kernel(int n, const double* __restrict__ share, const double* __restrict__ vsum, Scalars* sc) {
   double acc = 0.0;                                          // U_terminal = -sum_w share_w V_w (C16)
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) acc = fma(share[i], vsum[i], acc);
@@ -218,6 +226,135 @@ __global__ void scatter_scaled_kernel(int n, const double* __restrict__ src, con
                                       double* __restrict__ dst, double scale) {
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
     dst[perm ? perm[i] : i] = scale * src[i];
+}
+
+// ---- fused step kernels (qs_step with constraint groups): few launches per step, no host round trip before the CG's
+// first convergence test ---------------------------------------------------------------------------------------------
+__global__ void step_begin_kernel(StepBegin a, Scalars* sc) {
+  const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+  // state backups, CG start (plain warm start or the linear extrapolation 2 I'_k - I'_{k-1}), ring currents I = a J
+  for (int i = tid; i < a.N; i += nth) {
+    const double Ji = a.J[i];
+    a.Jold[i] = Ji;
+    a.Hold[i] = a.H[i];
+    const double xi = a.x[i];
+    a.xold[i] = xi;
+    if (a.extrapolate) a.x[i] = fma(2.0, xi, -a.xprev2[i]);
+    a.xprev2[i] = xi;
+    a.cur[i] = a.area[i] * Ji;
+  }
+  // the two contiguous backup blocks (derived fields; per-turn event state), 8 bytes at a time
+  for (size_t i = tid; i < a.fld_words; i += nth) a.fld_backup[i] = a.fld[i];
+  for (size_t i = tid; i < a.ev_words; i += nth) a.ev_backup[i] = a.ev[i];
+  // sweep accumulators + work counter, per-turn scratch, event observables of the material pass, solver scalars
+  for (size_t i = tid; i < a.acc_words; i += nth) a.acc[i] = 0ull;
+  for (int w = tid; w < a.n_turns; w += nth) {
+    a.vsum[w] = 0.0;
+    a.tw[w] = 0.0;
+    if (a.xmax_bits) {
+      a.xmax_bits[w] = 0ull;
+      a.rmin_bits[w] = ~0ull;
+    }
+  }
+  if (tid == 0) {
+    sc->rg[0] = sc->rg[1] = sc->pq[0] = sc->pq[1] = sc->nu2 = 0.0;
+    sc->done = 0;
+    sc->iters = 0;
+    sc->blocks_done = 0u;
+    sc->thresh2 = 0.0;
+    sc->uterm = sc->joule = 0.0;
+    sc->tmax = 0.0;
+    sc->djmax = 0.0;
+    sc->nonfinite = 0;
+    sc->event_or = 0;
+  }
+}
+
+constexpr int kTurnBlock = 128;
+__device__ __forceinline__ double turn_block_sum(double v, double* sh) {   // sum over the CTA, result in every thread
+  v = warp_sum(v);
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double s = 0.0;
+#pragma unroll
+  for (int k = 0; k < kTurnBlock / 32; ++k) s += sh[k];
+  return s;
+}
+
+// one CTA per constraint group: deficit_w = d share_w - sum_{i in w} x_i ; x_i += deficit_w / (H_i s_w)  (C8: moves a
+// warm start onto the constraint; H = diag(M), s_w its per-turn Schur scalar)
+__global__ void __launch_bounds__(kTurnBlock) turn_fix_kernel(const int* __restrict__ ptr, const int* __restrict__ idx,
+                                                              const double* __restrict__ share, double d,
+                                                              const double* __restrict__ Hd, const double* __restrict__ sw,
+                                                              double* __restrict__ x) {
+  __shared__ double sh[kTurnBlock / 32];
+  const int w = blockIdx.x, k0 = ptr[w], k1 = ptr[w + 1];
+  double acc = 0.0;
+  for (int k = k0 + threadIdx.x; k < k1; k += kTurnBlock) acc += x[idx[k]];
+  const double def = fma(d, share[w], -turn_block_sum(acc, sh)) / sw[w];
+  for (int k = k0 + threadIdx.x; k < k1; k += kTurnBlock) {
+    const int i = idx[k];
+    x[i] += def / Hd[i];
+  }
+}
+
+// one CTA per constraint group, after the material pass: everything between the sweep and the first convergence test
+// of the projected CG (C8), for BOTH residuals at once -
+//   r1 = I_ramp (M xp1 + shift xp1) - b   (cold start: its projected norm is the reference norm nu)
+//   r2 = M x + shift x - b                (the warm start x, already on the constraint)
+// s_w = sum 1/H, v = (sum r/H)/s_w, r <- r - v, g = r/H, nu2 += r1.g1, rg[0] += r2.g2, p = -g2; the multipliers of the
+// two projections go to vnu[w] and vsum[w].
+__global__ void __launch_bounds__(kTurnBlock) turn_start_kernel(TurnStart a, Scalars* sc) {
+  __shared__ double sh[kTurnBlock / 32];
+  const int w = blockIdx.x, k0 = a.ptr[w], k1 = a.ptr[w + 1];
+  double s = 0.0, a1 = 0.0, a2 = 0.0;
+  for (int k = k0 + threadIdx.x; k < k1; k += kTurnBlock) {
+    const int i = a.idx[k];
+    const double hinv = 1.0 / a.Hd[i], bi = rhs_at(a.b, i), sh_i = a.shift[i];
+    const double r1 = a.I_ramp * fma(sh_i, a.xp1[i], a.Mxp1[i]) - bi;
+    const double r2 = fma(sh_i, a.x[i], a.cM * a.yacc[i]) - bi;
+    a.g[i] = r1;          // parked until the second pass
+    a.r[i] = r2;
+    s += hinv;
+    a1 = fma(r1, hinv, a1);
+    a2 = fma(r2, hinv, a2);
+  }
+  s = turn_block_sum(s, sh);
+  const double v1 = turn_block_sum(a1, sh) / s, v2 = turn_block_sum(a2, sh) / s;
+  double nu2 = 0.0, rg = 0.0;
+  for (int k = k0 + threadIdx.x; k < k1; k += kTurnBlock) {
+    const int i = a.idx[k];
+    const double hinv = 1.0 / a.Hd[i];
+    const double r1 = a.g[i] - v1, r2 = a.r[i] - v2;
+    const double g2 = r2 * hinv;
+    nu2 = fma(r1 * hinv, r1, nu2);
+    rg = fma(r2, g2, rg);
+    a.r[i] = r2;
+    a.g[i] = g2;
+    a.p[i] = -g2;
+  }
+  nu2 = turn_block_sum(nu2, sh);
+  rg = turn_block_sum(rg, sh);
+  if (threadIdx.x == 0) {
+    a.sw[w] = s;
+    a.vnu[w] = v1;
+    a.vsum[w] = v2;
+    atomicAdd(&sc->nu2, nu2);
+    atomicAdd(&sc->rg[0], rg);
+  }
+}
+
+// S5 (J += dt I'/a) and the terminal voltage sum_w share_w vsum_w in one launch
+__global__ void step_update_kernel(int n, double dt, const double* __restrict__ x, const double* __restrict__ area,
+                                   double* __restrict__ J, int n_turns, const double* __restrict__ share,
+                                   const double* __restrict__ vsum, Scalars* sc) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) J[i] += dt * x[i] / area[i];
+  if (blockIdx.x == 0) {
+    double acc = 0.0;
+    for (int w = threadIdx.x; w < n_turns; w += blockDim.x) acc = fma(share[w], vsum[w], acc);
+    block_atomic_sum(acc, &sc->uterm);
+  }
 }
 
 // ---- fused CG iteration ---------------------------------------------------------------------------------------------
@@ -323,7 +460,7 @@ __global__ void cg_direction_kernel(int n, int npad, int n_turns, CgIter it, Sca
 }
 }  // namespace
 
-#define QS_LAUNCH(v) (++*(v).launches)
+#define QS_LAUNCH(v) (g_sm_count = (v).sm_count, ++*(v).launches)
 
 void k_finish_Ap(const VecCtx& v, const double* yacc, const double* shift, const double* p, double* q, double cM) {
   QS_LAUNCH(v);
@@ -401,6 +538,24 @@ void k_cg_direction(const VecCtx& v, const CgIter& it) {
   QS_LAUNCH(v);
   cg_direction_kernel<<<grid_for(v.Np), kBlock, 0, v.stream>>>(v.N, v.Np, v.n_turns, it, v.sc);
 }
+void k_step_begin(const VecCtx& v, const StepBegin& a) {
+  QS_LAUNCH(v);
+  const size_t most = a.acc_words > static_cast<size_t>(a.N) ? a.acc_words : static_cast<size_t>(a.N);
+  step_begin_kernel<<<grid_for(static_cast<int>(most < (1u << 30) ? most : (1u << 30))), kBlock, 0, v.stream>>>(a, v.sc);
+}
+void k_turn_fix(const VecCtx& v, double d, const double* Hd, const double* sw, double* x) {
+  if (!v.n_turns) return;
+  QS_LAUNCH(v);
+  turn_fix_kernel<<<v.n_turns, kTurnBlock, 0, v.stream>>>(v.turn_ptr, v.turn_idx, v.share, d, Hd, sw, x);
+}
+void k_turn_start(const VecCtx& v, const TurnStart& a) {
+  QS_LAUNCH(v);
+  turn_start_kernel<<<v.n_turns, kTurnBlock, 0, v.stream>>>(a, v.sc);
+}
+void k_step_update(const VecCtx& v, double dt, const double* x, const double* area, double* J, const double* vsum) {
+  QS_LAUNCH(v);
+  step_update_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, dt, x, area, J, v.n_turns, v.share, vsum, v.sc);
+}
 void k_axpy(const VecCtx& v, double a, const double* x, double* y) {
   QS_LAUNCH(v);
   axpy_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, a, x, y);
@@ -433,6 +588,11 @@ void k_nu_residual(const VecCtx& v, double I_ramp, const double* Mxp1, const dou
                    const Rhs& b, double* r) {
   QS_LAUNCH(v);
   nu_residual_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, I_ramp, Mxp1, shift, xp1, b, r);
+}
+void k_field_scale(const VecCtx& v, const double* bracc, const double* bzacc, const double* r, const double* selfcoef,
+                   const double* cur, double* Br, double* Bz) {
+  QS_LAUNCH(v);
+  field_scale_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, bracc, bzacc, r, selfcoef, cur, Br, Bz);
 }
 void k_sum_uterm(const VecCtx& v, const double* vsum) {
   if (!v.n_turns) return;

@@ -39,15 +39,17 @@ def test_matvec_free_rings_full(pkg, n):
     assert st["pair_evals"] >= nb * (nb + 1) // 2 * 1024 and st["launches"] > 0
 
 
-@pytest.mark.parametrize("n,rows", [(65536, 256), (262144, 128), (1048576, 64)])
+@pytest.mark.parametrize("n,rows", [(65536, 1024), (262144, 1024), (1048576, 1024)])
 def test_matvec_free_rings_sampled_rows(pkg, n, rows):
-    # BASELINE.json configs[4] sizes; the oracle evaluates exact rows sum_j M_ij x_j on a seeded row sample
+    # BASELINE.json configs[4] sizes; the oracle evaluates exact rows sum_j M_ij x_j on a seeded sample of 1024 target
+    # rows (SURVEY.md §8(d) parity protocol), pair by pair against all n sources
     geo, x = wl.free_rings(n)
     idx = wl.sample_rows(n, rows, seed=n)
     with pkg.QS(geo, wl.Material()) as sim:
         y = sim.matvec(x)
     yo = qo.matvec_rows(geo, x, idx, chunk=16)
     assert rel(y[idx], yo) <= 1e-9
+    assert np.max(np.abs(y[idx] - yo)) <= 1e-9 * np.max(np.abs(yo))
     assert np.all(np.isfinite(y))
 
 
@@ -214,6 +216,7 @@ def test_pair_arithmetic_every_class_at_its_threshold(pkg):
     # per-pair K, E, M of the sweeps against the oracle's library route (scipy Cephes K/E + Maxwell bracket),
     # each evaluation class probed from its own k'^2 threshold upwards (where its truncation error is largest)
     from paper_2403_07666_b200 import pair_eval
+    # classes (NIT, ORD): (2,2) (2,4) (3,2) (3,4) (4,2) (4,4) (5,2) (5,4) (6,2) (7,2)
     thr = [0.3965, 0.1394, 0.01529, 1.374e-3, 1.453e-5, 1.157e-7, 1.293e-11, 8.2e-16, 1.03e-23, 1e-27]
     ri = 0.05
     for cls, t in enumerate(thr):

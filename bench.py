@@ -63,7 +63,11 @@ def parse_args():
                     help="pairs: on-the-fly AGM pair sweeps (north_star, default); tables: lattice-aware operator (f1)")
     ap.add_argument("--leg", default="all", choices=["all", "hbm", "operator"],
                     help="hbm / operator: run only that extra leg and print its JSON (used for the ncu captures)")
+    ap.add_argument("--sizes", default="4096,65536,262144,1048576", help="ring counts of the config-4 operator leg")
+    ap.add_argument("--cg-budget-s", type=float, default=45.0,
+                    help="operator leg: seconds of CG per size above 65,536 rings (0: matvec only)")
     a = ap.parse_args()
+    a.sizes = tuple(int(v) for v in a.sizes.split(",") if v)
     k, w = DEFAULTS[a.workload]
     a.steps = a.steps or k
     a.warmup = max(a.warmup or w, 3)
@@ -366,6 +370,9 @@ def operator_leg(torch, pkg, fp64_peak, sizes=(4096, 65536, 262144, 1048576), bu
             rec = {"matvec_ms": ms, "pair_evals_per_s": pe / ms * 1e3, "pair_interactions_per_s": n * n / ms * 1e3,
                    "nominal_tflops": tf, "frac_of_fp64_peak": tf / fp64_peak}
             # CG: to tolerance, or the iterations that fit the time budget of this size (at least 20)
+            if budget_s <= 0.0:
+                out[f"N{n}"] = rec
+                continue
             per_it_s = ms * 1e-3 * 1.05
             maxit = to_tol.get(n) or int(max(20, min(200, budget_s / per_it_s)))
             sim.solve_device(bd, xh, maxit=2)                 # graph capture, first-touch
@@ -440,7 +447,8 @@ def gpu_arm(args):
     hbm_peak, hbm_src = load_measured_peaks()
     fp64_tf, fp64_mhz = pkg.fp64_peak()
     if args.leg != "all":
-        leg = hbm_roofline_leg(torch, pkg, hbm_peak) if args.leg == "hbm" else operator_leg(torch, pkg, fp64_tf)
+        leg = (hbm_roofline_leg(torch, pkg, hbm_peak) if args.leg == "hbm"
+               else operator_leg(torch, pkg, fp64_tf, args.sizes, args.cg_budget_s))
         print(json.dumps({"leg": args.leg, **leg}), flush=True)
         return
 
@@ -571,7 +579,7 @@ def gpu_arm(args):
         line["roofline_hbm"]["peak_source"] = f"MEASURED_PEAKS.json hbm_gbs ({hbm_src})"
         line["roofline_hbm"]["traffic_source"] = NCU_SOURCE
         line["cg_active"] = cg_active_leg(torch, pkg)
-        line["operator_cfg4"] = operator_leg(torch, pkg, fp64_tf)
+        line["operator_cfg4"] = operator_leg(torch, pkg, fp64_tf, args.sizes, args.cg_budget_s)
         line["cpu_baseline"] = cpu_baseline
     if rank == 0:
         print(json.dumps(line), flush=True)

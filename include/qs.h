@@ -66,6 +66,11 @@ typedef struct qs_ctx qs_ctx;
                                   Toeplitz products instead of on-the-fly pair sweeps.  Same
                                   arithmetic per unique pair, same results up to summation order.  */
 
+#define QS_GEO_NO_PATCH_PRECOND 4 /* lattice geometries whose constraint groups are the wires: do NOT build the patch
+                                    (block-Jacobi over p x p cells of a wire, p <= 8) constraint preconditioner of the
+                                    projected CG (2 x 8 N p^2 bytes of workspace); the solver then keeps diag(A) (C8).
+                                    The preconditioner is free: the solution of a step is unique (C4).  */
+
 typedef struct {
   int32_t  n_rings;                 /* N                                                         */
   const double *r, *z, *area;       /* [N] ring centre radius, height, cross-section [m, m, m^2] */

@@ -163,6 +163,7 @@ struct qs_ctx {
   // CUDA graphs of two fused CG iterations (parities 0, 1), keyed by the vectors they were captured with
   struct CgGraph {
     const double *x = nullptr, *shift = nullptr, *Hd = nullptr, *sw = nullptr;
+    bool patch = false;
     cudaGraphExec_t exec = nullptr;
     int launches = 0;
   } cg_graph[2];
@@ -183,6 +184,9 @@ struct qs_ctx {
   int tabNr = 0, tabNz = 0;
   double4* bbox;
   double* Lblk = nullptr;            // [nb][32][32] block-Jacobi factors of M (free rings: unconstrained solves)
+  PatchPrec patch;                   // patch preconditioner of the lattice solves (pp = 0: off)
+  int* pidx = nullptr;               // [N] patch slot -> cell
+  int* pturn = nullptr;              // [N / pp] patch -> constraint group
   Scalars* sc;
   Scalars* h_sc = nullptr;           // pinned
   double* h_stage = nullptr;         // pinned staging, 2N doubles
@@ -271,6 +275,15 @@ void carve(qs_ctx* c, void* base, size_t* total) {
   c->d_perm = k.take<int>(N);
   c->bbox = k.take<double4>(std::max(c->nb, 1));
   if (c->blockprec) c->Lblk = k.take<double>(static_cast<size_t>(c->nb) * 1024);
+  if (c->patch.pp > 0) {
+    const size_t pp = c->patch.pp;
+    c->pidx = k.take<int>(N);
+    c->pturn = k.take<int>(N / pp);
+    c->patch.Pm = k.take<double>(N * pp);
+    c->patch.Pinv = k.take<double>(N * pp);
+    c->patch.h1 = k.take<double>(N);
+    c->patch.sw = k.take<double>(nt);
+  }
   if (c->tables) {
     const size_t nt3 = static_cast<size_t>(c->tabNr) * c->tabNr * c->tabNz;
     c->TM = k.take<double>(nt3);
@@ -302,6 +315,21 @@ int check_geometry(const qs_geometry* g) {
     if (Nr * Nz != g->n_rings) return fail(QS_ERR_ARG, "geometry: n_rings != Nr*Nz");
   }
   return QS_OK;
+}
+
+// Side p of the square patches of the patch preconditioner (0: not applicable): lattices whose constraint groups are
+// the wires in canonical numbering; p = the largest divisor of the cells per wire side that is <= 8.
+int patch_side(const qs_geometry* g) {
+  if (!g->lattice || (g->flags & (QS_GEO_NO_OPERATOR | QS_GEO_NO_PATCH_PRECOND)) || g->n_turns <= 0) return 0;
+  const int n = g->cells_per_side;
+  if (n < 2 || g->n_turns != g->layers * g->turns_per_layer) return 0;
+  const long long Nz = static_cast<long long>(g->turns_per_layer) * n;
+  for (long long k = 0; k < g->n_rings; ++k)
+    if (g->turn_id[k] != (k / Nz / n) * g->turns_per_layer + (k % Nz) / n) return 0;
+  int p = 1;
+  for (int d = 2; d <= 8 && d <= n; ++d)
+    if (n % d == 0) p = d;
+  return p >= 2 ? p : 0;
 }
 
 int sync_scalars(qs_ctx* c) {
@@ -431,6 +459,15 @@ int cg_core(qs_ctx* c, const Rhs& b, double* x, const double* shift, const doubl
   it.cM = kCM;
   it.Lblk = Lblk;
   it.nb = c->nb;
+  // lattice solves with wires as constraint groups: patch (block-Jacobi) preconditioner, set up only now that the solve
+  // really iterates - the block projection replaces the diagonal one from here on (the multipliers keep accumulating)
+  const bool use_patch = c->patch.pp > 0 && c->n_turns > 0 && !Lblk;
+  if (use_patch) {
+    it.patch = c->patch;
+    it.sw = c->patch.sw;
+    it.par = 0;
+    k_patch_start(v, it, shift);
+  }
   // one iteration = sweep + four vector kernels; pairs of iterations are replayed from a CUDA graph (captured on
   // first use for this set of vectors) unless the event profiler is recording
   auto enqueue_iteration = [&](int par) -> int {
@@ -448,7 +485,8 @@ int cg_core(qs_ctx* c, const Rhs& b, double* x, const double* shift, const doubl
   qs_ctx::CgGraph* graph = nullptr;
   if (!c->prof.on) {
     for (auto& gslot : c->cg_graph)
-      if (gslot.exec && gslot.x == x && gslot.shift == shift && gslot.Hd == Hd && gslot.sw == sw) graph = &gslot;
+      if (gslot.exec && gslot.x == x && gslot.shift == shift && gslot.Hd == Hd && gslot.sw == sw && gslot.patch == use_patch)
+        graph = &gslot;
     if (!graph) {
       qs_ctx::CgGraph& gslot = c->cg_graph[c->cg_graph[0].exec ? 1 : 0];
       if (gslot.exec) {
@@ -462,7 +500,7 @@ int cg_core(qs_ctx* c, const Rhs& b, double* x, const double* shift, const doubl
         const bool ok = enqueue_iteration(0) == QS_OK && enqueue_iteration(1) == QS_OK;
         const cudaError_t ec = cudaStreamEndCapture(c->stream, &gr);
         if (ok && ec == cudaSuccess && gr && cudaGraphInstantiate(&gslot.exec, gr, 0) == cudaSuccess) {
-          gslot.x = x, gslot.shift = shift, gslot.Hd = Hd, gslot.sw = sw;
+          gslot.x = x, gslot.shift = shift, gslot.Hd = Hd, gslot.sw = sw, gslot.patch = use_patch;
           gslot.launches = static_cast<int>(c->launches - l0);
           graph = &gslot;
         } else {
@@ -896,6 +934,11 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
   c->has_operator = !(geo->flags & QS_GEO_NO_OPERATOR);
   c->tables = c->lattice && c->has_operator && (geo->flags & QS_GEO_LATTICE_TABLES);
   c->blockprec = !c->lattice && c->has_operator && geo->n_turns == 0;
+  {
+    const int ps = patch_side(geo);
+    c->patch.pp = ps * ps;
+    c->patch.n_patches = ps ? N / (ps * ps) : 0;
+  }
   c->Bext0 = geo->Bext0;
   c->Bext_rate = geo->Bext_rate;
   c->Bext_max = geo->Bext_max;
@@ -1123,6 +1166,28 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
         return bail(fail(QS_ERR_CUDA, "block preconditioner build failed"));
       ++c->launches;
     }
+    if (c->patch.pp > 0) {   // patch preconditioner: slot -> cell map, patch -> wire map, constant part M_patch
+      const int ps = static_cast<int>(std::lround(std::sqrt(static_cast<double>(c->patch.pp)))), pp = c->patch.pp;
+      const int n = lp.n, per = n / ps;                 // patches per wire side
+      std::vector<int> hidx(N), hturn(c->patch.n_patches);
+      int pch = 0;
+      for (int l = 0; l < geo->layers; ++l)
+        for (int tq = 0; tq < geo->turns_per_layer; ++tq)
+          for (int a = 0; a < per; ++a)
+            for (int b = 0; b < per; ++b, ++pch) {
+              hturn[pch] = l * geo->turns_per_layer + tq;
+              for (int i = 0; i < ps; ++i)
+                for (int j = 0; j < ps; ++j)
+                  hidx[pch * pp + i * ps + j] = (l * n + a * ps + i) * lp.Nz + tq * n + b * ps + j;
+            }
+      if (cudaMemcpyAsync(c->pidx, hidx.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+          cudaMemcpyAsync(c->pturn, hturn.data(), sizeof(int) * hturn.size(), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+          cudaStreamSynchronize(c->stream) != cudaSuccess)
+        return bail(fail(QS_ERR_CUDA, "upload of the patch tables failed"));
+      c->patch.pidx = c->pidx;
+      c->patch.pturn = c->pturn;
+      k_patch_build(v, c->patch, c->r, c->z, c->soft_all, c->soft_self);
+    }
     if (c->n_turns) {
       // unit-ramp particular solution x_p1 = H_M^-1 C (share/s_M) and M x_p1 (reference norm of the CG, C8, C16)
       k_turn_schur(v, c->diagM, c->swM);
@@ -1164,6 +1229,10 @@ size_t qs_workspace_bytes(const qs_geometry* geo) {
     tmp.tables = (geo->flags & QS_GEO_LATTICE_TABLES) && !(geo->flags & QS_GEO_NO_OPERATOR);
   }
   tmp.blockprec = !geo->lattice && !(geo->flags & QS_GEO_NO_OPERATOR) && geo->n_turns == 0;
+  {
+    const int ps = patch_side(geo);
+    tmp.patch.pp = ps * ps;
+  }
   size_t need = 0;
   carve(&tmp, nullptr, &need);
   return need;

@@ -96,6 +96,17 @@ struct VecCtx {
 
 // ---- fused projected-CG iteration (C8): four launches after the sweep, no host round trip; every kernel returns at
 // once when sc->done is set, so a batch of iterations can be enqueued blind -----------------------------------------
+// patch (block-Jacobi) constraint preconditioner of the lattice solves (qs_vector.cu)
+struct PatchPrec {
+  int pp = 0;               // cells per patch (0: off), p x p inside one wire
+  int n_patches = 0;
+  const int* pidx = nullptr;    // [n_patches][pp] cell of slot t of the patch
+  const int* pturn = nullptr;   // [n_patches] constraint group of the patch
+  double* Pm = nullptr;         // [n_patches][pp][pp] constant part M_patch [H]
+  double* Pinv = nullptr;       // [n_patches][pp][pp] (M_patch + diag(shift))^-1 of the current solve
+  double* h1 = nullptr;         // [N] Pinv 1
+  double* sw = nullptr;         // [n_turns] per-turn Schur scalars sum h1
+};
 struct CgIter {
   int par;                   // parity of this iteration: rg[par] old, rg[par^1] new, pq[par]
   const double* yacc_in;     // sweep accumulators of p
@@ -110,12 +121,16 @@ struct CgIter {
   double cM;
   const double* Lblk;        // non-null: block-Jacobi factors (unconstrained solves): g = B^-1 r instead of r / Hd
   int nb;                    // blocks of 32
+  PatchPrec patch;           // pp > 0: patch preconditioner (sw then points to patch.sw)
 };
 void k_cg_Ap(const VecCtx& v, const CgIter& it);          // q = shift p + cM yacc ; pq[par] += p.q
 void k_cg_update(const VecCtx& v, const CgIter& it);      // alpha = rg[par]/pq[par]; x += alpha p; r += alpha q; tw += r/H
 void k_cg_project(const VecCtx& v, const CgIter& it);     // r -= tw/sw; g = r/H; rg[par^1] += r.g
 void k_cg_direction(const VecCtx& v, const CgIter& it);   // p = -g + beta p; clears accumulators; last block: bookkeeping
 void k_cg_begin(const VecCtx& v, double thresh2);         // done = 0, iters = 0, pq = 0, blocks_done = 0
+void k_patch_build(const VecCtx& v, const PatchPrec& pc, const double* r, const double* z, double soft_all,
+                   double soft_self);
+void k_patch_start(const VecCtx& v, const CgIter& it, const double* shift);   // Pinv, then g, p, rg[0], vsum from the current r
 
 // Right-hand side of the circuit equations: a given array, or (inside qs_step) evaluated on the fly from the
 // material law's E as b_i = -2 pi r_i (E_i + r_i Bdot_ext / 2)   (C4)

@@ -5,6 +5,7 @@
 // needs no host round trip.  Reductions: warp shuffles -> one shared-memory stage -> one FP64 atomic per CTA.
 // Streaming kernels use grid-stride loops over a grid that is a multiple of the SM count.
 #include "qs_internal.h"
+#include "qs_pair.cuh"
 
 namespace qs {
 
@@ -357,6 +358,159 @@ __global__ void step_update_kernel(int n, double dt, const double* __restrict__ 
   }
 }
 
+// ---- patch (block-Jacobi) constraint preconditioner of the lattice solves -------------------------------------------
+// H = blockdiag over square patches of p x p cells inside one wire of (M_patch + diag(shift)); the projection of C8 with
+// a block H:  t = H^-1 r,  s_w = sum_{i in w} (H^-1 1)_i,  v_w = (sum_{i in w} t_i)/s_w,  g = t - v_w H^-1 1,  r <- r - v_w.
+// Patches never straddle a constraint group, so the per-turn Schur complement stays diagonal.
+constexpr int kPatchMax = 64;   // cells per patch (p <= 8)
+
+// once per qs_init: the constant part M_patch [H] of every patch, pair by pair with the sweeps' arithmetic
+__global__ void __launch_bounds__(kPatchMax) patch_build_kernel(int pp, const int* __restrict__ pidx,
+                                                               const double* __restrict__ r, const double* __restrict__ z,
+                                                               double soft_all, double soft_self, double* __restrict__ Pm) {
+  const int pch = blockIdx.x, t = threadIdx.x;
+  if (t >= pp) return;
+  const int i = pidx[pch * pp + t];
+  const double ri = r[i], zi = z[i];
+  double* row = Pm + (static_cast<size_t>(pch) * pp + t) * pp;
+  for (int u = 0; u < pp; ++u) {
+    const int j = pidx[pch * pp + u];
+    const double rj = r[j], dz = zi - z[j];
+    const double dz2 = fma(dz, dz, soft_all) + (u == t ? soft_self : 0.0);
+    const double dif = ri - rj;
+    const double B2 = fma(dif, dif, dz2), A2 = fma(4.0 * ri, rj, B2);
+    const PairAGM a = agm_pair<7, 2, false>(A2, B2);
+    row[u] = (0.5 * kMu0 * kPi) * a.S * a.yinf;
+  }
+}
+
+// per solve: Pinv = (M_patch + diag(shift))^-1 by in-place Gauss-Jordan elimination in shared memory (SPD: no pivoting),
+// h1 = Pinv 1, s_w += sum h1.  One CTA per patch, one thread per row.
+__global__ void __launch_bounds__(kPatchMax) patch_invert_kernel(int pp, const int* __restrict__ pidx,
+                                                                const int* __restrict__ pturn,
+                                                                const double* __restrict__ Pm,
+                                                                const double* __restrict__ shift, double* __restrict__ Pinv,
+                                                                double* __restrict__ h1, double* __restrict__ sw) {
+  __shared__ double A[kPatchMax][kPatchMax + 1];
+  __shared__ double part[kPatchMax / 32];
+  const int pch = blockIdx.x, t = threadIdx.x;
+  const bool act = t < pp;
+  const int i = act ? pidx[pch * pp + t] : 0;
+  if (act) {
+    const double* row = Pm + (static_cast<size_t>(pch) * pp + t) * pp;
+    for (int u = 0; u < pp; ++u) A[t][u] = row[u];
+    A[t][t] += shift[i];
+  }
+  __syncthreads();
+  for (int k = 0; k < pp; ++k) {
+    const double piv = 1.0 / A[k][k];
+    const double f = act ? A[t][k] : 0.0;
+    __syncthreads();
+    if (t == k) {
+      for (int u = 0; u < pp; ++u) A[k][u] *= piv;
+      A[k][k] = piv;
+    }
+    __syncthreads();
+    if (act && t != k) {
+      for (int u = 0; u < pp; ++u) A[t][u] = (u == k) ? -f * A[k][k] : fma(-f, A[k][u], A[t][u]);
+    }
+    __syncthreads();
+  }
+  double hs = 0.0;
+  if (act) {
+    double* row = Pinv + (static_cast<size_t>(pch) * pp + t) * pp;
+    for (int u = 0; u < pp; ++u) {
+      // symmetrised on the way out (the elimination leaves rounding-level asymmetry)
+      const double v = 0.5 * (A[t][u] + A[u][t]);
+      row[u] = v;
+      hs += v;
+    }
+    h1[i] = hs;
+  }
+  hs = warp_sum(hs);
+  if ((t & 31) == 0) part[t >> 5] = hs;
+  __syncthreads();
+  if (t == 0) {
+    double s = 0.0;
+    for (int k = 0; k < (pp + 31) / 32; ++k) s += part[k];
+    atomicAdd(sw + pturn[pch], s);
+  }
+}
+
+// t = Pinv r over one patch; parks t in g and adds sum t to tw[turn].  UPDATE: first x += alpha p, r += alpha q
+// (the fused CG iteration's update); else r is taken as it is (start of the solve).
+template <bool UPDATE>
+__global__ void __launch_bounds__(kPatchMax) patch_apply_kernel(int pp, const int* __restrict__ pidx,
+                                                               const int* __restrict__ pturn,
+                                                               const double* __restrict__ Pinv, CgIter it, Scalars* sc) {
+  __shared__ double rs[kPatchMax];
+  __shared__ double part[kPatchMax / 32];
+  if (UPDATE && sc->done) return;
+  double alpha = 0.0;
+  if (UPDATE) {
+    const double pq = sc->pq[it.par];
+    if (!(pq > 0.0)) {   // breakdown: every thread sees the same pq and leaves the state alone
+      if (blockIdx.x == 0 && threadIdx.x == 0) sc->done = 2;
+      return;
+    }
+    alpha = sc->rg[it.par] / pq;
+  }
+  const int pch = blockIdx.x, t = threadIdx.x;
+  const bool act = t < pp;
+  const int i = act ? pidx[pch * pp + t] : 0;
+  if (act) {
+    double ri = it.r[i];
+    if (UPDATE) {
+      it.x[i] = fma(alpha, it.p[i], it.x[i]);
+      ri = fma(alpha, it.q[i], ri);
+      it.r[i] = ri;
+    }
+    rs[t] = ri;
+  }
+  __syncthreads();
+  double acc = 0.0;
+  if (act) {
+    const double* col = Pinv + static_cast<size_t>(pch) * pp * pp + t;   // column t = row t (symmetric): coalesced
+    for (int u = 0; u < pp; ++u) acc = fma(col[static_cast<size_t>(u) * pp], rs[u], acc);
+    it.g[i] = acc;
+  }
+  acc = warp_sum(acc);
+  if ((t & 31) == 0) part[t >> 5] = acc;
+  __syncthreads();
+  if (t == 0) {
+    double s = 0.0;
+    for (int k = 0; k < (pp + 31) / 32; ++k) s += part[k];
+    atomicAdd(it.tw + pturn[pch], s);
+  }
+}
+
+// r -= v_w ; g = t - v_w h1 ; rg[slot] += r.g ; FIRST: p = -g (start of the solve)
+template <bool FIRST>
+__global__ void patch_project_kernel(int n, CgIter it, const int* __restrict__ turn, const double* __restrict__ h1,
+                                     Scalars* sc) {
+  if (!FIRST && sc->done) return;
+  double acc = 0.0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const int w = turn[i];
+    const double v = it.tw[w] / it.sw[w];
+    const double ri = it.r[i] - v;
+    const double gi = fma(-v, h1[i], it.g[i]);
+    it.r[i] = ri;
+    it.g[i] = gi;
+    if (FIRST) it.p[i] = -gi;
+    acc = fma(ri, gi, acc);
+  }
+  block_atomic_sum(acc, &sc->rg[FIRST ? 0 : it.par ^ 1]);
+}
+// vsum += tw/sw ; tw = 0  (the multipliers of the start projection; later ones are booked by the direction kernel)
+__global__ void turn_book_kernel(int n_turns, double* __restrict__ tw, const double* __restrict__ sw,
+                                 double* __restrict__ vsum) {
+  for (int w = blockIdx.x * blockDim.x + threadIdx.x; w < n_turns; w += gridDim.x * blockDim.x) {
+    vsum[w] += tw[w] / sw[w];
+    tw[w] = 0.0;
+  }
+}
+
 // ---- fused CG iteration ---------------------------------------------------------------------------------------------
 __global__ void cg_begin_kernel(Scalars* sc, double thresh2) {
   sc->done = 0;
@@ -524,10 +678,38 @@ void k_cg_Ap(const VecCtx& v, const CgIter& it) {
 }
 void k_cg_update(const VecCtx& v, const CgIter& it) {
   QS_LAUNCH(v);
+  if (it.patch.pp > 0) {   // patch preconditioner: update fused with t = Pinv r
+    patch_apply_kernel<true><<<it.patch.n_patches, kPatchMax, 0, v.stream>>>(it.patch.pp, it.patch.pidx, it.patch.pturn,
+                                                                           it.patch.Pinv, it, v.sc);
+    return;
+  }
   cg_update_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.n_turns ? v.turn_id : nullptr, v.sc);
+}
+void k_patch_build(const VecCtx& v, const PatchPrec& pc, const double* r, const double* z, double soft_all,
+                   double soft_self) {
+  QS_LAUNCH(v);
+  patch_build_kernel<<<pc.n_patches, kPatchMax, 0, v.stream>>>(pc.pp, pc.pidx, r, z, soft_all, soft_self, pc.Pm);
+}
+// start of a solve in patch mode: Pinv for this shift, then the block projection of the current (refined) residual
+void k_patch_start(const VecCtx& v, const CgIter& it, const double* shift) {
+  const PatchPrec& pc = it.patch;
+  cudaMemsetAsync(pc.sw, 0, sizeof(double) * v.n_turns, v.stream);
+  cudaMemsetAsync(&v.sc->rg[0], 0, sizeof(double), v.stream);
+  QS_LAUNCH(v);
+  patch_invert_kernel<<<pc.n_patches, kPatchMax, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pm, shift, pc.Pinv, pc.h1, pc.sw);
+  QS_LAUNCH(v);
+  patch_apply_kernel<false><<<pc.n_patches, kPatchMax, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pinv, it, v.sc);
+  QS_LAUNCH(v);
+  patch_project_kernel<true><<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.turn_id, pc.h1, v.sc);
+  QS_LAUNCH(v);
+  turn_book_kernel<<<(v.n_turns + kBlock - 1) / kBlock, kBlock, 0, v.stream>>>(v.n_turns, it.tw, it.sw, it.vsum);
 }
 void k_cg_project(const VecCtx& v, const CgIter& it) {
   QS_LAUNCH(v);
+  if (it.patch.pp > 0) {
+    patch_project_kernel<false><<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.turn_id, it.patch.h1, v.sc);
+    return;
+  }
   if (it.Lblk) {   // block-Jacobi preconditioner (unconstrained solves): g = B^-1 r, rg[par^1] += r.g
     launch_blockprec_apply(it.nb, v.N, it.Lblk, it.r, it.g, &v.sc->rg[it.par ^ 1], &v.sc->done, v.stream);
     return;

@@ -270,8 +270,8 @@ def test_handle_works_while_another_device_or_stream_context_is_current(pkg):
             got = sim.read()
         for _ in range(3):
             ref.step(w.dt, w.I_ramp)
-        for u, v in zip(got, ref.read()):
-            assert np.array_equal(u, v)
+        for u, v in zip(got, ref.read()):                      # (FP64 atomics: equal up to summation order)
+            assert rel(u, v) <= 1e-12 or np.linalg.norm(v) < 1e-30
 
 
 @pytest.mark.parametrize("cfg,rows", [(2, 256), (3, 128)])

@@ -61,7 +61,7 @@ def parse_args():
     ap.add_argument("--no-extras", action="store_true", help="skip the HBM-roofline leg, cfg4 operator leg and cpu_baseline")
     ap.add_argument("--operator", default="pairs", choices=["pairs", "tables"],
                     help="pairs: on-the-fly AGM pair sweeps (north_star, default); tables: lattice-aware operator (f1)")
-    ap.add_argument("--leg", default="all", choices=["all", "hbm", "operator"],
+    ap.add_argument("--leg", default="all", choices=["all", "hbm", "hbm_blocked", "operator"],
                     help="hbm / operator: run only that extra leg and print its JSON (used for the ncu captures)")
     ap.add_argument("--sizes", default="4096,65536,262144,1048576", help="ring counts of the config-4 operator leg")
     ap.add_argument("--cg-budget-s", type=float, default=45.0,
@@ -311,7 +311,7 @@ def pinned(torch, n):
     return torch.empty(n, dtype=torch.float64).pin_memory().numpy()
 
 
-def hbm_roofline_leg(torch, pkg, hbm_peak):
+def hbm_roofline_leg(torch, pkg, hbm_peak, blocked=False):
     """K5 / K6 on a lattice whose arrays exceed L2 (4096 x 4096 cells = 134 MB per array), no pair operator."""
     w = wl.lattice_workload("hbm_4096x4096", 64, 64, 64, 1.0e-3, 30e-3, 1e-4, 0.0, 1, 77, 0.01)
     N = w.geometry.n_rings
@@ -332,6 +332,22 @@ def hbm_roofline_leg(torch, pkg, hbm_peak):
         pr = sim.profile_read()
     ms_mat = pr["material"][0] / max(pr["material"][1], 1)
     ms_heat = pr["heat"][0] / max(pr["heat"][1], 1)
+    if blocked:   # ncu capture of the temporally blocked kernel on this HBM-resident lattice (not its production size)
+        mat = w.material
+        alpha0 = mat.k_in / (mat.C3 * w.geometry.T_bath ** 2 + mat.C1)
+        dt4 = 3.5 * 0.8 * w.geometry.h ** 2 / (4.0 * alpha0)           # m = 4 sub-steps per call = one launch
+        with pkg.QS(w.geometry, w.material, no_operator=True, heat_blocked=True) as sim:
+            sim.write(J=np.zeros(N), T=4.2 + g.random(N))
+            sim.set_fields(Q=1e3 * g.random(N))
+            sim.profile_enable(True)
+            m4 = sim.heat(dt4)
+            for _ in range(10):
+                sim.heat(dt4)
+            pr4 = sim.profile_read()
+        ms4 = pr4["heat"][0] / max(pr4["heat"][1], 1)
+        out["heat_K6_blocked_forced"] = {"substeps_per_launch": int(m4), "ms": ms4, "ms_per_substep": ms4 / max(m4, 1),
+                                         "note": "forced (QS_GEO_HEAT_BLOCKED): above 2 M cells the library runs one "
+                                                 "marching kernel per sub-step instead"}
     # algorithmic bytes per cell: K5 reads J, T, Br, Bz, jc0_scale (40) and
     # writes E, dE/dJ, Q, b (32) = 72; K6 reads H, Q and writes H = 24 per sub-step
     for name, ms, bpc in (("material_K5", ms_mat, 72.0), ("heat_K6", ms_heat, 24.0)):
@@ -447,7 +463,7 @@ def gpu_arm(args):
     hbm_peak, hbm_src = load_measured_peaks()
     fp64_tf, fp64_mhz = pkg.fp64_peak()
     if args.leg != "all":
-        leg = (hbm_roofline_leg(torch, pkg, hbm_peak) if args.leg == "hbm"
+        leg = (hbm_roofline_leg(torch, pkg, hbm_peak, blocked=args.leg == "hbm_blocked") if args.leg.startswith("hbm")
                else operator_leg(torch, pkg, fp64_tf, args.sizes, args.cg_budget_s))
         print(json.dumps({"leg": args.leg, **leg}), flush=True)
         return

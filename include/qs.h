@@ -71,6 +71,11 @@ typedef struct qs_ctx qs_ctx;
                                     projected CG (2 x 8 N p^2 bytes of workspace); the solver then keeps diag(A) (C8).
                                     The preconditioner is free: the solution of a step is unique (C4).  */
 
+#define QS_GEO_HEAT_BLOCKED 8     /* measurement: use the temporally blocked heat kernel (<= 4 explicit sub-steps per
+                                    launch from a shared-memory tile with a 4-cell halo) at ANY lattice size; by
+                                    default it serves lattices up to 2 M cells (L2-resident), larger ones run one
+                                    marching kernel per sub-step.  Same arithmetic per cell either way (C9).  */
+
 typedef struct {
   int32_t  n_rings;                 /* N                                                         */
   const double *r, *z, *area;       /* [N] ring centre radius, height, cross-section [m, m, m^2] */

@@ -175,6 +175,7 @@ struct qs_ctx {
     double sub = 0.0;
     cudaGraphExec_t exec = nullptr;
   } heat_graph[2];
+  bool heat_force_blocked = false;   // QS_GEO_HEAT_BLOCKED: temporally blocked heat kernel at any lattice size (measurement)
   bool canonical_turns = false;      // turn_id[c] == (ir / n) * turns_per_layer + iz / n for every cell
   bool aux_on = false;               // qs_material_eval also writes dE/dJ (after the first qs_read_aux)
   double last_eval_dt = 0.0;
@@ -381,7 +382,7 @@ int do_sweep(qs_ctx* c, const double* x, const double* cur, bool field, bool pre
   prm.minsep2 = c->minsep2;
   prm.diag_d2 = c->diag_d2;
   const int wpc = sweep_warps_per_cta();
-  int grid = sweep_grid(c->sm_count, field);
+  int grid = sweep_grid(c->sm_count, field, c->nb);
   const long long need = (prm.n_items + wpc - 1) / wpc;
   if (need < grid) grid = static_cast<int>(need);
   const long long warps = static_cast<long long>(grid) * wpc;
@@ -396,6 +397,7 @@ int do_sweep(qs_ctx* c, const double* x, const double* cur, bool field, bool pre
 }
 
 constexpr double kCM = 0.5 * kMu0 * kPi;   // yacc -> henry * ampere
+constexpr long long kHeatBlockedMaxCells = 2000000;   // H, Q, H' of 2 M cells = 48 MB: well inside the 126 MB L2
 
 // Projected CG (C8) on A = M + diag(shift), constraint C^T x = const kept by the projection.
 // In: x satisfies the constraint; if yacc_has_Mx the accumulators hold the sweep of x.  nu < 0: nu = start norm.
@@ -537,7 +539,7 @@ int cg_core(qs_ctx* c, const Rhs& b, double* x, const double* shift, const doubl
     batch = std::min(16, batch * 2);
   }
   const int done_it = c->h_sc->iters;
-  rg = c->h_sc->rg[done_it & 1];
+  rg = use_patch ? c->h_sc->rd[done_it & 1] : c->h_sc->rg[done_it & 1];
   *iters = done_it;
   *hit_max = c->h_sc->done != 1;
   *relres = std::sqrt(std::max(rg, 0.0)) / nu;
@@ -585,7 +587,13 @@ int run_heat(qs_ctx* c, double dt, int* m_out) {
     c->prof.end(c->stream, QS_PROF_HEAT, 1);
   } else {
     qs_ctx::HeatGraph* hg = nullptr;
-    if (!c->prof.on && m >= 4) {   // replay the m launches from a graph (captured on first use for this start buffer)
+    const int group = k_heat_block_max();   // sub-steps per temporally blocked launch
+    // Temporal blocking pays where the lattice lives in L2 (every config: <= 6.9 MB per array) and the launches are
+    // latency-bound: config 2, m = 28: 0.19 -> 0.074 ms per step.  On an HBM-resident lattice (4096 x 4096 cells) it
+    // does cut the traffic to ~28 B per cell per 4 sub-steps but is slower than four marching launches (0.364 vs
+    // 0.303 ms: 27 % halo recompute, one 1024-thread CTA per SM, FP64-bound), so those keep the marching kernel.
+    const bool blocked = m > 1 && (c->heat_force_blocked || static_cast<long long>(c->N) <= kHeatBlockedMaxCells);
+    if (blocked && !c->prof.on && m > 2 * group) {   // replay the m launches from a graph (captured on first use for this start buffer)
       for (auto& slot : c->heat_graph)
         if (slot.exec && slot.H == c->H && slot.m == m && slot.sub == sub) hg = &slot;
       if (!hg) {
@@ -598,8 +606,8 @@ int run_heat(qs_ctx* c, double dt, int* m_out) {
         cudaGraph_t gr = nullptr;
         if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed) == cudaSuccess) {
           double *a = c->H, *b = c->Halt;
-          for (int s = 0; s < m; ++s) {
-            k_heat_substep(c->v, c->mp, c->lp, a, c->Q, b, sub);
+          for (int s = 0; s < m; s += group) {
+            k_heat_block(c->v, c->mp, c->lp, std::min(group, m - s), a, c->Q, b, sub);
             std::swap(a, b);
           }
           const cudaError_t ec = cudaStreamEndCapture(c->stream, &gr);
@@ -615,17 +623,23 @@ int run_heat(qs_ctx* c, double dt, int* m_out) {
         c->launches = l0;   // capture enqueued nothing
       }
     }
+    const int n_launch = (m + group - 1) / group;
     if (hg) {
       QS_CUDA(cudaGraphLaunch(hg->exec, c->stream));
-      c->launches += m;
-      if (m & 1) std::swap(c->H, c->Halt);
-    } else {
+      c->launches += n_launch;
+      if (n_launch & 1) std::swap(c->H, c->Halt);
+    } else if (!blocked) {   // one marching TMA kernel per sub-step (24 B per cell and sub-step, no halo re-reads)
       for (int s = 0; s < m; ++s) {
         k_heat_substep(c->v, c->mp, c->lp, c->H, c->Q, c->Halt, sub);
         std::swap(c->H, c->Halt);
       }
+    } else {
+      for (int s = 0; s < m; s += group) {
+        k_heat_block(c->v, c->mp, c->lp, std::min(group, m - s), c->H, c->Q, c->Halt, sub);
+        std::swap(c->H, c->Halt);
+      }
     }
-    c->prof.end(c->stream, QS_PROF_HEAT, m);
+    c->prof.end(c->stream, QS_PROF_HEAT, blocked ? n_launch : m);
   }
   *m_out = m;
   QS_CUDA(cudaGetLastError());
@@ -856,9 +870,14 @@ int finish_step(qs_ctx* c, double dt, double I_ramp, int iters, double relres, b
   ev.ebar_prev = c->ebar_prev; ev.flags = c->flags; ev.t_first = c->t_first; ev.count = c->count;
   ev.dt = dt; ev.t_new = c->t + dt; ev.have_prev = c->have_prev_E;
   c->prof.begin(c->stream);
-  k_events(v, c->mp, ev);
-  k_step_stats(v, c->mp, c->J, c->Jold, c->H, c->Q, c->r, c->area);
-  c->prof.end(c->stream, QS_PROF_EVENTS, c->n_turns ? 2 : 1);
+  if (c->n_turns) {   // one pass: events, per-wire statistics and the step statistics
+    ev.J = c->J;
+    ev.Jold = c->Jold;
+    k_events(v, c->mp, ev);
+  } else {
+    k_step_stats(v, c->mp, c->J, c->Jold, c->H, c->Q, c->r, c->area);
+  }
+  c->prof.end(c->stream, QS_PROF_EVENTS, 1);
   if ((rc = sync_scalars(c)) != QS_OK) {
     restore_state(c);
     return rc;
@@ -933,6 +952,7 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
   c->lattice = geo->lattice != 0;
   c->has_operator = !(geo->flags & QS_GEO_NO_OPERATOR);
   c->tables = c->lattice && c->has_operator && (geo->flags & QS_GEO_LATTICE_TABLES);
+  c->heat_force_blocked = (geo->flags & QS_GEO_HEAT_BLOCKED) != 0;
   c->blockprec = !c->lattice && c->has_operator && geo->n_turns == 0;
   {
     const int ps = patch_side(geo);

@@ -28,7 +28,7 @@ struct SweepParams {
   double minsep2;         // lower bound on the squared centre distance of two distinct rings
   double diag_d2;         // smallest B2 inside a diagonal item (self pair included)
 };
-int sweep_grid(int sm_count, bool field);
+int sweep_grid(int sm_count, bool field, int nb);
 long long sweep_items(int nb, bool field);   // multi-target + triangle items covering every unordered block pair once
 int sweep_warps_per_cta();
 cudaError_t launch_sweep(const SweepParams& prm, bool field, int grid, cudaStream_t stream);
@@ -78,6 +78,8 @@ struct Scalars {
   int iters;             // fused CG: completed iterations
   unsigned int blocks_done;   // last-block-done counter of the direction kernel
   int pad;
+  double rd[2];          // patch-preconditioned solves: r^T diag(A)^-1 r, double buffered like rg - the quantity the
+                         // stopping rule tests, so that it is the same rule whatever the preconditioner
 };
 
 struct VecCtx {
@@ -252,6 +254,10 @@ void k_heat_substep(const VecCtx& v, const MaterialParams& mp, const LatticePara
 bool k_heat_all_substeps(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, int m, const double* Hin,
                          const double* Q, double* Hout, double dtsub);
 // one ADI sub-step (qs_adi.cu, C15); scratch: six arrays of N doubles; returns the number of launches
+// temporally blocked explicit heat sub-steps: msub <= k_heat_block_max() sub-steps of length dtsub in one launch
+int k_heat_block_max();
+void k_heat_block(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, int msub, const double* Hin,
+                  const double* Q, double* Hout, double dtsub);
 // opt-in shared-memory sizes of the heat kernels on the CURRENT device (cudaFuncSetAttribute is per device): called by
 // every qs_init with the handle's device current
 void pointwise_prepare_device();
@@ -261,6 +267,8 @@ struct EventArgs {
   const double *H, *E;
   const unsigned long long *xmax_bits, *rmin_bits;   // per turn, from the material pass
   const double *Q, *r, *area;   // Joule power density, ring radius and cross-section per cell (per-wire statistics)
+  const double *J = nullptr, *Jold = nullptr;   // non-null: the step statistics (max |dJ|, Tmax, Joule power, NaN/Inf check)
+                                                // are taken in this pass too and k_step_stats is not launched
   double* wire;          // [9][n_turns]: E_joule, Q_FJ, P_max, T_max, t_q, T_q, P_q, Q_q, E_at_first (f3)
   double* ebar_prev;     // [n_turns]
   int* flags;            // [n_turns]

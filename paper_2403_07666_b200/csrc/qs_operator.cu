@@ -61,15 +61,18 @@ __device__ __constant__ double kClassKp2Min[kNumClasses] = {0.3965,   0.1394,   
                                // T=2 at 7 CTAs (72 regs) 108.6 ms, at 6 CTAs 110.1 ms; T=3 at 5 CTAs 107.7 ms;
                                // T=4 at 5 CTAs (96 regs, spills) 107.7 ms, at 4 CTAs (128 regs) 105.0 ms
 #endif
+#ifndef QS_SW_MINB_M12
+#define QS_SW_MINB_M12 7       // M-only sweep at T = 1, 2: 28 warps at 72 registers
+#endif
 #ifndef QS_SW_UNROLL
 #define QS_SW_UNROLL 2         // source steps unrolled in the off-diagonal item loop (1: +3 %, 4: +17 % on K2)
 #endif
 constexpr int kSweepUnroll = QS_SW_UNROLL;
-#ifndef QS_SW_T_FIELD
-#define QS_SW_T_FIELD 2        // target blocks per multi-target item of the fused sweep (32 T targets x 32 sources)
+#ifndef QS_SW_NB_T2
+#define QS_SW_NB_T2 1024       // blocks of 32 rings from which items hold T = 2 target blocks (both sweeps)
 #endif
-#ifndef QS_SW_T_M
-#define QS_SW_T_M 4            // the same for the M-only sweep
+#ifndef QS_SW_NB_T4
+#define QS_SW_NB_T4 4096       // ... and T = 4 (M-only sweep)
 #endif
 #ifndef QS_SW_MULTI_UNROLL
 #define QS_SW_MULTI_UNROLL 1   // source steps unrolled in the multi-target loop (each step already holds T pair chains)
@@ -318,8 +321,11 @@ struct WorkList {
   }
 };
 
+// resident CTAs per SM the register budget is sized for (measured, see QS_SW_MINB_*): fused 5 (96 registers);
+// M-only 7 at T <= 2 (72 registers), 4 at T = 4 (128 registers)
+constexpr int sweep_minb(bool field, int T) { return field ? QS_SW_MINB_FIELD : (T >= 4 ? QS_SW_MINB_M : QS_SW_MINB_M12); }
 template <bool FIELD, int T>
-__global__ void __launch_bounds__(kThreads, FIELD ? QS_SW_MINB_FIELD : QS_SW_MINB_M) sweep_kernel(SweepParams prm) {
+__global__ void __launch_bounds__(kThreads, sweep_minb(FIELD, T)) sweep_kernel(SweepParams prm) {
   constexpr int NA = FIELD ? 4 : 3;
   __shared__ __align__(128) double sbuf[kWarpsPerCta][2][kMaxArrays][64];   // every array twice: no wrap of lane + s
   __shared__ __align__(8) uint64_t sbar[kWarpsPerCta][2];
@@ -732,17 +738,43 @@ cudaError_t issue_probe(int mode, double* cycles_per_dfma) {
   return cudaSuccess;
 }
 
-int sweep_grid(int sm_count, bool field) { return sm_count * (field ? QS_SW_MINB_FIELD : QS_SW_MINB_M); }
+
+// Target blocks per multi-target item, by problem size: small ring sets have too few items for big ones, large ones
+// gain from the shared source loads and shuffles.  Measured, T = 1 / 2 / 4 (ms): matvec on free
+// rings N = 4,096: 0.054 / 0.060 / 0.070; 16,384: 0.500 / 0.498 / 0.637; 65,536: 7.32 / 7.16 / 7.43; 262,144: 112.2 /
+// 106.9 / 104.1; lattice matvec config 0: 0.024 / 0.032 / 0.040, config 1: 0.058 / 0.064 / 0.069, N = 34,560:
+// 2.38 / 2.28 / 3.04; fused sweep config 0: 0.019 / 0.029, config 1: 0.065 / 0.066.  QS_SW_T_FORCE_* pin the choice.
+int sweep_T(int nb, bool field) {
+#ifdef QS_SW_T_FORCE_FIELD
+  if (field) return QS_SW_T_FORCE_FIELD;
+#endif
+#ifdef QS_SW_T_FORCE_M
+  if (!field) return QS_SW_T_FORCE_M;
+#endif
+  if (field) return nb >= QS_SW_NB_T2 ? 2 : 1;
+  return nb >= QS_SW_NB_T4 ? 4 : (nb >= QS_SW_NB_T2 ? 2 : 1);
+}
+
+int sweep_grid(int sm_count, bool field, int nb) { return sm_count * sweep_minb(field, sweep_T(nb, field)); }
 
 long long sweep_items(int nb, bool field) {
-  return field ? WorkList<QS_SW_T_FIELD>(nb).total() : WorkList<QS_SW_T_M>(nb).total();
+  switch (sweep_T(nb, field)) {
+    case 1: return WorkList<1>(nb).total();
+    case 2: return WorkList<2>(nb).total();
+    default: return WorkList<4>(nb).total();
+  }
 }
 
 cudaError_t launch_sweep(const SweepParams& prm, bool field, int grid, cudaStream_t stream) {
-  if (field)
-    sweep_kernel<true, QS_SW_T_FIELD><<<grid, kThreads, 0, stream>>>(prm);
-  else
-    sweep_kernel<false, QS_SW_T_M><<<grid, kThreads, 0, stream>>>(prm);
+  const int T = sweep_T(prm.nb, field);
+  if (field) {
+    if (T == 1) sweep_kernel<true, 1><<<grid, kThreads, 0, stream>>>(prm);
+    else sweep_kernel<true, 2><<<grid, kThreads, 0, stream>>>(prm);
+  } else {
+    if (T == 1) sweep_kernel<false, 1><<<grid, kThreads, 0, stream>>>(prm);
+    else if (T == 2) sweep_kernel<false, 2><<<grid, kThreads, 0, stream>>>(prm);
+    else sweep_kernel<false, 4><<<grid, kThreads, 0, stream>>>(prm);
+  }
   return cudaGetLastError();
 }
 

@@ -588,27 +588,149 @@ __global__ void __launch_bounds__(kHeatSmallThreads, 1) heat_small_kernel(Materi
   }
 }
 
+// ---- K6, temporally blocked variant: up to kHbHalo sub-steps per launch.  A CTA owns a TILE x TILE block of cells,
+// loads it with a halo of kHbHalo cells on every side (H, Q once from HBM / L2), keeps H and Q of its cells in
+// registers and T^2 of the region in shared memory (two buffers, one barrier per sub-step), advances the WHOLE region
+// msub <= kHbHalo sub-steps - the error of the missing outer neighbours moves inward one cell per sub-step and never
+// reaches the tile - and writes the tile.  Per step of m sub-steps the enthalpy and the source cross HBM m/4 times
+// instead of m times (the algorithmic minimum becomes 24 B per cell per launch group).
+constexpr int kHbHalo = 4;
+template <int TILE, int THREADS>
+__global__ void __launch_bounds__(THREADS) heat_block_kernel(MaterialParams mp, LatticeParams lp, int msub,
+                                                             const double* __restrict__ Hin, const double* __restrict__ Q,
+                                                             double* __restrict__ Hout, double dtsub) {
+  constexpr int W = TILE + 2 * kHbHalo, NC = W * W, PER = (NC + THREADS - 1) / THREADS;
+  extern __shared__ __align__(16) double hb_smem[];
+  double* U0 = hb_smem;                 // [NC] T^2, ping
+  double* U1 = U0 + NC;                 // [NC] pong
+  double* crp = U1 + NC;                // [W] x 3 row coefficients, [W] x 3 column coefficients (0 outside the pack)
+  double* crm = crp + W;
+  double* crb = crm + W;
+  double* czp = crb + W;
+  double* czm = czp + W;
+  double* czb = czm + W;
+  const int Nr = lp.Nr, Nz = lp.Nz;
+  const int r0 = blockIdx.y * TILE - kHbHalo, c0 = blockIdx.x * TILE - kHbHalo;
+  for (int i = threadIdx.x; i < W; i += THREADS) {
+    const int gr = r0 + i, gc = c0 + i;
+    const bool rin = gr >= 0 && gr < Nr, cin = gc >= 0 && gc < Nz;
+    crp[i] = rin ? lp.hr_p[gr] : 0.0, crm[i] = rin ? lp.hr_m[gr] : 0.0, crb[i] = rin ? lp.rb_r[gr] : 0.0;
+    czp[i] = cin ? lp.hz_p[gc] : 0.0, czm[i] = cin ? lp.hz_m[gc] : 0.0, czb[i] = cin ? lp.rb_z[gc] : 0.0;
+  }
+  const double C3 = mp.C3, qC1sq = 0.25 * mp.C1 * mp.C1, hC1 = 0.5 * mp.C1, inv_hC3 = 2.0 / mp.C3;
+  double H[PER], q[PER];
+#pragma unroll
+  for (int k = 0; k < PER; ++k) {
+    const int idx = threadIdx.x + k * THREADS;
+    H[k] = q[k] = 0.0;
+    if (idx < NC) {
+      const int row = idx / W, col = idx - row * W;
+      const int gr = r0 + row, gc = c0 + col;
+      if (gr >= 0 && gr < Nr && gc >= 0 && gc < Nz) {
+        const long long g = static_cast<long long>(gr) * Nz + gc;
+        H[k] = Hin[g];
+        q[k] = Q[g];
+      }
+      U0[idx] = tsq_fast(H[k], C3, qC1sq, hC1, inv_hC3);
+    }
+  }
+  __syncthreads();
+  for (int s = 0; s < msub; ++s) {
+    const double* Uc = (s & 1) ? U1 : U0;
+    double* Un = (s & 1) ? U0 : U1;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+      const int idx = threadIdx.x + k * THREADS;
+      if (idx < NC) {
+        const int row = idx / W, col = idx - row * W;
+        const double u = Uc[idx];
+        // neighbours outside the region: the cell itself (pack borders have coefficient 0; region borders are halo)
+        const double un = row + 1 < W ? Uc[idx + W] : u, up = row > 0 ? Uc[idx - W] : u;
+        const double ur = col + 1 < W ? Uc[idx + 1] : u, ul = col > 0 ? Uc[idx - 1] : u;
+        double a = fma(crp[row], un - u, q[k]);
+        a = fma(crm[row], up - u, a);
+        a = fma(czp[col], ur - u, a);
+        a = fma(czm[col], ul - u, a);
+        const double rb = crb[row] + czb[col];
+        // (u > 0: region cells outside the pack hold T^2 = 0 up to rounding and must stay finite - a NaN there would
+        // reach the pack through 0 * NaN)
+        if (rb != 0.0 && u > 0.0) a = fma(-rb, sqrt_fast(u) - lp.T_bath, a);
+        H[k] = fma(dtsub, a, H[k]);
+        if (s + 1 < msub) Un[idx] = tsq_fast(H[k], C3, qC1sq, hC1, inv_hC3);
+      }
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int k = 0; k < PER; ++k) {
+    const int idx = threadIdx.x + k * THREADS;
+    if (idx < NC) {
+      const int row = idx / W, col = idx - row * W;
+      const int gr = r0 + row, gc = c0 + col;
+      if (row >= kHbHalo && row < kHbHalo + TILE && col >= kHbHalo && col < kHbHalo + TILE && gr < Nr && gc < Nz)
+        Hout[static_cast<long long>(gr) * Nz + gc] = H[k];
+    }
+  }
+}
+constexpr size_t heat_block_smem(int tile) {
+  return sizeof(double) * (2 * static_cast<size_t>(tile + 2 * kHbHalo) * (tile + 2 * kHbHalo) + 6 * (tile + 2 * kHbHalo));
+}
+
 // ---- K7 ---------------------------------------------------------------------------------------------------
-__global__ void events_kernel(int n_turns, const int* __restrict__ ptr, const int* __restrict__ idx,
-                              MaterialParams mp, EventArgs e, Scalars* sc) {
-  const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-  if (w >= n_turns) return;
-  double tsq = 0.0, esum = 0.0, qv = 0.0, pmax = 0.0;
-  for (int k = ptr[w] + lane; k < ptr[w + 1]; k += 32) {
+// One CTA per constraint group (32 .. 256 threads: the power of two next to the group's cell count).
+constexpr int kEventBlockMax = 256;
+__global__ void __launch_bounds__(kEventBlockMax) events_kernel(int n_turns, const int* __restrict__ ptr,
+                                                                const int* __restrict__ idx, MaterialParams mp,
+                                                                EventArgs e, Scalars* sc) {
+  __shared__ double red[5][kEventBlockMax / 32];
+  __shared__ int redbad[kEventBlockMax / 32];
+  const int w = blockIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  double tsq = 0.0, esum = 0.0, qv = 0.0, pmax = 0.0, dj = 0.0;
+  int bad = 0;
+  for (int k = ptr[w] + threadIdx.x; k < ptr[w + 1]; k += blockDim.x) {
     const int i = idx[k];
-    tsq = fmax(tsq, tsq_of_H(e.H[i], mp.C3, mp.C1));
+    const double t2 = tsq_of_H(e.H[i], mp.C3, mp.C1);
+    tsq = fmax(tsq, t2);
     esum += fabs(e.E[i]);
     const double q = e.Q[i];
     qv = fma(q, 2.0 * kPi * e.r[i] * e.area[i], qv);       // Joule power of the wire [W]
     pmax = fmax(pmax, q);
+    if (e.J) {   // step statistics folded into this pass (every cell belongs to one group)
+      const double Ji = e.J[i];
+      dj = fmax(dj, fabs(Ji - e.Jold[i]));
+      if (!isfinite(Ji) || !isfinite(t2) || !(t2 > 0.0)) bad = 1;
+    }
   }
   tsq = warp_max(tsq);
   esum = warp_sum(esum);
   qv = warp_sum(qv);
   pmax = warp_max(pmax);
+  dj = warp_max(dj);
+  bad = __any_sync(0xffffffffu, bad);
+  if (nw > 1) {   // combine the warps of the CTA
+    if (lane == 0) red[0][wid] = tsq, red[1][wid] = esum, red[2][wid] = qv, red[3][wid] = pmax, red[4][wid] = dj, redbad[wid] = bad;
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    for (int k = 1; k < nw; ++k) {
+      tsq = fmax(tsq, red[0][k]);
+      esum += red[1][k];
+      qv += red[2][k];
+      pmax = fmax(pmax, red[3][k]);
+      dj = fmax(dj, red[4][k]);
+      bad |= redbad[k];
+    }
+  }
+  if (e.J) {
+    if (threadIdx.x == 0) {
+      if (dj > 0.0 && isfinite(dj)) atomic_max_pos(&sc->djmax, dj);
+      if (tsq > 0.0 && isfinite(tsq)) atomic_max_pos(&sc->tmax, sqrt(tsq));
+      atomicAdd(&sc->joule, qv);
+      if (bad) atomicOr(&sc->nonfinite, 1);
+    }
+  }
   const double xmax = __longlong_as_double(static_cast<long long>(e.xmax_bits[w]));
   const double rmin = __longlong_as_double(static_cast<long long>(e.rmin_bits[w])) / mp.rho_n;
-  if (lane != 0) return;
+  if (threadIdx.x != 0) return;
   const double Tmax = sqrt(tsq);
   const double ebar = esum / static_cast<double>(ptr[w + 1] - ptr[w]);
   int fl = 0;
@@ -748,14 +870,32 @@ bool k_heat_all_substeps(const VecCtx& v, const MaterialParams& mp, const Lattic
                                                                                                  dtsub);
   return true;
 }
+int k_heat_block_max() { return kHbHalo; }
+// msub <= kHbHalo sub-steps in one launch (lattices too large for the in-SM kernel)
+void k_heat_block(const VecCtx& v, const MaterialParams& mp, const LatticeParams& lp, int msub, const double* Hin,
+                  const double* Q, double* Hout, double dtsub) {
+  QS_LAUNCH(v);
+  const long long tiles64 = static_cast<long long>((lp.Nr + 63) / 64) * ((lp.Nz + 63) / 64);
+  if (tiles64 >= 4ll * g_sm_count) {   // big lattices: 64 x 64 tiles (halo overhead 27 %), two CTAs per SM
+    dim3 grid((lp.Nz + 63) / 64, (lp.Nr + 63) / 64);
+    heat_block_kernel<64, 1024><<<grid, 1024, heat_block_smem(64), v.stream>>>(mp, lp, msub, Hin, Q, Hout, dtsub);
+  } else {                             // the coil configs: 32 x 32 tiles so that every SM has work
+    dim3 grid((lp.Nz + 31) / 32, (lp.Nr + 31) / 32);
+    heat_block_kernel<32, 256><<<grid, 256, heat_block_smem(32), v.stream>>>(mp, lp, msub, Hin, Q, Hout, dtsub);
+  }
+}
 void pointwise_prepare_device() {
+  cudaFuncSetAttribute(heat_block_kernel<64, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(heat_block_smem(64)));
+  cudaFuncSetAttribute(heat_block_kernel<32, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(heat_block_smem(32)));
   cudaFuncSetAttribute(heat_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(sizeof(HeatSmem)));
   cudaFuncSetAttribute(heat_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);   // N + 3 (Nr + Nz) doubles <= 131 KB
 }
 void k_events(const VecCtx& v, const MaterialParams& mp, const EventArgs& e) {
   if (!v.n_turns) return;
   QS_LAUNCH(v);
-  events_kernel<<<(v.n_turns * 32 + kBlock - 1) / kBlock, kBlock, 0, v.stream>>>(v.n_turns, v.turn_ptr, v.turn_idx, mp,
+  int bt = 32;
+  while (bt < (v.N + v.n_turns - 1) / v.n_turns && bt < kEventBlockMax) bt <<= 1;
+  events_kernel<<<v.n_turns, bt, 0, v.stream>>>(v.n_turns, v.turn_ptr, v.turn_idx, mp,
                                                                                 e, v.sc);
 }
 void k_step_stats(const VecCtx& v, const MaterialParams& mp, const double* J, const double* Jold, const double* H,

@@ -185,6 +185,7 @@ __global__ void mul_kernel(int n, const double* __restrict__ a, const double* __
 }
 __global__ void set_scalars_kernel(Scalars* sc) {
   sc->rg[0] = sc->rg[1] = sc->pq[0] = sc->pq[1] = sc->nu2 = 0.0;
+  sc->rd[0] = sc->rd[1] = 0.0;
   sc->done = 0;
   sc->iters = 0;
   sc->blocks_done = 0u;
@@ -259,6 +260,7 @@ __global__ void step_begin_kernel(StepBegin a, Scalars* sc) {
   }
   if (tid == 0) {
     sc->rg[0] = sc->rg[1] = sc->pq[0] = sc->pq[1] = sc->nu2 = 0.0;
+    sc->rd[0] = sc->rd[1] = 0.0;
     sc->done = 0;
     sc->iters = 0;
     sc->blocks_done = 0u;
@@ -271,30 +273,35 @@ __global__ void step_begin_kernel(StepBegin a, Scalars* sc) {
   }
 }
 
-constexpr int kTurnBlock = 128;
+constexpr int kTurnBlockMax = 1024;   // threads per constraint group: the power of two next to its cell count, 64..1024
 __device__ __forceinline__ double turn_block_sum(double v, double* sh) {   // sum over the CTA, result in every thread
   v = warp_sum(v);
   __syncthreads();
   if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
   __syncthreads();
   double s = 0.0;
-#pragma unroll
-  for (int k = 0; k < kTurnBlock / 32; ++k) s += sh[k];
+  for (int k = 0; k < static_cast<int>(blockDim.x >> 5); ++k) s += sh[k];
   return s;
+}
+inline int turn_block(const VecCtx& v) {
+  const int per = (v.N + v.n_turns - 1) / (v.n_turns > 0 ? v.n_turns : 1);
+  int b = 64;
+  while (b < per && b < kTurnBlockMax) b <<= 1;
+  return b;
 }
 
 // one CTA per constraint group: deficit_w = d share_w - sum_{i in w} x_i ; x_i += deficit_w / (H_i s_w)  (C8: moves a
 // warm start onto the constraint; H = diag(M), s_w its per-turn Schur scalar)
-__global__ void __launch_bounds__(kTurnBlock) turn_fix_kernel(const int* __restrict__ ptr, const int* __restrict__ idx,
+__global__ void __launch_bounds__(kTurnBlockMax) turn_fix_kernel(const int* __restrict__ ptr, const int* __restrict__ idx,
                                                               const double* __restrict__ share, double d,
                                                               const double* __restrict__ Hd, const double* __restrict__ sw,
                                                               double* __restrict__ x) {
-  __shared__ double sh[kTurnBlock / 32];
-  const int w = blockIdx.x, k0 = ptr[w], k1 = ptr[w + 1];
+  __shared__ double sh[kTurnBlockMax / 32];
+  const int w = blockIdx.x, k0 = ptr[w], k1 = ptr[w + 1], nt = blockDim.x;
   double acc = 0.0;
-  for (int k = k0 + threadIdx.x; k < k1; k += kTurnBlock) acc += x[idx[k]];
+  for (int k = k0 + threadIdx.x; k < k1; k += nt) acc += x[idx[k]];
   const double def = fma(d, share[w], -turn_block_sum(acc, sh)) / sw[w];
-  for (int k = k0 + threadIdx.x; k < k1; k += kTurnBlock) {
+  for (int k = k0 + threadIdx.x; k < k1; k += nt) {
     const int i = idx[k];
     x[i] += def / Hd[i];
   }
@@ -306,9 +313,9 @@ __global__ void __launch_bounds__(kTurnBlock) turn_fix_kernel(const int* __restr
 //   r2 = M x + shift x - b                (the warm start x, already on the constraint)
 // s_w = sum 1/H, v = (sum r/H)/s_w, r <- r - v, g = r/H, nu2 += r1.g1, rg[0] += r2.g2, p = -g2; the multipliers of the
 // two projections go to vnu[w] and vsum[w].
-__global__ void __launch_bounds__(kTurnBlock) turn_start_kernel(TurnStart a, Scalars* sc) {
-  __shared__ double sh[kTurnBlock / 32];
-  const int w = blockIdx.x, k0 = a.ptr[w], k1 = a.ptr[w + 1];
+__global__ void __launch_bounds__(kTurnBlockMax) turn_start_kernel(TurnStart a, Scalars* sc) {
+  __shared__ double sh[kTurnBlockMax / 32];
+  const int w = blockIdx.x, k0 = a.ptr[w], k1 = a.ptr[w + 1], kTurnBlock = blockDim.x;
   double s = 0.0, a1 = 0.0, a2 = 0.0;
   for (int k = k0 + threadIdx.x; k < k1; k += kTurnBlock) {
     const int i = a.idx[k];
@@ -385,55 +392,59 @@ __global__ void __launch_bounds__(kPatchMax) patch_build_kernel(int pp, const in
 }
 
 // per solve: Pinv = (M_patch + diag(shift))^-1 by in-place Gauss-Jordan elimination in shared memory (SPD: no pivoting),
-// h1 = Pinv 1, s_w += sum h1.  One CTA per patch, one thread per row.
-__global__ void __launch_bounds__(kPatchMax) patch_invert_kernel(int pp, const int* __restrict__ pidx,
-                                                                const int* __restrict__ pturn,
-                                                                const double* __restrict__ Pm,
-                                                                const double* __restrict__ shift, double* __restrict__ Pinv,
-                                                                double* __restrict__ h1, double* __restrict__ sw) {
+// h1 = Pinv 1, s_w += sum h1.  One CTA per patch, kPinvSplit threads per row (each owns every kPinvSplit-th column).
+constexpr int kPinvSplit = 4;
+__global__ void __launch_bounds__(kPatchMax * kPinvSplit) patch_invert_kernel(int pp, const int* __restrict__ pidx,
+                                                                              const int* __restrict__ pturn,
+                                                                              const double* __restrict__ Pm,
+                                                                              const double* __restrict__ shift,
+                                                                              double* __restrict__ Pinv, double* __restrict__ h1,
+                                                                              double* __restrict__ sw) {
   __shared__ double A[kPatchMax][kPatchMax + 1];
-  __shared__ double part[kPatchMax / 32];
-  const int pch = blockIdx.x, t = threadIdx.x;
-  const bool act = t < pp;
-  const int i = act ? pidx[pch * pp + t] : 0;
-  if (act) {
-    const double* row = Pm + (static_cast<size_t>(pch) * pp + t) * pp;
-    for (int u = 0; u < pp; ++u) A[t][u] = row[u];
-    A[t][t] += shift[i];
-  }
+  __shared__ double part[kPatchMax * kPinvSplit / 32];
+  const int pch = blockIdx.x, nthr = pp * kPinvSplit;
+  const int t = threadIdx.x / kPinvSplit, c = threadIdx.x % kPinvSplit;   // row, column phase
+  const bool act = static_cast<int>(threadIdx.x) < nthr;
+  const double* src = Pm + static_cast<size_t>(pch) * pp * pp;
+  for (int e = threadIdx.x; e < pp * pp; e += blockDim.x) A[e / pp][e % pp] = src[e];
+  __syncthreads();
+  if (threadIdx.x < pp) A[threadIdx.x][threadIdx.x] += shift[pidx[pch * pp + threadIdx.x]];
   __syncthreads();
   for (int k = 0; k < pp; ++k) {
     const double piv = 1.0 / A[k][k];
     const double f = act ? A[t][k] : 0.0;
     __syncthreads();
-    if (t == k) {
-      for (int u = 0; u < pp; ++u) A[k][u] *= piv;
-      A[k][k] = piv;
+    if (act && t == k) {
+      for (int u = c; u < pp; u += kPinvSplit) A[k][u] = (u == k) ? piv : A[k][u] * piv;
     }
     __syncthreads();
     if (act && t != k) {
-      for (int u = 0; u < pp; ++u) A[t][u] = (u == k) ? -f * A[k][k] : fma(-f, A[k][u], A[t][u]);
+      for (int u = c; u < pp; u += kPinvSplit) A[t][u] = (u == k) ? -f * piv : fma(-f, A[k][u], A[t][u]);
     }
     __syncthreads();
   }
   double hs = 0.0;
   if (act) {
     double* row = Pinv + (static_cast<size_t>(pch) * pp + t) * pp;
-    for (int u = 0; u < pp; ++u) {
+    for (int u = c; u < pp; u += kPinvSplit) {
       // symmetrised on the way out (the elimination leaves rounding-level asymmetry)
       const double v = 0.5 * (A[t][u] + A[u][t]);
       row[u] = v;
       hs += v;
     }
-    h1[i] = hs;
   }
-  hs = warp_sum(hs);
-  if ((t & 31) == 0) part[t >> 5] = hs;
+  // row sums: the kPinvSplit threads of a row are adjacent lanes
+#pragma unroll
+  for (int o = kPinvSplit / 2; o > 0; o >>= 1) hs += __shfl_xor_sync(0xffffffffu, hs, o);
+  if (act && c == 0) h1[pidx[pch * pp + t]] = hs;
+  double tot = (act && c == 0) ? hs : 0.0;
+  tot = warp_sum(tot);
+  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = tot;
   __syncthreads();
-  if (t == 0) {
-    double s = 0.0;
-    for (int k = 0; k < (pp + 31) / 32; ++k) s += part[k];
-    atomicAdd(sw + pturn[pch], s);
+  if (threadIdx.x == 0) {
+    double ssum = 0.0;
+    for (int k = 0; k < static_cast<int>(blockDim.x >> 5); ++k) ssum += part[k];
+    atomicAdd(sw + pturn[pch], ssum);
   }
 }
 
@@ -489,7 +500,7 @@ template <bool FIRST>
 __global__ void patch_project_kernel(int n, CgIter it, const int* __restrict__ turn, const double* __restrict__ h1,
                                      Scalars* sc) {
   if (!FIRST && sc->done) return;
-  double acc = 0.0;
+  double acc = 0.0, accd = 0.0;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     const int w = turn[i];
     const double v = it.tw[w] / it.sw[w];
@@ -499,8 +510,11 @@ __global__ void patch_project_kernel(int n, CgIter it, const int* __restrict__ t
     it.g[i] = gi;
     if (FIRST) it.p[i] = -gi;
     acc = fma(ri, gi, acc);
+    accd = fma(ri / it.Hd[i], ri, accd);          // the stopping rule's norm: r^T diag(A)^-1 r
   }
   block_atomic_sum(acc, &sc->rg[FIRST ? 0 : it.par ^ 1]);
+  __syncthreads();
+  block_atomic_sum(accd, &sc->rd[FIRST ? 0 : it.par ^ 1]);
 }
 // vsum += tw/sw ; tw = 0  (the multipliers of the start projection; later ones are booked by the direction kernel)
 __global__ void turn_book_kernel(int n_turns, double* __restrict__ tw, const double* __restrict__ sw,
@@ -516,6 +530,7 @@ __global__ void cg_begin_kernel(Scalars* sc, double thresh2) {
   sc->done = 0;
   sc->iters = 0;
   sc->pq[0] = sc->pq[1] = 0.0;
+  sc->rd[0] = sc->rd[1] = 0.0;
   sc->blocks_done = 0u;
   sc->thresh2 = thresh2;
 }
@@ -603,13 +618,15 @@ __global__ void cg_direction_kernel(int n, int npad, int n_turns, CgIter it, Sca
     it.tw[w] = 0.0;
   }
   if (threadIdx.x == 0) {
+    const double test = it.patch.pp > 0 ? sc->rd[it.par ^ 1] : rg_new;   // same stopping rule with either preconditioner
     sc->rg[it.par] = 0.0;
+    sc->rd[it.par] = 0.0;
     sc->pq[it.par] = 0.0;
     sc->blocks_done = 0u;
     *it.counter = 0ull;
     sc->iters += 1;
     if (!(rg_new == rg_new)) sc->done = 2;
-    else if (rg_new <= sc->thresh2) sc->done = 1;
+    else if (test <= sc->thresh2) sc->done = 1;
   }
 }
 }  // namespace
@@ -695,8 +712,9 @@ void k_patch_start(const VecCtx& v, const CgIter& it, const double* shift) {
   const PatchPrec& pc = it.patch;
   cudaMemsetAsync(pc.sw, 0, sizeof(double) * v.n_turns, v.stream);
   cudaMemsetAsync(&v.sc->rg[0], 0, sizeof(double), v.stream);
+  cudaMemsetAsync(&v.sc->rd[0], 0, 2 * sizeof(double), v.stream);
   QS_LAUNCH(v);
-  patch_invert_kernel<<<pc.n_patches, kPatchMax, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pm, shift, pc.Pinv, pc.h1, pc.sw);
+  patch_invert_kernel<<<pc.n_patches, kPatchMax * kPinvSplit, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pm, shift, pc.Pinv, pc.h1, pc.sw);
   QS_LAUNCH(v);
   patch_apply_kernel<false><<<pc.n_patches, kPatchMax, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pinv, it, v.sc);
   QS_LAUNCH(v);
@@ -728,11 +746,11 @@ void k_step_begin(const VecCtx& v, const StepBegin& a) {
 void k_turn_fix(const VecCtx& v, double d, const double* Hd, const double* sw, double* x) {
   if (!v.n_turns) return;
   QS_LAUNCH(v);
-  turn_fix_kernel<<<v.n_turns, kTurnBlock, 0, v.stream>>>(v.turn_ptr, v.turn_idx, v.share, d, Hd, sw, x);
+  turn_fix_kernel<<<v.n_turns, turn_block(v), 0, v.stream>>>(v.turn_ptr, v.turn_idx, v.share, d, Hd, sw, x);
 }
 void k_turn_start(const VecCtx& v, const TurnStart& a) {
   QS_LAUNCH(v);
-  turn_start_kernel<<<v.n_turns, kTurnBlock, 0, v.stream>>>(a, v.sc);
+  turn_start_kernel<<<v.n_turns, turn_block(v), 0, v.stream>>>(a, v.sc);
 }
 void k_step_update(const VecCtx& v, double dt, const double* x, const double* area, double* J, const double* vsum) {
   QS_LAUNCH(v);

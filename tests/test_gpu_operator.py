@@ -190,6 +190,57 @@ def test_heat_substeps_pointwise(pkg, shape):
     assert np.max(np.abs(Tg - qo.temperature(mat, Ho))) <= 1e-12 * 12.0
 
 
+@pytest.mark.parametrize("shape,msub", [((7, 9, 11), 6), ((20, 17, 8), 4), ((5, 3, 24), 9), ((9, 13, 7), 1), ((9, 13, 7), 3)])
+def test_heat_temporally_blocked_kernel(pkg, shape, msub):
+    # lattices above 4096 cells: groups of <= 4 sub-steps per launch from a shared-memory tile with a 4-cell halo.
+    # Odd sizes (tiles cut by all four pack borders), sub-step counts that are not multiples of 4 (a short last group),
+    # Robin loss on all borders, strong gradients: cell by cell against the oracle's sub-step loop.
+    L, Tn, n = shape
+    geo = wl.lattice_geometry(L, Tn, n, 1e-3, 30e-3)
+    geo = dataclasses.replace(geo, h_conv=(500.0, 300.0, 200.0, 100.0))
+    mat = wl.Material()
+    N = geo.n_rings
+    assert N > 4096
+    g = np.random.default_rng(100 + msub)
+    T = g.uniform(4.2, 12.0, N)
+    Q = g.uniform(0, 5e6, N)
+    alpha0 = mat.k_in / (mat.C3 * geo.T_bath ** 2 + mat.C1)
+    dt = (msub - 0.5) * 0.8 * geo.h ** 2 / (4.0 * alpha0)
+    assert qo.heat_substeps_count(geo, mat, dt) == msub
+    with pkg.QS(geo, mat, no_operator=True) as sim:
+        sim.write(np.zeros(N), T, 0.0, 0.0)
+        sim.set_fields(Q=Q)
+        for _ in range(3):                                       # three steps: ping-pong buffers, graph replay (msub > 8)
+            assert sim.heat(dt) == msub
+        _, Tg, _, _ = sim.read(J=False, B=False, E=False)
+    Ho = qo.enthalpy(mat, T)
+    for _ in range(3):
+        Ho, _ = qo.heat_substeps(geo, mat, Ho, Q, dt, msub)
+    assert np.max(np.abs(Tg - qo.temperature(mat, Ho))) <= 1e-12 * 12.0
+
+
+def test_heat_temporally_blocked_kernel_forced_on_a_large_lattice(pkg):
+    # 2048 x 2048 cells: above the size the library blocks by itself (QS_GEO_HEAT_BLOCKED forces it: the 64 x 64-tile
+    # variant); 4 sub-steps in one launch, and 6 (4 + 2), cell by cell against the oracle
+    geo = wl.lattice_geometry(32, 32, 64, 1e-3, 30e-3)
+    geo = dataclasses.replace(geo, h_conv=(500.0, 300.0, 200.0, 100.0))
+    mat = wl.Material()
+    N = geo.n_rings
+    g = np.random.default_rng(404)
+    T = g.uniform(4.2, 12.0, N)
+    Q = g.uniform(0, 5e6, N)
+    alpha0 = mat.k_in / (mat.C3 * geo.T_bath ** 2 + mat.C1)
+    for msub in (4, 6):
+        dt = (msub - 0.5) * 0.8 * geo.h ** 2 / (4.0 * alpha0)
+        with pkg.QS(geo, mat, no_operator=True, heat_blocked=True) as sim:
+            sim.write(np.zeros(N), T, 0.0, 0.0)
+            sim.set_fields(Q=Q)
+            assert sim.heat(dt) == msub
+            _, Tg, _, _ = sim.read(J=False, B=False, E=False)
+        Ho, _ = qo.heat_substeps(geo, mat, qo.enthalpy(mat, T), Q, dt, msub)
+        assert np.max(np.abs(Tg - qo.temperature(mat, Ho))) <= 1e-12 * 12.0
+
+
 def test_errors_and_no_operator_mode(pkg):
     geo, x = wl.free_rings(64)
     with pkg.QS(geo, wl.Material()) as sim:

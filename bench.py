@@ -43,11 +43,12 @@ FLOP_K1, FLOP_K2 = 76.0, 100.0
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9 / 1e12
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the ncu --set full captures summarised
 # under profiles/ (r01_sweep_field_cfg2.md, r01_hbm_passes.md); None where no capture of that workload exists
-NCU_TRAFFIC = {"sweep_field:cfg2_mid_solenoid_20x40x16": 11.8e6, "material_K5": 671.4e6 + 498.2e6, "heat_K6": 275.0e6 + 102.4e6}   # r01 captures
+NCU_TRAFFIC = {"sweep_field:cfg3_real_coil_60x100x12": 50.1e6 + 0.8e6,      # profiles/r02_sweep_field_cfg3.md
+               "material_K5": 671.3e6 + 498.7e6, "heat_K6": 275.2e6 + 102.3e6}  # profiles/r02_hbm_passes.md
 NCU_SOURCE = "committed ncu capture (profiles/), not a quantity of this run"
 # executed FP64 flop per launch (dadd + dmul + 2 dfma thread instructions) of the same captures: ncu counts what the
 # kernel really issues (square roots and the series tail expand to several FP64 instructions), the nominal count does not
-NCU_EXEC_FLOP = {"sweep_field:cfg2_mid_solenoid_20x40x16": (1178.569285 + 2342.123003 + 2 * 4037.256723) * 1.963764e9 * 102.601792e-3}
+NCU_EXEC_FLOP = {"sweep_field:cfg3_real_coil_60x100x12": (809.524212 + 2449.661278 + 2 * 4568.629332) * 1.963472e9 * 1.643487}
 DEFAULTS = {"cfg0": (50, 5), "cfg1": (100, 5), "cfg2": (10, 3), "cfg3": (5, 3)}
 
 
@@ -560,7 +561,7 @@ def gpu_arm(args):
     if ex is not None:   # executed flop per launch from the committed ncu capture / this run's launch time
         ex_tf = ex / (d_ms / max(d_n, 1) * 1e-3) / 1e12
         roofline["executed"] = {"achieved": ex_tf, "unit": "TFLOP/s", "frac": ex_tf / fp64_tf,
-                                "source": NCU_SOURCE + ": profiles/r01_sweep_field_cfg2.md (sass_thread_inst_executed_op_d{add,mul,fma})"}
+                                "source": NCU_SOURCE + ": profiles/r02_sweep_field_cfg3.md (sass_thread_inst_executed_op_d{add,mul,fma})"}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",

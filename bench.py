@@ -42,7 +42,7 @@ FLOP_K1, FLOP_K2 = 76.0, 100.0
 # FP64 peak derived from unit counts: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz
 FP64_PEAK_NOMINAL = 148 * 64 * 2 * 1.965e9 / 1e12
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the ncu --set full captures summarised
-# under profiles/ (r01_sweep_field_cfg2.md, r01_hbm_passes.md); None where no capture of that workload exists
+# under profiles/ (r02_sweep_field_cfg3.md, r02_hbm_passes.md); None where no capture of that workload exists
 NCU_TRAFFIC = {"sweep_field:cfg3_real_coil_60x100x12": 50.1e6 + 0.8e6,      # profiles/r02_sweep_field_cfg3.md
                "material_K5": 671.3e6 + 498.7e6, "heat_K6": 275.2e6 + 102.3e6}  # profiles/r02_hbm_passes.md
 NCU_SOURCE = "committed ncu capture (profiles/), not a quantity of this run"

@@ -195,6 +195,25 @@ int  qs_write_rate(qs_ctx *ctx, const double *Idot);
 int  qs_matvec(qs_ctx *ctx, const double *x, double *y);
 int  qs_matvec_device(qs_ctx *ctx, const double *d_x, double *d_y);
 
+/* y = M x on FREE rings (C2: dz^2 + softening^2 for all pairs; the config-4 operator) WITHOUT ANY ALLOCATION, for
+ * callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it).  No handle:
+ * the sweep's scratch memory (padded copies of r, z, x, block boxes, FP64 accumulators, work counter) is one
+ * file-scope static __device__ array of 557,312 bytes, sized for at most QS_NOALLOC_MAX_RINGS rings, which every GPU
+ * that loads the library holds until the process exits.
+ *   d_r, d_z, d_x [n_rings]: DEVICE pointers, inputs (r > 0, finite; the ring set must satisfy qs_init's validity
+ *   domain k'^2 <= 0.98 - not checked here, the data are on the device); d_y [n_rings]: DEVICE pointer, output [Wb],
+ *   may alias d_x; stream: a cudaStream_t of the CURRENT device (NULL = default stream).
+ * Enqueues three kernels on `stream` and returns without synchronising; calls no cudaMalloc / cudaFree / allocating
+ * library routine.  The first call on a device takes the array's device address (cudaGetSymbolAddress) - a call with
+ * n_rings == 0 does only that.  Rings are swept in the caller's order (no Morton re-ordering as qs_init does), so
+ * scattered sets take deeper AGM classes: same numbers, more work.
+ * SHARED STATE: every call uses the same array, which keeps the last call's contents; each call rewrites its inputs
+ * and clears the accumulators first.  Calls that overlap on the GPU (two streams, two threads) RACE: serialise them.
+ * Returns QS_OK; QS_ERR_ARG for n_rings < 0 or > QS_NOALLOC_MAX_RINGS, NULL arrays, softening <= 0; QS_ERR_CUDA.  */
+#define QS_NOALLOC_MAX_RINGS 16384
+int  qs_matvec_noalloc(int32_t n_rings, const double *d_r, const double *d_z, double softening,
+                       const double *d_x, double *d_y, void *stream);
+
 /* Br, Bz [N each, B = Br then Bz] of ring currents I [A] (C3), without B_ext; lattice only.  */
 int  qs_field(qs_ctx *ctx, const double *I, double *B);
 

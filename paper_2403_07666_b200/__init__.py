@@ -5,3 +5,4 @@ Nothing here imports the CPU oracle; without a CUDA device ``QS(...)`` raises.
 """
 from .build import build  # noqa: F401
 from .binding import QS, QsError, load_library, SYMBOLS, fp64_peak, pair_eval, issue_probe  # noqa: F401
+from .binding import matvec_noalloc, NOALLOC_MAX_RINGS  # noqa: F401

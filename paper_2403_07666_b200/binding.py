@@ -66,6 +66,7 @@ SYMBOLS = [
     ("qs_debug_inject_failure", C.c_int, [_VP, C.c_int32]),
     ("qs_matvec", C.c_int, [_VP, c_double_p, c_double_p]),
     ("qs_matvec_device", C.c_int, [_VP, _VP, _VP]),
+    ("qs_matvec_noalloc", C.c_int, [C.c_int32, _VP, _VP, C.c_double, _VP, _VP, _VP]),
     ("qs_field", C.c_int, [_VP, c_double_p, c_double_p]),
     ("qs_solve", C.c_int, [_VP, c_double_p, c_double_p, C.c_int32, c_int32_p, c_double_p]),
     ("qs_solve_device", C.c_int, [_VP, _VP, _VP, C.c_int32, c_int32_p, c_double_p]),
@@ -122,6 +123,23 @@ def _f64(a, n=None) -> np.ndarray:
     if n is not None and out.size != n:
         raise ValueError(f"expected {n} elements, got {out.size}")
     return out
+
+
+NOALLOC_MAX_RINGS = 16384
+
+
+def matvec_noalloc(r, z, softening: float, x, y, stream=None) -> None:
+    """qs_matvec_noalloc: y = M x on free rings with all scratch in the library's static device array (no allocation,
+    no handle).  r, z, x, y: float64 CUDA tensors of n elements on the current device; enqueued on `stream` (a
+    torch.cuda.Stream, default: the current stream).  Calls that overlap on the GPU race on the shared array."""
+    import torch
+    lib = load_library()
+    n = int(r.numel())
+    st = torch.cuda.current_stream() if stream is None else stream
+    rc = lib.qs_matvec_noalloc(n, _VP(r.data_ptr()), _VP(z.data_ptr()), float(softening), _VP(x.data_ptr()),
+                               _VP(y.data_ptr()), _VP(st.cuda_stream))
+    if rc < 0:
+        raise QsError(rc, lib.qs_last_error().decode())
 
 
 def fp64_peak():

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqs.so")
-SOURCES = ["qs_api.cu", "qs_operator.cu", "qs_vector.cu", "qs_pointwise.cu", "qs_lattice.cu", "qs_adi.cu"]
+SOURCES = ["qs_api.cu", "qs_operator.cu", "qs_vector.cu", "qs_pointwise.cu", "qs_lattice.cu", "qs_adi.cu", "qs_noalloc.cu"]
 HEADERS = ["qs_internal.h", "qs_pair.cuh", "qs_tma.cuh", os.path.join("..", "..", "include", "qs.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--shared", "-cudart", "static"]

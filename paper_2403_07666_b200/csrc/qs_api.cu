@@ -33,6 +33,11 @@ int fail(int code, const std::string& msg) {
   } while (0)
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+}  // namespace
+namespace qs {
+int set_error(int code, const char* msg) { return fail(code, msg); }
+}  // namespace qs
+namespace {
 
 // Carves named arrays out of one device buffer; used twice (size query with base == nullptr, then for real).
 struct Carver {

@@ -8,6 +8,9 @@ namespace qs {
 constexpr double kMu0 = 1.2566370614359172953850573533118e-6;   // 4 pi 1e-7
 constexpr double kPi = 3.1415926535897932384626433832795;
 
+// records the message qs_last_error() returns for the calling thread and hands back `code` (qs_api.cu)
+int set_error(int code, const char* msg);
+
 // ---- pair sweeps (qs_operator.cu) -------------------------------------------------------------
 struct SweepParams {
   const double* r;        // [Np] ring radius, padded to a multiple of 32

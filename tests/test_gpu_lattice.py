@@ -21,8 +21,9 @@ def pkg():
     return p
 
 
-# (layers, turns, n): Nz = turns * n covers every thread/output shape of the sweep: 8, 18 (ragged), 65 (odd), 96, 130
-@pytest.mark.parametrize("shape", [(1, 1, 8), (2, 3, 6), (2, 5, 13), (3, 4, 24), (2, 10, 13)])
+# (layers, turns, n): Nz = turns * n covers every thread/output shape of the sweeps: 8, 18 (ragged), 65 (odd), 96, and
+# for the tensor-core kernel (Nz >= 128) 130, 143 (odd: padded table rows, folded offset window) and 328 (several warps)
+@pytest.mark.parametrize("shape", [(1, 1, 8), (2, 3, 6), (2, 5, 13), (3, 4, 24), (2, 10, 13), (2, 11, 13), (1, 41, 8)])
 def test_tables_matvec_and_field_equal_the_dense_oracle(pkg, shape):
     L, Tn, n = shape
     geo = wl.lattice_geometry(L, Tn, n, 0.9e-3, 35e-3)

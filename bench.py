@@ -428,6 +428,29 @@ def cg_active_leg(torch, pkg, steps=50, warm=20):
             "gpu_launches": int(launches)}
 
 
+def nonlinear_cfg2_leg(torch, pkg, reach=150, steps=2):
+    """Config 2 beyond its linear first ~100 steps (C13): the surface cells of the wires are at Jc and every
+    step iterates the projected CG.  The state of step `reach` is produced by a lattice-tables handle (f1: ~6 s) and
+    carried over (state + rate) to a pair-sweep handle, which takes one untimed and `steps` timed steps."""
+    w = wl.config(2)
+    N = w.geometry.n_rings
+    with pkg.QS(w.geometry, w.material, lattice_tables=True) as tab:
+        for _ in range(reach):
+            tab.step(w.dt, w.I_ramp)
+        J, T = tab.read(B=False, E=False)[:2]
+        st = tab.stats()
+        rate = tab.read_rate()
+    its = []
+    with pkg.QS(w.geometry, w.material) as sim:
+        sim.write(J, T, st["t"], st["I"])
+        sim.write_rate(rate)
+        sim.step(w.dt, w.I_ramp)
+        ms, launches = timed_steps(torch, sim, w, steps, cg_iters=its)
+    return {"workload": w.name, "operator": "pairs", "window": f"steps {reach + 2}..{reach + 1 + steps} of the trajectory",
+            "value": N * steps / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms / steps,
+            "cg_iterations_per_step_mean": float(np.mean(its)), "gpu_launches": int(launches)}
+
+
 def gpu_arm(args):
     # the CPU oracle first (rank 0, one GPU, unless --no-extras): its worker pool is forked before this process
     # creates a CUDA context
@@ -475,13 +498,14 @@ def gpu_arm(args):
     # coils that first step is taken by a second handle with the lattice-tables operator (f1, ~0.2 s per sweep) and the
     # state AND the rate I' are carried over through qs_read / qs_read_rate -> qs_write / qs_write_rate; the W warm-up
     # steps and the K timed steps then run on the timed (pair-sweep) handle.
-    sim_tab, cold_start = None, "qs_step on the timed handle"
+    sim_tab, cold_start, first_timed = None, "qs_step on the timed handle", 1
     if args.operator == "pairs" and N > 100000:
         sim_tab = pkg.QS(w.geometry, w.material, device=local, lattice_tables=True)
         sim_tab.step(w.dt, w.I_ramp)
         J1, T1 = sim_tab.read(B=False, E=False)[:2]
         sim.write(J1, T1, sim_tab.stats()["t"], sim_tab.stats()["I"])
         sim.write_rate(sim_tab.read_rate())
+        first_timed = 2
         cold_start = ("first step (cold CG solve) on a lattice-tables handle, state + I' carried over by qs_write / "
                       "qs_write_rate; all warm-up and timed steps on the pair-sweep handle")
         if rank > 0 or world > 1 or args.no_extras:
@@ -572,6 +596,9 @@ def gpu_arm(args):
                        "cg_iterations_timed": int(np.sum(cg_its)), "cg_iterations_per_step_mean": float(np.mean(cg_its)),
                        "cg_note": "linear-regime steps: the warm-started CG is converged on entry, a step is one fused K2 "
                                   "sweep + O(N) passes; see cg_active for steps that iterate" if int(np.sum(cg_its)) == 0 else None,
+                       "window": f"steps {args.warmup + first_timed}..{args.warmup + first_timed - 1 + args.steps} of the trajectory from J = 0 (the coil "
+                                 "configs are in the linear regime for their first ~100 steps; later steps iterate the CG: "
+                                 "nonlinear_cfg2, cg_active, profiles/r02_full_runs.md)",
                        "cold_start": cold_start, "heat_substeps": st["heat_substeps"]},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "kernel_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()}}
@@ -596,6 +623,7 @@ def gpu_arm(args):
         line["roofline_hbm"]["peak_source"] = f"MEASURED_PEAKS.json hbm_gbs ({hbm_src})"
         line["roofline_hbm"]["traffic_source"] = NCU_SOURCE
         line["cg_active"] = cg_active_leg(torch, pkg)
+        line["nonlinear_cfg2"] = nonlinear_cfg2_leg(torch, pkg)
         line["operator_cfg4"] = operator_leg(torch, pkg, fp64_tf, args.sizes, args.cg_budget_s)
         line["cpu_baseline"] = cpu_baseline
     if rank == 0:

@@ -149,6 +149,7 @@ struct qs_ctx {
   char *fld_begin = nullptr, *fld_backup = nullptr, *ev_begin = nullptr, *ev_backup = nullptr;
   size_t fld_bytes = 0, ev_bytes = 0;
   bool have_prev_E_old = false;
+  bool backup_valid = false;         // the backups belong to the step in flight (restore_state copies them back only then)
   double *r, *z, *area, *jc0s, *selfcoef, *diagM;
   double *J, *Jold, *Ha, *Hb, *Hold, *Br, *Bz, *E, *dEdJ, *Q, *b, *shift, *Hd, *Jc, *rho;
   double *x, *xold, *cur, *p, *q, *rr, *g, *xp1, *Mxp1, *tmp, *tmp2, *zero;
@@ -713,12 +714,14 @@ MaterialArgs material_args(qs_ctx* c, double Bext, double Bdot, double dt, bool 
 // per-turn event state (wire statistics, mean-E history, first-event times, flag words, counters).
 int backup_state(qs_ctx* c) {
   const size_t nb8 = sizeof(double) * c->N;
+  c->backup_valid = false;
   QS_CUDA(cudaMemcpyAsync(c->Jold, c->J, nb8, cudaMemcpyDeviceToDevice, c->stream));
   QS_CUDA(cudaMemcpyAsync(c->Hold, c->H, nb8, cudaMemcpyDeviceToDevice, c->stream));
   QS_CUDA(cudaMemcpyAsync(c->xold, c->x, nb8, cudaMemcpyDeviceToDevice, c->stream));
   QS_CUDA(cudaMemcpyAsync(c->fld_backup, c->fld_begin, c->fld_bytes, cudaMemcpyDeviceToDevice, c->stream));
   if (c->n_turns) QS_CUDA(cudaMemcpyAsync(c->ev_backup, c->ev_begin, c->ev_bytes, cudaMemcpyDeviceToDevice, c->stream));
   c->have_prev_E_old = c->have_prev_E;
+  c->backup_valid = true;
   return QS_OK;
 }
 // Called on every negative return after backup_state: puts the state back (best effort if the device itself failed).
@@ -726,6 +729,9 @@ int backup_state(qs_ctx* c) {
 void restore_state(qs_ctx* c) {
   const size_t nb8 = sizeof(double) * c->N;
   cudaGetLastError();
+  c->n_prev = 0;
+  if (!c->backup_valid) return;   // the backup itself never ran (launch failure): the state was not touched either
+  c->backup_valid = false;
   cudaMemcpyAsync(c->J, c->Jold, nb8, cudaMemcpyDeviceToDevice, c->stream);
   cudaMemcpyAsync(c->H, c->Hold, nb8, cudaMemcpyDeviceToDevice, c->stream);
   cudaMemcpyAsync(c->x, c->xold, nb8, cudaMemcpyDeviceToDevice, c->stream);
@@ -819,7 +825,11 @@ int em_stage_fused(qs_ctx* c, bool extrapolate, double Bext, double Bdot, double
   const bool ev = c->lattice && c->n_turns > 0;
   sb.xmax_bits = ev ? c->xmax_bits : nullptr;
   sb.rmin_bits = ev ? c->rmin_bits : nullptr;
+  c->backup_valid = false;
   k_step_begin(v, sb);
+  if (cudaPeekAtLastError() != cudaSuccess)
+    return fail(QS_ERR_CUDA, std::string("step_begin launch failed: ") + cudaGetErrorString(cudaGetLastError()));
+  c->backup_valid = true;
   c->have_prev_E_old = c->have_prev_E;
   k_turn_fix(v, I_ramp, c->diagM, c->swM, c->x);
   if ((rc = do_sweep(c, c->x, c->cur, true, /*prezeroed=*/true)) != QS_OK) return rc;

@@ -258,6 +258,42 @@ def test_rate_checkpoint_resumes_like_the_uninterrupted_run(pkg):
         assert rel(b.read_rate(), a.read_rate()) <= 1e-9
 
 
+def test_patch_preconditioner_changes_iterations_not_the_solution(pkg):
+    # C8: the preconditioner is free, the solution of a step is unique.  Same nonlinear trajectory (single wire under a
+    # fast field ramp, |J| ~ Jc) with the patch (block-Jacobi) constraint preconditioner and with the diagonal one
+    # (QS_GEO_NO_PATCH_PRECOND): same states and terminal voltage to the CG tolerance, fewer iterations; and a coil in
+    # the linear regime (several turns: the per-turn Schur complement of the block projection), cold solve included
+    w = wl.shrunk(1, 1, 1, 32)
+    geo = dataclasses.replace(w.geometry, Bext_rate=20.0)
+    mat = dataclasses.replace(w.material, cg_tol=1e-12)
+    res = {}
+    for patch in (True, False):
+        its = 0
+        with pkg.QS(geo, mat, patch_precond=patch) as sim:
+            for _ in range(60):
+                assert sim.step(w.dt, 0.0) >= 0
+                its += sim.stats()["cg_iters"]
+            res[patch] = (sim.read(), sim.stats()["U_terminal"], its)
+    for u, v in zip(res[True][0], res[False][0]):
+        assert rel(u, v) <= 1e-8 or np.linalg.norm(v) < 1e-30
+    assert abs(res[True][1] - res[False][1]) <= 1e-8 * abs(res[False][1]) + 1e-20
+    assert 0 < res[True][2] < 0.7 * res[False][2], (res[True][2], res[False][2])
+    w = wl.shrunk(0, 3, 2, 8)
+    mat = dataclasses.replace(w.material, cg_tol=1e-12)
+    res = {}
+    for patch in (True, False):
+        with pkg.QS(w.geometry, mat, patch_precond=patch) as sim:
+            sim.step(w.dt, w.I_ramp)
+            first = sim.stats()["cg_iters"]
+            for _ in range(4):
+                sim.step(w.dt, w.I_ramp)
+            res[patch] = (sim.read(), sim.stats()["U_terminal"], first)
+    for u, v in zip(res[True][0], res[False][0]):
+        assert rel(u, v) <= 1e-9 or np.linalg.norm(v) < 1e-30
+    assert abs(res[True][1] - res[False][1]) <= 1e-9 * abs(res[False][1])
+    assert 0 < res[True][2] < res[False][2]
+
+
 def test_handle_works_while_another_device_or_stream_context_is_current(pkg):
     # a handle remembers its device: calls are valid whatever device is current in the calling thread (one GPU here:
     # the guard must at least be a no-op; with two visible devices the second one is made current around the calls)

@@ -155,10 +155,16 @@ __global__ void __launch_bounds__(256) table_sweep_kernel(LatticeSweepParams prm
 // is, for 8 consecutive p and a fixed block offset d, an (8 x 8) += (8 x 8)(8 x 8) product = two m8n8k4 steps whose
 // A operand is a block of 8 x 8 source values (rows = source blocks p - d) and whose B operand is the Toeplitz block
 // T_d[b][q] = t[8d + q - b].  A warp owns NT tiles of 64 outputs which share every B fragment; the fused sweep shares
-// the A fragment of the ring currents between the Bz and Br tables.  Fragments are read from shared memory: the source
-// row in 8-blocks padded to a stride of 12 doubles (conflict-free for the row-strided A pattern), the mirrored table
-// row as for the multiply-add kernel.
+// the A fragment of the ring currents between the Bz and Br tables.  Fragments are read from shared memory:
+//   * the source row in 8-blocks padded to a stride of 12 slots (conflict-free for the row-strided A pattern); in the
+//     fused sweep a slot is the pair {x, ring current}, so one LDS.128 fetches both A fragments;
+//   * the mirrored table row t_ext[e]; in the fused sweep the three tables are interleaved per offset, so the three
+//     B fragments are one pointer with immediate offsets (stride 3 is odd: conflict-free).
+// The offset loop is split into segments with a compile-time tile mask (the first 8 offsets reach only tile 0, the last
+// 8 only tile 1), its pointers advance by constants, and the fragments of the next k-step are loaded before the DMMAs
+// of the current one are issued (two register sets alternate, no copies).
 constexpr int kMmaNT = 2;
+constexpr int kMmaBlk = 12;                                        // slots per source 8-block in shared memory
 
 __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -167,26 +173,77 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
 }
 
 template <bool FIELD>
+struct MmaFrag {
+  double b[FIELD ? 3 : 1];                                         // B fragments: k = lk (+4 kk), n = li, per table
+  double ax[kMmaNT], ac[FIELD ? kMmaNT : 1];                       // A fragments: row li = output block, k = lk (+4 kk)
+};
+
+template <bool FIELD, int MASK>
+__device__ __forceinline__ void mma_load(MmaFrag<FIELD>& f, const double* pa, const double* pb) {
+  f.b[0] = pb[0];
+  if constexpr (FIELD) f.b[1] = pb[1], f.b[2] = pb[2];
+#pragma unroll
+  for (int j = 0; j < kMmaNT; ++j) {
+    if (!((MASK >> j) & 1)) continue;
+    if constexpr (FIELD) {
+      const double2 v = *reinterpret_cast<const double2*>(pa + j * 8 * kMmaBlk * 2);
+      f.ax[j] = v.x, f.ac[j] = v.y;
+    } else {
+      f.ax[j] = pa[j * 8 * kMmaBlk];
+    }
+  }
+}
+
+template <bool FIELD, int MASK>
+__device__ __forceinline__ void mma_issue(double (&acc)[kMmaNT][FIELD ? 3 : 1][2], const MmaFrag<FIELD>& f) {
+#pragma unroll
+  for (int j = 0; j < kMmaNT; ++j) {
+    if (!((MASK >> j) & 1)) continue;
+    dmma(acc[j][0], f.ax[j], f.b[0]);
+    if constexpr (FIELD) {
+      dmma(acc[j][1], f.ac[j], f.b[1]);
+      dmma(acc[j][2], f.ac[j], f.b[2]);
+    }
+  }
+}
+
+// Offsets d0..d1 for the tiles in MASK.  pa / pb: this lane's A / B fragment of k-step 0 at offset d0.  The last trip
+// loads the fragments of offset d1 + 1, which are not used: the shared arrays carry one guard block for that.
+template <bool FIELD, int MASK>
+__device__ __forceinline__ void mma_segment(double (&acc)[kMmaNT][FIELD ? 3 : 1][2], const double* pa, const double* pb,
+                                            int d0, int d1) {
+  constexpr int W = FIELD ? 2 : 1, TW = FIELD ? 3 : 1;
+  if (d0 > d1) return;
+  MmaFrag<FIELD> f0, f1;
+  mma_load<FIELD, MASK>(f0, pa, pb);
+  for (int d = d0; d <= d1; ++d) {
+    mma_load<FIELD, MASK>(f1, pa + 4 * W, pb - 4 * TW);            // k-step 1 of offset d
+    mma_issue<FIELD, MASK>(acc, f0);
+    pa -= kMmaBlk * W;
+    pb += 8 * TW;
+    mma_load<FIELD, MASK>(f0, pa, pb);                             // k-step 0 of offset d + 1
+    mma_issue<FIELD, MASK>(acc, f1);
+  }
+}
+
+template <bool FIELD>
 __global__ void __launch_bounds__(512) table_sweep_mma_kernel(LatticeSweepParams prm, int P, int n_asplit, int A_c) {
   // The CTA owns the outputs of its warps (8 NT p-blocks each) and the SOURCE blocks a in [a_lo, a_hi): splitting the
   // sources as well as the outputs keeps the shared-memory windows near 50 KB (four CTAs per SM) on long rows.
   extern __shared__ __align__(16) double lsm[];
-  constexpr int NT = kMmaNT, NTAB = FIELD ? 3 : 1;
+  constexpr int NT = kMmaNT, NTAB = FIELD ? 3 : 1, W = FIELD ? 2 : 1, TW = FIELD ? 3 : 1;
+  static_assert(NT == 2, "the segment split below is written for two tiles per warp");
   const int Nz = prm.Nz, T = blockDim.x;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = T >> 5;
   const int zt = blockIdx.z / n_asplit, as = blockIdx.z - zt * n_asplit;
   const int a_lo = as * A_c, a_hi = min(a_lo + A_c, P);
   const int p_lo = zt * nwarps * 8 * NT;                          // first p-block of the CTA's outputs
   const int np_cta = nwarps * 8 * NT;
-  const int xblocks = A_c + 14;                                   // source blocks a_lo - 7 .. a_lo + A_c + 6
-  const int xlen = xblocks * 12;
+  const int xblocks = A_c + 15;                                   // source blocks a_lo - 8 .. a_lo + A_c + 6
   const int e0 = 8 * (p_lo - (a_lo + A_c) + 1) - 8;               // first offset iz - jz of the table window
-  const int tlen = 8 * (np_cta + A_c + 8) + 24;
-  double* xs = lsm;
-  double* cs = FIELD ? xs + xlen : nullptr;
-  double* tM = (FIELD ? cs : xs) + xlen;                          // t_ext[e] at [e - e0]
-  double* tBz = FIELD ? tM + tlen : nullptr;
-  double* tBr = FIELD ? tBz + tlen : nullptr;
+  const int tlen = 8 * (np_cta + A_c + 8) + 32;                   // incl. the guard of the look-ahead load
+  double* xc = lsm;                                               // slot (blk, b) at [(blk * 12 + b) * W (+ 1: current)]
+  double* tt = xc + xblocks * kMmaBlk * W;                        // t_ext[e] of table k at [(e - e0) * TW + k]
   if (prm.done != nullptr && *prm.done != 0) return;
   const int ir = blockIdx.y;
   const int j0 = blockIdx.x * prm.jr_chunk, j1 = min(j0 + prm.jr_chunk, prm.Nr);
@@ -197,49 +254,47 @@ __global__ void __launch_bounds__(512) table_sweep_mma_kernel(LatticeSweepParams
   for (int j = 0; j < NT; ++j)
 #pragma unroll
     for (int t = 0; t < NTAB; ++t) acc[j][t][0] = acc[j][t][1] = 0.0;
+  // offset ranges of the two tiles (tile 1 = tile 0 shifted by 8 blocks) and the three segments of the union
+  const int lo0 = pw - (a_hi - 1), hi0 = pw + 7 - a_lo, lo1 = lo0 + 8, hi1 = hi0 + 8;
+  const bool two = pw + 8 < P;                                    // tile 1 inside the row
   for (int jr = j0; jr < j1; ++jr) {
     __syncthreads();
     const long long trow = (static_cast<long long>(ir) * prm.Nr + jr) * Nz;
     const long long xrow = static_cast<long long>(jr) * Nz;
     for (int s = threadIdx.x; s < xblocks * 8; s += T) {          // source blocks of this CTA, zero outside its range
-      const int a = a_lo - 7 + (s >> 3), b = s & 7, j = 8 * a + b;
+      const int blk = s >> 3, b = s & 7;
+      const int a = a_lo - 8 + blk, j = 8 * a + b;
       const bool in = a >= a_lo && a < a_hi && j < Nz;
-      xs[(s >> 3) * 12 + b] = in ? prm.x[xrow + j] : 0.0;
-      if (FIELD) cs[(s >> 3) * 12 + b] = in ? prm.cur[xrow + j] : 0.0;
+      const double xv = in ? prm.x[xrow + j] : 0.0;
+      if constexpr (FIELD) {
+        const double cv = in ? prm.cur[xrow + j] : 0.0;
+        reinterpret_cast<double2*>(xc)[blk * kMmaBlk + b] = make_double2(xv, cv);
+      } else {
+        xc[blk * kMmaBlk + b] = xv;
+      }
     }
     for (int s = threadIdx.x; s < tlen; s += T) {                 // mirrored table row, zero outside |e| < Nz
       const int e = s + e0, d = abs(e);
       const bool in = d < Nz;
-      tM[s] = in ? prm.TM[trow + d] : 0.0;
-      if (FIELD) {
-        tBz[s] = in ? prm.TBz[trow + d] : 0.0;
+      tt[s * TW] = in ? prm.TM[trow + d] : 0.0;
+      if constexpr (FIELD) {
+        tt[s * TW + 1] = in ? prm.TBz[trow + d] : 0.0;
         const double br = in ? prm.TBr[trow + d] : 0.0;
-        tBr[s] = e < 0 ? -br : br;
+        tt[s * TW + 2] = e < 0 ? -br : br;
       }
     }
     __syncthreads();
     if (pw >= P) continue;                                        // warp beyond the row: only helps with the fills
-    const int dlo = pw - (a_hi - 1), dhi = pw + 8 * (NT - 1) + 7 - a_lo;
-    for (int d = dlo; d <= dhi; ++d) {
-#pragma unroll
-      for (int kk = 0; kk < 2; ++kk) {
-        const int e = 8 * d + li - lk - 4 * kk - e0;              // B fragment: k = lk (+4 kk), n = li
-        const double bM = tM[e];
-        const double bBz = FIELD ? tBz[e] : 0.0, bBr = FIELD ? tBr[e] : 0.0;
-#pragma unroll
-        for (int j = 0; j < NT; ++j) {
-          const int pj = pw + 8 * j;
-          if (pj >= P || d < pj - (a_hi - 1) || d > pj + 7 - a_lo) continue;   // tile beyond the row, or no source block
-                                                                               // of this CTA at this offset (uniform)
-          const int ai = (pj + li - d - a_lo + 7) * 12 + lk + 4 * kk;   // A fragment: row li = output block, k = lk (+4 kk)
-          dmma(acc[j][0], xs[ai], bM);
-          if (FIELD) {
-            const double ac = cs[ai];
-            dmma(acc[j][1], ac, bBz);
-            dmma(acc[j][2], ac, bBr);
-          }
-        }
-      }
+    // fragment addresses at offset d: A (tile 0) slot ((pw + li - d - a_lo + 8) * 12 + lk), B element 8 d + li - lk - e0
+    auto pa_at = [&](int d) { return xc + ((pw + li - d - a_lo + 8) * kMmaBlk + lk) * W; };
+    auto pb_at = [&](int d) { return tt + (8 * d + li - lk - e0) * TW; };
+    if (!two) {
+      mma_segment<FIELD, 1>(acc, pa_at(lo0), pb_at(lo0), lo0, hi0);
+    } else {
+      const int a1 = min(hi0, lo1 - 1), c0 = max(hi0 + 1, lo1);
+      mma_segment<FIELD, 1>(acc, pa_at(lo0), pb_at(lo0), lo0, a1);
+      mma_segment<FIELD, 3>(acc, pa_at(lo1), pb_at(lo1), lo1, hi0);
+      mma_segment<FIELD, 2>(acc, pa_at(c0), pb_at(c0), c0, hi1);
     }
   }
   const long long orow = static_cast<long long>(ir) * Nz;
@@ -321,8 +376,8 @@ static cudaError_t launch_table_sweep_mma(LatticeSweepParams prm, bool field, in
   splits = (prm.Nr + prm.jr_chunk - 1) / prm.jr_chunk;
   const dim3 grid(splits, prm.Nr, ztiles * n_asplit);
   const int np_cta = nwarps * per_warp;
-  const size_t smem = sizeof(double) * (static_cast<size_t>(field ? 2 : 1) * (A_c + 14) * 12 +
-                                        static_cast<size_t>(field ? 3 : 1) * (8 * (np_cta + A_c + 8) + 24));
+  const size_t smem = sizeof(double) * (static_cast<size_t>(field ? 2 : 1) * (A_c + 15) * kMmaBlk +
+                                        static_cast<size_t>(field ? 3 : 1) * (8 * (np_cta + A_c + 8) + 32));
   if (field) {
     cudaFuncSetAttribute(table_sweep_mma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     table_sweep_mma_kernel<true><<<grid, nwarps * 32, smem, stream>>>(prm, P, n_asplit, A_c);

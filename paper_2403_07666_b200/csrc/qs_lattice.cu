@@ -226,8 +226,10 @@ __device__ __forceinline__ void mma_segment(double (&acc)[kMmaNT][FIELD ? 3 : 1]
   }
 }
 
+// <= 8 warps per CTA; the register budget of three 8-warp CTAs (<= 80 per thread, 78 used by the fused sweep) keeps the
+// warp count shared-memory bound (102 registers unbounded: config 2 8.07 ms, this budget 7.87 ms; 64 registers: 8.18 ms)
 template <bool FIELD>
-__global__ void __launch_bounds__(512) table_sweep_mma_kernel(LatticeSweepParams prm, int P, int n_asplit, int A_c) {
+__global__ void __launch_bounds__(256, 3) table_sweep_mma_kernel(LatticeSweepParams prm, int P, int n_asplit, int A_c) {
   // The CTA owns the outputs of its warps (8 NT p-blocks each) and the SOURCE blocks a in [a_lo, a_hi): splitting the
   // sources as well as the outputs keeps the shared-memory windows near 50 KB (four CTAs per SM) on long rows.
   extern __shared__ __align__(16) double lsm[];
@@ -359,13 +361,65 @@ static cudaError_t launch_R(const LatticeSweepParams& prm, bool field, dim3 grid
 }
 
 // tensor-core variant
-static cudaError_t launch_table_sweep_mma(LatticeSweepParams prm, bool field, int sm_count, cudaStream_t stream) {
+static size_t mma_sweep_smem(bool field, int nwarps, int A_c) {
+  const int np_cta = nwarps * 8 * kMmaNT;
+  return sizeof(double) * (static_cast<size_t>(field ? 2 : 1) * (A_c + 15) * kMmaBlk +
+                           static_cast<size_t>(field ? 3 : 1) * (8 * (np_cta + A_c + 8) + 32));
+}
+
+// Launch shape of the tensor-core sweep: warps per CTA (each owns 8 NT output blocks), CTAs per row, and the number of
+// source-block ranges a row is split into.  Measured on B200 (config 2: 80 blocks = 5 warp tiles, config 3: 150 blocks
+// = 10 warp tiles; fused / M-only sweep in ms):
+//   config 2: one 5-warp CTA per row 7.87 / 2.65 (four / six CTAs resident per SM); 3 + 2 warps 9.18 / 2.67; 2 + 2 + 1
+//             warps 9.85 / 3.19; sources split in two 9.18 / 2.94
+//   config 3: 4 + 4 + 2 warps 143.6 / 46.2 (three 74 KB CTAs = 12 warps per SM); 5 + 5 warps 185.4 / 49.8 (two 77 KB
+//             CTAs = 10 warps: 3, 3, 2, 2 per sub-partition); 3 + 3 + 3 + 1 190.8 / 48.8; 5 + 5 on half the sources each
+//             149.3 / 52.8 (four CTAs = 20 warps, but a tile of 8 output blocks sweeps A_c + 7 block offsets for A_c
+//             source blocks: 9 % padding instead of 4.5 %)
+// The DMMA pipe is per sub-partition, so a launch is as fast as its most loaded sub-partition; beyond ~12 resident warps
+// the count itself matters little; CTAs of 1-2 warps pay for their window fills.  So: among >= 3 warps per CTA (fewer
+// only if the row has fewer tiles) with the sources unsplit (split only when the windows do not fit otherwise), estimate
+// the resident warps R per SM from shared memory and registers and take the smallest ceil(R / 4) / (R / 4); on a tie
+// fewer CTAs per row, then more resident warps.
+static void mma_sweep_shape(bool field, int P, int regs_per_thread, int* nwarps_out, int* ztiles_out, int* nas_out) {
+  const int wn = (P + 8 * kMmaNT - 1) / (8 * kMmaNT);
+  const int regs_per_warp = ((regs_per_thread * 32 + 511) / 512) * 512;
+  *nwarps_out = std::min(wn, 8), *ztiles_out = (wn + 7) / 8, *nas_out = 1;
+  for (int nas = 1; nas <= 16; ++nas) {
+    const int A_c = (P + nas - 1) / nas;
+    double best = 1e300;
+    int bestR = 0, bestZ = 0;
+    for (int nw = std::min(wn, 3); nw <= 8; ++nw) {
+      const int ztiles = (wn + nw - 1) / nw, nwarps = (wn + ztiles - 1) / ztiles;
+      if (nwarps != nw) continue;                                  // the equalised shape is enumerated under its own nw
+      const size_t smem = mma_sweep_smem(field, nwarps, A_c);
+      if (smem > 227u * 1024u) continue;
+      const int by_smem = static_cast<int>((228u * 1024u) / (smem + 1024u));
+      const int by_regs = 65536 / (regs_per_warp * nwarps);
+      const int ctas = std::min(std::min(by_smem, by_regs), std::min(32, 64 / nwarps));
+      if (ctas < 1) continue;
+      const int R = ctas * nwarps;
+      const double cost = static_cast<double>((R + 3) / 4) / (R / 4.0) * (R < 8 ? 8.0 / R : 1.0);
+      const bool better = cost < best - 1e-9 ||
+                          (cost < best + 1e-9 && (ztiles < bestZ || (ztiles == bestZ && R > bestR)));
+      if (better) best = cost, bestR = R, bestZ = ztiles, *nwarps_out = nwarps, *ztiles_out = ztiles, *nas_out = nas;
+    }
+    if (bestR > 0) return;                                         // a shape fits with this split
+  }
+}
+
+template <bool FIELD>
+static cudaError_t launch_mma_T(LatticeSweepParams prm, int sm_count, cudaStream_t stream) {
+  static int regs = 0;                                               // of this instantiation (the same on every device)
+  if (regs == 0) {
+    cudaFuncAttributes at;
+    const cudaError_t e = cudaFuncGetAttributes(&at, table_sweep_mma_kernel<FIELD>);
+    if (e != cudaSuccess) return e;
+    regs = at.numRegs;
+  }
   const int P = (prm.Nz + 7) / 8;
-  const int per_warp = 8 * kMmaNT;                                   // 8-blocks per warp
-  const int warps_needed = (P + per_warp - 1) / per_warp;
-  const int ztiles = (warps_needed + 4) / 5;                         // at most 5 warps (640 outputs) per CTA ...
-  const int nwarps = (warps_needed + ztiles - 1) / ztiles;
-  const int n_asplit = (P + 79) / 80;                                // ... and at most 80 source blocks
+  int nwarps, ztiles, n_asplit;
+  mma_sweep_shape(FIELD, P, regs, &nwarps, &ztiles, &n_asplit);
   const int A_c = (P + n_asplit - 1) / n_asplit;
   // many small CTAs (a few source rows each): the fill of one CTA overlaps the DMMA phase of its neighbours on the SM
   // and the tail of the launch stays short (measured: 10.7 ms at 12 CTAs per SM, 9.3 ms at one source row per CTA)
@@ -375,17 +429,15 @@ static cudaError_t launch_table_sweep_mma(LatticeSweepParams prm, bool field, in
   prm.jr_chunk = (prm.Nr + splits - 1) / splits;
   splits = (prm.Nr + prm.jr_chunk - 1) / prm.jr_chunk;
   const dim3 grid(splits, prm.Nr, ztiles * n_asplit);
-  const int np_cta = nwarps * per_warp;
-  const size_t smem = sizeof(double) * (static_cast<size_t>(field ? 2 : 1) * (A_c + 15) * kMmaBlk +
-                                        static_cast<size_t>(field ? 3 : 1) * (8 * (np_cta + A_c + 8) + 32));
-  if (field) {
-    cudaFuncSetAttribute(table_sweep_mma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
-    table_sweep_mma_kernel<true><<<grid, nwarps * 32, smem, stream>>>(prm, P, n_asplit, A_c);
-  } else {
-    cudaFuncSetAttribute(table_sweep_mma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
-    table_sweep_mma_kernel<false><<<grid, nwarps * 32, smem, stream>>>(prm, P, n_asplit, A_c);
-  }
+  const size_t smem = mma_sweep_smem(FIELD, nwarps, A_c);
+  cudaFuncSetAttribute(table_sweep_mma_kernel<FIELD>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+  table_sweep_mma_kernel<FIELD><<<grid, nwarps * 32, smem, stream>>>(prm, P, n_asplit, A_c);
   return cudaGetLastError();
+}
+
+// tensor-core variant
+static cudaError_t launch_table_sweep_mma(const LatticeSweepParams& prm, bool field, int sm_count, cudaStream_t stream) {
+  return field ? launch_mma_T<true>(prm, sm_count, stream) : launch_mma_T<false>(prm, sm_count, stream);
 }
 
 cudaError_t launch_table_sweep(const LatticeSweepParams& prm_in, bool field, int sm_count, cudaStream_t stream) {

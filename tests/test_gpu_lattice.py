@@ -63,6 +63,29 @@ def test_tables_config2_full_size_sampled_rows(pkg):
     assert rel(B[idx], Br) <= 1e-9 and rel(B[geo.n_rings + idx], Bz) <= 1e-9
 
 
+# long rows of the tensor-core sweep, one case per launch shape (mma_sweep_shape): Nz = 128 (one warp, both of its
+# tiles), 200 (second warp with its second tile beyond the row), 1200 (config 3's rows: three CTAs per row of 4 + 4 + 2
+# active warps) and 8192 (the source blocks of a row split between CTAs: the windows of the fused sweep do not fit
+# otherwise); exact oracle rows on a seeded sample, the on-the-fly sweeps on every ring
+# (layers, turns, n, inner radius): the 0.82 m tall stack needs a radius the library accepts (k'^2 <= 0.98)
+@pytest.mark.parametrize("shape", [(2, 16, 8, 50e-3), (2, 25, 8, 50e-3), (1, 100, 12, 50e-3), (1, 1024, 8, 0.2)])
+def test_tables_long_rows_sampled(pkg, shape):
+    L, Tn, n, r_in = shape
+    geo = wl.lattice_geometry(L, Tn, n, 0.8e-3, r_in)
+    N = geo.n_rings
+    x = np.random.default_rng(77 + N).standard_normal(N)
+    idx = wl.sample_rows(N, 64, seed=N)
+    with pkg.QS(geo, wl.Material(), lattice_tables=True) as sim:
+        y, B = sim.matvec(x), sim.field(x)
+    with pkg.QS(geo, wl.Material()) as fly:
+        y2, B2 = fly.matvec(x), fly.field(x)
+    assert rel(y, y2) <= 1e-12 and rel(B, B2) <= 1e-12
+    assert np.max(np.abs(y - y2)) <= 1e-11 * np.max(np.abs(y2)) and np.max(np.abs(B - B2)) <= 1e-11 * np.max(np.abs(B2))
+    assert rel(y[idx], qo.matvec_rows(geo, x, idx, chunk=16)) <= 1e-9
+    Br, Bz = qo.field_eval_rows(geo, x, idx, chunk=8)
+    assert rel(B[idx], Br) <= 1e-9 and rel(B[N + idx], Bz) <= 1e-9
+
+
 def test_tables_steps_config0_and_shrunk_config2(pkg):
     for w, steps in ((wl.config(0), 50), (wl.shrunk(2, 3, 5), 100)):
         geo = w.geometry

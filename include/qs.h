@@ -67,9 +67,14 @@ typedef struct qs_ctx qs_ctx;
                                   arithmetic per unique pair, same results up to summation order.  */
 
 #define QS_GEO_NO_PATCH_PRECOND 4 /* lattice geometries whose constraint groups are the wires: do NOT build the patch
-                                    (block-Jacobi over p x p cells of a wire, p <= 8) constraint preconditioner of the
-                                    projected CG (2 x 8 N p^2 bytes of workspace); the solver then keeps diag(A) (C8).
+                                    (block-Jacobi over p x p cells of a wire, p <= 16: whole wires of up to 16 x 16
+                                    cells) constraint preconditioner of the projected CG (up to 2 x 8 N p^2 bytes of
+                                    workspace); the solver then keeps diag(A) (C8).
                                     The preconditioner is free: the solution of a step is unique (C4).  */
+
+#define QS_GEO_PATCH_SUBWIRE 16   /* keep the patches of the constraint preconditioner at p <= 8 (inverted in shared
+                                    memory) instead of p <= 16 (whole wires of up to 16 x 16 cells; inverted per solve
+                                    in global memory); either is a preconditioner only (C8).  */
 
 #define QS_GEO_HEAT_BLOCKED 8     /* measurement: use the temporally blocked heat kernel (<= 4 explicit sub-steps per
                                     launch from a shared-memory tile with a 4-cell halo) at ANY lattice size; by

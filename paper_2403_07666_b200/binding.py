@@ -183,7 +183,8 @@ class QS:
     ``qs_geometry`` / ``qs_material`` (e.g. ``workloads.Geometry`` / ``workloads.Material``)."""
 
     def __init__(self, geometry, material, device: int = 0, no_operator: bool = False, torch_memory: bool = True,
-                 lattice_tables: bool = False, patch_precond: bool = True, heat_blocked: bool = False):
+                 lattice_tables: bool = False, patch_precond: bool = True, heat_blocked: bool = False,
+                 patch_subwire: bool = False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2403_07666_b200 needs a CUDA device: there is no CPU path")
@@ -209,7 +210,8 @@ class QS:
         g.h_conv = (C.c_double * 4)(*[float(v) for v in geometry.h_conv])
         g.T_bath = float(geometry.T_bath)
         g.Bext0, g.Bext_rate, g.Bext_max = float(geometry.Bext0), float(geometry.Bext_rate), float(geometry.Bext_max)
-        g.flags = (1 if no_operator else 0) | (2 if lattice_tables else 0) | (0 if patch_precond else 4) | (8 if heat_blocked else 0)
+        g.flags = (1 if no_operator else 0) | (2 if lattice_tables else 0) | (0 if patch_precond else 4) | (8 if heat_blocked else 0) | \
+                  (16 if patch_subwire else 0)
         share = getattr(geometry, "turn_share", None)
         if share is not None and self.n_turns > 0:
             sh = _f64(share, self.n_turns)

@@ -286,7 +286,7 @@ void carve(qs_ctx* c, void* base, size_t* total) {
     const size_t pp = c->patch.pp;
     c->pidx = k.take<int>(N);
     c->pturn = k.take<int>(N / pp);
-    c->patch.Pm = k.take<double>(N * pp);
+    c->patch.Pm = k.take<double>(c->patch.big ? static_cast<size_t>(c->patch.layers) * c->patch.per * pp * pp : N * pp);
     c->patch.Pinv = k.take<double>(N * pp);
     c->patch.h1 = k.take<double>(N);
     c->patch.sw = k.take<double>(nt);
@@ -326,6 +326,9 @@ int check_geometry(const qs_geometry* g) {
 
 // Side p of the square patches of the patch preconditioner (0: not applicable): lattices whose constraint groups are
 // the wires in canonical numbering; p = the largest divisor of the cells per wire side that is <= 8.
+// Side p of the square patches of the patch preconditioner (0: not applicable): lattices whose constraint groups are
+// the wires in canonical numbering; p = the largest divisor of the cells per wire side that is <= 16 (the whole wire
+// up to 16 x 16 cells: configs 0, 2, 3; 16 x 16 patches of config 1's 64 x 64), <= 8 with QS_GEO_PATCH_SUBWIRE.
 int patch_side(const qs_geometry* g) {
   if (!g->lattice || (g->flags & (QS_GEO_NO_OPERATOR | QS_GEO_NO_PATCH_PRECOND)) || g->n_turns <= 0) return 0;
   const int n = g->cells_per_side;
@@ -333,10 +336,20 @@ int patch_side(const qs_geometry* g) {
   const long long Nz = static_cast<long long>(g->turns_per_layer) * n;
   for (long long k = 0; k < g->n_rings; ++k)
     if (g->turn_id[k] != (k / Nz / n) * g->turns_per_layer + (k % Nz) / n) return 0;
+  const int pmax = (g->flags & QS_GEO_PATCH_SUBWIRE) ? 8 : 16;
   int p = 1;
-  for (int d = 2; d <= 8 && d <= n; ++d)
+  for (int d = 2; d <= pmax && d <= n; ++d)
     if (n % d == 0) p = d;
   return p >= 2 ? p : 0;
+}
+void patch_setup(PatchPrec* pc, const qs_geometry* g, int N) {
+  const int ps = patch_side(g);
+  pc->pp = ps * ps;
+  pc->n_patches = ps ? N / (ps * ps) : 0;
+  pc->big = ps > 8;
+  pc->per = ps ? g->cells_per_side / ps : 1;
+  pc->layers = g->layers;
+  pc->per_layer = g->turns_per_layer;
 }
 
 int sync_scalars(qs_ctx* c) {
@@ -969,11 +982,7 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
   c->tables = c->lattice && c->has_operator && (geo->flags & QS_GEO_LATTICE_TABLES);
   c->heat_force_blocked = (geo->flags & QS_GEO_HEAT_BLOCKED) != 0;
   c->blockprec = !c->lattice && c->has_operator && geo->n_turns == 0;
-  {
-    const int ps = patch_side(geo);
-    c->patch.pp = ps * ps;
-    c->patch.n_patches = ps ? N / (ps * ps) : 0;
-  }
+  patch_setup(&c->patch, geo, N);
   c->Bext0 = geo->Bext0;
   c->Bext_rate = geo->Bext_rate;
   c->Bext_max = geo->Bext_max;
@@ -1264,10 +1273,7 @@ size_t qs_workspace_bytes(const qs_geometry* geo) {
     tmp.tables = (geo->flags & QS_GEO_LATTICE_TABLES) && !(geo->flags & QS_GEO_NO_OPERATOR);
   }
   tmp.blockprec = !geo->lattice && !(geo->flags & QS_GEO_NO_OPERATOR) && geo->n_turns == 0;
-  {
-    const int ps = patch_side(geo);
-    tmp.patch.pp = ps * ps;
-  }
+  patch_setup(&tmp.patch, geo, geo->n_rings);
   size_t need = 0;
   carve(&tmp, nullptr, &need);
   return need;

@@ -105,9 +105,13 @@ struct VecCtx {
 struct PatchPrec {
   int pp = 0;               // cells per patch (0: off), p x p inside one wire
   int n_patches = 0;
+  int big = 0;              // 1: patches of more than 64 cells (p = 9..16): inverse per solve in global memory, the
+                            //    constant part shared between the patches of one (layer, radial slot of the wire)
+  int per = 1;              // patches per wire side (patches are numbered ((layer * per_layer + turn) * per + a) * per + b)
+  int layers = 0, per_layer = 0;
   const int* pidx = nullptr;    // [n_patches][pp] cell of slot t of the patch
   const int* pturn = nullptr;   // [n_patches] constraint group of the patch
-  double* Pm = nullptr;         // [n_patches][pp][pp] constant part M_patch [H]
+  double* Pm = nullptr;         // [n_patches][pp][pp] constant part M_patch [H]   (big: [layers * per][pp][pp])
   double* Pinv = nullptr;       // [n_patches][pp][pp] (M_patch + diag(shift))^-1 of the current solve
   double* h1 = nullptr;         // [N] Pinv 1
   double* sw = nullptr;         // [n_turns] per-turn Schur scalars sum h1

@@ -370,16 +370,19 @@ __global__ void step_update_kernel(int n, double dt, const double* __restrict__ 
 // a block H:  t = H^-1 r,  s_w = sum_{i in w} (H^-1 1)_i,  v_w = (sum_{i in w} t_i)/s_w,  g = t - v_w H^-1 1,  r <- r - v_w.
 // Patches never straddle a constraint group, so the per-turn Schur complement stays diagonal.
 constexpr int kPatchMax = 64;   // cells per patch (p <= 8)
+constexpr int kWireMax = 256;   // cells per patch of the big patches (p <= 16: whole wires of up to 16 x 16 cells)
 
 // once per qs_init: the constant part M_patch [H] of every patch, pair by pair with the sweeps' arithmetic
-__global__ void __launch_bounds__(kPatchMax) patch_build_kernel(int pp, const int* __restrict__ pidx,
-                                                               const double* __restrict__ r, const double* __restrict__ z,
-                                                               double soft_all, double soft_self, double* __restrict__ Pm) {
-  const int pch = blockIdx.x, t = threadIdx.x;
+// (big patches: one matrix per (layer, radial slot) = blockIdx.x, evaluated on that slot's first patch of the layer)
+__global__ void __launch_bounds__(kWireMax) patch_build_kernel(int pp, int per, int per_layer, const int* __restrict__ pidx,
+                                                              const double* __restrict__ r, const double* __restrict__ z,
+                                                              double soft_all, double soft_self, double* __restrict__ Pm) {
+  const int pch = per > 0 ? ((blockIdx.x / per) * per_layer * per + blockIdx.x % per) * per : blockIdx.x;
+  const int t = threadIdx.x;
   if (t >= pp) return;
   const int i = pidx[pch * pp + t];
   const double ri = r[i], zi = z[i];
-  double* row = Pm + (static_cast<size_t>(pch) * pp + t) * pp;
+  double* row = Pm + (static_cast<size_t>(blockIdx.x) * pp + t) * pp;
   for (int u = 0; u < pp; ++u) {
     const int j = pidx[pch * pp + u];
     const double rj = r[j], dz = zi - z[j];
@@ -451,11 +454,11 @@ __global__ void __launch_bounds__(kPatchMax * kPinvSplit) patch_invert_kernel(in
 // t = Pinv r over one patch; parks t in g and adds sum t to tw[turn].  UPDATE: first x += alpha p, r += alpha q
 // (the fused CG iteration's update); else r is taken as it is (start of the solve).
 template <bool UPDATE>
-__global__ void __launch_bounds__(kPatchMax) patch_apply_kernel(int pp, const int* __restrict__ pidx,
-                                                               const int* __restrict__ pturn,
-                                                               const double* __restrict__ Pinv, CgIter it, Scalars* sc) {
-  __shared__ double rs[kPatchMax];
-  __shared__ double part[kPatchMax / 32];
+__global__ void __launch_bounds__(kWireMax) patch_apply_kernel(int pp, const int* __restrict__ pidx,
+                                                              const int* __restrict__ pturn,
+                                                              const double* __restrict__ Pinv, CgIter it, Scalars* sc) {
+  __shared__ double rs[kWireMax];
+  __shared__ double part[kWireMax / 32];
   if (UPDATE && sc->done) return;
   double alpha = 0.0;
   if (UPDATE) {
@@ -492,6 +495,72 @@ __global__ void __launch_bounds__(kPatchMax) patch_apply_kernel(int pp, const in
     double s = 0.0;
     for (int k = 0; k < (pp + 31) / 32; ++k) s += part[k];
     atomicAdd(it.tw + pturn[pch], s);
+  }
+}
+
+// ---- patches of more than 64 cells (p = 9..16: whole wires of configs 2 and 3, 16 x 16 sub-wire patches of config 1) ----
+// A 256 x 256 block does not fit shared memory, so the per-solve inverse is formed by the same Gauss-Jordan elimination
+// IN GLOBAL MEMORY (the block stays in L2 while its CTA of 1024 threads works on it: ~0.05-0.2 ms per block, a few
+// blocks per SM, ~1 ms per solve at config 3).  The constant part is shared: patches in the same layer and radial slot
+// of their wire are translates of each other along z, so Pm holds one matrix per (layer, radial slot).
+// Why whole wires: measured on the host on mid-trajectory systems of shrunk configs 2 / 3 with the surface cells at Jc
+// (warm start), 2 x 2 ... 8 x 8 sub-wire patches all need 87-97 iterations, the whole wire 41 / 44: only the full block
+// carries the wire's screening-current modes.  A fixed inverse of M_wire with a diagonal scaling for the shift (no
+// per-solve inversion) does as well there (43 / 44) but not when the shift is comparable to diag(M) (single wire of
+// 32 x 32 cells under a fast field ramp, shift / diag(M) up to 3: 165 iterations against 50), so the inverse is exact.
+__device__ __forceinline__ int patch_pm_index(const PatchPrec& pc, int pch) {
+  return (pch / (pc.per_layer * pc.per * pc.per)) * pc.per + (pch / pc.per) % pc.per;   // (layer, radial slot)
+}
+__global__ void __launch_bounds__(1024) patch_invert_big_kernel(PatchPrec pc, const double* __restrict__ shift) {
+  __shared__ double rowk[kWireMax], colk[kWireMax];
+  __shared__ double part[32];
+  const int pp = pc.pp, pch = blockIdx.x, nthr = blockDim.x;
+  const double* src = pc.Pm + static_cast<size_t>(patch_pm_index(pc, pch)) * pp * pp;
+  double* A = pc.Pinv + static_cast<size_t>(pch) * pp * pp;
+  const int* idx = pc.pidx + static_cast<size_t>(pch) * pp;
+  for (int e = threadIdx.x; e < pp * pp; e += nthr) {
+    const int i = e / pp, u = e - i * pp;
+    A[e] = src[e] + (i == u ? shift[idx[i]] : 0.0);
+  }
+  __syncthreads();
+  for (int k = 0; k < pp; ++k) {
+    for (int u = threadIdx.x; u < pp; u += nthr) rowk[u] = A[k * pp + u], colk[u] = A[u * pp + k];
+    __syncthreads();
+    const double piv = 1.0 / rowk[k];
+    for (int e = threadIdx.x; e < pp * pp; e += nthr) {
+      const int i = e / pp, u = e - i * pp;
+      double v;
+      if (i == k) v = (u == k) ? piv : rowk[u] * piv;
+      else if (u == k) v = -colk[i] * piv;
+      else v = fma(-colk[i] * piv, rowk[u], A[e]);
+      A[e] = v;
+    }
+    __syncthreads();
+  }
+  for (int e = threadIdx.x; e < pp * pp; e += nthr) {             // symmetrise (rounding-level asymmetry of the elimination)
+    const int i = e / pp, u = e - i * pp;
+    if (u > i) {
+      const double v = 0.5 * (A[e] + A[u * pp + i]);
+      A[e] = v;
+      A[u * pp + i] = v;
+    }
+  }
+  __syncthreads();
+  // h1 = Pinv 1 (one warp per row), s_w += sum h1
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = nthr >> 5;
+  double tot = 0.0;
+  for (int i = warp; i < pp; i += nwarps) {
+    double hs = 0.0;
+    for (int u = lane; u < pp; u += 32) hs += A[i * pp + u];
+    hs = warp_sum(hs);
+    if (lane == 0) pc.h1[idx[i]] = hs, tot += hs;
+  }
+  if (lane == 0) part[warp] = tot;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double ssum = 0.0;
+    for (int k = 0; k < nwarps; ++k) ssum += part[k];
+    atomicAdd(pc.sw + pc.pturn[pch], ssum);
   }
 }
 
@@ -693,10 +762,11 @@ void k_cg_Ap(const VecCtx& v, const CgIter& it) {
   QS_LAUNCH(v);
   cg_Ap_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.sc);
 }
+static int patch_threads(const PatchPrec& pc) { return pc.big ? (pc.pp + 31) / 32 * 32 : kPatchMax; }
 void k_cg_update(const VecCtx& v, const CgIter& it) {
   QS_LAUNCH(v);
   if (it.patch.pp > 0) {   // patch preconditioner: update fused with t = Pinv r
-    patch_apply_kernel<true><<<it.patch.n_patches, kPatchMax, 0, v.stream>>>(it.patch.pp, it.patch.pidx, it.patch.pturn,
+    patch_apply_kernel<true><<<it.patch.n_patches, patch_threads(it.patch), 0, v.stream>>>(it.patch.pp, it.patch.pidx, it.patch.pturn,
                                                                            it.patch.Pinv, it, v.sc);
     return;
   }
@@ -705,7 +775,12 @@ void k_cg_update(const VecCtx& v, const CgIter& it) {
 void k_patch_build(const VecCtx& v, const PatchPrec& pc, const double* r, const double* z, double soft_all,
                    double soft_self) {
   QS_LAUNCH(v);
-  patch_build_kernel<<<pc.n_patches, kPatchMax, 0, v.stream>>>(pc.pp, pc.pidx, r, z, soft_all, soft_self, pc.Pm);
+  if (pc.big) {   // one matrix per (layer, radial slot)
+    patch_build_kernel<<<pc.layers * pc.per, patch_threads(pc), 0, v.stream>>>(pc.pp, pc.per, pc.per_layer, pc.pidx, r, z,
+                                                                              soft_all, soft_self, pc.Pm);
+    return;
+  }
+  patch_build_kernel<<<pc.n_patches, kPatchMax, 0, v.stream>>>(pc.pp, 0, 0, pc.pidx, r, z, soft_all, soft_self, pc.Pm);
 }
 // start of a solve in patch mode: Pinv for this shift, then the block projection of the current (refined) residual
 void k_patch_start(const VecCtx& v, const CgIter& it, const double* shift) {
@@ -714,9 +789,10 @@ void k_patch_start(const VecCtx& v, const CgIter& it, const double* shift) {
   cudaMemsetAsync(&v.sc->rg[0], 0, sizeof(double), v.stream);
   cudaMemsetAsync(&v.sc->rd[0], 0, 2 * sizeof(double), v.stream);
   QS_LAUNCH(v);
-  patch_invert_kernel<<<pc.n_patches, kPatchMax * kPinvSplit, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pm, shift, pc.Pinv, pc.h1, pc.sw);
+  if (pc.big) patch_invert_big_kernel<<<pc.n_patches, 1024, 0, v.stream>>>(pc, shift);
+  else patch_invert_kernel<<<pc.n_patches, kPatchMax * kPinvSplit, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pm, shift, pc.Pinv, pc.h1, pc.sw);
   QS_LAUNCH(v);
-  patch_apply_kernel<false><<<pc.n_patches, kPatchMax, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pinv, it, v.sc);
+  patch_apply_kernel<false><<<pc.n_patches, patch_threads(pc), 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pinv, it, v.sc);
   QS_LAUNCH(v);
   patch_project_kernel<true><<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.turn_id, pc.h1, v.sc);
   QS_LAUNCH(v);

@@ -294,6 +294,36 @@ def test_patch_preconditioner_changes_iterations_not_the_solution(pkg):
     assert 0 < res[True][2] < res[False][2]
 
 
+def test_whole_wire_patches_of_the_preconditioner(pkg):
+    # wires of 12 x 12 (config 3) and 16 x 16 (config 2) cells: the patch is the whole wire (inverted per solve in global
+    # memory, the constant part shared per layer) against the sub-wire patches of at most 8 x 8 cells
+    # (QS_GEO_PATCH_SUBWIRE) and the diagonal (QS_GEO_NO_PATCH_PRECOND), on a trajectory ramped fast enough that the
+    # surface cells of the wires sit at Jc (C13): same states and terminal voltage (C8: the preconditioner is
+    # free), and about half the iterations of the sub-wire patches; last a single wire of 32 x 32 cells in a fast field
+    # ramp (16 x 16 patches against 8 x 8: four matrices for the four radial slots and z-translates of each)
+    cases = [(wl.shrunk(3, 2, 3), 200.0, 0.0, 0.75), (wl.shrunk(2, 2, 2), 100.0, 0.0, 0.75), (wl.shrunk(1, 1, 1, 32), 1.0, 20.0, 0.9)]
+    for w, rampx, bext_rate, gain in cases:
+        geo = dataclasses.replace(w.geometry, Bext_rate=bext_rate) if bext_rate else w.geometry
+        mat = dataclasses.replace(w.material, cg_tol=1e-12)
+        res = {}
+        for mode, kw in (("whole", {}), ("sub", dict(patch_subwire=True)), ("diag", dict(patch_precond=False))):
+            its = 0
+            with pkg.QS(geo, mat, **kw) as sim:
+                for k in range(130):
+                    assert sim.step(w.dt, w.I_ramp * rampx) >= 0
+                    if k >= 110:
+                        its += sim.stats()["cg_iters"]
+                res[mode] = (sim.read(), sim.stats()["U_terminal"], its)
+        J = res["diag"][0][0]
+        assert np.abs(J).max() > 1e9                              # the nonlinear regime was reached
+        for mode in ("whole", "sub"):
+            for u, v in zip(res[mode][0], res["diag"][0]):
+                assert rel(u, v) <= 1e-8 or np.linalg.norm(v) < 1e-30
+            assert abs(res[mode][1] - res["diag"][1]) <= 1e-8 * abs(res["diag"][1]) + 1e-20
+        print("cg iterations over 20 steps (p <= 16, p <= 8, diagonal):", res["whole"][2], res["sub"][2], res["diag"][2])
+        assert 0 < res["whole"][2] < gain * res["sub"][2] < res["diag"][2], (res["whole"][2], res["sub"][2], res["diag"][2])
+
+
 def test_handle_works_while_another_device_or_stream_context_is_current(pkg):
     # a handle remembers its device: calls are valid whatever device is current in the calling thread (one GPU here:
     # the guard must at least be a no-op; with two visible devices the second one is made current around the calls)

@@ -499,10 +499,9 @@ __global__ void __launch_bounds__(kWireMax) patch_apply_kernel(int pp, const int
 }
 
 // ---- patches of more than 64 cells (p = 9..16: whole wires of configs 2 and 3, 16 x 16 sub-wire patches of config 1) ----
-// A 256 x 256 block does not fit shared memory, so the per-solve inverse is formed by the same Gauss-Jordan elimination
-// IN GLOBAL MEMORY (the block stays in L2 while its CTA of 1024 threads works on it: ~0.05-0.2 ms per block, a few
-// blocks per SM, ~1 ms per solve at config 3).  The constant part is shared: patches in the same layer and radial slot
-// of their wire are translates of each other along z, so Pm holds one matrix per (layer, radial slot).
+// A 256 x 256 block does not fit shared memory, so the per-solve inverse is formed by a Gauss-Jordan elimination IN GLOBAL
+// MEMORY (the block stays in L2 while its CTA works on it).  The constant part is shared: patches in the same layer and
+// radial slot of their wire are translates of each other along z, so Pm holds one matrix per (layer, radial slot).
 // Why whole wires: measured on the host on mid-trajectory systems of shrunk configs 2 / 3 with the surface cells at Jc
 // (warm start), 2 x 2 ... 8 x 8 sub-wire patches all need 87-97 iterations, the whole wire 41 / 44: only the full block
 // carries the wire's screening-current modes.  A fixed inverse of M_wire with a diagonal scaling for the shift (no
@@ -511,29 +510,115 @@ __global__ void __launch_bounds__(kWireMax) patch_apply_kernel(int pp, const int
 __device__ __forceinline__ int patch_pm_index(const PatchPrec& pc, int pch) {
   return (pch / (pc.per_layer * pc.per * pc.per)) * pc.per + (pch / pc.per) % pc.per;   // (layer, radial slot)
 }
-__global__ void __launch_bounds__(1024) patch_invert_big_kernel(PatchPrec pc, const double* __restrict__ shift) {
-  __shared__ double rowk[kWireMax], colk[kWireMax];
-  __shared__ double part[32];
-  const int pp = pc.pp, pch = blockIdx.x, nthr = blockDim.x;
+// BLOCKED elimination with block size p (the wire side: pp = p blocks of p): per block step K the pivot block is inverted
+// in shared memory, the row panel P^-1 A[K, :] and the column panel A[:, K] are staged in shared memory, and every
+// other element takes ONE rank-p update from them (4 x 4 register tiles), so the block is read and written p times
+// instead of p^2 times (element-wise elimination in global memory: 45 ms per solve at config 2, L2-bandwidth bound):
+//   A[K,K] <- P^-1;  A[K,j] <- P^-1 A[K,j];  A[i,j] <- A[i,j] - A[i,K] (P^-1 A[K,j]);  A[i,K] <- -A[i,K] P^-1   (i, j != K)
+constexpr int kBigThreads = 512;
+__host__ __device__ inline int big_ldr(int pp) { return (pp + 3) / 4 * 4; }
+static size_t big_invert_smem(int p) {
+  const int pp = p * p, ldr = big_ldr(pp);
+  return sizeof(double) * (static_cast<size_t>(p) * (p + 1) + static_cast<size_t>(p) * ldr + static_cast<size_t>(ldr) * (p + 1));
+}
+__global__ void __launch_bounds__(kBigThreads, 2) patch_invert_big_kernel(PatchPrec pc, int p, const double* __restrict__ shift) {
+  extern __shared__ __align__(16) double bsm[];
+  __shared__ double part[kBigThreads / 32];
+  const int pp = pc.pp, pch = blockIdx.x, nthr = blockDim.x, tid = threadIdx.x;
+  const int ldr = big_ldr(pp), ldc = p + 1;
+  double* Pb = bsm;                    // [p][p + 1]   pivot block, then its inverse
+  double* R = Pb + p * (p + 1);        // [p][ldr]     row panel (columns past pp: zero)
+  double* Cp = R + p * ldr;            // [ldr][p + 1] column panel (rows past pp: zero)
   const double* src = pc.Pm + static_cast<size_t>(patch_pm_index(pc, pch)) * pp * pp;
   double* A = pc.Pinv + static_cast<size_t>(pch) * pp * pp;
   const int* idx = pc.pidx + static_cast<size_t>(pch) * pp;
-  for (int e = threadIdx.x; e < pp * pp; e += nthr) {
+  for (int e = tid; e < pp * pp; e += nthr) {                      // A = M_patch + diag(shift)
     const int i = e / pp, u = e - i * pp;
     A[e] = src[e] + (i == u ? shift[idx[i]] : 0.0);
   }
+  for (int e = tid; e < p * ldr; e += nthr) R[e] = 0.0;
+  for (int e = tid; e < ldr * ldc; e += nthr) Cp[e] = 0.0;
   __syncthreads();
-  for (int k = 0; k < pp; ++k) {
-    for (int u = threadIdx.x; u < pp; u += nthr) rowk[u] = A[k * pp + u], colk[u] = A[u * pp + k];
+  const int ri = tid / p, ci = tid % p;                            // element of the pivot block (tid < p * p)
+  const bool inP = tid < p * p;
+  const int ntile = ldr / 4;
+  for (int K = 0; K < p; ++K) {
+    const int k0 = K * p;
+    if (inP) Pb[ri * ldc + ci] = A[(k0 + ri) * pp + k0 + ci];
+    for (int e = tid; e < p * pp; e += nthr) {
+      const int m = e / pp, j = e - m * pp;
+      R[m * ldr + j] = A[(k0 + m) * pp + j];
+    }
+    for (int e = tid; e < pp * p; e += nthr) {
+      const int i = e / p, m = e - i * p;
+      Cp[i * ldc + m] = A[i * pp + k0 + m];
+    }
     __syncthreads();
-    const double piv = 1.0 / rowk[k];
-    for (int e = threadIdx.x; e < pp * pp; e += nthr) {
-      const int i = e / pp, u = e - i * pp;
-      double v;
-      if (i == k) v = (u == k) ? piv : rowk[u] * piv;
-      else if (u == k) v = -colk[i] * piv;
-      else v = fma(-colk[i] * piv, rowk[u], A[e]);
-      A[e] = v;
+    for (int k = 0; k < p; ++k) {                                  // pivot block: element-wise elimination in shared memory
+      double v = 0.0;
+      if (inP) {
+        const double piv = 1.0 / Pb[k * ldc + k];
+        const double f = Pb[ri * ldc + k], rv = Pb[k * ldc + ci];
+        if (ri == k) v = (ci == k) ? piv : rv * piv;
+        else if (ci == k) v = -f * piv;
+        else v = fma(-f * piv, rv, Pb[ri * ldc + ci]);
+      }
+      __syncthreads();
+      if (inP) Pb[ri * ldc + ci] = v;
+      __syncthreads();
+    }
+    if (tid < pp) {                                                // row panel in place, one column per thread
+      const int j = tid;
+      if (j >= k0 && j < k0 + p) {
+        for (int m = 0; m < p; ++m) R[m * ldr + j] = Pb[m * ldc + (j - k0)];
+      } else {
+        double col[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) col[q] = q < p ? R[q * ldr + j] : 0.0;
+        for (int m = 0; m < p; ++m) {
+          double acc = 0.0;
+#pragma unroll
+          for (int q = 0; q < 16; ++q)
+            if (q < p) acc = fma(Pb[m * ldc + q], col[q], acc);
+          R[m * ldr + j] = acc;
+        }
+      }
+    }
+    __syncthreads();
+    for (int tile = tid; tile < ntile * ntile; tile += nthr) {     // rank-p update, 4 x 4 elements per tile
+      const int i0 = (tile / ntile) * 4, j0 = (tile % ntile) * 4;
+      double acc[4][4];
+#pragma unroll
+      for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) acc[a][b] = 0.0;
+      for (int m = 0; m < p; ++m) {
+        const double2 r01 = *reinterpret_cast<const double2*>(R + m * ldr + j0);
+        const double2 r23 = *reinterpret_cast<const double2*>(R + m * ldr + j0 + 2);
+        const double rr[4] = {r01.x, r01.y, r23.x, r23.y};
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+          const double c = Cp[(i0 + a) * ldc + m];
+#pragma unroll
+          for (int b = 0; b < 4; ++b) acc[a][b] = fma(c, rr[b], acc[a][b]);
+        }
+      }
+#pragma unroll
+      for (int a = 0; a < 4; ++a) {
+        const int i = i0 + a;
+        if (i >= pp) continue;
+        const bool rowK = i >= k0 && i < k0 + p;
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+          const int j = j0 + b;
+          if (j >= pp) continue;
+          const bool colK = j >= k0 && j < k0 + p;
+          double v;
+          if (rowK) v = R[(i - k0) * ldr + j];
+          else v = (colK ? 0.0 : A[i * pp + j]) - acc[a][b];
+          A[i * pp + j] = v;
+        }
+      }
     }
     __syncthreads();
   }
@@ -789,7 +874,12 @@ void k_patch_start(const VecCtx& v, const CgIter& it, const double* shift) {
   cudaMemsetAsync(&v.sc->rg[0], 0, sizeof(double), v.stream);
   cudaMemsetAsync(&v.sc->rd[0], 0, 2 * sizeof(double), v.stream);
   QS_LAUNCH(v);
-  if (pc.big) patch_invert_big_kernel<<<pc.n_patches, 1024, 0, v.stream>>>(pc, shift);
+  if (pc.big) {
+    const int p = static_cast<int>(std::lround(std::sqrt(static_cast<double>(pc.pp))));
+    const size_t smem = big_invert_smem(p);
+    cudaFuncSetAttribute(patch_invert_big_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    patch_invert_big_kernel<<<pc.n_patches, kBigThreads, smem, v.stream>>>(pc, p, shift);
+  }
   else patch_invert_kernel<<<pc.n_patches, kPatchMax * kPinvSplit, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pm, shift, pc.Pinv, pc.h1, pc.sw);
   QS_LAUNCH(v);
   patch_apply_kernel<false><<<pc.n_patches, patch_threads(pc), 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pinv, it, v.sc);

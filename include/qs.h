@@ -72,9 +72,9 @@ typedef struct qs_ctx qs_ctx;
                                     workspace); the solver then keeps diag(A) (C8).
                                     The preconditioner is free: the solution of a step is unique (C4).  */
 
-#define QS_GEO_PATCH_SUBWIRE 16   /* keep the patches of the constraint preconditioner at p <= 8 (inverted in shared
-                                    memory) instead of p <= 16 (whole wires of up to 16 x 16 cells; inverted per solve
-                                    in global memory); either is a preconditioner only (C8).  */
+#define QS_GEO_PATCH_SUBWIRE 16   /* constraint preconditioner: plain patches of p x p cells, p <= 8, only - no whole-wire
+                                    blocks (wires of up to 16 x 16 cells) and no second level of patch-wise constants
+                                    (larger wires); a preconditioner only either way (C8).  */
 
 #define QS_GEO_HEAT_BLOCKED 8     /* measurement: use the temporally blocked heat kernel (<= 4 explicit sub-steps per
                                     launch from a shared-memory tile with a 4-cell halo) at ANY lattice size; by

@@ -194,6 +194,7 @@ struct qs_ctx {
   PatchPrec patch;                   // patch preconditioner of the lattice solves (pp = 0: off)
   int* pidx = nullptr;               // [N] patch slot -> cell
   int* pturn = nullptr;              // [N / pp] patch -> constraint group
+  int* pid = nullptr;                // [N] cell -> patch (second level of the patch preconditioner)
   Scalars* sc;
   Scalars* h_sc = nullptr;           // pinned
   double* h_stage = nullptr;         // pinned staging, 2N doubles
@@ -288,6 +289,14 @@ void carve(qs_ctx* c, void* base, size_t* total) {
     c->pturn = k.take<int>(N / pp);
     c->patch.Pm = k.take<double>(c->patch.big ? static_cast<size_t>(c->patch.layers) * c->patch.per * pp * pp : N * pp);
     c->patch.Pinv = k.take<double>(N * pp);
+    if (c->patch.nc > 0) {
+      const size_t nc = c->patch.nc;
+      c->patch.C0m = k.take<double>(static_cast<size_t>(c->patch.layers) * nc * nc);
+      c->patch.C0inv = k.take<double>(static_cast<size_t>(nt) * nc * nc);
+      c->patch.rc = k.take<double>(N / pp);
+      c->patch.yc = k.take<double>(N / pp);
+      c->pid = k.take<int>(N);
+    }
     c->patch.h1 = k.take<double>(N);
     c->patch.sw = k.take<double>(nt);
   }
@@ -348,6 +357,8 @@ void patch_setup(PatchPrec* pc, const qs_geometry* g, int N) {
   pc->n_patches = ps ? N / (ps * ps) : 0;
   pc->big = ps > 8;
   pc->per = ps ? g->cells_per_side / ps : 1;
+  // second level for wires of several patches (at most 64 patches per wire), unless the plain patches are asked for
+  pc->nc = (ps && pc->per > 1 && pc->per * pc->per <= 64 && !(g->flags & QS_GEO_PATCH_SUBWIRE)) ? pc->per * pc->per : 0;
   pc->layers = g->layers;
   pc->per_layer = g->turns_per_layer;
 }
@@ -1230,6 +1241,15 @@ int init_common(const qs_geometry* geo, const qs_material* mat, void* workspace,
         return bail(fail(QS_ERR_CUDA, "upload of the patch tables failed"));
       c->patch.pidx = c->pidx;
       c->patch.pturn = c->pturn;
+      if (c->patch.nc > 0) {
+        std::vector<int> hpid(N);
+        for (int q = 0; q < c->patch.n_patches; ++q)
+          for (int t = 0; t < pp; ++t) hpid[hidx[q * pp + t]] = q;
+        if (cudaMemcpyAsync(c->pid, hpid.data(), sizeof(int) * N, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+            cudaStreamSynchronize(c->stream) != cudaSuccess)
+          return bail(fail(QS_ERR_CUDA, "upload of the patch tables failed"));
+        c->patch.pid = c->pid;
+      }
       k_patch_build(v, c->patch, c->r, c->z, c->soft_all, c->soft_self);
     }
     if (c->n_turns) {

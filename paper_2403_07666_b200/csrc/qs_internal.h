@@ -113,7 +113,15 @@ struct PatchPrec {
   const int* pturn = nullptr;   // [n_patches] constraint group of the patch
   double* Pm = nullptr;         // [n_patches][pp][pp] constant part M_patch [H]   (big: [layers * per][pp][pp])
   double* Pinv = nullptr;       // [n_patches][pp][pp] (M_patch + diag(shift))^-1 of the current solve
-  double* h1 = nullptr;         // [N] Pinv 1
+  // second level (wires larger than one patch): piecewise constants per patch, H^-1 = B + Z C Z^T with B the patch
+  // inverses, Z the patch indicators and C = blockdiag over wires of (Z_w^T (M + shift) Z_w)^-1
+  int nc = 0;                   // coarse unknowns per wire = per * per (0: no second level)
+  double* C0m = nullptr;        // [layers][nc][nc] constant part Z^T M Z of a wire of the layer [H]
+  double* C0inv = nullptr;      // [n_turns][nc][nc] coarse inverses of the current solve
+  double* rc = nullptr;         // [n_patches] restricted residual Z^T r
+  double* yc = nullptr;         // [n_patches] coarse correction C Z^T r
+  const int* pid = nullptr;     // [N] cell -> patch
+  double* h1 = nullptr;         // [N] H^-1 1
   double* sw = nullptr;         // [n_turns] per-turn Schur scalars sum h1
 };
 struct CgIter {

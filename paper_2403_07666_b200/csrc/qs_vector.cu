@@ -495,8 +495,128 @@ __global__ void __launch_bounds__(kWireMax) patch_apply_kernel(int pp, const int
     double s = 0.0;
     for (int k = 0; k < (pp + 31) / 32; ++k) s += part[k];
     atomicAdd(it.tw + pturn[pch], s);
+    if (it.patch.nc > 0) {             // second level: restricted residual of this patch
+      double rsum = 0.0;
+      for (int u = 0; u < pp; ++u) rsum += rs[u];
+      it.patch.rc[pch] = rsum;
+    }
   }
 }
+
+// ---- second level: piecewise constants per patch (wires larger than one patch: config 1) -----------------------------
+// Host experiment (single wire of 32 x 32 cells in a fast field ramp, surface at Jc, warm start): 8 x 8 patches alone 85
+// iterations, 16 x 16 patches 50, 8 x 8 patches + this coarse space 45 (4 x 4 + coarse: 46): what the patches miss are
+// the wire-scale screening-current modes, and patch-wise constants carry them.
+// once per qs_init: C0m[layer][P][Q] = sum_{i in P, j in Q} M_ij on the first wire of the layer, one CTA per (layer, P, Q)
+__global__ void __launch_bounds__(kPatchMax) coarse_build_kernel(PatchPrec pc, const double* __restrict__ r,
+                                                                const double* __restrict__ z, double soft_all,
+                                                                double soft_self) {
+  __shared__ double part[kPatchMax / 32];
+  const int nc = pc.nc, pp = pc.pp, t = threadIdx.x;
+  const int Q = blockIdx.x % nc, P = (blockIdx.x / nc) % nc, layer = blockIdx.x / (nc * nc);
+  const int w0 = layer * pc.per_layer;                            // first wire of the layer
+  const int* iP = pc.pidx + (static_cast<size_t>(w0) * nc + P) * pp;
+  const int* iQ = pc.pidx + (static_cast<size_t>(w0) * nc + Q) * pp;
+  double acc = 0.0;
+  if (t < pp) {
+    const int i = iP[t];
+    const double ri = r[i], zi = z[i];
+    for (int u = 0; u < pp; ++u) {
+      const int j = iQ[u];
+      const double rj = r[j], dz = zi - z[j];
+      const double dz2 = fma(dz, dz, soft_all) + (i == j ? soft_self : 0.0);
+      const double dif = ri - rj;
+      const double B2 = fma(dif, dif, dz2), A2 = fma(4.0 * ri, rj, B2);
+      const PairAGM a = agm_pair<7, 2, false>(A2, B2);
+      acc += (0.5 * kMu0 * kPi) * a.S * a.yinf;
+    }
+  }
+  acc = warp_sum(acc);
+  if ((t & 31) == 0) part[t >> 5] = acc;
+  __syncthreads();
+  if (t == 0) {
+    double s = 0.0;
+    for (int k = 0; k < static_cast<int>(blockDim.x >> 5); ++k) s += part[k];
+    pc.C0m[blockIdx.x] = s;
+  }
+}
+
+// per solve, after the patch inverses: C0inv[w] = (C0m[layer] + diag(sum of the shift over each patch))^-1 by the same
+// elimination in shared memory; h1 += Z C Z^T 1, s_w += its sum.  One CTA per wire, one thread per coarse unknown.
+__global__ void __launch_bounds__(kPatchMax) coarse_invert_kernel(PatchPrec pc, const double* __restrict__ shift) {
+  __shared__ double A[kPatchMax][kPatchMax + 1];
+  __shared__ double hc[kPatchMax];
+  const int nc = pc.nc, pp = pc.pp, w = blockIdx.x, t = threadIdx.x;
+  const bool act = t < nc;
+  const double* src = pc.C0m + static_cast<size_t>(w / pc.per_layer) * nc * nc;
+  for (int e = t; e < nc * nc; e += blockDim.x) A[e / nc][e % nc] = src[e];
+  __syncthreads();
+  if (act) {
+    const int* idx = pc.pidx + (static_cast<size_t>(w) * nc + t) * pp;
+    double ssum = 0.0;
+    for (int u = 0; u < pp; ++u) ssum += shift[idx[u]];
+    A[t][t] += ssum;
+  }
+  __syncthreads();
+  for (int k = 0; k < nc; ++k) {
+    const double piv = 1.0 / A[k][k];
+    const double f = act ? A[t][k] : 0.0;
+    __syncthreads();
+    if (act && t == k)
+      for (int u = 0; u < nc; ++u) A[k][u] = (u == k) ? piv : A[k][u] * piv;
+    __syncthreads();
+    if (act && t != k)
+      for (int u = 0; u < nc; ++u) A[t][u] = (u == k) ? -f * piv : fma(-f, A[k][u], A[t][u]);
+    __syncthreads();
+  }
+  double h = 0.0;
+  if (act) {
+    double* row = pc.C0inv + (static_cast<size_t>(w) * nc + t) * nc;
+    for (int u = 0; u < nc; ++u) {
+      const double v = 0.5 * (A[t][u] + A[u][t]);                 // symmetrised on the way out
+      row[u] = v;
+      h += v;
+    }
+    h *= pp;                                                       // (C Z^T 1)_t : Z^T 1 = pp on every patch
+    hc[t] = h;
+  }
+  __syncthreads();
+  for (int e = t; e < nc * pp; e += blockDim.x) {                  // h1 += Z hc over the cells of the wire
+    const int c = e / pp;
+    pc.h1[pc.pidx[(static_cast<size_t>(w) * nc + c) * pp + (e - c * pp)]] += hc[c];
+  }
+  if (t == 0) {
+    double s = 0.0;
+    for (int c = 0; c < nc; ++c) s += hc[c];
+    atomicAdd(pc.sw + w, s * pp);
+  }
+}
+
+// per iteration, after the patch products: yc = C0inv (Z^T r) per wire, tw[w] += sum of Z yc
+template <bool UPDATE>
+__global__ void __launch_bounds__(kPatchMax) coarse_apply_kernel(PatchPrec pc, double* __restrict__ tw, Scalars* sc) {
+  __shared__ double rs[kPatchMax];
+  __shared__ double part[kPatchMax / 32];
+  if (UPDATE && sc->done) return;
+  const int nc = pc.nc, w = blockIdx.x, t = threadIdx.x;
+  if (t < nc) rs[t] = pc.rc[static_cast<size_t>(w) * nc + t];
+  __syncthreads();
+  double acc = 0.0;
+  if (t < nc) {
+    const double* col = pc.C0inv + static_cast<size_t>(w) * nc * nc + t;   // symmetric: column t, coalesced
+    for (int u = 0; u < nc; ++u) acc = fma(col[static_cast<size_t>(u) * nc], rs[u], acc);
+    pc.yc[static_cast<size_t>(w) * nc + t] = acc;
+  }
+  acc = warp_sum(acc);
+  if ((t & 31) == 0) part[t >> 5] = acc;
+  __syncthreads();
+  if (t == 0) {
+    double s = 0.0;
+    for (int k = 0; k < static_cast<int>(blockDim.x >> 5); ++k) s += part[k];
+    atomicAdd(tw + w, s * pc.pp);
+  }
+}
+
 
 // ---- patches of more than 64 cells (p = 9..16: whole wires of configs 2 and 3, 16 x 16 sub-wire patches of config 1) ----
 // A 256 x 256 block does not fit shared memory, so the per-solve inverse is formed by a Gauss-Jordan elimination IN GLOBAL
@@ -659,7 +779,8 @@ __global__ void patch_project_kernel(int n, CgIter it, const int* __restrict__ t
     const int w = turn[i];
     const double v = it.tw[w] / it.sw[w];
     const double ri = it.r[i] - v;
-    const double gi = fma(-v, h1[i], it.g[i]);
+    const double ti = it.patch.nc > 0 ? it.g[i] + it.patch.yc[it.patch.pid[i]] : it.g[i];   // t = B r + Z yc
+    const double gi = fma(-v, h1[i], ti);
     it.r[i] = ri;
     it.g[i] = gi;
     if (FIRST) it.p[i] = -gi;
@@ -853,6 +974,10 @@ void k_cg_update(const VecCtx& v, const CgIter& it) {
   if (it.patch.pp > 0) {   // patch preconditioner: update fused with t = Pinv r
     patch_apply_kernel<true><<<it.patch.n_patches, patch_threads(it.patch), 0, v.stream>>>(it.patch.pp, it.patch.pidx, it.patch.pturn,
                                                                            it.patch.Pinv, it, v.sc);
+    if (it.patch.nc > 0) {
+      QS_LAUNCH(v);
+      coarse_apply_kernel<true><<<v.n_turns, kPatchMax, 0, v.stream>>>(it.patch, it.tw, v.sc);
+    }
     return;
   }
   cg_update_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.n_turns ? v.turn_id : nullptr, v.sc);
@@ -866,6 +991,10 @@ void k_patch_build(const VecCtx& v, const PatchPrec& pc, const double* r, const 
     return;
   }
   patch_build_kernel<<<pc.n_patches, kPatchMax, 0, v.stream>>>(pc.pp, 0, 0, pc.pidx, r, z, soft_all, soft_self, pc.Pm);
+  if (pc.nc > 0) {
+    QS_LAUNCH(v);
+    coarse_build_kernel<<<pc.layers * pc.nc * pc.nc, kPatchMax, 0, v.stream>>>(pc, r, z, soft_all, soft_self);
+  }
 }
 // start of a solve in patch mode: Pinv for this shift, then the block projection of the current (refined) residual
 void k_patch_start(const VecCtx& v, const CgIter& it, const double* shift) {
@@ -881,8 +1010,16 @@ void k_patch_start(const VecCtx& v, const CgIter& it, const double* shift) {
     patch_invert_big_kernel<<<pc.n_patches, kBigThreads, smem, v.stream>>>(pc, p, shift);
   }
   else patch_invert_kernel<<<pc.n_patches, kPatchMax * kPinvSplit, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pm, shift, pc.Pinv, pc.h1, pc.sw);
+  if (pc.nc > 0) {
+    QS_LAUNCH(v);
+    coarse_invert_kernel<<<v.n_turns, kPatchMax, 0, v.stream>>>(pc, shift);
+  }
   QS_LAUNCH(v);
   patch_apply_kernel<false><<<pc.n_patches, patch_threads(pc), 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pinv, it, v.sc);
+  if (pc.nc > 0) {
+    QS_LAUNCH(v);
+    coarse_apply_kernel<false><<<v.n_turns, kPatchMax, 0, v.stream>>>(pc, it.tw, v.sc);
+  }
   QS_LAUNCH(v);
   patch_project_kernel<true><<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.turn_id, pc.h1, v.sc);
   QS_LAUNCH(v);

@@ -299,9 +299,12 @@ def test_whole_wire_patches_of_the_preconditioner(pkg):
     # memory, the constant part shared per layer) against the sub-wire patches of at most 8 x 8 cells
     # (QS_GEO_PATCH_SUBWIRE) and the diagonal (QS_GEO_NO_PATCH_PRECOND), on a trajectory ramped fast enough that the
     # surface cells of the wires sit at Jc (C13): same states and terminal voltage (C8: the preconditioner is
-    # free), and about half the iterations of the sub-wire patches; last wires of 10 x 10 cells (a block size that is not
-    # a multiple of the update's 4 x 4 tiles)
-    cases = [(wl.shrunk(3, 2, 3), 200.0, 0.0, 0.75), (wl.shrunk(2, 2, 2), 100.0, 0.0, 0.75), (wl.shrunk(3, 3, 2, 10), 200.0, 0.0, 0.75)]
+    # free), and about half the iterations of the sub-wire patches; wires of 10 x 10 cells (a block size that is not a
+    # multiple of the update's 4 x 4 tiles); last wires larger than a patch, where a second level of patch-wise constants
+    # stands in for the whole-wire block: one wire of 32 x 32 cells in a fast field ramp (16 coarse unknowns) and two
+    # layers of two wires of 24 x 24 cells (9 coarse unknowns per wire, one coarse matrix per layer)
+    cases = [(wl.shrunk(3, 2, 3), 200.0, 0.0, 0.75), (wl.shrunk(2, 2, 2), 100.0, 0.0, 0.75), (wl.shrunk(3, 3, 2, 10), 200.0, 0.0, 0.75),
+             (wl.shrunk(1, 1, 1, 32), 1.0, 20.0, 0.8), (wl.shrunk(3, 2, 2, 24), 200.0, 0.0, 0.8)]
     for w, rampx, bext_rate, gain in cases:
         geo = dataclasses.replace(w.geometry, Bext_rate=bext_rate) if bext_rate else w.geometry
         mat = dataclasses.replace(w.material, cg_tol=1e-12)

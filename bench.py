@@ -11,7 +11,7 @@ largest single-GPU configuration (864,000 rings).  Prints ONE JSON line.
   cpu_baseline  the CPU oracle as it stands, timed on a bounded row sample of the same workload on ALL host cores
                 (a process pool over target rows; rank 0, N = 1)
   operator_cfg4 the config-4 sweep: y = M x and the CG solve at N = 4,096 / 65,536 / 262,144 / 1,048,576
-  cg_active     config 1 (the nonlinear config: ~200 CG iterations per step) next to the headline, whose timed steps
+  cg_active     config 1 (the nonlinear config: ~26 CG iterations per step with the two-level patch preconditioner) next to the headline, whose timed steps
                 are linear-regime steps in which the warm-started CG has nothing left to do
 N > 1: independent replicas (one coil per GPU, different Jc0 seeds), no data-path collective ("replicas only").
 --impl reference: the oracle on the host cores (rank 0 only); no CUDA is touched.
@@ -415,7 +415,7 @@ def operator_leg(torch, pkg, fp64_peak, sizes=(4096, 65536, 262144, 1048576), bu
 
 def cg_active_leg(torch, pkg, steps=50, warm=20):
     """Config 1 (single wire, 64 x 64 cells, ramped background field): the config whose steps really iterate the
-    projected CG (~200 iterations per step: K1 sweeps + K3/K4 vector kernels), timed next to the headline."""
+    projected CG (~26 iterations per step: K1 sweeps + K3/K4 vector kernels), timed next to the headline."""
     w = wl.config(1)
     its = []
     with pkg.QS(w.geometry, w.material) as sim:
@@ -493,7 +493,7 @@ def gpu_arm(args):
         return
 
     sim = pkg.QS(w.geometry, w.material, device=local, lattice_tables=args.operator == "tables")
-    # The very first step of a run solves for I' from a cold start: ~250 CG iterations, each a full K1 sweep (minutes at
+    # The very first step of a run solves for I' from a cold start: ~60 CG iterations, each a full K1 sweep (minutes at
     # 864,000 rings) - a cost of the first step only, the timed steps are steps of the running trajectory.  For the big
     # coils that first step is taken by a second handle with the lattice-tables operator (f1, ~0.2 s per sweep) and the
     # state AND the rate I' are carried over through qs_read / qs_read_rate -> qs_write / qs_write_rate; the W warm-up

@@ -542,81 +542,90 @@ __global__ void __launch_bounds__(kPatchMax) coarse_build_kernel(PatchPrec pc, c
 }
 
 // per solve, after the patch inverses: C0inv[w] = (C0m[layer] + diag(sum of the shift over each patch))^-1 by the same
-// elimination in shared memory; h1 += Z C Z^T 1, s_w += its sum.  One CTA per wire, one thread per coarse unknown.
-__global__ void __launch_bounds__(kPatchMax) coarse_invert_kernel(PatchPrec pc, const double* __restrict__ shift) {
+// elimination in shared memory; h1 += Z C Z^T 1, s_w += its sum.  One CTA per wire, kPinvSplit threads per coarse
+// unknown (each owns every kPinvSplit-th column; a single wire is a single CTA, so the row work is spread).
+__global__ void __launch_bounds__(kPatchMax * kPinvSplit) coarse_invert_kernel(PatchPrec pc, const double* __restrict__ shift) {
   __shared__ double A[kPatchMax][kPatchMax + 1];
   __shared__ double hc[kPatchMax];
-  const int nc = pc.nc, pp = pc.pp, w = blockIdx.x, t = threadIdx.x;
+  const int nc = pc.nc, pp = pc.pp, w = blockIdx.x;
+  const int t = threadIdx.x / kPinvSplit, c = threadIdx.x % kPinvSplit;   // row, column phase
   const bool act = t < nc;
   const double* src = pc.C0m + static_cast<size_t>(w / pc.per_layer) * nc * nc;
-  for (int e = t; e < nc * nc; e += blockDim.x) A[e / nc][e % nc] = src[e];
+  for (int e = threadIdx.x; e < nc * nc; e += blockDim.x) A[e / nc][e % nc] = src[e];
   __syncthreads();
+  double ssum = 0.0;
   if (act) {
     const int* idx = pc.pidx + (static_cast<size_t>(w) * nc + t) * pp;
-    double ssum = 0.0;
-    for (int u = 0; u < pp; ++u) ssum += shift[idx[u]];
-    A[t][t] += ssum;
+    for (int u = c; u < pp; u += kPinvSplit) ssum += shift[idx[u]];
   }
+#pragma unroll
+  for (int o = kPinvSplit / 2; o > 0; o >>= 1) ssum += __shfl_xor_sync(0xffffffffu, ssum, o);
+  if (act && c == 0) A[t][t] += ssum;
   __syncthreads();
   for (int k = 0; k < nc; ++k) {
     const double piv = 1.0 / A[k][k];
     const double f = act ? A[t][k] : 0.0;
     __syncthreads();
     if (act && t == k)
-      for (int u = 0; u < nc; ++u) A[k][u] = (u == k) ? piv : A[k][u] * piv;
+      for (int u = c; u < nc; u += kPinvSplit) A[k][u] = (u == k) ? piv : A[k][u] * piv;
     __syncthreads();
     if (act && t != k)
-      for (int u = 0; u < nc; ++u) A[t][u] = (u == k) ? -f * piv : fma(-f, A[k][u], A[t][u]);
+      for (int u = c; u < nc; u += kPinvSplit) A[t][u] = (u == k) ? -f * piv : fma(-f, A[k][u], A[t][u]);
     __syncthreads();
   }
   double h = 0.0;
   if (act) {
     double* row = pc.C0inv + (static_cast<size_t>(w) * nc + t) * nc;
-    for (int u = 0; u < nc; ++u) {
+    for (int u = c; u < nc; u += kPinvSplit) {
       const double v = 0.5 * (A[t][u] + A[u][t]);                 // symmetrised on the way out
       row[u] = v;
       h += v;
     }
-    h *= pp;                                                       // (C Z^T 1)_t : Z^T 1 = pp on every patch
-    hc[t] = h;
   }
+#pragma unroll
+  for (int o = kPinvSplit / 2; o > 0; o >>= 1) h += __shfl_xor_sync(0xffffffffu, h, o);
+  if (act && c == 0) hc[t] = h * pp;                               // (C Z^T 1)_t : Z^T 1 = pp on every patch
   __syncthreads();
-  for (int e = t; e < nc * pp; e += blockDim.x) {                  // h1 += Z hc over the cells of the wire
-    const int c = e / pp;
-    pc.h1[pc.pidx[(static_cast<size_t>(w) * nc + c) * pp + (e - c * pp)]] += hc[c];
+  for (int e = threadIdx.x; e < nc * pp; e += blockDim.x) {        // h1 += Z hc over the cells of the wire
+    const int q = e / pp;
+    pc.h1[pc.pidx[(static_cast<size_t>(w) * nc + q) * pp + (e - q * pp)]] += hc[q];
   }
-  if (t == 0) {
+  if (threadIdx.x == 0) {
     double s = 0.0;
-    for (int c = 0; c < nc; ++c) s += hc[c];
+    for (int q = 0; q < nc; ++q) s += hc[q];
     atomicAdd(pc.sw + w, s * pp);
   }
 }
 
-// per iteration, after the patch products: yc = C0inv (Z^T r) per wire, tw[w] += sum of Z yc
+// per iteration, after the patch products: yc = C0inv (Z^T r) per wire, tw[w] += sum of Z yc.  kPinvSplit threads per
+// coarse unknown (adjacent lanes, each a quarter of the row product).
 template <bool UPDATE>
-__global__ void __launch_bounds__(kPatchMax) coarse_apply_kernel(PatchPrec pc, double* __restrict__ tw, Scalars* sc) {
+__global__ void __launch_bounds__(kPatchMax * kPinvSplit) coarse_apply_kernel(PatchPrec pc, double* __restrict__ tw, Scalars* sc) {
   __shared__ double rs[kPatchMax];
-  __shared__ double part[kPatchMax / 32];
+  __shared__ double part[kPatchMax * kPinvSplit / 32];
   if (UPDATE && sc->done) return;
-  const int nc = pc.nc, w = blockIdx.x, t = threadIdx.x;
-  if (t < nc) rs[t] = pc.rc[static_cast<size_t>(w) * nc + t];
+  const int nc = pc.nc, w = blockIdx.x;
+  const int t = threadIdx.x / kPinvSplit, c = threadIdx.x % kPinvSplit;
+  if (threadIdx.x < nc) rs[threadIdx.x] = pc.rc[static_cast<size_t>(w) * nc + threadIdx.x];
   __syncthreads();
   double acc = 0.0;
   if (t < nc) {
-    const double* col = pc.C0inv + static_cast<size_t>(w) * nc * nc + t;   // symmetric: column t, coalesced
-    for (int u = 0; u < nc; ++u) acc = fma(col[static_cast<size_t>(u) * nc], rs[u], acc);
-    pc.yc[static_cast<size_t>(w) * nc + t] = acc;
+    const double* row = pc.C0inv + (static_cast<size_t>(w) * nc + t) * nc;
+    for (int u = c; u < nc; u += kPinvSplit) acc = fma(row[u], rs[u], acc);
   }
-  acc = warp_sum(acc);
-  if ((t & 31) == 0) part[t >> 5] = acc;
+#pragma unroll
+  for (int o = kPinvSplit / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (t < nc && c == 0) pc.yc[static_cast<size_t>(w) * nc + t] = acc;
+  double tot = (t < nc && c == 0) ? acc : 0.0;
+  tot = warp_sum(tot);
+  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = tot;
   __syncthreads();
-  if (t == 0) {
+  if (threadIdx.x == 0) {
     double s = 0.0;
     for (int k = 0; k < static_cast<int>(blockDim.x >> 5); ++k) s += part[k];
     atomicAdd(tw + w, s * pc.pp);
   }
 }
-
 
 // ---- patches of more than 64 cells (p = 9..16: whole wires of configs 2 and 3, 16 x 16 sub-wire patches of config 1) ----
 // A 256 x 256 block does not fit shared memory, so the per-solve inverse is formed by a Gauss-Jordan elimination IN GLOBAL
@@ -976,7 +985,7 @@ void k_cg_update(const VecCtx& v, const CgIter& it) {
                                                                            it.patch.Pinv, it, v.sc);
     if (it.patch.nc > 0) {
       QS_LAUNCH(v);
-      coarse_apply_kernel<true><<<v.n_turns, kPatchMax, 0, v.stream>>>(it.patch, it.tw, v.sc);
+      coarse_apply_kernel<true><<<v.n_turns, kPatchMax * kPinvSplit, 0, v.stream>>>(it.patch, it.tw, v.sc);
     }
     return;
   }
@@ -1012,13 +1021,13 @@ void k_patch_start(const VecCtx& v, const CgIter& it, const double* shift) {
   else patch_invert_kernel<<<pc.n_patches, kPatchMax * kPinvSplit, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pm, shift, pc.Pinv, pc.h1, pc.sw);
   if (pc.nc > 0) {
     QS_LAUNCH(v);
-    coarse_invert_kernel<<<v.n_turns, kPatchMax, 0, v.stream>>>(pc, shift);
+    coarse_invert_kernel<<<v.n_turns, kPatchMax * kPinvSplit, 0, v.stream>>>(pc, shift);
   }
   QS_LAUNCH(v);
   patch_apply_kernel<false><<<pc.n_patches, patch_threads(pc), 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pinv, it, v.sc);
   if (pc.nc > 0) {
     QS_LAUNCH(v);
-    coarse_apply_kernel<false><<<v.n_turns, kPatchMax, 0, v.stream>>>(pc, it.tw, v.sc);
+    coarse_apply_kernel<false><<<v.n_turns, kPatchMax * kPinvSplit, 0, v.stream>>>(pc, it.tw, v.sc);
   }
   QS_LAUNCH(v);
   patch_project_kernel<true><<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.turn_id, pc.h1, v.sc);

@@ -8,6 +8,7 @@
 //      algorithmic traffic is read H, Q + write H = 24 B per cell per sub-step.
 //   K7 one warp per turn over the CSR cell list: Tmax, mean|E|, max|J|/Jc, min rho/rho_n -> flags (C10).
 #include <algorithm>
+#include <cooperative_groups.h>
 
 #include "qs_internal.h"
 #include "qs_pair.cuh"
@@ -588,6 +589,101 @@ __global__ void __launch_bounds__(kHeatSmallThreads, 1) heat_small_kernel(Materi
   }
 }
 
+// ---- K6, cluster variant of the in-SM kernel: the same "all m sub-steps in one launch", spread over a thread-block
+// CLUSTER of 8 CTAs (8 SMs instead of one: the single-CTA kernel is FP64-bound on its SM, 2 us per sub-step at config 1).
+// CTA c owns a band of rows_per rows; T^2 of its band lives in its shared memory in two buffers (sub-step parity), the
+// rows just above and below the band are read from the neighbour CTAs' shared memory (DSMEM), and ONE cluster barrier
+// per sub-step separates "publish" from "read": a CTA overwrites buffer b again only two sub-steps later, after a
+// barrier that every reader of b has passed.  Same arithmetic per cell, in the same order, as heat_small_kernel.
+constexpr int kHeatClusterCtas = 8;
+constexpr int kHeatClusterThreads = 512;
+constexpr int kHeatClusterPer = 2;                                  // cells per thread: bands of <= 1024 cells
+
+__global__ void __launch_bounds__(kHeatClusterThreads, 1) heat_cluster_kernel(MaterialParams mp, LatticeParams lp, int m,
+                                                                              int rows_per, const double* __restrict__ Hin,
+                                                                              const double* __restrict__ Q,
+                                                                              double* __restrict__ Hout, double dtsub) {
+  extern __shared__ __align__(16) double hc_smem[];
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  const int rank = static_cast<int>(cluster.block_rank());
+  const int Nz = lp.Nz, Nr = lp.Nr;
+  const int band = rows_per * Nz;                                   // cells of a full band (buffer stride)
+  const int r0 = rank * rows_per, r1 = min(r0 + rows_per, Nr);      // this CTA's rows [r0, r1): may be empty
+  const int cells = max(r1 - r0, 0) * Nz;
+  double* U[2] = {hc_smem, hc_smem + band};                         // T^2 of the band, by sub-step parity
+  double* crp = hc_smem + 2 * band;                                 // per-row coefficients of the band x 3, per-column x 3
+  double* crm = crp + rows_per;
+  double* crb = crm + rows_per;
+  double* czp = crb + rows_per;
+  double* czm = czp + Nz;
+  double* czb = czm + Nz;
+  for (int i = threadIdx.x; i < r1 - r0; i += blockDim.x)
+    crp[i] = lp.hr_p[r0 + i], crm[i] = lp.hr_m[r0 + i], crb[i] = lp.rb_r[r0 + i];
+  for (int i = threadIdx.x; i < Nz; i += blockDim.x) czp[i] = lp.hz_p[i], czm[i] = lp.hz_m[i], czb[i] = lp.rb_z[i];
+  // the neighbours' buffers: the band above ends with row r0 - 1 (its last row), the band below starts with row r1
+  const bool has_up = r0 > 0 && cells > 0, has_dn = r1 < Nr && cells > 0;
+  const double* Uup[2] = {nullptr, nullptr};
+  const double* Udn[2] = {nullptr, nullptr};
+  if (has_up) {
+    double* base = cluster.map_shared_rank(hc_smem, rank - 1);
+    Uup[0] = base + (rows_per - 1) * Nz, Uup[1] = base + band + (rows_per - 1) * Nz;
+  }
+  if (has_dn) {
+    double* base = cluster.map_shared_rank(hc_smem, rank + 1);
+    Udn[0] = base, Udn[1] = base + band;
+  }
+  const double C3 = mp.C3, qC1sq = 0.25 * mp.C1 * mp.C1, hC1 = 0.5 * mp.C1, inv_hC3 = 2.0 / mp.C3;
+  double H[kHeatClusterPer], q[kHeatClusterPer];
+  int lr[kHeatClusterPer], iz[kHeatClusterPer];
+#pragma unroll
+  for (int k = 0; k < kHeatClusterPer; ++k) {
+    const int i = threadIdx.x + k * kHeatClusterThreads;
+    H[k] = q[k] = 0.0;
+    lr[k] = iz[k] = 0;
+    if (i < cells) {
+      lr[k] = i / Nz, iz[k] = i - lr[k] * Nz;
+      H[k] = Hin[r0 * Nz + i];
+      q[k] = Q[r0 * Nz + i];
+    }
+  }
+  for (int s = 0; s < m; ++s) {
+    double* Us = U[s & 1];
+#pragma unroll
+    for (int k = 0; k < kHeatClusterPer; ++k) {
+      const int i = threadIdx.x + k * kHeatClusterThreads;
+      if (i < cells) Us[i] = tsq_fast(H[k], C3, qC1sq, hC1, inv_hC3);
+    }
+    cluster.sync();
+#pragma unroll
+    for (int k = 0; k < kHeatClusterPer; ++k) {
+      const int i = threadIdx.x + k * kHeatClusterThreads;
+      if (i < cells) {
+        const double u = Us[i];
+        const int gr = r0 + lr[k];
+        // neighbours outside the pack have coefficient 0: read the cell itself instead
+        double un = u, up = u;
+        if (gr + 1 < Nr) un = gr + 1 < r1 ? Us[i + Nz] : Udn[s & 1][iz[k]];
+        if (gr > 0) up = lr[k] > 0 ? Us[i - Nz] : Uup[s & 1][iz[k]];
+        const double ur = iz[k] + 1 < Nz ? Us[i + 1] : u, ul = iz[k] > 0 ? Us[i - 1] : u;
+        double a = fma(crp[lr[k]], un - u, q[k]);
+        a = fma(crm[lr[k]], up - u, a);
+        a = fma(czp[iz[k]], ur - u, a);
+        a = fma(czm[iz[k]], ul - u, a);
+        const double rb = crb[lr[k]] + czb[iz[k]];
+        if (rb != 0.0) a = fma(-rb, sqrt_fast(u) - lp.T_bath, a);
+        H[k] = fma(dtsub, a, H[k]);
+      }
+    }
+  }
+  cluster.sync();                                                  // nobody leaves while a neighbour may still read its band
+#pragma unroll
+  for (int k = 0; k < kHeatClusterPer; ++k) {
+    const int i = threadIdx.x + k * kHeatClusterThreads;
+    if (i < cells) Hout[r0 * Nz + i] = H[k];
+  }
+}
+
 // ---- K6, temporally blocked variant: up to kHbHalo sub-steps per launch.  A CTA owns a TILE x TILE block of cells,
 // loads it with a halo of kHbHalo cells on every side (H, Q once from HBM / L2), keeps H and Q of its cells in
 // registers and T^2 of the region in shared memory (two buffers, one barrier per sub-step), advances the WHOLE region
@@ -866,6 +962,23 @@ bool k_heat_all_substeps(const VecCtx& v, const MaterialParams& mp, const Lattic
   const long long N = static_cast<long long>(lp.Nr) * lp.Nz;
   if (N > kHeatSmallMax || m < 2) return false;
   QS_LAUNCH(v);
+  const int rows_per = (lp.Nr + kHeatClusterCtas - 1) / kHeatClusterCtas;
+  if (lp.Nr >= 2 * kHeatClusterCtas && rows_per * lp.Nz <= kHeatClusterThreads * kHeatClusterPer) {   // 8 SMs instead of one
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(kHeatClusterCtas);
+    cfg.blockDim = dim3(kHeatClusterThreads);
+    cfg.dynamicSmemBytes = sizeof(double) * (2 * static_cast<size_t>(rows_per) * lp.Nz + 3 * (rows_per + lp.Nz));
+    cfg.stream = v.stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = kHeatClusterCtas;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, heat_cluster_kernel, mp, lp, m, rows_per, Hin, Q, Hout, dtsub) == cudaSuccess) return true;
+    cudaGetLastError();                                            // cluster launch refused: the single-CTA kernel below
+  }
   heat_small_kernel<<<1, kHeatSmallThreads, sizeof(double) * (N + 3 * (lp.Nr + lp.Nz)), v.stream>>>(mp, lp, m, Hin, Q, Hout,
                                                                                                  dtsub);
   return true;

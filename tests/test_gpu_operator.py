@@ -168,7 +168,10 @@ def test_material_law_pointwise(pkg):
         assert rel(got, ref) <= 1e-12, key
 
 
-@pytest.mark.parametrize("shape", [(1, 1, 8), (3, 2, 4), (2, 5, 13), (5, 3, 24)])
+# lattices of <= 4096 cells run all sub-steps in one launch: one CTA below 16 rows ((1, 1, 8), (3, 2, 4)), a cluster of
+# 8 CTAs with DSMEM halo rows from there: 16 rows = 2 per CTA (1, 1, 16), ragged bands with an empty last CTA
+# ((2, 5, 13): 26 rows, (2, 3, 10): 20 rows), configs 0 and 1 ((4, 4, 8), (1, 1, 64)); (5, 3, 24) is the blocked kernel
+@pytest.mark.parametrize("shape", [(1, 1, 8), (3, 2, 4), (2, 5, 13), (5, 3, 24), (1, 1, 16), (2, 3, 10), (4, 4, 8), (1, 1, 64)])
 def test_heat_substeps_pointwise(pkg, shape):
     L, Tn, n = shape
     geo = wl.lattice_geometry(L, Tn, n, 1e-3, 30e-3)

@@ -5,7 +5,8 @@
 //      Jc, rho (C5, C4, C7).
 //   K6 one explicit finite-volume sub-step in enthalpy form (C9; PAPER.md:75 heat equation with Robin borders):
 //      a CTA stages T^2 of its tile plus a one-cell halo in shared memory (one sqrt per staged cell), so the
-//      algorithmic traffic is read H, Q + write H = 24 B per cell per sub-step.
+//      algorithmic traffic is read H, Q + write H = 24 B per cell per sub-step.  Lattices of <= 4096 cells run all
+//      sub-steps of a step in one launch: one CTA, or a thread-block cluster of 8 CTAs with DSMEM halo rows.
 //   K7 one warp per turn over the CSR cell list: Tmax, mean|E|, max|J|/Jc, min rho/rho_n -> flags (C10).
 #include <algorithm>
 #include <cooperative_groups.h>

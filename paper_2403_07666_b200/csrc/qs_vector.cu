@@ -369,6 +369,9 @@ __global__ void step_update_kernel(int n, double dt, const double* __restrict__ 
 // H = blockdiag over square patches of p x p cells inside one wire of (M_patch + diag(shift)); the projection of C8 with
 // a block H:  t = H^-1 r,  s_w = sum_{i in w} (H^-1 1)_i,  v_w = (sum_{i in w} t_i)/s_w,  g = t - v_w H^-1 1,  r <- r - v_w.
 // Patches never straddle a constraint group, so the per-turn Schur complement stays diagonal.
+// Three shapes (qs_api.cu patch_setup): p <= 8 inverted in shared memory (patch_invert_kernel); the whole wire for wires
+// of 9 x 9 to 16 x 16 cells, inverted by a blocked elimination in global memory (patch_invert_big_kernel); and for wires
+// larger than that p <= 8 plus a second level of patch-wise constants per wire (coarse_* kernels).
 constexpr int kPatchMax = 64;   // cells per patch (p <= 8)
 constexpr int kWireMax = 256;   // cells per patch of the big patches (p <= 16: whole wires of up to 16 x 16 cells)
 

@@ -400,15 +400,14 @@ __global__ void __launch_bounds__(kWireMax) patch_build_kernel(int pp, int per, 
 // per solve: Pinv = (M_patch + diag(shift))^-1 by in-place Gauss-Jordan elimination in shared memory (SPD: no pivoting),
 // h1 = Pinv 1, s_w += sum h1.  One CTA per patch, kPinvSplit threads per row (each owns every kPinvSplit-th column).
 constexpr int kPinvSplit = 4;
-__global__ void __launch_bounds__(kPatchMax * kPinvSplit) patch_invert_kernel(int pp, const int* __restrict__ pidx,
-                                                                              const int* __restrict__ pturn,
-                                                                              const double* __restrict__ Pm,
-                                                                              const double* __restrict__ shift,
-                                                                              double* __restrict__ Pinv, double* __restrict__ h1,
-                                                                              double* __restrict__ sw) {
-  __shared__ double A[kPatchMax][kPatchMax + 1];
-  __shared__ double part[kPatchMax * kPinvSplit / 32];
-  const int pch = blockIdx.x, nthr = pp * kPinvSplit;
+// (H1_ATOMIC: h1 is accumulated, not stored - the coarse level of the same launch adds its part in any order)
+template <bool H1_ATOMIC>
+__device__ __forceinline__ void patch_invert_body(double (*A)[kPatchMax + 1], double* part, int pch, int pp,
+                                                  const int* __restrict__ pidx, const int* __restrict__ pturn,
+                                                  const double* __restrict__ Pm, const double* __restrict__ shift,
+                                                  double* __restrict__ Pinv, double* __restrict__ h1,
+                                                  double* __restrict__ sw) {
+  const int nthr = pp * kPinvSplit;
   const int t = threadIdx.x / kPinvSplit, c = threadIdx.x % kPinvSplit;   // row, column phase
   const bool act = static_cast<int>(threadIdx.x) < nthr;
   const double* src = Pm + static_cast<size_t>(pch) * pp * pp;
@@ -442,7 +441,10 @@ __global__ void __launch_bounds__(kPatchMax * kPinvSplit) patch_invert_kernel(in
   // row sums: the kPinvSplit threads of a row are adjacent lanes
 #pragma unroll
   for (int o = kPinvSplit / 2; o > 0; o >>= 1) hs += __shfl_xor_sync(0xffffffffu, hs, o);
-  if (act && c == 0) h1[pidx[pch * pp + t]] = hs;
+  if (act && c == 0) {
+    if (H1_ATOMIC) atomicAdd(h1 + pidx[pch * pp + t], hs);
+    else h1[pidx[pch * pp + t]] = hs;
+  }
   double tot = (act && c == 0) ? hs : 0.0;
   tot = warp_sum(tot);
   if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = tot;
@@ -452,6 +454,16 @@ __global__ void __launch_bounds__(kPatchMax * kPinvSplit) patch_invert_kernel(in
     for (int k = 0; k < static_cast<int>(blockDim.x >> 5); ++k) ssum += part[k];
     atomicAdd(sw + pturn[pch], ssum);
   }
+}
+__global__ void __launch_bounds__(kPatchMax * kPinvSplit) patch_invert_kernel(int pp, const int* __restrict__ pidx,
+                                                                              const int* __restrict__ pturn,
+                                                                              const double* __restrict__ Pm,
+                                                                              const double* __restrict__ shift,
+                                                                              double* __restrict__ Pinv, double* __restrict__ h1,
+                                                                              double* __restrict__ sw) {
+  __shared__ double A[kPatchMax][kPatchMax + 1];
+  __shared__ double part[kPatchMax * kPinvSplit / 32];
+  patch_invert_body<false>(A, part, blockIdx.x, pp, pidx, pturn, Pm, shift, Pinv, h1, sw);
 }
 
 // t = Pinv r over one patch; parks t in g and adds sum t to tw[turn].  UPDATE: first x += alpha p, r += alpha q
@@ -547,10 +559,9 @@ __global__ void __launch_bounds__(kPatchMax) coarse_build_kernel(PatchPrec pc, c
 // per solve, after the patch inverses: C0inv[w] = (C0m[layer] + diag(sum of the shift over each patch))^-1 by the same
 // elimination in shared memory; h1 += Z C Z^T 1, s_w += its sum.  One CTA per wire, kPinvSplit threads per coarse
 // unknown (each owns every kPinvSplit-th column; a single wire is a single CTA, so the row work is spread).
-__global__ void __launch_bounds__(kPatchMax * kPinvSplit) coarse_invert_kernel(PatchPrec pc, const double* __restrict__ shift) {
-  __shared__ double A[kPatchMax][kPatchMax + 1];
-  __shared__ double hc[kPatchMax];
-  const int nc = pc.nc, pp = pc.pp, w = blockIdx.x;
+__device__ __forceinline__ void coarse_invert_body(double (*A)[kPatchMax + 1], double* hc, int w, const PatchPrec& pc,
+                                                   const double* __restrict__ shift) {
+  const int nc = pc.nc, pp = pc.pp;
   const int t = threadIdx.x / kPinvSplit, c = threadIdx.x % kPinvSplit;   // row, column phase
   const bool act = t < nc;
   const double* src = pc.C0m + static_cast<size_t>(w / pc.per_layer) * nc * nc;
@@ -591,13 +602,25 @@ __global__ void __launch_bounds__(kPatchMax * kPinvSplit) coarse_invert_kernel(P
   __syncthreads();
   for (int e = threadIdx.x; e < nc * pp; e += blockDim.x) {        // h1 += Z hc over the cells of the wire
     const int q = e / pp;
-    pc.h1[pc.pidx[(static_cast<size_t>(w) * nc + q) * pp + (e - q * pp)]] += hc[q];
+    atomicAdd(pc.h1 + pc.pidx[(static_cast<size_t>(w) * nc + q) * pp + (e - q * pp)], hc[q]);
   }
   if (threadIdx.x == 0) {
     double s = 0.0;
     for (int q = 0; q < nc; ++q) s += hc[q];
     atomicAdd(pc.sw + w, s * pp);
   }
+}
+// both levels in ONE launch (CTAs 0 .. n_patches-1: the patches, the rest: one per wire); h1 and s_w are accumulated with
+// atomics into zeroed arrays, so the two levels need no order (config 1: the single coarse CTA of 0.13 ms hides behind
+// the 64 patch CTAs instead of following them)
+__global__ void __launch_bounds__(kPatchMax * kPinvSplit) two_level_invert_kernel(PatchPrec pc, const double* __restrict__ shift) {
+  __shared__ double A[kPatchMax][kPatchMax + 1];
+  __shared__ double part[kPatchMax * kPinvSplit / 32];
+  __shared__ double hc[kPatchMax];
+  if (static_cast<int>(blockIdx.x) < pc.n_patches)
+    patch_invert_body<true>(A, part, blockIdx.x, pc.pp, pc.pidx, pc.pturn, pc.Pm, shift, pc.Pinv, pc.h1, pc.sw);
+  else
+    coarse_invert_body(A, hc, static_cast<int>(blockIdx.x) - pc.n_patches, pc, shift);
 }
 
 // per iteration, after the patch products: yc = C0inv (Z^T r) per wire, tw[w] += sum of Z yc.  kPinvSplit threads per
@@ -1021,11 +1044,11 @@ void k_patch_start(const VecCtx& v, const CgIter& it, const double* shift) {
     cudaFuncSetAttribute(patch_invert_big_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     patch_invert_big_kernel<<<pc.n_patches, kBigThreads, smem, v.stream>>>(pc, p, shift);
   }
-  else patch_invert_kernel<<<pc.n_patches, kPatchMax * kPinvSplit, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pm, shift, pc.Pinv, pc.h1, pc.sw);
-  if (pc.nc > 0) {
-    QS_LAUNCH(v);
-    coarse_invert_kernel<<<v.n_turns, kPatchMax * kPinvSplit, 0, v.stream>>>(pc, shift);
+  else if (pc.nc > 0) {   // patches and coarse level in one launch
+    cudaMemsetAsync(pc.h1, 0, sizeof(double) * v.N, v.stream);
+    two_level_invert_kernel<<<pc.n_patches + v.n_turns, kPatchMax * kPinvSplit, 0, v.stream>>>(pc, shift);
   }
+  else patch_invert_kernel<<<pc.n_patches, kPatchMax * kPinvSplit, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pm, shift, pc.Pinv, pc.h1, pc.sw);
   QS_LAUNCH(v);
   patch_apply_kernel<false><<<pc.n_patches, patch_threads(pc), 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pinv, it, v.sc);
   if (pc.nc > 0) {

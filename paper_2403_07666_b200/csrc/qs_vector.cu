@@ -467,8 +467,10 @@ __global__ void __launch_bounds__(kPatchMax * kPinvSplit) patch_invert_kernel(in
 }
 
 // t = Pinv r over one patch; parks t in g and adds sum t to tw[turn].  UPDATE: first x += alpha p, r += alpha q
-// (the fused CG iteration's update); else r is taken as it is (start of the solve).
-template <bool UPDATE>
+// (the fused CG iteration's update); else r is taken as it is (start of the solve).  SPLIT threads per row (adjacent
+// lanes, each a part of the row product): 4 for the patches of <= 64 cells (few, small CTAs: the product is a latency
+// chain), 1 for the big patches.
+template <bool UPDATE, int SPLIT>
 __global__ void __launch_bounds__(kWireMax) patch_apply_kernel(int pp, const int* __restrict__ pidx,
                                                               const int* __restrict__ pturn,
                                                               const double* __restrict__ Pinv, CgIter it, Scalars* sc) {
@@ -484,10 +486,10 @@ __global__ void __launch_bounds__(kWireMax) patch_apply_kernel(int pp, const int
     }
     alpha = sc->rg[it.par] / pq;
   }
-  const int pch = blockIdx.x, t = threadIdx.x;
+  const int pch = blockIdx.x, t = threadIdx.x / SPLIT, c = threadIdx.x % SPLIT;
   const bool act = t < pp;
   const int i = act ? pidx[pch * pp + t] : 0;
-  if (act) {
+  if (act && c == 0) {
     double ri = it.r[i];
     if (UPDATE) {
       it.x[i] = fma(alpha, it.p[i], it.x[i]);
@@ -500,15 +502,18 @@ __global__ void __launch_bounds__(kWireMax) patch_apply_kernel(int pp, const int
   double acc = 0.0;
   if (act) {
     const double* col = Pinv + static_cast<size_t>(pch) * pp * pp + t;   // column t = row t (symmetric): coalesced
-    for (int u = 0; u < pp; ++u) acc = fma(col[static_cast<size_t>(u) * pp], rs[u], acc);
-    it.g[i] = acc;
+    for (int u = c; u < pp; u += SPLIT) acc = fma(col[static_cast<size_t>(u) * pp], rs[u], acc);
   }
-  acc = warp_sum(acc);
-  if ((t & 31) == 0) part[t >> 5] = acc;
+#pragma unroll
+  for (int o = SPLIT / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (act && c == 0) it.g[i] = acc;
+  double tot = (act && c == 0) ? acc : 0.0;
+  tot = warp_sum(tot);
+  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = tot;
   __syncthreads();
-  if (t == 0) {
+  if (threadIdx.x == 0) {
     double s = 0.0;
-    for (int k = 0; k < (pp + 31) / 32; ++k) s += part[k];
+    for (int k = 0; k < static_cast<int>((blockDim.x + 31) >> 5); ++k) s += part[k];
     atomicAdd(it.tw + pturn[pch], s);
     if (it.patch.nc > 0) {             // second level: restricted residual of this patch
       double rsum = 0.0;
@@ -1003,12 +1008,16 @@ void k_cg_Ap(const VecCtx& v, const CgIter& it) {
   QS_LAUNCH(v);
   cg_Ap_kernel<<<grid_for(v.N), kBlock, 0, v.stream>>>(v.N, it, v.sc);
 }
-static int patch_threads(const PatchPrec& pc) { return pc.big ? (pc.pp + 31) / 32 * 32 : kPatchMax; }
+static int patch_threads(const PatchPrec& pc) { return pc.big ? (pc.pp + 31) / 32 * 32 : (pc.pp * kPinvSplit + 31) / 32 * 32; }
 void k_cg_update(const VecCtx& v, const CgIter& it) {
   QS_LAUNCH(v);
   if (it.patch.pp > 0) {   // patch preconditioner: update fused with t = Pinv r
-    patch_apply_kernel<true><<<it.patch.n_patches, patch_threads(it.patch), 0, v.stream>>>(it.patch.pp, it.patch.pidx, it.patch.pturn,
-                                                                           it.patch.Pinv, it, v.sc);
+    if (it.patch.big)
+      patch_apply_kernel<true, 1><<<it.patch.n_patches, patch_threads(it.patch), 0, v.stream>>>(it.patch.pp, it.patch.pidx,
+                                                                                             it.patch.pturn, it.patch.Pinv, it, v.sc);
+    else
+      patch_apply_kernel<true, kPinvSplit><<<it.patch.n_patches, patch_threads(it.patch), 0, v.stream>>>(
+          it.patch.pp, it.patch.pidx, it.patch.pturn, it.patch.Pinv, it, v.sc);
     if (it.patch.nc > 0) {
       QS_LAUNCH(v);
       coarse_apply_kernel<true><<<v.n_turns, kPatchMax * kPinvSplit, 0, v.stream>>>(it.patch, it.tw, v.sc);
@@ -1050,7 +1059,8 @@ void k_patch_start(const VecCtx& v, const CgIter& it, const double* shift) {
   }
   else patch_invert_kernel<<<pc.n_patches, kPatchMax * kPinvSplit, 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pm, shift, pc.Pinv, pc.h1, pc.sw);
   QS_LAUNCH(v);
-  patch_apply_kernel<false><<<pc.n_patches, patch_threads(pc), 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pinv, it, v.sc);
+  if (pc.big) patch_apply_kernel<false, 1><<<pc.n_patches, patch_threads(pc), 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pinv, it, v.sc);
+  else patch_apply_kernel<false, kPinvSplit><<<pc.n_patches, patch_threads(pc), 0, v.stream>>>(pc.pp, pc.pidx, pc.pturn, pc.Pinv, it, v.sc);
   if (pc.nc > 0) {
     QS_LAUNCH(v);
     coarse_apply_kernel<false><<<v.n_turns, kPatchMax * kPinvSplit, 0, v.stream>>>(pc, it.tw, v.sc);
